@@ -1,0 +1,128 @@
+/* bg_moe.h -- C ABI of the B200-native combined MoE layer (the hot path behind BatchGen's
+ * `combine` primitive).
+ *
+ * What the library computes.  The paper's runtime yields sequence coroutines at the MoE module
+ * boundary and COMBINEs them -- a concatenation of their hidden-state tensors (PAPER.md:192-194,
+ * §4.2) -- so that each expert receives a larger batch; what then runs is
+ *     h_out <- MoE(h_combined, l)            (Algorithm 1 line 8; prose PAPER.md:263)
+ * The paper does not spell out the MoE arithmetic; BASELINE.json `north_star` fixes it (restated
+ * in DESIGN.md §1): fp32 router -> top-k (ties to the lower expert index, softmax-renormalised
+ * gates) -> per-expert histogram -> exclusive scan -> stable permutation into expert-contiguous
+ * rows -> grouped SwiGLU expert FFN (gate/up GEMM, SiLU.mul, down GEMM) -> gate-weighted
+ * un-permute that sums each token's top-k results in slot order.
+ *
+ * Conventions (all entry points):
+ *  - Every data pointer is a DEVICE pointer owned by the caller (e.g. a torch tensor), 16-byte
+ *    aligned, valid until the work enqueued on `stream` has completed.  The only HOST-pointer
+ *    entry point is bg_moe_combined_forward_host (named so).  The library owns only its context
+ *    and workspace.  Inputs are never modified; outputs are fully overwritten.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Every call
+ *    is asynchronous on that stream: no host synchronisation, no allocation after bg_moe_create.
+ *  - All tensors are row-major (last index contiguous).  bf16 tensors are passed as void*.
+ *    T = combined tokens, d = hidden, E = experts, k = top-k, f = expert intermediate, R = T*k.
+ *  - Indices are int32 (R <= 2^31-1); byte offsets are computed in 64 bits.
+ *  - Return value: BG_OK (0) or a negative bg_moe_status.  Nothing aborts or throws across the
+ *    ABI.  T == 0 is BG_OK and a no-op.  A context is not thread-safe: one call at a time.
+ *  - Supported ranges: 1 <= E <= 256, 1 <= k <= min(E, 8), d and f multiples of 8 (d >= 64,
+ *    f >= 64), 0 <= T <= max_tokens.  Device must be sm_100 (B200).  There is no CPU fallback.
+ */
+#ifndef BG_MOE_H_
+#define BG_MOE_H_
+
+#include <stdint.h>
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bg_moe_ctx bg_moe_ctx;
+
+typedef enum {
+  BG_OK = 0,
+  BG_ERR_INVALID_ARG = -1,  /* NULL, T<0, T>max_tokens, k<1, k>E, misaligned pointer, d/f not /8 */
+  BG_ERR_UNSUPPORTED = -2,  /* E>256, k>8, gate_fn != 0, device is not sm_100 */
+  BG_ERR_CUDA = -3,         /* a CUDA call failed; bg_moe_last_error(ctx) has the string */
+  BG_ERR_NOMEM = -4,        /* workspace allocation failed */
+  BG_ERR_NO_WEIGHTS = -5    /* bg_moe_set_weights has not been called */
+} bg_moe_status;
+
+typedef struct {
+  int32_t d;          /* hidden size */
+  int32_t f;          /* expert intermediate size */
+  int32_t E;          /* number of routed experts */
+  int32_t k;          /* experts per token */
+  int32_t max_tokens; /* workspace is sized for T <= max_tokens */
+  int32_t gate_fn;    /* 0 = softmax over the k selected logits (the only one defined) */
+  int32_t device;     /* CUDA device ordinal */
+} bg_moe_config;
+
+/* Allocates the context and its device workspace (logits, routing tables, x_perm, H, Y).
+ * *out is set only on BG_OK. */
+int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out);
+int bg_moe_destroy(bg_moe_ctx* ctx);
+
+/* Borrows (does not copy) the layer's parameters.  W_r fp32 [d,E]; b_r fp32 [E] or NULL (reading
+ * S7: added to the logits in fp32, used for selection and gates); W_gate, W_up bf16 [E,d,f];
+ * W_down bf16 [E,f,d].  Consumed in these layouts as given (reading S14). */
+int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, const void* W_gate,
+                       const void* W_up, const void* W_down);
+
+/* Steps a1-a4: router logits, top-k + gates, histogram, exclusive scan.
+ *   hidden     bf16 [T,d]
+ *   logits_in  NULL, or fp32 [T,E]: use these logits instead of computing a1
+ *   logits_out NULL, or fp32 [T,E]: receives the logits used
+ *   topk_idx   int32 [T,k]  slot s = s-th largest under (logit desc, expert index asc)
+ *   topk_w     fp32 [T,k]   softmax over the k selected logits
+ *   counts     int32 [E];  offsets int32 [E+1], offsets[E] = T*k */
+int bg_moe_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits_in,
+                 float* logits_out, int32_t* topk_idx, float* topk_w, int32_t* counts,
+                 int32_t* offsets, void* stream);
+
+/* Steps a5-a6: stable counting sort of flat index i = t*k+s by expert, and the row gather.
+ *   row_src  int32 [T*k]: row_src[r] = i;   inv_perm int32 [T*k]: inv_perm[i] = r
+ *   x_perm   bf16 [T*k,d]: x_perm[r,:] = hidden[row_src[r]/k,:]   (may be NULL: skip the gather) */
+int bg_moe_permute(bg_moe_ctx* ctx, const void* hidden, int32_t T, const int32_t* topk_idx,
+                   const int32_t* offsets, int32_t* row_src, int32_t* inv_perm, void* x_perm,
+                   void* stream);
+
+/* Steps a7-a8, un-fused form: y_perm[r,:] = (silu(x W_gate[e]) . (x W_up[e])) W_down[e] for the
+ * rows r in [offsets[e], offsets[e+1]); bf16 in, fp32 accumulate, H rounded to bf16 between the
+ * two GEMMs, y_perm bf16 [T*k,d] in expert order, NOT gate-weighted. */
+int bg_moe_expert_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t T,
+                      void* y_perm, void* stream);
+
+/* Step a9, un-fused form: out[t,:] = sum_{s<k} topk_w[t,s] * y_perm[inv_perm[t*k+s],:], summed in
+ * slot order in fp32, rounded once (RNE) to bf16.  No floating-point atomics. */
+int bg_moe_unpermute(bg_moe_ctx* ctx, const void* y_perm, const int32_t* inv_perm,
+                     const float* topk_w, int32_t T, void* out, void* stream);
+
+/* The fused chain a1-a9 on the context's workspace: hidden bf16 [T,d] -> out bf16 [T,d].
+ * Same math as the split calls except that the down-GEMM epilogue applies the gate weight (in
+ * fp32, before the bf16 rounding of Y) and the final reduce only sums. */
+int bg_moe_combined_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void* out, void* stream);
+
+/* Same, but `hidden_host` and `out_host` are HOST pointers (pinned memory recommended): copies
+ * hidden host->device, runs the fused chain, copies out device->host, all on `stream`. */
+int bg_moe_combined_forward_host(bg_moe_ctx* ctx, const void* hidden_host, int32_t T,
+                                 void* out_host, void* stream);
+
+/* Device pointers into the workspace holding the routing artefacts of the LAST fused call
+ * (valid until the next call on this context).  Any out-pointer may be NULL. */
+int bg_moe_debug_views(bg_moe_ctx* ctx, const float** logits, const int32_t** topk_idx,
+                       const float** topk_w, const int32_t** counts, const int32_t** offsets,
+                       const int32_t** row_src, const int32_t** inv_perm);
+
+/* Number of kernels this library has launched through `ctx` since creation. */
+int64_t bg_moe_launch_count(const bg_moe_ctx* ctx);
+/* Bytes of device workspace owned by `ctx`. */
+int64_t bg_moe_workspace_bytes(const bg_moe_ctx* ctx);
+
+const char* bg_moe_strerror(int status);
+/* Text of the last CUDA error seen by `ctx` ("" if none).  Owned by the context. */
+const char* bg_moe_last_error(const bg_moe_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BG_MOE_H_ */

@@ -1,0 +1,207 @@
+"""ctypes binding with the same names as the C ABI (include/bg_moe.h).  Marshalling only."""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libbg_moe.so")
+
+BG_OK, BG_ERR_INVALID_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA, BG_ERR_NOMEM, BG_ERR_NO_WEIGHTS = 0, -1, -2, -3, -4, -5
+
+EXPORTS = ["bg_moe_create", "bg_moe_destroy", "bg_moe_set_weights", "bg_moe_route", "bg_moe_permute",
+           "bg_moe_expert_ffn", "bg_moe_unpermute", "bg_moe_combined_forward", "bg_moe_combined_forward_host",
+           "bg_moe_debug_views", "bg_moe_launch_count", "bg_moe_workspace_bytes", "bg_moe_strerror",
+           "bg_moe_last_error"]
+
+
+class BgMoeConfig(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("d", "f", "E", "k", "max_tokens", "gate_fn", "device")]
+
+
+class BgMoeError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"bg_moe status {status}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """Loads libbg_moe.so; raises (no fallback) if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2606_21712_b200.build` "
+                              "(there is no CPU fallback)")
+        lib = ctypes.CDLL(LIB_PATH)
+        vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+        lib.bg_moe_create.argtypes = [ctypes.POINTER(BgMoeConfig), ctypes.POINTER(vp)]
+        lib.bg_moe_destroy.argtypes = [vp]
+        lib.bg_moe_set_weights.argtypes = [vp] * 6
+        lib.bg_moe_route.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
+        lib.bg_moe_permute.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp]
+        lib.bg_moe_expert_ffn.argtypes = [vp, vp, vp, i32, vp, vp]
+        lib.bg_moe_unpermute.argtypes = [vp, vp, vp, vp, i32, vp, vp]
+        lib.bg_moe_combined_forward.argtypes = [vp, vp, i32, vp, vp]
+        lib.bg_moe_combined_forward_host.argtypes = [vp, vp, i32, vp, vp]
+        lib.bg_moe_debug_views.argtypes = [vp] + [ctypes.POINTER(vp)] * 7
+        lib.bg_moe_launch_count.argtypes = [vp]
+        lib.bg_moe_launch_count.restype = i64
+        lib.bg_moe_workspace_bytes.argtypes = [vp]
+        lib.bg_moe_workspace_bytes.restype = i64
+        lib.bg_moe_strerror.argtypes = [ctypes.c_int]
+        lib.bg_moe_strerror.restype = ctypes.c_char_p
+        lib.bg_moe_last_error.argtypes = [vp]
+        lib.bg_moe_last_error.restype = ctypes.c_char_p
+        _lib = lib
+    return _lib
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream: Optional[torch.cuda.Stream]):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+class MoELayer:
+    """One combined MoE layer context (`bg_moe_ctx`).  Methods mirror the C entry points."""
+
+    def __init__(self, d: int, f: int, E: int, k: int, max_tokens: int, device: int = 0, gate_fn: int = 0):
+        self.lib = load_library()
+        self.d, self.f, self.E, self.k, self.max_tokens, self.device = d, f, E, k, max_tokens, device
+        self._ctx = ctypes.c_void_p()
+        cfg = BgMoeConfig(d, f, E, k, max_tokens, gate_fn, device)
+        self._check(self.lib.bg_moe_create(ctypes.byref(cfg), ctypes.byref(self._ctx)), ctx=False)
+        self._weights = None
+
+    # ------------------------------------------------------------------ helpers
+    def _check(self, rc: int, ctx: bool = True):
+        if rc != BG_OK:
+            msg = self.lib.bg_moe_strerror(rc).decode()
+            if ctx and rc == BG_ERR_CUDA and self._ctx:
+                msg += " -- " + self.lib.bg_moe_last_error(self._ctx).decode()
+            raise BgMoeError(rc, msg)
+
+    def _dev(self):
+        return torch.device("cuda", self.device)
+
+    def close(self):
+        if getattr(self, "_ctx", None):
+            self.lib.bg_moe_destroy(self._ctx)
+            self._ctx = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def launch_count(self) -> int:
+        return int(self.lib.bg_moe_launch_count(self._ctx))
+
+    @property
+    def workspace_bytes(self) -> int:
+        return int(self.lib.bg_moe_workspace_bytes(self._ctx))
+
+    # ------------------------------------------------------------------ C ABI mirrors
+    def set_weights(self, W_r, b_r, W_gate, W_up, W_down):
+        assert W_r.dtype == torch.float32 and W_r.shape == (self.d, self.E) and W_r.is_contiguous()
+        assert b_r is None or (b_r.dtype == torch.float32 and b_r.shape == (self.E,))
+        for w, shp in ((W_gate, (self.E, self.d, self.f)), (W_up, (self.E, self.d, self.f)),
+                       (W_down, (self.E, self.f, self.d))):
+            assert w.dtype == torch.bfloat16 and tuple(w.shape) == shp and w.is_contiguous() and w.is_cuda
+        self._weights = (W_r, b_r, W_gate, W_up, W_down)          # keep the borrowed tensors alive
+        self._check(self.lib.bg_moe_set_weights(self._ctx, _ptr(W_r), _ptr(b_r), _ptr(W_gate), _ptr(W_up),
+                                                _ptr(W_down)))
+
+    def route(self, hidden, logits_in=None, want_logits=True, stream=None):
+        T = hidden.shape[0] if hidden is not None else logits_in.shape[0]
+        dev = self._dev()
+        logits = torch.empty(T, self.E, dtype=torch.float32, device=dev) if want_logits else None
+        idx = torch.empty(T, self.k, dtype=torch.int32, device=dev)
+        w = torch.empty(T, self.k, dtype=torch.float32, device=dev)
+        counts = torch.empty(self.E, dtype=torch.int32, device=dev)
+        offsets = torch.empty(self.E + 1, dtype=torch.int32, device=dev)
+        self._check(self.lib.bg_moe_route(self._ctx, _ptr(hidden), T, _ptr(logits_in), _ptr(logits), _ptr(idx),
+                                          _ptr(w), _ptr(counts), _ptr(offsets), _stream(stream)))
+        return dict(logits=logits, idx=idx, w=w, counts=counts, offsets=offsets)
+
+    def permute(self, hidden, topk_idx, offsets, gather=True, stream=None):
+        T = topk_idx.shape[0]
+        dev = self._dev()
+        row_src = torch.empty(T * self.k, dtype=torch.int32, device=dev)
+        inv_perm = torch.empty(T * self.k, dtype=torch.int32, device=dev)
+        x_perm = torch.empty(T * self.k, self.d, dtype=torch.bfloat16, device=dev) if gather else None
+        self._check(self.lib.bg_moe_permute(self._ctx, _ptr(hidden), T, _ptr(topk_idx), _ptr(offsets), _ptr(row_src),
+                                            _ptr(inv_perm), _ptr(x_perm), _stream(stream)))
+        return dict(row_src=row_src, inv_perm=inv_perm, x_perm=x_perm)
+
+    def expert_ffn(self, x_perm, offsets, T=None, stream=None):
+        T = x_perm.shape[0] // self.k if T is None else T
+        y = torch.empty(T * self.k, self.d, dtype=torch.bfloat16, device=self._dev())
+        self._check(self.lib.bg_moe_expert_ffn(self._ctx, _ptr(x_perm), _ptr(offsets), T, _ptr(y), _stream(stream)))
+        return y
+
+    def unpermute(self, y_perm, inv_perm, topk_w, stream=None):
+        T = topk_w.shape[0]
+        out = torch.empty(T, self.d, dtype=torch.bfloat16, device=self._dev())
+        self._check(self.lib.bg_moe_unpermute(self._ctx, _ptr(y_perm), _ptr(inv_perm), _ptr(topk_w), T, _ptr(out),
+                                              _stream(stream)))
+        return out
+
+    def combined_forward(self, hidden, out=None, stream=None):
+        T = hidden.shape[0]
+        assert hidden.dtype == torch.bfloat16 and hidden.is_cuda and hidden.is_contiguous()
+        if out is None:
+            out = torch.empty(T, self.d, dtype=torch.bfloat16, device=self._dev())
+        self._check(self.lib.bg_moe_combined_forward(self._ctx, _ptr(hidden), T, _ptr(out), _stream(stream)))
+        return out
+
+    def combined_forward_host(self, hidden_host, out_host=None, stream=None):
+        """hidden_host / out_host: CPU (ideally pinned) bf16 tensors; copies run on `stream`."""
+        T = hidden_host.shape[0]
+        assert hidden_host.dtype == torch.bfloat16 and not hidden_host.is_cuda and hidden_host.is_contiguous()
+        if out_host is None:
+            out_host = torch.empty(T, self.d, dtype=torch.bfloat16).pin_memory()
+        self._check(self.lib.bg_moe_combined_forward_host(self._ctx, _ptr(hidden_host), T, _ptr(out_host),
+                                                          _stream(stream)))
+        return out_host
+
+    def debug_views(self, T: int) -> dict:
+        """Routing artefacts of the last fused call, as torch tensors copied out of the workspace."""
+        ptrs = [ctypes.c_void_p() for _ in range(7)]
+        self._check(self.lib.bg_moe_debug_views(self._ctx, *[ctypes.byref(p) for p in ptrs]))
+        R = T * self.k
+        spec = [("logits", torch.float32, (T, self.E)), ("idx", torch.int32, (T, self.k)),
+                ("w", torch.float32, (T, self.k)), ("counts", torch.int32, (self.E,)),
+                ("offsets", torch.int32, (self.E + 1,)), ("row_src", torch.int32, (R,)),
+                ("inv_perm", torch.int32, (R,))]
+        out = {}
+        typestr = {torch.float32: "<f4", torch.int32: "<i4"}
+        for p, (name, dt, shape) in zip(ptrs, spec):
+            n = 1
+            for s in shape:
+                n *= s
+            if n == 0:
+                out[name] = torch.empty(shape, dtype=dt, device=self._dev())
+                continue
+            view = _DeviceArray(p.value, shape, typestr[dt])
+            out[name] = torch.as_tensor(view, device=self._dev()).clone()
+        return out
+
+
+class _DeviceArray:
+    """Zero-copy view of library-owned device memory through `__cuda_array_interface__`."""
+
+    def __init__(self, ptr: int, shape, typestr: str):
+        self.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": typestr, "data": (ptr, False),
+                                         "version": 2, "strides": None}

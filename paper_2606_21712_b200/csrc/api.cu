@@ -1,0 +1,383 @@
+// api.cu -- the C ABI declared in include/bg_moe.h: argument validation, workspace, TMA tensor-map
+// encoding and kernel sequencing.  No arithmetic of the layer happens on the host.
+#include "../../include/bg_moe.h"
+#include "kernels.h"
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+struct bg_moe_ctx {
+  bg_moe_config cfg;
+  int num_sms = 0;
+  // borrowed parameters
+  const float* W_r = nullptr;
+  const float* b_r = nullptr;
+  const void* W_gate = nullptr;
+  const void* W_up = nullptr;
+  const void* W_down = nullptr;
+  // workspace (one allocation)
+  uint8_t* ws = nullptr;
+  int64_t ws_bytes = 0;
+  float* logits = nullptr;
+  int32_t* topk_idx = nullptr;
+  float* topk_w = nullptr;
+  int32_t* counts = nullptr;
+  int32_t* offsets = nullptr;
+  int32_t* block_counts = nullptr;
+  int32_t* block_base = nullptr;
+  int32_t* row_src = nullptr;
+  int32_t* inv_perm = nullptr;
+  void* x_perm = nullptr;
+  void* H = nullptr;
+  void* Y = nullptr;
+  void* hidden_dev = nullptr;   // staging for the host-pointer entry point
+  void* out_dev = nullptr;
+  // weight tensor maps (encoded in set_weights)
+  CUtensorMap tm_wg, tm_wu, tm_wd;
+  int64_t launches = 0;
+  std::string last_error;
+};
+
+namespace {
+
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (fn == nullptr) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+// [rows, K] bf16 row-major, box {64 k, 128 rows}, 128B swizzle.
+bool encode_act_map(CUtensorMap* tm, const void* ptr, int64_t rows, int64_t K) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(rows)};
+  cuuint64_t strides[1] = {static_cast<cuuint64_t>(K) * 2};
+  cuuint32_t box[2] = {64, 128};
+  cuuint32_t estr[2] = {1, 1};
+  return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// [E, K, N] bf16 row-major (N contiguous), box {64 n, 64 k, 1 expert}, 128B swizzle.
+bool encode_weight_map(CUtensorMap* tm, const void* ptr, int64_t E, int64_t K, int64_t N) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[3] = {static_cast<cuuint64_t>(N), static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(E)};
+  cuuint64_t strides[2] = {static_cast<cuuint64_t>(N) * 2, static_cast<cuuint64_t>(N) * K * 2};
+  cuuint32_t box[3] = {64, 64, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(ptr), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+int cuda_fail(bg_moe_ctx* ctx, cudaError_t e, const char* where) {
+  if (ctx) ctx->last_error = std::string(where) + ": " + cudaGetErrorString(e);
+  return BG_ERR_CUDA;
+}
+
+#define BG_CUDA(ctx, call, where)                          \
+  do {                                                     \
+    cudaError_t e__ = (call);                              \
+    if (e__ != cudaSuccess) return cuda_fail(ctx, e__, where); \
+  } while (0)
+
+#define BG_LAUNCH(ctx, call, where) \
+  do {                              \
+    BG_CUDA(ctx, call, where);      \
+    (ctx)->launches += 1;           \
+  } while (0)
+
+int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
+
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+    if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
+int check_T(const bg_moe_ctx* ctx, int32_t T) {
+  if (ctx == nullptr) return BG_ERR_INVALID_ARG;
+  if (T < 0 || T > ctx->cfg.max_tokens) return BG_ERR_INVALID_ARG;
+  return BG_OK;
+}
+
+// a1-a4 on explicit buffers.
+int do_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits_in, float* logits_buf,
+             int32_t* topk_idx, float* topk_w, int32_t* counts, int32_t* offsets, cudaStream_t st) {
+  const bg_moe_config& c = ctx->cfg;
+  const float* L = logits_in;
+  if (L == nullptr) {
+    BG_LAUNCH(ctx, bg::launch_router_logits(hidden, ctx->W_r, ctx->b_r, T, c.d, c.E, logits_buf, st), "router_logits");
+    L = logits_buf;
+  }
+  BG_LAUNCH(ctx, bg::launch_topk_hist(L, T, c.E, c.k, topk_idx, topk_w, ctx->block_counts, st), "topk_hist");
+  BG_LAUNCH(ctx, bg::launch_scan(ctx->block_counts, bg::route_num_blocks(T, c.k), c.E, ctx->block_base, counts,
+                                 offsets, st), "scan");
+  return BG_OK;
+}
+
+int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t T, void* y, const float* row_scale,
+           const int32_t* row_src, cudaStream_t st) {
+  const bg_moe_config& c = ctx->cfg;
+  const int64_t R = static_cast<int64_t>(T) * c.k;
+  bg::GemmLaunch g1;
+  if (!encode_act_map(&g1.tm_a, x_perm, R, c.d)) { ctx->last_error = "cuTensorMapEncodeTiled(x_perm) failed"; return BG_ERR_CUDA; }
+  g1.tm_b0 = ctx->tm_wg;
+  g1.tm_b1 = ctx->tm_wu;
+  g1.offsets = offsets;
+  g1.E = c.E; g1.K = c.d; g1.N = c.f;
+  g1.out = ctx->H;
+  g1.row_scale = nullptr; g1.row_src = nullptr;
+  g1.num_sms = ctx->num_sms;
+  BG_LAUNCH(ctx, bg::launch_gateup_swiglu(g1, st), "gateup_swiglu");
+  bg::GemmLaunch g2;
+  if (!encode_act_map(&g2.tm_a, ctx->H, R, c.f)) { ctx->last_error = "cuTensorMapEncodeTiled(H) failed"; return BG_ERR_CUDA; }
+  g2.tm_b0 = ctx->tm_wd;
+  g2.tm_b1 = ctx->tm_wd;
+  g2.offsets = offsets;
+  g2.E = c.E; g2.K = c.f; g2.N = c.d;
+  g2.out = y;
+  g2.row_scale = row_scale; g2.row_src = row_src;
+  g2.num_sms = ctx->num_sms;
+  BG_LAUNCH(ctx, bg::launch_down(g2, st), "down");
+  return BG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* bg_moe_strerror(int status) {
+  switch (status) {
+    case BG_OK: return "ok";
+    case BG_ERR_INVALID_ARG: return "invalid argument";
+    case BG_ERR_UNSUPPORTED: return "unsupported configuration or device";
+    case BG_ERR_CUDA: return "CUDA error (see bg_moe_last_error)";
+    case BG_ERR_NOMEM: return "out of device memory";
+    case BG_ERR_NO_WEIGHTS: return "weights not set";
+    default: return "unknown status";
+  }
+}
+
+const char* bg_moe_last_error(const bg_moe_ctx* ctx) { return ctx ? ctx->last_error.c_str() : ""; }
+int64_t bg_moe_launch_count(const bg_moe_ctx* ctx) { return ctx ? ctx->launches : 0; }
+int64_t bg_moe_workspace_bytes(const bg_moe_ctx* ctx) { return ctx ? ctx->ws_bytes : 0; }
+
+int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
+  if (cfg == nullptr || out == nullptr) return BG_ERR_INVALID_ARG;
+  const bg_moe_config& c = *cfg;
+  if (c.d < 64 || c.f < 64 || c.d % 8 || c.f % 8 || c.E < 1 || c.k < 1 || c.k > c.E || c.max_tokens < 0 ||
+      c.device < 0)
+    return BG_ERR_INVALID_ARG;
+  if (c.E > 256 || c.k > 8 || c.gate_fn != 0) return BG_ERR_UNSUPPORTED;
+  if (static_cast<int64_t>(c.max_tokens) * c.k > 0x7fffffffLL) return BG_ERR_INVALID_ARG;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || c.device >= ndev) return BG_ERR_UNSUPPORTED;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, c.device) != cudaSuccess) return BG_ERR_CUDA;
+  if (prop.major != 10) return BG_ERR_UNSUPPORTED;   // tcgen05 / TMEM: sm_100 only, no fallback
+  DeviceGuard guard(c.device);
+  if (!guard.ok) return BG_ERR_CUDA;
+  if (get_encode_fn() == nullptr) return BG_ERR_CUDA;
+  if (bg::gemm_kernels_init() != cudaSuccess) return BG_ERR_CUDA;
+
+  bg_moe_ctx* ctx = new (std::nothrow) bg_moe_ctx();
+  if (!ctx) return BG_ERR_NOMEM;
+  ctx->cfg = c;
+  ctx->num_sms = prop.multiProcessorCount;
+  const int64_t Tm = c.max_tokens > 0 ? c.max_tokens : 1;
+  const int64_t Rm = Tm * c.k;
+  const int64_t nblk = bg::route_num_blocks(static_cast<int>(Tm), c.k);
+  int64_t off = 0;
+  auto carve = [&](int64_t bytes) { int64_t o = off; off = align_up(off + bytes, 1024); return o; };
+  const int64_t o_logits = carve(Tm * c.E * 4), o_idx = carve(Rm * 4), o_w = carve(Rm * 4);
+  const int64_t o_counts = carve(c.E * 4), o_offsets = carve((c.E + 1) * 4);
+  const int64_t o_bc = carve(nblk * c.E * 4), o_bb = carve(nblk * c.E * 4);
+  const int64_t o_rs = carve(Rm * 4), o_ip = carve(Rm * 4);
+  const int64_t o_x = carve(Rm * c.d * 2), o_h = carve(Rm * c.f * 2), o_y = carve(Rm * c.d * 2);
+  const int64_t o_hd = carve(Tm * c.d * 2), o_od = carve(Tm * c.d * 2);
+  ctx->ws_bytes = off;
+  void* p = nullptr;
+  if (cudaMalloc(&p, static_cast<size_t>(off)) != cudaSuccess) {
+    cudaGetLastError();
+    delete ctx;
+    return BG_ERR_NOMEM;
+  }
+  ctx->ws = static_cast<uint8_t*>(p);
+  ctx->logits = reinterpret_cast<float*>(ctx->ws + o_logits);
+  ctx->topk_idx = reinterpret_cast<int32_t*>(ctx->ws + o_idx);
+  ctx->topk_w = reinterpret_cast<float*>(ctx->ws + o_w);
+  ctx->counts = reinterpret_cast<int32_t*>(ctx->ws + o_counts);
+  ctx->offsets = reinterpret_cast<int32_t*>(ctx->ws + o_offsets);
+  ctx->block_counts = reinterpret_cast<int32_t*>(ctx->ws + o_bc);
+  ctx->block_base = reinterpret_cast<int32_t*>(ctx->ws + o_bb);
+  ctx->row_src = reinterpret_cast<int32_t*>(ctx->ws + o_rs);
+  ctx->inv_perm = reinterpret_cast<int32_t*>(ctx->ws + o_ip);
+  ctx->x_perm = ctx->ws + o_x;
+  ctx->H = ctx->ws + o_h;
+  ctx->Y = ctx->ws + o_y;
+  ctx->hidden_dev = ctx->ws + o_hd;
+  ctx->out_dev = ctx->ws + o_od;
+  *out = ctx;
+  return BG_OK;
+}
+
+int bg_moe_destroy(bg_moe_ctx* ctx) {
+  if (ctx == nullptr) return BG_OK;
+  DeviceGuard guard(ctx->cfg.device);
+  if (ctx->ws) cudaFree(ctx->ws);
+  delete ctx;
+  return BG_OK;
+}
+
+int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, const void* W_gate, const void* W_up,
+                       const void* W_down) {
+  if (!ctx || !W_r || !W_gate || !W_up || !W_down) return BG_ERR_INVALID_ARG;
+  if (!aligned16(W_r) || !aligned16(W_gate) || !aligned16(W_up) || !aligned16(W_down)) return BG_ERR_INVALID_ARG;
+  const bg_moe_config& c = ctx->cfg;
+  if (!encode_weight_map(&ctx->tm_wg, W_gate, c.E, c.d, c.f) || !encode_weight_map(&ctx->tm_wu, W_up, c.E, c.d, c.f) ||
+      !encode_weight_map(&ctx->tm_wd, W_down, c.E, c.f, c.d)) {
+    ctx->last_error = "cuTensorMapEncodeTiled(weights) failed";
+    return BG_ERR_CUDA;
+  }
+  ctx->W_r = W_r; ctx->b_r = b_r; ctx->W_gate = W_gate; ctx->W_up = W_up; ctx->W_down = W_down;
+  return BG_OK;
+}
+
+int bg_moe_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits_in, float* logits_out,
+                 int32_t* topk_idx, float* topk_w, int32_t* counts, int32_t* offsets, void* stream) {
+  int rc = check_T(ctx, T);
+  if (rc) return rc;
+  if (!counts || !offsets) return BG_ERR_INVALID_ARG;
+  if (T == 0) {   // nothing routed: counts and offsets are all zero
+    DeviceGuard guard0(ctx->cfg.device);
+    BG_LAUNCH(ctx, bg::launch_scan(ctx->block_counts, 0, ctx->cfg.E, ctx->block_base, counts, offsets,
+                                   static_cast<cudaStream_t>(stream)), "scan");
+    return BG_OK;
+  }
+  if (!topk_idx || !topk_w) return BG_ERR_INVALID_ARG;
+  if (logits_in == nullptr && (hidden == nullptr || !aligned16(hidden))) return BG_ERR_INVALID_ARG;
+  if (logits_in == nullptr && ctx->W_r == nullptr) return BG_ERR_NO_WEIGHTS;
+  DeviceGuard guard(ctx->cfg.device);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  float* lbuf = logits_out ? logits_out : ctx->logits;
+  rc = do_route(ctx, hidden, T, logits_in, lbuf, topk_idx, topk_w, counts, offsets, st);
+  if (rc) return rc;
+  if (logits_in && logits_out && logits_in != logits_out && T > 0)
+    BG_CUDA(ctx, cudaMemcpyAsync(logits_out, logits_in, sizeof(float) * T * ctx->cfg.E, cudaMemcpyDeviceToDevice, st),
+            "copy logits");
+  return BG_OK;
+}
+
+int bg_moe_permute(bg_moe_ctx* ctx, const void* hidden, int32_t T, const int32_t* topk_idx, const int32_t* offsets,
+                   int32_t* row_src, int32_t* inv_perm, void* x_perm, void* stream) {
+  int rc = check_T(ctx, T);
+  if (rc) return rc;
+  if (T == 0) return BG_OK;
+  if (!topk_idx || !offsets || !row_src || !inv_perm) return BG_ERR_INVALID_ARG;
+  if (x_perm && (!hidden || !aligned16(hidden) || !aligned16(x_perm))) return BG_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->cfg.device);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const bg_moe_config& c = ctx->cfg;
+  BG_LAUNCH(ctx, bg::launch_block_hist(topk_idx, T, c.E, c.k, ctx->block_counts, st), "block_hist");
+  BG_LAUNCH(ctx, bg::launch_scan(ctx->block_counts, bg::route_num_blocks(T, c.k), c.E, ctx->block_base, nullptr,
+                                 nullptr, st), "scan");
+  BG_LAUNCH(ctx, bg::launch_rank(topk_idx, ctx->block_base, T, c.E, c.k, row_src, inv_perm, st), "rank");
+  if (x_perm) BG_LAUNCH(ctx, bg::launch_gather(hidden, row_src, T * c.k, c.k, c.d, x_perm, ctx->num_sms, st), "gather");
+  return BG_OK;
+}
+
+int bg_moe_expert_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t T, void* y_perm,
+                      void* stream) {
+  int rc = check_T(ctx, T);
+  if (rc) return rc;
+  if (T == 0) return BG_OK;
+  if (!x_perm || !offsets || !y_perm || !aligned16(x_perm) || !aligned16(y_perm)) return BG_ERR_INVALID_ARG;
+  if (ctx->W_gate == nullptr) return BG_ERR_NO_WEIGHTS;
+  DeviceGuard guard(ctx->cfg.device);
+  return do_ffn(ctx, x_perm, offsets, T, y_perm, nullptr, nullptr, static_cast<cudaStream_t>(stream));
+}
+
+int bg_moe_unpermute(bg_moe_ctx* ctx, const void* y_perm, const int32_t* inv_perm, const float* topk_w, int32_t T,
+                     void* out, void* stream) {
+  int rc = check_T(ctx, T);
+  if (rc) return rc;
+  if (T == 0) return BG_OK;
+  if (!y_perm || !inv_perm || !topk_w || !out || !aligned16(y_perm) || !aligned16(out)) return BG_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->cfg.device);
+  BG_LAUNCH(ctx, bg::launch_unpermute(y_perm, inv_perm, topk_w, T, ctx->cfg.k, ctx->cfg.d, out, ctx->num_sms,
+                                      static_cast<cudaStream_t>(stream)), "unpermute");
+  return BG_OK;
+}
+
+int bg_moe_combined_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void* out, void* stream) {
+  int rc = check_T(ctx, T);
+  if (rc) return rc;
+  if (T == 0) return BG_OK;
+  if (!hidden || !out || !aligned16(hidden) || !aligned16(out)) return BG_ERR_INVALID_ARG;
+  if (ctx->W_r == nullptr) return BG_ERR_NO_WEIGHTS;
+  DeviceGuard guard(ctx->cfg.device);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const bg_moe_config& c = ctx->cfg;
+  rc = do_route(ctx, hidden, T, nullptr, ctx->logits, ctx->topk_idx, ctx->topk_w, ctx->counts, ctx->offsets, st);
+  if (rc) return rc;
+  BG_LAUNCH(ctx, bg::launch_rank(ctx->topk_idx, ctx->block_base, T, c.E, c.k, ctx->row_src, ctx->inv_perm, st), "rank");
+  BG_LAUNCH(ctx, bg::launch_gather(hidden, ctx->row_src, T * c.k, c.k, c.d, ctx->x_perm, ctx->num_sms, st), "gather");
+  rc = do_ffn(ctx, ctx->x_perm, ctx->offsets, T, ctx->Y, ctx->topk_w, ctx->row_src, st);
+  if (rc) return rc;
+  BG_LAUNCH(ctx, bg::launch_unpermute(ctx->Y, ctx->inv_perm, nullptr, T, c.k, c.d, out, ctx->num_sms, st), "unpermute");
+  return BG_OK;
+}
+
+int bg_moe_combined_forward_host(bg_moe_ctx* ctx, const void* hidden_host, int32_t T, void* out_host, void* stream) {
+  int rc = check_T(ctx, T);
+  if (rc) return rc;
+  if (T == 0) return BG_OK;
+  if (!hidden_host || !out_host) return BG_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->cfg.device);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const size_t bytes = static_cast<size_t>(T) * ctx->cfg.d * 2;
+  BG_CUDA(ctx, cudaMemcpyAsync(ctx->hidden_dev, hidden_host, bytes, cudaMemcpyHostToDevice, st), "H2D hidden");
+  rc = bg_moe_combined_forward(ctx, ctx->hidden_dev, T, ctx->out_dev, stream);
+  if (rc) return rc;
+  BG_CUDA(ctx, cudaMemcpyAsync(out_host, ctx->out_dev, bytes, cudaMemcpyDeviceToHost, st), "D2H out");
+  return BG_OK;
+}
+
+int bg_moe_debug_views(bg_moe_ctx* ctx, const float** logits, const int32_t** topk_idx, const float** topk_w,
+                       const int32_t** counts, const int32_t** offsets, const int32_t** row_src,
+                       const int32_t** inv_perm) {
+  if (!ctx) return BG_ERR_INVALID_ARG;
+  if (logits) *logits = ctx->logits;
+  if (topk_idx) *topk_idx = ctx->topk_idx;
+  if (topk_w) *topk_w = ctx->topk_w;
+  if (counts) *counts = ctx->counts;
+  if (offsets) *offsets = ctx->offsets;
+  if (row_src) *row_src = ctx->row_src;
+  if (inv_perm) *inv_perm = ctx->inv_perm;
+  return BG_OK;
+}
+
+}  // extern "C"

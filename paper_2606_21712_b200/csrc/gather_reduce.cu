@@ -1,0 +1,130 @@
+// gather_reduce.cu -- the two HBM-bound row movers of the combined MoE layer:
+//   a6 gather    x_perm[r,:] = hidden[row_src[r]/k,:]                        (16-byte vector copies)
+//   a9 reduce    out[t,:]    = sum_{s<k} (w[t,s]) * Y[inv_perm[t*k+s],:]     slot order, fp32, RNE->bf16
+// BASELINE.json north_star: "a gather kernel with 16-byte vectorised, coalesced row copies" and "a
+// gate-weighted un-permute that sums each token's top-k results", atomic-free.
+// One warp moves one row at a time; consecutive lanes touch consecutive 16-byte vectors, several
+// vectors in flight per lane.  Grid = a multiple of the SM count, warps stride over rows.
+#include "kernels.h"
+#include <cuda_bf16.h>
+
+namespace bg {
+namespace {
+
+__device__ __forceinline__ uint4 ld_stream(const uint4* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_stream(uint4* p, const uint4& v) {
+  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
+               "r"(v.w) : "memory");
+}
+
+__global__ void __launch_bounds__(256) gather_kernel(const uint4* __restrict__ hidden,
+                                                     const int32_t* __restrict__ row_src, int R, int k,
+                                                     int vec_per_row, uint4* __restrict__ x_perm) {
+  const int lane = threadIdx.x & 31;
+  const int warps_total = gridDim.x * (blockDim.x >> 5);
+  for (int r = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); r < R; r += warps_total) {
+    const int t = __ldg(row_src + r) / k;
+    const uint4* src = hidden + static_cast<int64_t>(t) * vec_per_row;
+    uint4* dst = x_perm + static_cast<int64_t>(r) * vec_per_row;
+    int c = lane;
+    for (; c + 96 < vec_per_row; c += 128) {
+      const uint4 a0 = __ldg(src + c), a1 = __ldg(src + c + 32), a2 = __ldg(src + c + 64), a3 = __ldg(src + c + 96);
+      st_stream(dst + c, a0);
+      st_stream(dst + c + 32, a1);
+      st_stream(dst + c + 64, a2);
+      st_stream(dst + c + 96, a3);
+    }
+    for (; c < vec_per_row; c += 32) st_stream(dst + c, __ldg(src + c));
+  }
+}
+
+__device__ __forceinline__ void accum8(float* acc, const uint4& v, float w) {
+  const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&v);
+  #pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const float2 f = __bfloat1622float2(h[i]);
+    acc[2 * i] = fmaf(w, f.x, acc[2 * i]);
+    acc[2 * i + 1] = fmaf(w, f.y, acc[2 * i + 1]);
+  }
+}
+
+template <int KMAX>
+__global__ void __launch_bounds__(256) unpermute_kernel(const uint4* __restrict__ y_perm,
+                                                        const int32_t* __restrict__ inv_perm,
+                                                        const float* __restrict__ weights, int T, int k,
+                                                        int vec_per_row, uint4* __restrict__ out) {
+  const int lane = threadIdx.x & 31;
+  const int warps_total = gridDim.x * (blockDim.x >> 5);
+  for (int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); t < T; t += warps_total) {
+    const uint4* rows[KMAX];
+    float w[KMAX];
+    #pragma unroll
+    for (int s = 0; s < KMAX; ++s) {
+      rows[s] = y_perm;
+      w[s] = 0.0f;
+      if (s < k) {
+        rows[s] = y_perm + static_cast<int64_t>(__ldg(inv_perm + static_cast<int64_t>(t) * k + s)) * vec_per_row;
+        w[s] = weights ? __ldg(weights + static_cast<int64_t>(t) * k + s) : 1.0f;
+      }
+    }
+    uint4* dst = out + static_cast<int64_t>(t) * vec_per_row;
+    for (int c = lane; c < vec_per_row; c += 32) {
+      uint4 v[KMAX];
+      #pragma unroll
+      for (int s = 0; s < KMAX; ++s)
+        if (s < k) v[s] = ld_stream(rows[s] + c);
+      float acc[8];
+      #pragma unroll
+      for (int i = 0; i < 8; ++i) acc[i] = 0.0f;
+      #pragma unroll
+      for (int s = 0; s < KMAX; ++s)       // slot order s = 0..k-1 (reading S11)
+        if (s < k) accum8(acc, v[s], w[s]);
+      uint4 o;
+      __nv_bfloat162 p;
+      p = __floats2bfloat162_rn(acc[0], acc[1]); o.x = *reinterpret_cast<uint32_t*>(&p);
+      p = __floats2bfloat162_rn(acc[2], acc[3]); o.y = *reinterpret_cast<uint32_t*>(&p);
+      p = __floats2bfloat162_rn(acc[4], acc[5]); o.z = *reinterpret_cast<uint32_t*>(&p);
+      p = __floats2bfloat162_rn(acc[6], acc[7]); o.w = *reinterpret_cast<uint32_t*>(&p);
+      st_stream(dst + c, o);
+    }
+  }
+}
+
+inline int row_mover_grid(int rows, int num_sms) {
+  const int blocks_needed = (rows + 7) / 8;
+  const int cap = num_sms * 8;     // 8 resident blocks of 256 threads per SM
+  return blocks_needed < cap ? (blocks_needed > 0 ? blocks_needed : 1) : cap;
+}
+
+}  // namespace
+
+cudaError_t launch_gather(const void* hidden, const int32_t* row_src, int R, int k, int d, void* x_perm,
+                          int num_sms, cudaStream_t st) {
+  if (R == 0) return cudaSuccess;
+  gather_kernel<<<row_mover_grid(R, num_sms), 256, 0, st>>>(static_cast<const uint4*>(hidden), row_src, R, k, d / 8,
+                                                            static_cast<uint4*>(x_perm));
+  return cudaGetLastError();
+}
+
+cudaError_t launch_unpermute(const void* y_perm, const int32_t* inv_perm, const float* weights, int T, int k,
+                             int d, void* out, int num_sms, cudaStream_t st) {
+  if (T == 0) return cudaSuccess;
+  const int grid = row_mover_grid(T, num_sms);
+  if (k <= 2)
+    unpermute_kernel<2><<<grid, 256, 0, st>>>(static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
+                                              static_cast<uint4*>(out));
+  else if (k <= 4)
+    unpermute_kernel<4><<<grid, 256, 0, st>>>(static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
+                                              static_cast<uint4*>(out));
+  else
+    unpermute_kernel<8><<<grid, 256, 0, st>>>(static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
+                                              static_cast<uint4*>(out));
+  return cudaGetLastError();
+}
+
+}  // namespace bg

@@ -1,0 +1,57 @@
+// kernels.h -- internal launcher interface between api.cu and the kernel translation units.
+// Not part of the public ABI (include/bg_moe.h is).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace bg {
+
+// ---- routing (routing.cu): steps a1-a5 of DESIGN.md §1
+// Tokens handled by one block of the top-k / rank kernels: chosen so that a block owns at most
+// 256 flat (token,slot) entries, one per thread of the rank kernel.
+inline int route_tokens_per_block(int k) { return 256 / k; }
+inline int route_num_blocks(int T, int k) {
+  const int tb = route_tokens_per_block(k);
+  return (T + tb - 1) / tb;
+}
+
+cudaError_t launch_router_logits(const void* hidden, const float* W_r, const float* b_r, int T, int d, int E,
+                                 float* logits, cudaStream_t st);
+cudaError_t launch_topk_hist(const float* logits, int T, int E, int k, int32_t* topk_idx, float* topk_w,
+                             int32_t* block_counts, cudaStream_t st);
+// block_counts [nblk,E]: per-block counts -> block_base [nblk,E]: expert offset + exclusive prefix
+// over blocks (the first row of block b inside expert e).  counts / offsets may be NULL.
+cudaError_t launch_scan(const int32_t* block_counts, int nblk, int E, int32_t* block_base, int32_t* counts,
+                        int32_t* offsets, cudaStream_t st);
+// Recomputes block_counts from topk_idx (used by the split bg_moe_permute, which receives only
+// topk_idx and offsets).
+cudaError_t launch_block_hist(const int32_t* topk_idx, int T, int E, int k, int32_t* block_counts,
+                              cudaStream_t st);
+cudaError_t launch_rank(const int32_t* topk_idx, const int32_t* block_base, int T, int E, int k,
+                        int32_t* row_src, int32_t* inv_perm, cudaStream_t st);
+
+// ---- gather / reduce (gather_reduce.cu): steps a6 and a9
+cudaError_t launch_gather(const void* hidden, const int32_t* row_src, int R, int k, int d, void* x_perm,
+                          int num_sms, cudaStream_t st);
+// weights == nullptr: plain sum (fused path, Y already gate-weighted).
+cudaError_t launch_unpermute(const void* y_perm, const int32_t* inv_perm, const float* weights, int T, int k,
+                             int d, void* out, int num_sms, cudaStream_t st);
+
+// ---- grouped GEMM (grouped_gemm.cu): steps a7 and a8
+struct GemmLaunch {
+  CUtensorMap tm_a;    // activations [rows_cap, K] bf16, box {64, 128}
+  CUtensorMap tm_b0;   // weights [E, K, N] bf16, box {64, 64, 1}: W_gate (gate/up GEMM) or W_down
+  CUtensorMap tm_b1;   // W_up (gate/up GEMM only)
+  const int32_t* offsets;  // [E+1]
+  int E, K, N;         // N = output columns (f for gate/up, d for down)
+  void* out;           // bf16 [rows, N]
+  const float* row_scale;   // down GEMM, fused path: topk_w flat [T*k] (else nullptr)
+  const int32_t* row_src;   // down GEMM, fused path: row -> flat index
+  int num_sms;
+};
+cudaError_t launch_gateup_swiglu(const GemmLaunch& g, cudaStream_t st);
+cudaError_t launch_down(const GemmLaunch& g, cudaStream_t st);
+cudaError_t gemm_kernels_init();   // sets the dynamic shared-memory attributes once
+
+}  // namespace bg

@@ -1,0 +1,269 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Bars (BASELINE.json north_star):
+  * routing artefacts (idx, counts, offsets, row_src, inv_perm) bit-exact given the same fp32 logits;
+  * logits |L_gpu - L_ref| <= 1e-4 * max(1,|L|); gate weights |w_gpu - w_ref| <= 2e-6;
+  * expert outputs max|err| <= 2e-2 * max|ref| and relative L2 <= 5e-3 (bf16 I/O, fp32 accumulate).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+MAX_TOL, L2_TOL = 2e-2, 5e-3
+
+
+def to_dev(lay):
+    dev = torch.device("cuda", 0)
+    return {k: (v.to(dev) if isinstance(v, torch.Tensor) else v) for k, v in lay.items()}
+
+
+def make(cfg, max_tokens=None):
+    from paper_2606_21712_b200 import MoELayer
+    lay = wl.make_layer(cfg)
+    g = to_dev(lay)
+    layer = MoELayer(cfg.d, cfg.f, cfg.E, cfg.k, max_tokens or max(cfg.T, 1))
+    layer.set_weights(g["W_r"], g["b_r"], g["W_gate"], g["W_up"], g["W_down"])
+    return lay, g, layer
+
+
+def check_out(out_gpu: torch.Tensor, ref: np.ndarray, what=""):
+    got = out_gpu.to(torch.float64).cpu().numpy()
+    assert np.all(np.isfinite(got)), f"{what}: non-finite output"
+    scale = np.max(np.abs(ref))
+    err = np.abs(got - ref)
+    max_err = err.max() if err.size else 0.0
+    l2 = np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-300) if err.size else 0.0
+    assert max_err <= MAX_TOL * scale, f"{what}: max|err| {max_err:.3e} > {MAX_TOL}*max|ref| ({scale:.3e}); relL2 {l2:.3e}"
+    assert l2 <= L2_TOL, f"{what}: relative L2 {l2:.3e} > {L2_TOL}"
+    return max_err / max(scale, 1e-300), l2
+
+
+def check_routing_against_oracle(logits_gpu, idx, w, counts, offsets, row_src, inv_perm, E, k):
+    """Feed the GPU's fp32 logits to the oracle's top-k / hist / scan / perm: integers bit-exact."""
+    L = logits_gpu.cpu().numpy()
+    o_idx, o_w = oracle.topk_gate(L, k)
+    assert np.array_equal(idx.cpu().numpy(), o_idx), "topk_idx differs from the oracle on the same logits"
+    assert np.max(np.abs(w.cpu().numpy() - o_w)) <= 2e-6 if o_w.size else True
+    assert np.all(np.abs(w.cpu().numpy().astype(np.float64).sum(1) - 1) <= 4 * k * 2.0**-24)
+    o_counts, o_offsets, o_rs, o_ip = oracle.hist_scan_perm(o_idx, E)
+    assert np.array_equal(counts.cpu().numpy(), o_counts)
+    assert np.array_equal(offsets.cpu().numpy(), o_offsets)
+    if row_src is not None:
+        assert np.array_equal(row_src.cpu().numpy(), o_rs)
+        assert np.array_equal(inv_perm.cpu().numpy(), o_ip)
+    return o_idx, o_w, o_counts, o_offsets, o_rs, o_ip
+
+
+ROUTE_SHAPES = [
+    # T, d, E, k
+    (256, 512, 8, 2), (1, 64, 4, 2), (127, 128, 8, 2), (129, 96, 33, 3), (300, 256, 128, 8),
+    (64, 128, 256, 8), (200, 72, 5, 5), (77, 64, 1, 1), (513, 320, 64, 6), (1000, 64, 16, 1),
+]
+
+
+@pytest.mark.parametrize("T,d,E,k", ROUTE_SHAPES)
+def test_route_and_permute_parity(T, d, E, k):
+    cfg = wl.small_config(T=T, d=d, E=E, k=k, f=64, index=11)
+    lay, g, layer = make(cfg)
+    r = layer.route(g["hidden"])
+    Lref = oracle.router_logits(lay["hidden"], lay["W_r"], lay["b_r"])
+    Lg = r["logits"].cpu().numpy()
+    assert np.all(np.abs(Lg - Lref) <= 1e-4 * np.maximum(1.0, np.abs(Lref))), "router logits out of tolerance"
+    p = layer.permute(g["hidden"], r["idx"], r["offsets"])
+    check_routing_against_oracle(r["logits"], r["idx"], r["w"], r["counts"], r["offsets"], p["row_src"],
+                                 p["inv_perm"], E, k)
+    xo = oracle.gather(lay["hidden"], p["row_src"].cpu().numpy(), k)
+    xg = p["x_perm"].view(torch.int16).cpu().numpy().view(np.uint16)
+    assert np.array_equal(xg, xo), "gathered rows differ"
+    torch.cuda.synchronize()
+
+
+def test_route_logits_in_ties_and_bias():
+    """Reverse direction of S5: oracle-made logits (with exact ties, +-0) go INTO the GPU top-k."""
+    T, E, k = 333, 40, 4
+    rng = np.random.default_rng(3)
+    L = rng.standard_normal((T, E)).astype(np.float32)
+    L[0] = 0.5                       # all equal -> experts 0..k-1
+    L[1] = np.round(L[1])            # many duplicates
+    L[2, :4] = [0.0, -0.0, 0.0, -0.0]
+    L[2, 4:] = -1.0
+    L[3, ::2] = L[3, 1::2]           # pairwise ties
+    cfg = wl.small_config(T=T, d=64, E=E, k=k, f=64, index=12)
+    lay, g, layer = make(cfg)
+    r = layer.route(None, logits_in=torch.from_numpy(L).cuda())
+    assert torch.equal(r["logits"].cpu(), torch.from_numpy(L))
+    o_idx, *_ = check_routing_against_oracle(r["logits"], r["idx"], r["w"], r["counts"], r["offsets"], None, None,
+                                             E, k)
+    assert o_idx[0].tolist() == [0, 1, 2, 3] and o_idx[2].tolist() == [0, 1, 2, 3]
+    # Zipf-style bias (reading S7): used for selection and gates
+    b = torch.linspace(-3, 0, E)
+    layer.set_weights(g["W_r"], b.cuda(), g["W_gate"], g["W_up"], g["W_down"])
+    r = layer.route(g["hidden"])
+    Lref = oracle.router_logits(lay["hidden"], lay["W_r"], b)
+    assert np.all(np.abs(r["logits"].cpu().numpy() - Lref) <= 1e-4 * np.maximum(1.0, np.abs(Lref)))
+    check_routing_against_oracle(r["logits"], r["idx"], r["w"], r["counts"], r["offsets"], None, None, E, k)
+
+
+def test_one_expert_gets_everything_and_empty_experts():
+    T, E, k = 500, 16, 2
+    L = np.full((T, E), -5.0, np.float32)
+    L[:, 7] = 3.0
+    L[:, 9] = 1.0                      # every token -> experts (7, 9); 14 experts empty
+    cfg = wl.small_config(T=T, d=64, E=E, k=k, f=64, index=13)
+    lay, g, layer = make(cfg)
+    r = layer.route(None, logits_in=torch.from_numpy(L).cuda())
+    p = layer.permute(g["hidden"], r["idx"], r["offsets"])
+    check_routing_against_oracle(r["logits"], r["idx"], r["w"], r["counts"], r["offsets"], p["row_src"],
+                                 p["inv_perm"], E, k)
+    c = r["counts"].cpu().numpy()
+    assert c[7] == T and c[9] == T and c.sum() == 2 * T
+
+
+FFN_SHAPES = [
+    # R rows per expert list, d, f
+    ([64] * 8, 512, 1024),             # C1-like: half-filled tiles
+    ([128, 256, 130, 1, 0, 127, 129, 3], 256, 384),   # ragged: tails, empty expert, multi-tile
+    ([300], 64, 64),                   # minimum d, f; one expert
+    ([5, 0, 0, 700, 2], 192, 200),     # f not a multiple of 128, K not a multiple of 64
+    ([33, 90], 1024, 136),             # N tail of 8
+]
+
+
+@pytest.mark.parametrize("rows,d,f", FFN_SHAPES)
+def test_expert_ffn_parity(rows, d, f):
+    E = len(rows)
+    R = sum(rows)
+    cfg = wl.MoEConfig("ffn", 14, T=R, d=d, E=E, k=1, f=f)
+    lay, g, layer = make(cfg)
+    offsets = np.concatenate([[0], np.cumsum(rows)]).astype(np.int32)
+    x = lay["hidden"]                                   # [R, d] rows already "expert-contiguous"
+    y = layer.expert_ffn(g["hidden"], torch.from_numpy(offsets).cuda(), T=R)
+    torch.cuda.synchronize()
+    ref = oracle.expert_ffn(x, offsets, lay["W_gate"], lay["W_up"], lay["W_down"])
+    m, l2 = check_out(y, ref, f"expert_ffn rows={rows} d={d} f={f}")
+    # per-expert check too: a wrong expert's weights would still pass a global norm only by luck
+    for e in range(E):
+        if rows[e]:
+            check_out(y[offsets[e]:offsets[e + 1]], ref[offsets[e]:offsets[e + 1]], f"expert {e}")
+
+
+def test_unpermute_parity():
+    T, k, d, E = 257, 3, 136, 7
+    rng = np.random.default_rng(4)
+    L = rng.standard_normal((T, E)).astype(np.float32)
+    idx, w = oracle.topk_gate(L, k)
+    _, _, _, inv_perm = oracle.hist_scan_perm(idx, E)
+    cfg = wl.small_config(T=T, d=d, E=E, k=k, f=64, index=15)
+    lay, g, layer = make(cfg)
+    y = (torch.randn(T * k, d, generator=torch.Generator().manual_seed(1)) * 0.3).to(torch.bfloat16)
+    out = layer.unpermute(y.cuda(), torch.from_numpy(inv_perm).cuda(), torch.from_numpy(w).cuda())
+    ref = oracle.unpermute(y.to(torch.float64).numpy(), inv_perm, w)
+    got = out.to(torch.float64).cpu().numpy()
+    # only the final RNE to bf16 (2^-9 relative) plus fp32 summation noise
+    assert np.all(np.abs(got - ref) <= 2.0**-8 * np.abs(ref) + 1e-6)
+
+
+FUSED_SHAPES = [
+    wl.C1,
+    wl.small_config(T=1, d=64, E=4, k=2, f=64, index=21, name="T1"),
+    wl.small_config(T=127, d=128, E=8, k=2, f=256, index=22, name="T127"),
+    wl.small_config(T=129, d=256, E=5, k=5, f=192, index=23, name="k=E"),
+    wl.small_config(T=384, d=512, E=1, k=1, f=512, index=24, name="dense"),
+    wl.small_config(T=600, d=256, E=130, k=8, f=128, index=25, name="E130"),
+    wl.small_config(T=96, d=320, E=256, k=8, f=200, index=26, name="E256-sparse"),
+]
+
+
+@pytest.mark.parametrize("cfg", FUSED_SHAPES, ids=lambda c: c.name)
+def test_fused_forward_parity(cfg):
+    lay, g, layer = make(cfg)
+    n0 = layer.launch_count
+    out = layer.combined_forward(g["hidden"])
+    torch.cuda.synchronize()
+    assert layer.launch_count - n0 == 8          # router, topk, scan, rank, gather, 2 GEMMs, reduce
+    v = layer.debug_views(cfg.T)
+    check_routing_against_oracle(v["logits"], v["idx"], v["w"], v["counts"], v["offsets"], v["row_src"],
+                                 v["inv_perm"], cfg.E, cfg.k)
+    # expert outputs: oracle routed by the GPU's logits (reading S5), fp64, no intermediate rounding
+    ref = oracle.forward_batched(lay["hidden"], lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"],
+                                 cfg.k, logits_in=v["logits"].cpu().numpy())
+    m, l2 = check_out(out, ref["out"], cfg.name)
+    # and the oracle's own logits agree with the GPU's
+    own = oracle.router_logits(lay["hidden"], lay["W_r"], lay["b_r"])
+    assert np.all(np.abs(v["logits"].cpu().numpy() - own) <= 1e-4 * np.maximum(1.0, np.abs(own)))
+
+
+def test_fused_equals_split_and_is_deterministic():
+    cfg = wl.small_config(T=700, d=256, E=12, k=3, f=320, index=27)
+    lay, g, layer = make(cfg)
+    out1 = layer.combined_forward(g["hidden"])
+    out2 = layer.combined_forward(g["hidden"])
+    assert torch.equal(out1, out2), "fused path is not bitwise deterministic run to run"
+    r = layer.route(g["hidden"])
+    p = layer.permute(g["hidden"], r["idx"], r["offsets"])
+    y = layer.expert_ffn(p["x_perm"], r["offsets"])
+    out_split = layer.unpermute(y, p["inv_perm"], r["w"])
+    torch.cuda.synchronize()
+    ref = oracle.forward_batched(lay["hidden"], lay["W_r"], None, lay["W_gate"], lay["W_up"], lay["W_down"], cfg.k,
+                                 logits_in=r["logits"].cpu().numpy())["out"]
+    check_out(out_split, ref, "split")
+    check_out(out1, ref, "fused")
+    # the two differ only in where the gate weight is applied (before vs after Y's bf16 rounding)
+    a, b = out1.float(), out_split.float()
+    assert (a - b).abs().max().item() <= 2e-2 * b.abs().max().item()
+
+
+def test_combine_invariance_on_gpu():
+    """forward(concat(S1,S2)) == concat(forward(S1), forward(S2)), row for row."""
+    cfg = wl.small_config(T=300, d=128, E=8, k=2, f=128, index=28)
+    lay, g, layer = make(cfg)
+    h = g["hidden"]
+    full = layer.combined_forward(h).clone()
+    a = layer.combined_forward(h[:111].contiguous()).clone()
+    b = layer.combined_forward(h[111:].contiguous()).clone()
+    assert torch.equal(torch.cat([a, b]), full), "per-row results depend on what the row was combined with"
+    perm = torch.randperm(300, generator=torch.Generator().manual_seed(2)).cuda()
+    shuf = layer.combined_forward(h[perm].contiguous())
+    assert torch.equal(shuf, full[perm])
+
+
+def test_host_entry_point_and_zero_tokens():
+    cfg = wl.small_config(T=200, d=128, E=8, k=2, f=128, index=29)
+    lay, g, layer = make(cfg)
+    dev_out = layer.combined_forward(g["hidden"])
+    host_out = layer.combined_forward_host(lay["hidden"].pin_memory())
+    torch.cuda.synchronize()
+    assert torch.equal(host_out, dev_out.cpu())
+    empty = torch.empty(0, cfg.d, dtype=torch.bfloat16, device="cuda")
+    assert layer.combined_forward(empty).shape == (0, cfg.d)          # T == 0: BG_OK, no-op
+    r = layer.route(empty)
+    assert r["counts"].sum().item() == 0 and r["offsets"].abs().sum().item() == 0
+
+
+def test_argument_errors():
+    from paper_2606_21712_b200 import MoELayer, BgMoeError, BG_ERR_INVALID_ARG, BG_ERR_UNSUPPORTED, BG_ERR_NO_WEIGHTS
+    with pytest.raises(BgMoeError) as ei:
+        MoELayer(512, 1024, 300, 2, 16)          # E > 256
+    assert ei.value.status == BG_ERR_UNSUPPORTED
+    with pytest.raises(BgMoeError) as ei:
+        MoELayer(512, 1024, 8, 9, 16)            # k > E
+    assert ei.value.status == BG_ERR_INVALID_ARG
+    with pytest.raises(BgMoeError) as ei:
+        MoELayer(100, 1024, 8, 2, 16)            # d not a multiple of 8
+    assert ei.value.status == BG_ERR_INVALID_ARG
+    layer = MoELayer(64, 64, 4, 2, 16)
+    h = torch.zeros(32, 64, dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(BgMoeError) as ei:
+        layer.combined_forward(h[:8].contiguous())   # weights not set
+    assert ei.value.status == BG_ERR_NO_WEIGHTS
+    cfg = wl.small_config(T=16, d=64, E=4, k=2, f=64, index=30)
+    g = to_dev(wl.make_layer(cfg))
+    layer.set_weights(g["W_r"], None, g["W_gate"], g["W_up"], g["W_down"])
+    with pytest.raises(BgMoeError) as ei:
+        layer.combined_forward(h)                # T > max_tokens
+    assert ei.value.status == BG_ERR_INVALID_ARG
