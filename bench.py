@@ -1,0 +1,328 @@
+#!/usr/bin/env python
+"""bench.py -- combined MoE layer throughput on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--T tokens] [--impl reference]
+
+A "step" is one pass of the whole hot path (router -> top-k -> histogram/scan -> permutation ->
+gather -> grouped gate/up GEMM + SwiGLU -> grouped down GEMM -> un-permute reduce) over one
+batch of T combined tokens of seeded synthetic data (workloads.py).  Default workload: C2, the
+Mixtral-8x7B-shaped layer at T=4096 (BASELINE.json configs[1]).  One JSON line on stdout.
+
+N > 1 (launched under torch.distributed.run): token data parallelism, "replicas only" -- every
+rank holds all experts and its own T tokens, no data-path collective; the only
+communication is the barrier and the max-over-ranks of the device time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+import workloads as wl  # noqa: E402
+
+METRIC = "combined MoE layer TFLOP/s & roofline fraction vs combined tokens T (1xB200)"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+NOMINAL = {"hbm_gbs": 8000.0, "bf16_tflops": 2250.0}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": float(d["bf16_tflops"]),
+                    "bf16_tflops_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"]))}, "measured"
+        except Exception:
+            pass
+    return dict(FALLBACK_PEAKS), "fallback"
+
+
+def get_config(args) -> wl.MoEConfig:
+    cfg = wl.CONFIGS[args.config]
+    if args.T:
+        cfg = cfg.with_T(args.T)
+    return cfg
+
+
+# ----------------------------------------------------------------------------- clocks
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device_index: int):
+        self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(device_index), f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.tmp,
+                                         stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.tmp.flush()
+        rows = [ln.strip().split(", ") for ln in open(self.tmp.name) if ln.strip()]
+        os.unlink(self.tmp.name)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+                for nm, v in zip(names, r[4:8]):
+                    if v.strip().lower() == "active":
+                        reasons.add(nm)
+            except Exception:
+                continue
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------- oracle legs
+def oracle_sample_tokens(cfg: wl.MoEConfig, n: int) -> np.ndarray:
+    rng = np.random.default_rng(1234)
+    return np.sort(rng.choice(cfg.T, size=min(n, cfg.T), replace=False)).astype(np.int32)
+
+
+def time_oracle(cfg, cpu_layer, n_tokens: int):
+    """Times the oracle's per-token brute force on a bounded sample; returns (TFLOP/s, seconds, cores)."""
+    import oracle
+    toks = oracle_sample_tokens(cfg, n_tokens)
+    t0 = time.perf_counter()
+    oracle.forward_tokens(cpu_layer["hidden"], cpu_layer["W_r"], cpu_layer["b_r"], cpu_layer["W_gate"],
+                          cpu_layer["W_up"], cpu_layer["W_down"], cfg.k, toks)
+    dt = time.perf_counter() - t0
+    flops = len(toks) * (6.0 * cfg.k * cfg.d * cfg.f + 2.0 * cfg.d * cfg.E)
+    return flops / dt / 1e12, dt, oracle.num_threads(), len(toks)
+
+
+def oracle_tokens_per_step(cfg: wl.MoEConfig, target_s: float, cores: int) -> int:
+    per_tok = 6.0 * cfg.k * cfg.d * cfg.f + 2.0 * cfg.d * cfg.E
+    gflops = 2.5 * cores            # the fp64 oracle runs at roughly 2-3 GFLOP/s per core
+    return int(max(cores, min(cfg.T, target_s * gflops * 1e9 / per_tok)))
+
+
+def to_cpu_layer(lay: dict) -> dict:
+    return {k: (v.cpu() if isinstance(v, torch.Tensor) else v) for k, v in lay.items()}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on this box's host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    cfg = get_config(args)
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    lay = to_cpu_layer(wl.make_layer(cfg, dev))
+    cores = oracle.num_threads()
+    n = oracle_tokens_per_step(cfg, 1.0, cores)
+    for _ in range(args.warmup):
+        time_oracle(cfg, lay, n)
+    t0 = time.perf_counter()
+    tf = []
+    for _ in range(args.steps):
+        tf.append(time_oracle(cfg, lay, n)[0])
+    total = time.perf_counter() - t0
+    flops = args.steps * n * (6.0 * cfg.k * cfg.d * cfg.f + 2.0 * cfg.d * cfg.E)
+    value = flops / total / 1e12
+    sample = f"{n} of {cfg.T} tokens per step (seeded sample), per-token brute force, fp64"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "TFLOP/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": total / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "T": cfg.T, "d": cfg.d, "E": cfg.E, "k": cfg.k, "f": cfg.f,
+                       "sample": sample},
+            "tokens_per_s": args.steps * n / total,
+            "cpu_baseline": {"value": value, "unit": "TFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ----------------------------------------------------------------------------- our arm
+def run_ours(args):
+    from paper_2606_21712_b200 import MoELayer
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = get_config(args)
+    peaks, peak_src = load_peaks()
+
+    lay = wl.make_layer(cfg, "cuda")
+    if rank:
+        lay["hidden"] = lay["hidden"].roll(17 * rank, dims=0).contiguous()   # each replica: its own tokens
+    layer = MoELayer(cfg.d, cfg.f, cfg.E, cfg.k, cfg.T, device=local)
+    layer.set_weights(lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"])
+    hidden = lay["hidden"]
+    out = torch.empty_like(hidden)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps):
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        if dist is not None:
+            t = torch.tensor([ms], device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        barrier()
+        return ms
+
+    step = lambda: layer.combined_forward(hidden, out, stream)
+    for _ in range(max(args.warmup, 3)):
+        step()
+    sampler = ClockSampler(local) if rank == 0 else None
+    n0 = layer.launch_count
+    ms_total = timed(step, args.steps)
+    launches = layer.launch_count - n0
+    clocks = sampler.stop() if sampler else None
+    ms_step = ms_total / args.steps
+
+    # ---- end to end through the host-pointer entry point (H2D + chain + D2H inside the timed region)
+    h_host = hidden.cpu().pin_memory()
+    o_host = torch.empty_like(h_host).pin_memory()
+    e2e_step = lambda: layer.combined_forward_host(h_host, o_host, stream)
+    for _ in range(3):
+        e2e_step()
+    ms_e2e = timed(e2e_step, args.steps) / args.steps
+
+    # ---- per-kernel durations (CUDA events recorded by the library on the launching stream)
+    layer.profile_enable(True)
+    acc = {}
+    for _ in range(args.steps):
+        step()
+        for k_, v in layer.profile_read().items():
+            acc[k_] = acc.get(k_, 0.0) + v
+    layer.profile_enable(False)
+    stage_ms = {k_: v / args.steps for k_, v in acc.items()}
+
+    views = layer.debug_views(cfg.T)
+    counts = views["counts"].cpu().numpy()
+    E_act = int((counts > 0).sum())
+    R = cfg.T * cfg.k
+    F = cfg.flops()
+    B_min = cfg.min_bytes(E_act)
+    tflops = F * world / (ms_step * 1e-3) / 1e12
+    t_roof_burst = max(F / (peaks["bf16_tflops"] * 1e12), B_min / (peaks["hbm_gbs"] * 1e9))
+    t_roof_sust = max(F / (peaks["bf16_tflops_sustained"] * 1e12), B_min / (peaks["hbm_gbs"] * 1e9))
+    t_roof_nom = max(F / (NOMINAL["bf16_tflops"] * 1e12), B_min / (NOMINAL["hbm_gbs"] * 1e9))
+
+    # dominant kernel and its roofline (algorithmic work per launch)
+    alg = {
+        "router": ("alu", 2.0 * cfg.T * cfg.d * cfg.E),
+        "topk_hist": ("hbm", 4.0 * cfg.T * cfg.E + 8.0 * R),
+        "scan": ("hbm", 0.0),
+        "rank": ("hbm", 12.0 * R),
+        "gather": ("hbm", 2.0 * cfg.T * cfg.d + 2.0 * R * cfg.d + 4.0 * R),
+        "gateup_swiglu": ("tensor", 4.0 * R * cfg.d * cfg.f),
+        "down": ("tensor", 2.0 * R * cfg.d * cfg.f),
+        "unpermute": ("hbm", 2.0 * R * cfg.d + 2.0 * cfg.T * cfg.d + 4.0 * R),
+    }
+    dom = max(stage_ms, key=stage_ms.get)
+    bound, work = alg[dom]
+    dom_s = stage_ms[dom] * 1e-3
+    if bound == "tensor":
+        achieved, peak, unit = work / dom_s / 1e12, peaks["bf16_tflops"], "TFLOP/s"
+    elif bound == "hbm":
+        achieved, peak, unit = work / dom_s / 1e9, peaks["hbm_gbs"], "GB/s"
+    else:
+        achieved, peak, unit = work / dom_s / 1e12, 148 * 128 * 2 * 1.965e9 / 1e12, "TFLOP/s"
+    roofline = {"kernel": dom, "bound": bound, "achieved": achieved, "peak": peak, "unit": unit,
+                "frac": achieved / peak, "traffic": None, "peak_source": f"{peak_src} (burst)",
+                "ms_per_launch": stage_ms[dom], "share_of_step": stage_ms[dom] / sum(stage_ms.values())}
+
+    line = {
+        "metric": METRIC, "value": tflops, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": cfg.name, "T": cfg.T, "d": cfg.d, "E": cfg.E, "k": cfg.k, "f": cfg.f,
+                   "E_active": E_act, "rows_per_expert_min_max": [int(counts.min()), int(counts.max())],
+                   "parallelism": "replicas" if world > 1 else "single-gpu",
+                   "l2": "inputs larger than L2 (expert weights %.0f MB); no explicit flush" %
+                         (6.0 * cfg.d * cfg.f * cfg.E / 1e6)},
+        "tokens_per_s": cfg.T * world / (ms_step * 1e-3),
+        "layer_roofline": {"F_gflop": F / 1e9, "B_min_mb": B_min / 1e6,
+                           "frac_of_measured_burst": t_roof_burst / (ms_step * 1e-3),
+                           "frac_of_measured_sustained": t_roof_sust / (ms_step * 1e-3),
+                           "frac_of_nominal": t_roof_nom / (ms_step * 1e-3), "peaks": peaks,
+                           "peak_source": peak_src},
+        "stage_ms": stage_ms,
+        "roofline": roofline,
+        "e2e": {"value": F * world / (ms_e2e * 1e-3) / 1e12, "unit": "TFLOP/s", "ms_per_step": ms_e2e,
+                "h2d_bytes_per_step": int(cfg.T * cfg.d * 2), "d2h_bytes_per_step": int(cfg.T * cfg.d * 2)},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+    }
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        cores = oracle.num_threads()
+        n = oracle_tokens_per_step(cfg, 12.0, cores)
+        cpu_lay = to_cpu_layer(lay)
+        tf, dt, cores, n = time_oracle(cfg, cpu_lay, n)
+        line["cpu_baseline"] = {"value": tf, "unit": "TFLOP/s", "cores": cores, "kind": "oracle", "seconds": dt,
+                                "sample": f"{n} of {cfg.T} tokens (seeded sample), per-token brute force, fp64"}
+    elif rank == 0:
+        line["cpu_baseline"] = None
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C2", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--T", type=int, default=0, help="override the combined-token count (C3 sweep)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

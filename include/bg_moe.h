@@ -113,6 +113,15 @@ int bg_moe_debug_views(bg_moe_ctx* ctx, const float** logits, const int32_t** to
                        const float** topk_w, const int32_t** counts, const int32_t** offsets,
                        const int32_t** row_src, const int32_t** inv_perm);
 
+/* Per-kernel timing of the fused chain.  While enabled, bg_moe_combined_forward records a CUDA
+ * event on `stream` before and after each of its BG_MOE_NUM_STAGES kernels (in launch order:
+ * router, top-k+histogram, scan, rank, gather, gate/up GEMM+SwiGLU, down GEMM, un-permute reduce).
+ * bg_moe_profile_read waits for the last recorded call and writes that call's per-kernel
+ * durations in milliseconds to ms_out[BG_MOE_NUM_STAGES] (HOST pointer). */
+#define BG_MOE_NUM_STAGES 8
+int bg_moe_profile_enable(bg_moe_ctx* ctx, int enable);
+int bg_moe_profile_read(bg_moe_ctx* ctx, float* ms_out);
+
 /* Number of kernels this library has launched through `ctx` since creation. */
 int64_t bg_moe_launch_count(const bg_moe_ctx* ctx);
 /* Bytes of device workspace owned by `ctx`. */

@@ -14,7 +14,7 @@ BG_OK, BG_ERR_INVALID_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA, BG_ERR_NOMEM, BG_ERR
 
 EXPORTS = ["bg_moe_create", "bg_moe_destroy", "bg_moe_set_weights", "bg_moe_route", "bg_moe_permute",
            "bg_moe_expert_ffn", "bg_moe_unpermute", "bg_moe_combined_forward", "bg_moe_combined_forward_host",
-           "bg_moe_debug_views", "bg_moe_launch_count", "bg_moe_workspace_bytes", "bg_moe_strerror",
+           "bg_moe_debug_views", "bg_moe_profile_enable", "bg_moe_profile_read", "bg_moe_launch_count", "bg_moe_workspace_bytes", "bg_moe_strerror",
            "bg_moe_last_error"]
 
 
@@ -50,6 +50,8 @@ def load_library() -> ctypes.CDLL:
         lib.bg_moe_combined_forward.argtypes = [vp, vp, i32, vp, vp]
         lib.bg_moe_combined_forward_host.argtypes = [vp, vp, i32, vp, vp]
         lib.bg_moe_debug_views.argtypes = [vp] + [ctypes.POINTER(vp)] * 7
+        lib.bg_moe_profile_enable.argtypes = [vp, ctypes.c_int]
+        lib.bg_moe_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
         lib.bg_moe_launch_count.argtypes = [vp]
         lib.bg_moe_launch_count.restype = i64
         lib.bg_moe_workspace_bytes.argtypes = [vp]
@@ -175,6 +177,17 @@ class MoELayer:
         self._check(self.lib.bg_moe_combined_forward_host(self._ctx, _ptr(hidden_host), T, _ptr(out_host),
                                                           _stream(stream)))
         return out_host
+
+    STAGES = ("router", "topk_hist", "scan", "rank", "gather", "gateup_swiglu", "down", "unpermute")
+
+    def profile_enable(self, on: bool = True):
+        self._check(self.lib.bg_moe_profile_enable(self._ctx, int(on)))
+
+    def profile_read(self) -> dict:
+        """Per-kernel milliseconds of the last fused call made while profiling was enabled."""
+        buf = (ctypes.c_float * len(self.STAGES))()
+        self._check(self.lib.bg_moe_profile_read(self._ctx, buf))
+        return dict(zip(self.STAGES, [float(x) for x in buf]))
 
     def debug_views(self, T: int) -> dict:
         """Routing artefacts of the last fused call, as torch tensors copied out of the workspace."""

@@ -38,6 +38,10 @@ struct bg_moe_ctx {
   CUtensorMap tm_wg, tm_wu, tm_wd;
   int64_t launches = 0;
   std::string last_error;
+  // optional per-kernel timing of the fused chain
+  bool profile = false;
+  bool profile_valid = false;
+  cudaEvent_t ev[BG_MOE_NUM_STAGES + 1] = {};
 };
 
 namespace {
@@ -105,6 +109,10 @@ int cuda_fail(bg_moe_ctx* ctx, cudaError_t e, const char* where) {
 
 int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
+inline void mark(bg_moe_ctx* ctx, int i, cudaStream_t st) {
+  if (ctx->profile) cudaEventRecord(ctx->ev[i], st);
+}
+
 struct DeviceGuard {
   int prev = -1;
   bool ok = true;
@@ -139,7 +147,7 @@ int do_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits
 }
 
 int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t T, void* y, const float* row_scale,
-           const int32_t* row_src, cudaStream_t st) {
+           const int32_t* row_src, cudaStream_t st, int mark_between = -1) {
   const bg_moe_config& c = ctx->cfg;
   const int64_t R = static_cast<int64_t>(T) * c.k;
   bg::GemmLaunch g1;
@@ -152,6 +160,7 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g1.row_scale = nullptr; g1.row_src = nullptr;
   g1.num_sms = ctx->num_sms;
   BG_LAUNCH(ctx, bg::launch_gateup_swiglu(g1, st), "gateup_swiglu");
+  if (mark_between >= 0) mark(ctx, mark_between, st);
   bg::GemmLaunch g2;
   if (!encode_act_map(&g2.tm_a, ctx->H, R, c.f)) { ctx->last_error = "cuTensorMapEncodeTiled(H) failed"; return BG_ERR_CUDA; }
   g2.tm_b0 = ctx->tm_wd;
@@ -247,6 +256,8 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
 int bg_moe_destroy(bg_moe_ctx* ctx) {
   if (ctx == nullptr) return BG_OK;
   DeviceGuard guard(ctx->cfg.device);
+  for (cudaEvent_t e : ctx->ev)
+    if (e) cudaEventDestroy(e);
   if (ctx->ws) cudaFree(ctx->ws);
   delete ctx;
   return BG_OK;
@@ -341,13 +352,25 @@ int bg_moe_combined_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void
   DeviceGuard guard(ctx->cfg.device);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const bg_moe_config& c = ctx->cfg;
-  rc = do_route(ctx, hidden, T, nullptr, ctx->logits, ctx->topk_idx, ctx->topk_w, ctx->counts, ctx->offsets, st);
-  if (rc) return rc;
+  mark(ctx, 0, st);
+  BG_LAUNCH(ctx, bg::launch_router_logits(hidden, ctx->W_r, ctx->b_r, T, c.d, c.E, ctx->logits, st), "router_logits");
+  mark(ctx, 1, st);
+  BG_LAUNCH(ctx, bg::launch_topk_hist(ctx->logits, T, c.E, c.k, ctx->topk_idx, ctx->topk_w, ctx->block_counts, st),
+            "topk_hist");
+  mark(ctx, 2, st);
+  BG_LAUNCH(ctx, bg::launch_scan(ctx->block_counts, bg::route_num_blocks(T, c.k), c.E, ctx->block_base, ctx->counts,
+                                 ctx->offsets, st), "scan");
+  mark(ctx, 3, st);
   BG_LAUNCH(ctx, bg::launch_rank(ctx->topk_idx, ctx->block_base, T, c.E, c.k, ctx->row_src, ctx->inv_perm, st), "rank");
+  mark(ctx, 4, st);
   BG_LAUNCH(ctx, bg::launch_gather(hidden, ctx->row_src, T * c.k, c.k, c.d, ctx->x_perm, ctx->num_sms, st), "gather");
-  rc = do_ffn(ctx, ctx->x_perm, ctx->offsets, T, ctx->Y, ctx->topk_w, ctx->row_src, st);
+  mark(ctx, 5, st);
+  rc = do_ffn(ctx, ctx->x_perm, ctx->offsets, T, ctx->Y, ctx->topk_w, ctx->row_src, st, /*mark_between=*/6);
   if (rc) return rc;
+  mark(ctx, 7, st);
   BG_LAUNCH(ctx, bg::launch_unpermute(ctx->Y, ctx->inv_perm, nullptr, T, c.k, c.d, out, ctx->num_sms, st), "unpermute");
+  mark(ctx, 8, st);
+  ctx->profile_valid = ctx->profile;
   return BG_OK;
 }
 
@@ -363,6 +386,25 @@ int bg_moe_combined_forward_host(bg_moe_ctx* ctx, const void* hidden_host, int32
   rc = bg_moe_combined_forward(ctx, ctx->hidden_dev, T, ctx->out_dev, stream);
   if (rc) return rc;
   BG_CUDA(ctx, cudaMemcpyAsync(out_host, ctx->out_dev, bytes, cudaMemcpyDeviceToHost, st), "D2H out");
+  return BG_OK;
+}
+
+int bg_moe_profile_enable(bg_moe_ctx* ctx, int enable) {
+  if (!ctx) return BG_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->cfg.device);
+  if (enable && ctx->ev[0] == nullptr)
+    for (cudaEvent_t& e : ctx->ev) BG_CUDA(ctx, cudaEventCreate(&e), "cudaEventCreate");
+  ctx->profile = enable != 0;
+  ctx->profile_valid = false;
+  return BG_OK;
+}
+
+int bg_moe_profile_read(bg_moe_ctx* ctx, float* ms_out) {
+  if (!ctx || !ms_out || !ctx->profile_valid) return BG_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->cfg.device);
+  BG_CUDA(ctx, cudaEventSynchronize(ctx->ev[BG_MOE_NUM_STAGES]), "cudaEventSynchronize");
+  for (int i = 0; i < BG_MOE_NUM_STAGES; ++i)
+    BG_CUDA(ctx, cudaEventElapsedTime(ms_out + i, ctx->ev[i], ctx->ev[i + 1]), "cudaEventElapsedTime");
   return BG_OK;
 }
 
