@@ -117,7 +117,7 @@ def time_oracle(cfg, cpu_layer, n_tokens: int):
 
 def oracle_tokens_per_step(cfg: wl.MoEConfig, target_s: float, cores: int) -> int:
     per_tok = 6.0 * cfg.k * cfg.d * cfg.f + 2.0 * cfg.d * cfg.E
-    gflops = 2.5 * cores            # the fp64 oracle runs at roughly 2-3 GFLOP/s per core
+    gflops = 5.5 * cores            # the fp64 oracle runs at roughly 5-6 GFLOP/s per core (measured)
     return int(max(cores, min(cfg.T, target_s * gflops * 1e9 / per_tok)))
 
 
@@ -159,6 +159,21 @@ def run_reference(args):
     return 0
 
 
+# ----------------------------------------------------------------------------- multi-rank plumbing
+def max_over_ranks(ms_local: float, dist, device) -> float:
+    """Device time of the step = the slowest rank's (contract: max over ranks, never wall clock)."""
+    if dist is None:
+        return float(ms_local)
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank: float, world: int, ms: float) -> float:
+    """Replicas only: every rank processes `units_per_rank`; value = all units / time."""
+    return units_per_rank * world / (ms * 1e-3)
+
+
 # ----------------------------------------------------------------------------- our arm
 def run_ours(args):
     from paper_2606_21712_b200 import MoELayer
@@ -198,11 +213,7 @@ def run_ours(args):
             fn()
         e1.record(stream)
         torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1)
-        if dist is not None:
-            t = torch.tensor([ms], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = max_over_ranks(e0.elapsed_time(e1), dist, "cuda")
         barrier()
         return ms
 
@@ -240,7 +251,7 @@ def run_ours(args):
     R = cfg.T * cfg.k
     F = cfg.flops()
     B_min = cfg.min_bytes(E_act)
-    tflops = F * world / (ms_step * 1e-3) / 1e12
+    tflops = whole_job_rate(F, world, ms_step) / 1e12
     t_roof_burst = max(F / (peaks["bf16_tflops"] * 1e12), B_min / (peaks["hbm_gbs"] * 1e9))
     t_roof_sust = max(F / (peaks["bf16_tflops_sustained"] * 1e12), B_min / (peaks["hbm_gbs"] * 1e9))
     t_roof_nom = max(F / (NOMINAL["bf16_tflops"] * 1e12), B_min / (NOMINAL["hbm_gbs"] * 1e9))
@@ -278,7 +289,7 @@ def run_ours(args):
                    "parallelism": "replicas" if world > 1 else "single-gpu",
                    "l2": "inputs larger than L2 (expert weights %.0f MB); no explicit flush" %
                          (6.0 * cfg.d * cfg.f * cfg.E / 1e6)},
-        "tokens_per_s": cfg.T * world / (ms_step * 1e-3),
+        "tokens_per_s": whole_job_rate(cfg.T, world, ms_step),
         "layer_roofline": {"F_gflop": F / 1e9, "B_min_mb": B_min / 1e6,
                            "frac_of_measured_burst": t_roof_burst / (ms_step * 1e-3),
                            "frac_of_measured_sustained": t_roof_sust / (ms_step * 1e-3),
@@ -286,7 +297,7 @@ def run_ours(args):
                            "peak_source": peak_src},
         "stage_ms": stage_ms,
         "roofline": roofline,
-        "e2e": {"value": F * world / (ms_e2e * 1e-3) / 1e12, "unit": "TFLOP/s", "ms_per_step": ms_e2e,
+        "e2e": {"value": whole_job_rate(F, world, ms_e2e) / 1e12, "unit": "TFLOP/s", "ms_per_step": ms_e2e,
                 "h2d_bytes_per_step": int(cfg.T * cfg.d * 2), "d2h_bytes_per_step": int(cfg.T * cfg.d * 2)},
         "gpu_launches": int(launches),
         "clocks": clocks,
@@ -295,7 +306,7 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
         cores = oracle.num_threads()
-        n = oracle_tokens_per_step(cfg, 12.0, cores)
+        n = oracle_tokens_per_step(cfg, 15.0, cores)
         cpu_lay = to_cpu_layer(lay)
         tf, dt, cores, n = time_oracle(cfg, cpu_lay, n)
         line["cpu_baseline"] = {"value": tf, "unit": "TFLOP/s", "cores": cores, "kind": "oracle", "seconds": dt,

@@ -4,6 +4,7 @@
 #include "kernels.h"
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -21,6 +22,8 @@ struct bg_moe_ctx {
   uint8_t* ws = nullptr;
   int64_t ws_bytes = 0;
   float* logits = nullptr;
+  float* partial = nullptr;     // router split-K partials [ksplit][T][E]
+  void* wr_pieces = nullptr;    // bf16 [3][d][round_up(E,16)]: exact hi/mid/lo split of W_r
   int32_t* topk_idx = nullptr;
   float* topk_w = nullptr;
   int32_t* counts = nullptr;
@@ -35,7 +38,7 @@ struct bg_moe_ctx {
   void* hidden_dev = nullptr;   // staging for the host-pointer entry point
   void* out_dev = nullptr;
   // weight tensor maps (encoded in set_weights)
-  CUtensorMap tm_wg, tm_wu, tm_wd;
+  CUtensorMap tm_wg, tm_wu, tm_wd, tm_wr;
   int64_t launches = 0;
   std::string last_error;
   // optional per-kernel timing of the fused chain
@@ -90,6 +93,10 @@ bool encode_weight_map(CUtensorMap* tm, const void* ptr, int64_t E, int64_t K, i
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+inline void mark(bg_moe_ctx* ctx, int i, cudaStream_t st) {
+  if (ctx->profile) cudaEventRecord(ctx->ev[i], st);
+}
+
 int cuda_fail(bg_moe_ctx* ctx, cudaError_t e, const char* where) {
   if (ctx) ctx->last_error = std::string(where) + ": " + cudaGetErrorString(e);
   return BG_ERR_CUDA;
@@ -108,10 +115,6 @@ int cuda_fail(bg_moe_ctx* ctx, cudaError_t e, const char* where) {
   } while (0)
 
 int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
-
-inline void mark(bg_moe_ctx* ctx, int i, cudaStream_t st) {
-  if (ctx->profile) cudaEventRecord(ctx->ev[i], st);
-}
 
 struct DeviceGuard {
   int prev = -1;
@@ -135,19 +138,30 @@ int check_T(const bg_moe_ctx* ctx, int32_t T) {
 int do_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits_in, float* logits_buf,
              int32_t* topk_idx, float* topk_w, int32_t* counts, int32_t* offsets, cudaStream_t st) {
   const bg_moe_config& c = ctx->cfg;
-  const float* L = logits_in;
-  if (L == nullptr) {
-    BG_LAUNCH(ctx, bg::launch_router_logits(hidden, ctx->W_r, ctx->b_r, T, c.d, c.E, logits_buf, st), "router_logits");
-    L = logits_buf;
+  if (logits_in == nullptr) {
+    CUtensorMap tm_h;
+    if (!encode_act_map(&tm_h, hidden, T, c.d)) { ctx->last_error = "cuTensorMapEncodeTiled(hidden) failed"; return BG_ERR_CUDA; }
+    const int ks = bg::router_ksplit(T, c.d, ctx->num_sms);
+    mark(ctx, 0, st);
+    BG_LAUNCH(ctx, bg::launch_router_gemm(tm_h, ctx->tm_wr, T, c.d, c.E, ks, ctx->partial, ctx->block_counts,
+                                          bg::route_num_blocks(T, c.k) * c.E, st), "router_gemm");
+    mark(ctx, 1, st);
+    BG_LAUNCH(ctx, bg::launch_topk_hist(ctx->partial, ks, ctx->b_r, logits_buf, T, c.E, c.k, topk_idx, topk_w,
+                                        ctx->block_counts, st), "topk_hist");
+  } else {
+    BG_CUDA(ctx, cudaMemsetAsync(ctx->block_counts, 0, sizeof(int32_t) * bg::route_num_blocks(T, c.k) * c.E, st),
+            "memset block_counts");
+    BG_LAUNCH(ctx, bg::launch_topk_hist(logits_in, 1, nullptr, nullptr, T, c.E, c.k, topk_idx, topk_w,
+                                        ctx->block_counts, st), "topk_hist");
   }
-  BG_LAUNCH(ctx, bg::launch_topk_hist(L, T, c.E, c.k, topk_idx, topk_w, ctx->block_counts, st), "topk_hist");
+  mark(ctx, 2, st);
   BG_LAUNCH(ctx, bg::launch_scan(ctx->block_counts, bg::route_num_blocks(T, c.k), c.E, ctx->block_base, counts,
                                  offsets, st), "scan");
   return BG_OK;
 }
 
-int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t T, void* y, const float* row_scale,
-           const int32_t* row_src, cudaStream_t st, int mark_between = -1) {
+int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t T, void* y,
+           const float* row_scale, const int32_t* row_src, cudaStream_t st, int mark_between = -1) {
   const bg_moe_config& c = ctx->cfg;
   const int64_t R = static_cast<int64_t>(T) * c.k;
   bg::GemmLaunch g1;
@@ -210,7 +224,7 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   DeviceGuard guard(c.device);
   if (!guard.ok) return BG_ERR_CUDA;
   if (get_encode_fn() == nullptr) return BG_ERR_CUDA;
-  if (bg::gemm_kernels_init() != cudaSuccess) return BG_ERR_CUDA;
+  if (bg::gemm_kernels_init() != cudaSuccess || bg::router_kernels_init() != cudaSuccess) return BG_ERR_CUDA;
 
   bg_moe_ctx* ctx = new (std::nothrow) bg_moe_ctx();
   if (!ctx) return BG_ERR_NOMEM;
@@ -221,7 +235,10 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   const int64_t nblk = bg::route_num_blocks(static_cast<int>(Tm), c.k);
   int64_t off = 0;
   auto carve = [&](int64_t bytes) { int64_t o = off; off = align_up(off + bytes, 1024); return o; };
+  const int64_t Tpad = align_up(Tm, 128);
+  const int64_t part_rows = Tpad > static_cast<int64_t>(ctx->num_sms) * 128 ? Tpad : static_cast<int64_t>(ctx->num_sms) * 128;
   const int64_t o_logits = carve(Tm * c.E * 4), o_idx = carve(Rm * 4), o_w = carve(Rm * 4);
+  const int64_t o_part = carve(part_rows * c.E * 4), o_pieces = carve(3LL * c.d * ((c.E + 15) & ~15) * 2);
   const int64_t o_counts = carve(c.E * 4), o_offsets = carve((c.E + 1) * 4);
   const int64_t o_bc = carve(nblk * c.E * 4), o_bb = carve(nblk * c.E * 4);
   const int64_t o_rs = carve(Rm * 4), o_ip = carve(Rm * 4);
@@ -236,6 +253,8 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   }
   ctx->ws = static_cast<uint8_t*>(p);
   ctx->logits = reinterpret_cast<float*>(ctx->ws + o_logits);
+  ctx->partial = reinterpret_cast<float*>(ctx->ws + o_part);
+  ctx->wr_pieces = ctx->ws + o_pieces;
   ctx->topk_idx = reinterpret_cast<int32_t*>(ctx->ws + o_idx);
   ctx->topk_w = reinterpret_cast<float*>(ctx->ws + o_w);
   ctx->counts = reinterpret_cast<int32_t*>(ctx->ws + o_counts);
@@ -272,6 +291,24 @@ int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, cons
       !encode_weight_map(&ctx->tm_wd, W_down, c.E, c.f, c.d)) {
     ctx->last_error = "cuTensorMapEncodeTiled(weights) failed";
     return BG_ERR_CUDA;
+  }
+  // exact bf16 hi/mid/lo split of W_r for the tensor-core router (router_gemm.cu); [3][d][E_ld]
+  {
+    DeviceGuard guard(c.device);
+    const int64_t E_ld = (c.E + 15) & ~15;
+    EncodeTiledFn fn = get_encode_fn();
+    cuuint64_t dims[3] = {static_cast<cuuint64_t>(E_ld), static_cast<cuuint64_t>(c.d), 3};
+    cuuint64_t strides[2] = {static_cast<cuuint64_t>(E_ld) * 2, static_cast<cuuint64_t>(E_ld) * c.d * 2};
+    cuuint32_t box[3] = {64, 64, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    if (fn(&ctx->tm_wr, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, ctx->wr_pieces, dims, strides, box, estr,
+           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
+      ctx->last_error = "cuTensorMapEncodeTiled(W_r pieces) failed";
+      return BG_ERR_CUDA;
+    }
+    BG_LAUNCH(ctx, bg::launch_split_wr(W_r, c.d, c.E, ctx->wr_pieces, nullptr), "split_wr");
+    BG_CUDA(ctx, cudaStreamSynchronize(nullptr), "split_wr sync");   // set_weights is the one synchronous call
   }
   ctx->W_r = W_r; ctx->b_r = b_r; ctx->W_gate = W_gate; ctx->W_up = W_up; ctx->W_down = W_down;
   return BG_OK;
@@ -352,14 +389,8 @@ int bg_moe_combined_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void
   DeviceGuard guard(ctx->cfg.device);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const bg_moe_config& c = ctx->cfg;
-  mark(ctx, 0, st);
-  BG_LAUNCH(ctx, bg::launch_router_logits(hidden, ctx->W_r, ctx->b_r, T, c.d, c.E, ctx->logits, st), "router_logits");
-  mark(ctx, 1, st);
-  BG_LAUNCH(ctx, bg::launch_topk_hist(ctx->logits, T, c.E, c.k, ctx->topk_idx, ctx->topk_w, ctx->block_counts, st),
-            "topk_hist");
-  mark(ctx, 2, st);
-  BG_LAUNCH(ctx, bg::launch_scan(ctx->block_counts, bg::route_num_blocks(T, c.k), c.E, ctx->block_base, ctx->counts,
-                                 ctx->offsets, st), "scan");
+  rc = do_route(ctx, hidden, T, nullptr, ctx->logits, ctx->topk_idx, ctx->topk_w, ctx->counts, ctx->offsets, st);
+  if (rc) return rc;
   mark(ctx, 3, st);
   BG_LAUNCH(ctx, bg::launch_rank(ctx->topk_idx, ctx->block_base, T, c.E, c.k, ctx->row_src, ctx->inv_perm, st), "rank");
   mark(ctx, 4, st);

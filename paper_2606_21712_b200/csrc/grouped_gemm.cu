@@ -36,8 +36,14 @@ constexpr int B_BYTES = (BN / 64) * B_BLK_BYTES;   // 32 KB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;     // 48 KB
 constexpr int NUM_THREADS = 256;   // warp 0 TMA, warp 1 MMA, warp 2 TMEM alloc, warps 4-7 epilogue
 constexpr int MAX_E = 256;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/ +
-                           (MAX_E + 1) * 4 * 2 /*tile tables*/;
+// Epilogue staging: each epilogue warp transposes 32 rows x 64 bf16 columns through its own
+// padded shared-memory buffer (row pitch 144 B: conflict-free 16-byte accesses) so that global
+// stores are whole 128-byte lines instead of 32 scattered 16-byte pieces.
+constexpr int EPI_PITCH = 144;
+constexpr int EPI_WARP_BYTES = 32 * EPI_PITCH;               // 4608 B
+constexpr int TABLE_BYTES = 2064;                            // 2 x (MAX_E + 1) ints, 16-byte padded
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/ + TABLE_BYTES +
+                           4 * EPI_WARP_BYTES;
 
 constexpr uint32_t IDESC = umma_idesc_bf16(BM, BN, /*A K-major*/ 0, /*B MN-major*/ 1);
 // A: K-major SW128: 8-row groups 1024 B apart (SBO); LBO unused inside one swizzle span.
@@ -111,6 +117,7 @@ grouped_gemm_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_const
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + STAGES * STAGE_BYTES + 8 * (2 * STAGES + 4));
   int* tile_start = reinterpret_cast<int*>(smem + STAGES * STAGE_BYTES + 256);
   int* m_tiles = tile_start + (MAX_E + 1);
+  uint8_t* epi_smem = smem + STAGES * STAGE_BYTES + 256 + TABLE_BYTES;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int E = p.E;
@@ -168,6 +175,8 @@ grouped_gemm_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_const
 
   if (warp == 0) {
     // ===================== TMA producer (one thread) =====================
+    // (A tile::gather4 load of the rows straight from `hidden` was measured and rejected: 32 gather4
+    //  operations per k-block cost ~40 ns each and made this kernel 3.4x slower.)
     if (lane == 0) {
       int s = 0;
       uint32_t ph = 0;
@@ -239,39 +248,55 @@ grouped_gemm_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_const
       const int n0 = c.n_tile * OUT_COLS;
       float scale = 1.0f;
       if (!GATEUP && p.row_scale != nullptr && row_ok) scale = __ldg(p.row_scale + __ldg(p.row_src + grow));
-      __nv_bfloat16* orow = p.out + grow * p.N + n0;
       mbar_wait(tfull_bar(as), aph);
       tc_fence_after();
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + as * BN;
+      uint8_t* stage_buf = epi_smem + q * EPI_WARP_BYTES;
+      const uint32_t my_row_smem = smem_u32(stage_buf) + lane * EPI_PITCH;
+      // transposed read-out: lane -> (row = lane/8 + 4*j, 16-byte piece = lane%8)
+      const int piece = lane & 7, sub_row = lane >> 3;
       #pragma unroll 1
-      for (int ch = 0; ch < OUT_COLS / 32; ++ch) {
-        uint32_t packed[16];
-        if (GATEUP) {
-          uint32_t g[32], u[32];
-          tmem_ld_32x32(taddr + ch * 32, g);
-          tmem_ld_32x32(taddr + BN / 2 + ch * 32, u);
-          tmem_ld_wait();
+      for (int ch = 0; ch < OUT_COLS / 64; ++ch) {            // 64 output columns per round
+        #pragma unroll
+        for (int half = 0; half < 2; ++half) {
+          const int c32 = ch * 64 + half * 32;               // first of 32 output columns
+          uint32_t packed[16];
+          if (GATEUP) {
+            uint32_t g[32], u[32];
+            tmem_ld_32x32(taddr + c32, g);
+            tmem_ld_32x32(taddr + BN / 2 + c32, u);
+            tmem_ld_wait();
+            #pragma unroll
+            for (int j = 0; j < 16; ++j)
+              packed[j] = pack_bf16(silu_mul(__uint_as_float(g[2 * j]), __uint_as_float(u[2 * j])),
+                                    silu_mul(__uint_as_float(g[2 * j + 1]), __uint_as_float(u[2 * j + 1])));
+          } else {
+            uint32_t a[32];
+            tmem_ld_32x32(taddr + c32, a);
+            tmem_ld_wait();
+            #pragma unroll
+            for (int j = 0; j < 16; ++j)
+              packed[j] = pack_bf16(__uint_as_float(a[2 * j]) * scale, __uint_as_float(a[2 * j + 1]) * scale);
+          }
           #pragma unroll
-          for (int j = 0; j < 16; ++j)
-            packed[j] = pack_bf16(silu_mul(__uint_as_float(g[2 * j]), __uint_as_float(u[2 * j])),
-                                  silu_mul(__uint_as_float(g[2 * j + 1]), __uint_as_float(u[2 * j + 1])));
-        } else {
-          uint32_t a[32];
-          tmem_ld_32x32(taddr + ch * 32, a);
-          tmem_ld_wait();
-          #pragma unroll
-          for (int j = 0; j < 16; ++j)
-            packed[j] = pack_bf16(__uint_as_float(a[2 * j]) * scale, __uint_as_float(a[2 * j + 1]) * scale);
+          for (int v = 0; v < 4; ++v)
+            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(my_row_smem + half * 64 + v * 16),
+                         "r"(packed[4 * v]), "r"(packed[4 * v + 1]), "r"(packed[4 * v + 2]), "r"(packed[4 * v + 3])
+                         : "memory");
         }
-        if (row_ok) {
+        __syncwarp();
+        const int col = n0 + ch * 64 + piece * 8;
+        if (col + 8 <= p.N) {
           #pragma unroll
-          for (int v = 0; v < 4; ++v) {
-            const int col = n0 + ch * 32 + v * 8;
-            if (col + 8 <= p.N)
-              *reinterpret_cast<uint4*>(orow + ch * 32 + v * 8) =
-                  make_uint4(packed[4 * v], packed[4 * v + 1], packed[4 * v + 2], packed[4 * v + 3]);
+          for (int j = 0; j < 8; ++j) {
+            const int r = sub_row + 4 * j;                   // row inside this warp's 32
+            if (q * 32 + r < c.rows_valid) {
+              const uint4 val = *reinterpret_cast<const uint4*>(stage_buf + r * EPI_PITCH + piece * 16);
+              *reinterpret_cast<uint4*>(p.out + (static_cast<int64_t>(c.row0) + q * 32 + r) * p.N + col) = val;
+            }
           }
         }
+        __syncwarp();
       }
       tc_fence_before();
       mbar_arrive(tempty_bar(as));

@@ -7,19 +7,28 @@
 
 namespace bg {
 
-// ---- routing (routing.cu): steps a1-a5 of DESIGN.md §1
+// ---- router logits on tensor cores (router_gemm.cu): step a1
+cudaError_t router_kernels_init();
+// pieces: bf16 [3][d][round_up(E,16)] = exact hi/mid/lo split of W_r (zero padded)
+cudaError_t launch_split_wr(const float* W_r, int d, int E, void* pieces, cudaStream_t st);
+int router_ksplit(int T, int d, int num_sms);
+// partial: fp32 [ksplit][T][E].  Also zeroes zero_buf[0..zero_n) (the histogram the top-k kernel fills).
+cudaError_t launch_router_gemm(const CUtensorMap& tm_h, const CUtensorMap& tm_w, int T, int d, int E, int ksplit,
+                               float* partial, int32_t* zero_buf, int zero_n, cudaStream_t st);
+
+// ---- routing (routing.cu): steps a1 (sum of partials + bias) - a5 of DESIGN.md §1
 // Tokens handled by one block of the top-k / rank kernels: chosen so that a block owns at most
-// 256 flat (token,slot) entries, one per thread of the rank kernel.
-inline int route_tokens_per_block(int k) { return 256 / k; }
+// 1024 flat (token,slot) entries, one per thread of the rank kernel.
+inline int route_tokens_per_block(int k) { return 1024 / k; }
 inline int route_num_blocks(int T, int k) {
   const int tb = route_tokens_per_block(k);
   return (T + tb - 1) / tb;
 }
 
-cudaError_t launch_router_logits(const void* hidden, const float* W_r, const float* b_r, int T, int d, int E,
-                                 float* logits, cudaStream_t st);
-cudaError_t launch_topk_hist(const float* logits, int T, int E, int k, int32_t* topk_idx, float* topk_w,
-                             int32_t* block_counts, cudaStream_t st);
+// src: fp32 [n_src][T][E] slabs added in ascending order (+ b_r) -> logits_out (may be NULL).
+// block_counts [route_num_blocks][E] must be zero on entry (router kernel or a memset does that).
+cudaError_t launch_topk_hist(const float* src, int n_src, const float* b_r, float* logits_out, int T, int E, int k,
+                             int32_t* topk_idx, float* topk_w, int32_t* block_counts, cudaStream_t st);
 // block_counts [nblk,E]: per-block counts -> block_base [nblk,E]: expert offset + exclusive prefix
 // over blocks (the first row of block b inside expert e).  counts / offsets may be NULL.
 cudaError_t launch_scan(const int32_t* block_counts, int nblk, int E, int32_t* block_base, int32_t* counts,
@@ -40,7 +49,7 @@ cudaError_t launch_unpermute(const void* y_perm, const int32_t* inv_perm, const 
 
 // ---- grouped GEMM (grouped_gemm.cu): steps a7 and a8
 struct GemmLaunch {
-  CUtensorMap tm_a;    // activations [rows_cap, K] bf16, box {64, 128}
+  CUtensorMap tm_a;    // activations [rows, K] bf16, box {64, 128}
   CUtensorMap tm_b0;   // weights [E, K, N] bf16, box {64, 64, 1}: W_gate (gate/up GEMM) or W_down
   CUtensorMap tm_b1;   // W_up (gate/up GEMM only)
   const int32_t* offsets;  // [E+1]

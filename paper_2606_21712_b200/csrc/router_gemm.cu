@@ -1,0 +1,193 @@
+// router_gemm.cu -- step a1 (router logits) on tensor cores with fp32-exact products.
+//
+//   L[t,e] = sum_j float(hidden[t,j]) * W_r[j,e]            (BASELINE.json north_star "fp32 router")
+//
+// hidden is bf16 and an fp32 W_r[j,e] (24-bit significand) is EXACTLY the sum of three bf16 values
+// hi + mid + lo (8 significand bits each, reading S6), so
+//   hidden * W_r = hidden * hi + hidden * mid + hidden * lo
+// with every bf16 x bf16 product exact in the fp32 accumulator; only the accumulation order
+// differs from a scalar fp32 loop.  (A single TF32 pass would round W_r to 10 bits and is not used.)
+// The three pieces are produced once per bg_moe_set_weights by split_wr_kernel.
+//
+// Kernel: one CTA per (128-token tile, k-split).  tcgen05.mma kind::f16, M=128, N=round_up(E,16),
+// A = hidden [T,d] (K-major, TMA box {64 k,128 rows}), B = pieces [3,d,E_ld] (MN-major, TMA boxes
+// {64 n, 64 k, 1}); the pipeline iterates over (k-block, piece).  Split-K keeps the SMs busy when
+// T/128 < #SMs: CTA (m, s) writes its fp32 partial tile to partial[s][T][E]; the top-k kernel adds
+// the partials in ascending s (a fixed order => bitwise deterministic logits) plus the bias.
+#include "kernels.h"
+#include "ptx_sm100.cuh"
+
+namespace bg {
+namespace {
+
+constexpr int BM = 128, BK = 64, UK = 16, STAGES = 4;
+constexpr int A_BYTES = BM * BK * 2;             // 16 KB
+constexpr int B_BLK_BYTES = 64 * BK * 2;         // 8 KB per 64 experts
+constexpr int B_BYTES = 4 * B_BLK_BYTES;         // up to 256 experts
+constexpr int STAGE_BYTES = A_BYTES + B_BYTES;   // 48 KB
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 + 256;
+constexpr int NUM_THREADS = 256;                 // warp 0 TMA, warp 1 MMA, warp 2 TMEM alloc, warps 4-7 epilogue
+
+constexpr uint64_t ADESC_HI = umma_desc_sw128(16, 1024);
+constexpr uint64_t BDESC_HI = umma_desc_sw128(B_BLK_BYTES, 1024);
+
+// pieces: [3][d][E_ld] bf16, E_ld = round_up(E,16), zero padded (TMA needs 16-byte row strides).
+__global__ void split_wr_kernel(const float* __restrict__ W_r, int d, int E, int E_ld,
+                                __nv_bfloat16* __restrict__ pieces) {
+  const int64_t n = static_cast<int64_t>(d) * E_ld;
+  const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int j = static_cast<int>(i / E_ld), e = static_cast<int>(i - static_cast<int64_t>(j) * E_ld);
+  const float w = (e < E) ? W_r[static_cast<int64_t>(j) * E + e] : 0.0f;
+  const __nv_bfloat16 hi = __float2bfloat16_rn(w);
+  const float r1 = w - __bfloat162float(hi);                 // exact
+  const __nv_bfloat16 mid = __float2bfloat16_rn(r1);
+  const float r2 = r1 - __bfloat162float(mid);               // exact
+  const __nv_bfloat16 lo = __float2bfloat16_rn(r2);          // exact: <= 8 significant bits remain
+  pieces[i] = hi;
+  pieces[n + i] = mid;
+  pieces[2 * n + i] = lo;
+}
+
+__global__ void __launch_bounds__(NUM_THREADS, 1)
+router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_constant__ CUtensorMap tm_w, int T, int d,
+                   int E, int ksplit, float* __restrict__ partial, int32_t* __restrict__ zero_buf, int zero_n) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t raw = smem_u32(smem_raw);
+  const uint32_t base = (raw + 1023u) & ~1023u;
+  uint8_t* smem = smem_raw + (base - raw);
+  const uint32_t bar_base = base + STAGES * STAGE_BYTES;
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+  const uint32_t done_bar = bar_base + 8u * (2 * STAGES);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + STAGES * STAGE_BYTES + 8 * (2 * STAGES + 1));
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int m_tile = blockIdx.x, ks = blockIdx.y;
+  {  // zero the per-block expert histogram that the top-k kernel (next in the stream) accumulates into
+    const int n_cta = gridDim.x * gridDim.y, cta = blockIdx.y * gridDim.x + blockIdx.x;
+    const int per = (zero_n + n_cta - 1) / n_cta;
+    const int z0 = cta * per, z1 = min(zero_n, z0 + per);
+    for (int i = z0 + threadIdx.x; i < z1; i += NUM_THREADS) zero_buf[i] = 0;
+  }
+  const int k_blocks = (d + BK - 1) / BK;
+  const int kb_per = (k_blocks + ksplit - 1) / ksplit;
+  const int kb0 = ks * kb_per, kb1 = min(k_blocks, kb0 + kb_per);
+  const int n_iter = max(0, kb1 - kb0) * 3;                  // (k-block, piece) pairs
+  const int n_mma = (E + 15) & ~15;                          // UMMA N (multiple of 16 for M=128)
+  const int n_blk = (E + 63) / 64;                           // 64-expert TMA boxes
+  const uint32_t idesc = umma_idesc_bf16(BM, n_mma, 0, 1);
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tm_h);
+    tma_prefetch_desc(&tm_w);
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    mbar_init(done_bar, 1);
+    fence_barrier_init();
+  }
+  if (warp == 2) { tmem_alloc(smem_u32(tmem_slot), 256); tmem_relinquish(); }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    if (lane == 0) {                              // ---- TMA producer
+      const uint32_t stage_tx = A_BYTES + n_blk * B_BLK_BYTES;
+      for (int it = 0; it < n_iter; ++it) {
+        const int s = it % STAGES;
+        const uint32_t ph = (it / STAGES) & 1u;
+        mbar_wait(empty_bar(s), ph ^ 1u);
+        const int kb = kb0 + it / 3, piece = it % 3;
+        const uint32_t sa = base + s * STAGE_BYTES, sb = sa + A_BYTES;
+        mbar_expect_tx(full_bar(s), stage_tx);
+        tma_load_2d(sa, &tm_h, full_bar(s), kb * BK, m_tile * BM);
+        for (int j = 0; j < n_blk; ++j) tma_load_3d(sb + j * B_BLK_BYTES, &tm_w, full_bar(s), 64 * j, kb * BK, piece);
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {                              // ---- MMA issuer
+      for (int it = 0; it < n_iter; ++it) {
+        const int s = it % STAGES;
+        const uint32_t ph = (it / STAGES) & 1u;
+        mbar_wait(full_bar(s), ph);
+        tc_fence_after();
+        const uint32_t sa = base + s * STAGE_BYTES, sb = sa + A_BYTES;
+        const uint64_t ad = ADESC_HI | ((sa >> 4) & 0x3FFFu);
+        const uint64_t bd = BDESC_HI | ((sb >> 4) & 0x3FFFu);
+        #pragma unroll
+        for (int kk = 0; kk < BK / UK; ++kk)
+          umma_f16(tmem_base, ad + ((kk * UK * 2) >> 4), bd + ((kk * UK * 128) >> 4), idesc, (it | kk) != 0 ? 1u : 0u);
+        umma_commit(empty_bar(s));
+      }
+      umma_commit(done_bar);
+    }
+  } else if (warp >= 4) {
+    const int q = warp & 3;                       // TMEM lane quarter of this warp
+    const int row = m_tile * BM + q * 32 + lane;
+    float* dst = partial + (static_cast<int64_t>(ks) * T + row) * E;
+    if (n_iter == 0) {
+      if (row < T) for (int e = 0; e < E; ++e) dst[e] = 0.0f;
+    } else {
+      mbar_wait(done_bar, 0);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16);
+      for (int c0 = 0; c0 < n_mma; c0 += 32) {
+        uint32_t v[32];
+        tmem_ld_32x32(taddr + c0, v);             // columns past n_mma are never used below
+        tmem_ld_wait();
+        if (row < T) {
+          if ((E & 3) == 0) {
+            #pragma unroll
+            for (int j = 0; j < 32; j += 4)
+              if (c0 + j + 4 <= E)
+                *reinterpret_cast<float4*>(dst + c0 + j) =
+                    make_float4(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), __uint_as_float(v[j + 2]),
+                                __uint_as_float(v[j + 3]));
+          } else {
+            #pragma unroll
+            for (int j = 0; j < 32; ++j)
+              if (c0 + j < E) dst[c0 + j] = __uint_as_float(v[j]);
+          }
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) { tc_fence_after(); tmem_dealloc(tmem_base, 256); }
+}
+
+}  // namespace
+
+cudaError_t router_kernels_init() {
+  return cudaFuncSetAttribute(router_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+}
+
+cudaError_t launch_split_wr(const float* W_r, int d, int E, void* pieces, cudaStream_t st) {
+  const int E_ld = (E + 15) & ~15;
+  const int64_t n = static_cast<int64_t>(d) * E_ld;
+  split_wr_kernel<<<static_cast<unsigned>((n + 255) / 256), 256, 0, st>>>(W_r, d, E, E_ld,
+                                                                          static_cast<__nv_bfloat16*>(pieces));
+  return cudaGetLastError();
+}
+
+int router_ksplit(int T, int d, int num_sms) {
+  const int m_tiles = (T + BM - 1) / BM;
+  const int k_blocks = (d + BK - 1) / BK;
+  int ks = num_sms / (m_tiles > 0 ? m_tiles : 1);
+  if (ks > 8) ks = 8;
+  if (ks > k_blocks) ks = k_blocks;
+  if (ks < 1) ks = 1;
+  return ks;
+}
+
+cudaError_t launch_router_gemm(const CUtensorMap& tm_h, const CUtensorMap& tm_w, int T, int d, int E, int ksplit,
+                               float* partial, int32_t* zero_buf, int zero_n, cudaStream_t st) {
+  if (T == 0) return cudaSuccess;
+  dim3 grid((T + BM - 1) / BM, ksplit);
+  router_gemm_kernel<<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tm_h, tm_w, T, d, E, ksplit, partial, zero_buf, zero_n);
+  return cudaGetLastError();
+}
+
+}  // namespace bg

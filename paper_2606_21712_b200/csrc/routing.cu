@@ -1,5 +1,6 @@
 // routing.cu -- steps a1-a5 of the combined MoE layer:
-//   a1 router logits  L[t,e] = sum_j float(hidden[t,j]) * W_r[j,e] (+ b_r[e])      fp32 FMA
+//   a1 (tail)         L[t,e] = sum_s partial[s][t][e] (+ b_r[e]): the split-K partials of
+//                     router_gemm.cu added in ascending s (fixed order => deterministic logits)
 //   a2 top-k          k passes of a warp arg-max under (logit desc, expert index asc);
 //                     gates = softmax over the k selected logits
 //   a3 histogram      per-block shared-memory counts (integer atomics: order-independent)
@@ -16,156 +17,102 @@ namespace bg {
 namespace {
 
 constexpr int MAX_E = 256;
-constexpr int MAX_K = 8;
-
-// ------------------------------------------------------------------ a1 router logits
-// Block: 32 tokens x all E experts, 256 threads.  Warp w owns tokens 4w..4w+3; lane l owns experts
-// l, l+32, ... (NE = ceil(E/32) of them).  k is consumed in chunks of 32 staged in shared memory.
-constexpr int RT_TOK = 32;
-constexpr int RT_KC = 32;
-
-template <int NE>
-__global__ void __launch_bounds__(256) router_logits_kernel(const __nv_bfloat16* __restrict__ hidden,
-                                                            const float* __restrict__ W_r,
-                                                            const float* __restrict__ b_r, int T, int d, int E,
-                                                            float* __restrict__ logits) {
-  __shared__ float hs[RT_TOK][RT_KC + 1];
-  __shared__ float ws[RT_KC][NE * 32];
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int t0 = blockIdx.x * RT_TOK;
-  float acc[4][NE];
-  #pragma unroll
-  for (int i = 0; i < 4; ++i)
-    #pragma unroll
-    for (int j = 0; j < NE; ++j) acc[i][j] = 0.0f;
-
-  for (int k0 = 0; k0 < d; k0 += RT_KC) {
-    // hidden chunk: 32 tokens x 32 k; thread -> (token = tid/8, 4 consecutive k)
-    {
-      const int tt = threadIdx.x >> 3, kk = (threadIdx.x & 7) * 4;
-      const int t = t0 + tt;
-      float v[4] = {0.f, 0.f, 0.f, 0.f};
-      if (t < T) {
-        #pragma unroll
-        for (int i = 0; i < 4; ++i)
-          if (k0 + kk + i < d) v[i] = __bfloat162float(hidden[static_cast<int64_t>(t) * d + k0 + kk + i]);
-      }
-      #pragma unroll
-      for (int i = 0; i < 4; ++i) hs[tt][kk + i] = v[i];
-    }
-    // W_r chunk: 32 k x E
-    for (int idx = threadIdx.x; idx < RT_KC * NE * 32; idx += 256) {
-      const int kk = idx / (NE * 32), e = idx - kk * (NE * 32);
-      ws[kk][e] = (e < E && k0 + kk < d) ? __ldg(W_r + static_cast<int64_t>(k0 + kk) * E + e) : 0.0f;
-    }
-    __syncthreads();
-    #pragma unroll 8
-    for (int kk = 0; kk < RT_KC; ++kk) {
-      float h[4], w[NE];
-      #pragma unroll
-      for (int i = 0; i < 4; ++i) h[i] = hs[warp * 4 + i][kk];
-      #pragma unroll
-      for (int j = 0; j < NE; ++j) w[j] = ws[kk][lane + 32 * j];
-      #pragma unroll
-      for (int i = 0; i < 4; ++i)
-        #pragma unroll
-        for (int j = 0; j < NE; ++j) acc[i][j] = fmaf(h[i], w[j], acc[i][j]);
-    }
-    __syncthreads();
-  }
-  #pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int t = t0 + warp * 4 + i;
-    if (t >= T) continue;
-    #pragma unroll
-    for (int j = 0; j < NE; ++j) {
-      const int e = lane + 32 * j;
-      if (e < E) logits[static_cast<int64_t>(t) * E + e] = acc[i][j] + (b_r ? __ldg(b_r + e) : 0.0f);
-    }
-  }
-}
 
 // ------------------------------------------------------------------ a2 + a3
-// (value, index) order of reading S3: a beats b <=> va > vb or (va == vb and ia < ib).
-// An index < 0 marks "no candidate" and loses to everything.
-__device__ __forceinline__ bool beats(float va, int ia, float vb, int ib) {
-  if (ia < 0) return false;
-  if (ib < 0) return true;
-  return (va > vb) || (va == vb && ia < ib);
+// One warp per token.  (logit, expert) is packed into one 64-bit key whose unsigned order IS the
+// order of reading S3: larger logit first, equal logits -> lower expert index first
+// (-0.0 == +0.0: both map to the same key half).  Lane l holds the keys of experts l, l+32, ...
+constexpr int RB = 1024;     // flat (token,slot) entries owned by one block of the rank kernel
+
+__device__ __forceinline__ uint32_t float_to_ordered(float f) {
+  f = f + 0.0f;                                    // canonicalise -0.0 to +0.0 (they tie)
+  const uint32_t u = __float_as_uint(f);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float ordered_to_float(uint32_t o) {
+  return __uint_as_float((o & 0x80000000u) ? (o ^ 0x80000000u) : ~o);
 }
 
+// src: fp32 [n_src][T][E]: n_src >= 1 slabs added in ascending order (n_src = 1: plain logits),
+// plus b_r.  logits_out (never aliases src) receives the summed logits.  block_counts [nblk][E]
+// must be zero on entry; it receives the histogram of each rank block (integer RED: the result
+// does not depend on arrival order).
 template <int NE>
-__global__ void __launch_bounds__(256) topk_hist_kernel(const float* __restrict__ logits, int T, int E, int k,
+__global__ void __launch_bounds__(256) topk_hist_kernel(const float* __restrict__ src, int n_src,
+                                                        const float* __restrict__ b_r,
+                                                        float* __restrict__ logits_out, int T, int E, int k,
                                                         int tokens_per_block, int32_t* __restrict__ topk_idx,
                                                         float* __restrict__ topk_w,
                                                         int32_t* __restrict__ block_counts) {
-  __shared__ int hist[MAX_E];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  for (int e = threadIdx.x; e < E; e += 256) hist[e] = 0;
-  __syncthreads();
-  const int t_begin = blockIdx.x * tokens_per_block;
-  const int t_end = min(T, t_begin + tokens_per_block);
-  for (int t = t_begin + warp; t < t_end; t += 8) {
-    float v[NE];
-    bool taken[NE];
+  const int t = blockIdx.x * 8 + warp;
+  if (t >= T) return;
+  const int64_t slab = static_cast<int64_t>(T) * E;
+  // Sum of the n_src slabs in ascending order (+ bias); loads are issued SB slabs at a time so
+  // their latencies overlap while the additions stay in slab order (deterministic logits).
+  constexpr int SB = (NE <= 4) ? 4 : 2;
+  float v[NE];
+  {
+    const float* p = src + static_cast<int64_t>(t) * E + lane;
     #pragma unroll
-    for (int j = 0; j < NE; ++j) {
-      const int e = lane + 32 * j;
-      v[j] = (e < E) ? __ldg(logits + static_cast<int64_t>(t) * E + e) : 0.0f;
-      taken[j] = !(e < E);
-    }
-    float sel_v[MAX_K];
-    int sel_i[MAX_K];
-    #pragma unroll
-    for (int s = 0; s < MAX_K; ++s) {
-      sel_v[s] = 0.0f;
-      sel_i[s] = 0;
-      if (s < k) {
-        float bv = 0.0f;
-        int bi = -1;
+    for (int j = 0; j < NE; ++j) v[j] = (lane + 32 * j < E) ? __ldg(p + 32 * j) : 0.0f;
+    for (int s = 1; s < n_src; s += SB) {
+      float a[SB][NE];
+      #pragma unroll
+      for (int u = 0; u < SB; ++u)
         #pragma unroll
         for (int j = 0; j < NE; ++j)
-          if (!taken[j] && beats(v[j], lane + 32 * j, bv, bi)) { bv = v[j]; bi = lane + 32 * j; }
-        #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-          const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
-          const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-          if (beats(ov, oi, bv, bi)) { bv = ov; bi = oi; }
-        }
-        // every lane now holds the same winner
+          a[u][j] = (s + u < n_src && lane + 32 * j < E) ? __ldg(p + (s + u) * slab + 32 * j) : 0.0f;
+      #pragma unroll
+      for (int u = 0; u < SB; ++u)
         #pragma unroll
         for (int j = 0; j < NE; ++j)
-          if (bi == lane + 32 * j) taken[j] = true;
-        sel_v[s] = bv;
-        sel_i[s] = bi;
-      }
-    }
-    // gates: softmax over the k selected logits, slot 0 holds the maximum (reading S2)
-    float ex[MAX_K], denom = 0.0f;
-    #pragma unroll
-    for (int s = 0; s < MAX_K; ++s) {
-      ex[s] = (s < k) ? expf(sel_v[s] - sel_v[0]) : 0.0f;
-      denom += ex[s];
-    }
-    #pragma unroll
-    for (int s = 0; s < MAX_K; ++s) {
-      if (s < k && lane == s) {
-        topk_idx[static_cast<int64_t>(t) * k + s] = sel_i[s];
-        topk_w[static_cast<int64_t>(t) * k + s] = ex[s] / denom;
-        atomicAdd(&hist[sel_i[s]], 1);
-      }
+          if (s + u < n_src) v[j] += a[u][j];
     }
   }
-  __syncthreads();
-  for (int e = threadIdx.x; e < E; e += 256) block_counts[static_cast<int64_t>(blockIdx.x) * E + e] = hist[e];
+  unsigned long long key[NE];
+  #pragma unroll
+  for (int j = 0; j < NE; ++j) {
+    const int e = lane + 32 * j;
+    key[j] = 0ull;                                  // 0 = "no candidate": below every real key
+    if (e < E) {
+      if (b_r) v[j] += __ldg(b_r + e);
+      if (logits_out) logits_out[static_cast<int64_t>(t) * E + e] = v[j];
+      key[j] = (static_cast<unsigned long long>(float_to_ordered(v[j])) << 32) | (0xFFFFFFFFu - static_cast<uint32_t>(e));
+    }
+  }
+  int my_e = 0;
+  float my_v = 0.0f, v_max = 0.0f;
+  for (int s = 0; s < k; ++s) {
+    unsigned long long best = key[0];
+    #pragma unroll
+    for (int j = 1; j < NE; ++j) best = max(best, key[j]);
+    #pragma unroll
+    for (int o = 16; o > 0; o >>= 1) best = max(best, __shfl_xor_sync(0xffffffffu, best, o));
+    #pragma unroll
+    for (int j = 0; j < NE; ++j)
+      if (key[j] == best) key[j] = 0ull;            // taken
+    const float val = ordered_to_float(static_cast<uint32_t>(best >> 32));
+    if (s == 0) v_max = val;
+    if (lane == s) { my_e = static_cast<int>(0xFFFFFFFFu - static_cast<uint32_t>(best)); my_v = val; }
+  }
+  // gates: softmax over the k selected logits; slot 0 holds the maximum (reading S2)
+  const float ex = (lane < k) ? expf(my_v - v_max) : 0.0f;
+  float denom = 0.0f;
+  for (int s = 0; s < k; ++s) denom += __shfl_sync(0xffffffffu, ex, s);     // slot order
+  if (lane < k) {
+    topk_idx[static_cast<int64_t>(t) * k + lane] = my_e;
+    topk_w[static_cast<int64_t>(t) * k + lane] = ex / denom;
+    atomicAdd(block_counts + static_cast<int64_t>(t / tokens_per_block) * E + my_e, 1);
+  }
 }
 
 // Recount per-block histograms from topk_idx (split API: bg_moe_permute gets only idx + offsets).
-__global__ void __launch_bounds__(256) block_hist_kernel(const int32_t* __restrict__ topk_idx, int T, int E, int k,
+__global__ void __launch_bounds__(RB) block_hist_kernel(const int32_t* __restrict__ topk_idx, int T, int E, int k,
                                                          int tokens_per_block,
                                                          int32_t* __restrict__ block_counts) {
   __shared__ int hist[MAX_E];
-  for (int e = threadIdx.x; e < E; e += 256) hist[e] = 0;
+  for (int e = threadIdx.x; e < E; e += RB) hist[e] = 0;
   __syncthreads();
   const int64_t i0 = static_cast<int64_t>(blockIdx.x) * tokens_per_block * k;
   const int64_t n = min(static_cast<int64_t>(tokens_per_block) * k, static_cast<int64_t>(T) * k - i0);
@@ -174,43 +121,58 @@ __global__ void __launch_bounds__(256) block_hist_kernel(const int32_t* __restri
     if (e >= 0 && e < E) atomicAdd(&hist[e], 1);
   }
   __syncthreads();
-  for (int e = threadIdx.x; e < E; e += 256) block_counts[static_cast<int64_t>(blockIdx.x) * E + e] = hist[e];
+  for (int e = threadIdx.x; e < E; e += RB) block_counts[static_cast<int64_t>(blockIdx.x) * E + e] = hist[e];
 }
 
-// ------------------------------------------------------------------ a4 scans (one block of 256)
+// ------------------------------------------------------------------ a4 scans (one block of 1024)
 // counts[e] = sum_b block_counts[b][e]; offsets = exclusive scan over e; then
 // block_base[b][e] = offsets[e] + sum_{b'<b} block_counts[b'][e]   (first row of block b in expert e)
-__global__ void __launch_bounds__(256) scan_kernel(const int32_t* __restrict__ block_counts, int nblk, int E,
-                                                   int32_t* __restrict__ block_base,
-                                                   int32_t* __restrict__ counts, int32_t* __restrict__ offsets) {
+// Thread (g, e): expert e = tid % 256, block group g = tid / 256 owns blocks [g*per, (g+1)*per).
+__global__ void __launch_bounds__(1024) scan_kernel(const int32_t* __restrict__ block_counts, int nblk, int E,
+                                                    int32_t* __restrict__ block_base,
+                                                    int32_t* __restrict__ counts, int32_t* __restrict__ offsets) {
+  __shared__ int gtot[4][MAX_E];
+  __shared__ int excl_e[MAX_E];
   __shared__ int warp_tot[8];
-  const int e = threadIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  int total = 0;
+  const int e = threadIdx.x & 255, g = threadIdx.x >> 8;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int per = (nblk + 3) / 4;
+  const int b0 = min(nblk, g * per), b1 = min(nblk, b0 + per);
+  int part = 0;
   if (e < E) {
     #pragma unroll 8
-    for (int b = 0; b < nblk; ++b) total += __ldg(block_counts + static_cast<int64_t>(b) * E + e);
+    for (int b = b0; b < b1; ++b) part += __ldg(block_counts + static_cast<int64_t>(b) * E + e);
   }
-  int v = total;
-  #pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const int u = __shfl_up_sync(0xffffffffu, v, o);
-    if (lane >= o) v += u;
-  }
-  if (lane == 31) warp_tot[warp] = v;
+  gtot[g][e] = part;
   __syncthreads();
-  int add = 0;
-  for (int w = 0; w < warp; ++w) add += warp_tot[w];
-  const int incl = v + add;
-  const int excl = incl - total;
-  if (e < E) {
-    if (counts) counts[e] = total;
-    if (offsets) {
-      offsets[e] = excl;
-      if (e == E - 1) offsets[E] = incl;
+  if (g == 0) {
+    const int total = gtot[0][e] + gtot[1][e] + gtot[2][e] + gtot[3][e];
+    int v = total;
+    #pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int u = __shfl_up_sync(0xffffffffu, v, o);
+      if (lane >= o) v += u;
     }
-    int run = excl;
+    if (lane == 31) warp_tot[warp] = v;
+    asm volatile("bar.sync 1, 256;" ::: "memory");      // only the 256 threads of group 0
+    int add = 0;
+    for (int w = 0; w < warp; ++w) add += warp_tot[w];
+    const int incl = v + add, excl = incl - total;
+    excl_e[e] = excl;
+    if (e < E) {
+      if (counts) counts[e] = total;
+      if (offsets) {
+        offsets[e] = excl;
+        if (e == E - 1) offsets[E] = incl;
+      }
+    }
+  }
+  __syncthreads();
+  if (e < E) {
+    int run = excl_e[e];
+    for (int gg = 0; gg < g; ++gg) run += gtot[gg][e];
     #pragma unroll 8
-    for (int b = 0; b < nblk; ++b) {
+    for (int b = b0; b < b1; ++b) {
       const int64_t at = static_cast<int64_t>(b) * E + e;
       block_base[at] = run;
       run += __ldg(block_counts + at);
@@ -222,13 +184,13 @@ __global__ void __launch_bounds__(256) scan_kernel(const int32_t* __restrict__ b
 // One thread per flat entry of the block.  Entries of a block are in flat-index order, so the
 // rank of entry j inside its expert is (#lower warps' entries with the same expert) + (#lower
 // lanes of this warp with the same expert): independent of any arrival order.
-__global__ void __launch_bounds__(256) rank_kernel(const int32_t* __restrict__ topk_idx,
+__global__ void __launch_bounds__(RB) rank_kernel(const int32_t* __restrict__ topk_idx,
                                                    const int32_t* __restrict__ block_base, int T, int E, int k,
                                                    int tokens_per_block, int32_t* __restrict__ row_src,
                                                    int32_t* __restrict__ inv_perm) {
-  __shared__ int wcnt[8][MAX_E];
+  __shared__ int wcnt[RB / 32][MAX_E];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  for (int i = threadIdx.x; i < 8 * MAX_E; i += 256) (&wcnt[0][0])[i] = 0;
+  for (int i = threadIdx.x; i < (RB / 32) * MAX_E; i += RB) (&wcnt[0][0])[i] = 0;
   __syncthreads();
   const int64_t i0 = static_cast<int64_t>(blockIdx.x) * tokens_per_block * k;
   const int64_t n = min(static_cast<int64_t>(tokens_per_block) * k, static_cast<int64_t>(T) * k - i0);
@@ -252,54 +214,42 @@ __global__ void __launch_bounds__(256) rank_kernel(const int32_t* __restrict__ t
 
 }  // namespace
 
-cudaError_t launch_router_logits(const void* hidden, const float* W_r, const float* b_r, int T, int d, int E,
-                                 float* logits, cudaStream_t st) {
+cudaError_t launch_topk_hist(const float* src, int n_src, const float* b_r, float* logits_out, int T, int E, int k,
+                             int32_t* topk_idx, float* topk_w, int32_t* block_counts, cudaStream_t st) {
   if (T == 0) return cudaSuccess;
-  const __nv_bfloat16* h = static_cast<const __nv_bfloat16*>(hidden);
-  const int grid = (T + RT_TOK - 1) / RT_TOK;
+  const int tb = route_tokens_per_block(k);
   const int ne = (E + 31) / 32;
+#define BG_TOPK(NE_) topk_hist_kernel<NE_><<<(T + 7) / 8, 256, 0, st>>>(src, n_src, b_r, logits_out, T, E, k, tb, \
+                                                                       topk_idx, topk_w, block_counts)
   switch (ne) {
-    case 1: router_logits_kernel<1><<<grid, 256, 0, st>>>(h, W_r, b_r, T, d, E, logits); break;
-    case 2: router_logits_kernel<2><<<grid, 256, 0, st>>>(h, W_r, b_r, T, d, E, logits); break;
-    case 3: case 4: router_logits_kernel<4><<<grid, 256, 0, st>>>(h, W_r, b_r, T, d, E, logits); break;
-    default: router_logits_kernel<8><<<grid, 256, 0, st>>>(h, W_r, b_r, T, d, E, logits); break;
+    case 1: BG_TOPK(1); break;
+    case 2: BG_TOPK(2); break;
+    case 3: case 4: BG_TOPK(4); break;
+    default: BG_TOPK(8); break;
   }
-  return cudaGetLastError();
-}
-
-cudaError_t launch_topk_hist(const float* logits, int T, int E, int k, int32_t* topk_idx, float* topk_w,
-                             int32_t* block_counts, cudaStream_t st) {
-  if (T == 0) return cudaSuccess;
-  const int tb = route_tokens_per_block(k), grid = route_num_blocks(T, k);
-  const int ne = (E + 31) / 32;
-  switch (ne) {
-    case 1: topk_hist_kernel<1><<<grid, 256, 0, st>>>(logits, T, E, k, tb, topk_idx, topk_w, block_counts); break;
-    case 2: topk_hist_kernel<2><<<grid, 256, 0, st>>>(logits, T, E, k, tb, topk_idx, topk_w, block_counts); break;
-    case 3: case 4: topk_hist_kernel<4><<<grid, 256, 0, st>>>(logits, T, E, k, tb, topk_idx, topk_w, block_counts); break;
-    default: topk_hist_kernel<8><<<grid, 256, 0, st>>>(logits, T, E, k, tb, topk_idx, topk_w, block_counts); break;
-  }
+#undef BG_TOPK
   return cudaGetLastError();
 }
 
 cudaError_t launch_block_hist(const int32_t* topk_idx, int T, int E, int k, int32_t* block_counts,
                               cudaStream_t st) {
   if (T == 0) return cudaSuccess;
-  block_hist_kernel<<<route_num_blocks(T, k), 256, 0, st>>>(topk_idx, T, E, k, route_tokens_per_block(k),
-                                                             block_counts);
+  block_hist_kernel<<<route_num_blocks(T, k), RB, 0, st>>>(topk_idx, T, E, k, route_tokens_per_block(k),
+                                                            block_counts);
   return cudaGetLastError();
 }
 
 cudaError_t launch_scan(const int32_t* block_counts, int nblk, int E, int32_t* block_base, int32_t* counts,
                         int32_t* offsets, cudaStream_t st) {
-  scan_kernel<<<1, 256, 0, st>>>(block_counts, nblk, E, block_base, counts, offsets);
+  scan_kernel<<<1, 1024, 0, st>>>(block_counts, nblk, E, block_base, counts, offsets);
   return cudaGetLastError();
 }
 
 cudaError_t launch_rank(const int32_t* topk_idx, const int32_t* block_base, int T, int E, int k,
                         int32_t* row_src, int32_t* inv_perm, cudaStream_t st) {
   if (T == 0) return cudaSuccess;
-  rank_kernel<<<route_num_blocks(T, k), 256, 0, st>>>(topk_idx, block_base, T, E, k, route_tokens_per_block(k),
-                                                       row_src, inv_perm);
+  rank_kernel<<<route_num_blocks(T, k), RB, 0, st>>>(topk_idx, block_base, T, E, k, route_tokens_per_block(k),
+                                                      row_src, inv_perm);
   return cudaGetLastError();
 }
 
