@@ -14,6 +14,10 @@
 // For a7 the 256 accumulator columns are [gate n0..n0+128 | up n0..n0+128] so that SiLU(g)*u is
 // an epilogue over one thread's registers; for a8 they are 256 consecutive output columns.
 //
+// Fused gather (a6 inside a7, the fused chain only): instead of TMA-loading rows of a materialised
+// x_perm, four extra warps copy the tile's rows straight from hidden[row_src[r]/k, :] with 16-byte
+// cp.async into the same 128B-swizzled layout TMA would have produced; x_perm is never written.
+//
 // Tile scheduler: M-tiles never straddle experts.  Expert e owns ceil(n_e/128) M-tiles; its tiles
 // are ordered n-tile-major / m-tile-minor so that the CTAs running at the same time share one
 // weight strip through L2.  Tile t -> CTA (t mod gridDim.x).  Experts with no rows own no tiles
@@ -35,6 +39,7 @@ constexpr int B_BLK_BYTES = 64 * BK * 2;      // 8 KB: one 64-column block of B
 constexpr int B_BYTES = (BN / 64) * B_BLK_BYTES;   // 32 KB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;     // 48 KB
 constexpr int NUM_THREADS = 256;   // warp 0 TMA, warp 1 MMA, warp 2 TMEM alloc, warps 4-7 epilogue
+constexpr int GATHER_THREADS = 128;   // warps 8-11 of the fused-gather variant
 constexpr int MAX_E = 256;
 // Epilogue staging: each epilogue warp transposes 32 rows x 64 bf16 columns through its own
 // padded shared-memory buffer (row pitch 144 B: conflict-free 16-byte accesses) so that global
@@ -57,7 +62,17 @@ struct Params {
   __nv_bfloat16* out;
   const float* row_scale;
   const int32_t* row_src;
+  const uint8_t* gather_src;   // hidden (bf16 [T,K]) when the A rows are gathered in-kernel
+  int k;
 };
+
+__device__ __forceinline__ void cp_async_16(uint32_t dst, const void* src, uint32_t src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+// Arrive on `bar` (without raising its pending count) once all prior cp.async of this thread are done.
+__device__ __forceinline__ void cp_async_arrive_noinc(uint32_t bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
 
 struct TileCoord {
   int e, row0, rows_valid, n_tile;
@@ -99,9 +114,10 @@ __device__ __forceinline__ float silu_mul(float g, float u) {
 
 // GATEUP = true : a7 (B = [W_gate strip | W_up strip], SwiGLU epilogue, 128 output columns / tile)
 // GATEUP = false: a8 (B = W_down strip, optional row scale, 256 output columns / tile)
-template <bool GATEUP>
-__global__ void __launch_bounds__(NUM_THREADS, 1)
-grouped_gemm_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_b0,
+// GATHER (a7 only): A rows come from hidden through row_src (cp.async), not from x_perm by TMA
+template <bool GATEUP, bool GATHER>
+__global__ void __launch_bounds__(NUM_THREADS + (GATHER ? GATHER_THREADS : 0), 1)
+grouped_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__ CUtensorMap tm_b0,
                     const __grid_constant__ CUtensorMap tm_b1, const Params p) {
   constexpr int OUT_COLS = GATEUP ? BN / 2 : BN;     // output columns per tile
   extern __shared__ uint8_t smem_raw[];
@@ -140,21 +156,20 @@ grouped_gemm_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_const
       if (lane >= o) v += u;
     }
     __shared__ int warp_tot[NUM_THREADS / 32];
-    if (lane == 31) warp_tot[warp] = v;
+    if (lane == 31 && warp < NUM_THREADS / 32) warp_tot[warp] = v;
     __syncthreads();
     int add = 0;
-    for (int w = 0; w < warp; ++w) add += warp_tot[w];
+    for (int w = 0; w < warp && w < NUM_THREADS / 32; ++w) add += warp_tot[w];
     v += add;                                   // inclusive prefix for thread's expert
     if (threadIdx.x < E) tile_start[threadIdx.x + 1] = v;
     if (threadIdx.x == 0) tile_start[0] = 0;
   }
 
   if (warp == 0 && lane == 0) {
-    tma_prefetch_desc(&tm_a);
     tma_prefetch_desc(&tm_b0);
     if (GATEUP) tma_prefetch_desc(&tm_b1);
     for (int s = 0; s < STAGES; ++s) {
-      mbar_init(full_bar(s), 1);
+      mbar_init(full_bar(s), GATHER ? 1 + GATHER_THREADS : 1);   // TMA thread (+ every gather thread)
       mbar_init(empty_bar(s), 1);
     }
     for (int a = 0; a < 2; ++a) {
@@ -183,12 +198,17 @@ grouped_gemm_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_const
       for (int t = blockIdx.x; t < total_tiles; t += gridDim.x) {
         const TileCoord c = decode_tile(t, tile_start, m_tiles, p.offsets, E);
         const int n0 = c.n_tile * OUT_COLS;
+        // A rows: the smallest power-of-two box (>= 16 rows) that covers the tile's valid rows; the
+        // rest of the 128-row slot keeps stale rows, which only feed accumulator rows never stored
+        const int box = c.rows_valid <= 16 ? 16 : 1 << (32 - __clz(c.rows_valid - 1));
+        const CUtensorMap* tm_a = &tm_act.m[27 - __clz(box)];          // log2(box) - 4
+        const uint32_t tx = B_BYTES + (GATHER ? 0 : box * BK * 2);
         for (int kb = 0; kb < k_blocks; ++kb) {
           mbar_wait(empty_bar(s), ph ^ 1u);
           const uint32_t sa = base + s * STAGE_BYTES;
           const uint32_t sb = sa + A_BYTES;
-          mbar_expect_tx(full_bar(s), STAGE_BYTES);
-          tma_load_2d(sa, &tm_a, full_bar(s), kb * BK, c.row0);
+          mbar_expect_tx(full_bar(s), tx);
+          if (!GATHER) tma_load_2d(sa, tm_a, full_bar(s), kb * BK, c.row0);
           if (GATEUP) {
             tma_load_3d(sb + 0 * B_BLK_BYTES, &tm_b0, full_bar(s), n0, kb * BK, c.e);
             tma_load_3d(sb + 1 * B_BLK_BYTES, &tm_b0, full_bar(s), n0 + 64, kb * BK, c.e);
@@ -234,7 +254,7 @@ grouped_gemm_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_const
         umma_commit(tfull_bar(as));                   // accumulator complete -> epilogue
       }
     }
-  } else if (warp >= 4) {
+  } else if (warp >= 4 && warp < 8) {
     // ===================== epilogue: TMEM -> registers -> global =====================
     const int q = warp & 3;                            // TMEM lane quarter this warp may read
     int it = 0;
@@ -301,6 +321,45 @@ grouped_gemm_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_const
       tc_fence_before();
       mbar_arrive(tempty_bar(as));
     }
+  } else if (GATHER && warp >= 8) {
+    // ===================== fused gather (a6): hidden rows -> swizzled A slot, cp.async ============
+    // Eight consecutive lanes copy the eight 16-byte chunks of one row's 128-byte k-span (full
+    // sectors); a warp instruction covers 4 rows, the four warps 16 rows, 8 instructions the tile.
+    // Chunk c of row r lands at r*128 + ((c ^ (r & 7)) << 4): the 128B swizzle TMA applies.
+    // Completion is asynchronous: every thread attaches an arrival to the stage's full barrier
+    // (cp.async.mbarrier.arrive.noinc) that fires when its own copies have landed, so issue never
+    // waits for data (the same producer protocol as CUTLASS's sm100 cp.async mainloop).
+    const int gw = warp - 8, sub = lane >> 3, chunk = lane & 7;
+    const int r_in16 = gw * 4 + sub;                                  // row inside a 16-row round
+    const uint32_t dst0 = r_in16 * 128 + ((chunk ^ (r_in16 & 7)) << 4);
+    const int64_t row_bytes = static_cast<int64_t>(p.K) * 2;
+    int s = 0;
+    uint32_t ph = 0;
+    for (int t = blockIdx.x; t < total_tiles; t += gridDim.x) {
+      const TileCoord c = decode_tile(t, tile_start, m_tiles, p.offsets, E);
+      const uint8_t* src[8];
+      uint32_t ok = 0;
+      #pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int rr = j * 16 + r_in16;
+        int tok = 0;
+        if (rr < c.rows_valid) {
+          tok = __ldg(p.row_src + c.row0 + rr) / p.k;
+          ok |= 1u << j;
+        }
+        src[j] = p.gather_src + static_cast<int64_t>(tok) * row_bytes + chunk * 16;
+      }
+      for (int kb = 0; kb < k_blocks; ++kb) {
+        mbar_wait(empty_bar(s), ph ^ 1u);
+        const uint32_t sa = base + s * STAGE_BYTES + dst0;
+        const bool k_ok = kb * BK + chunk * 8 < p.K;                   // k past K must read as zero
+        #pragma unroll
+        for (int j = 0; j < 8; ++j)
+          cp_async_16(sa + j * 2048, src[j] + kb * (BK * 2), (k_ok && ((ok >> j) & 1u)) ? 16u : 0u);
+        cp_async_arrive_noinc(full_bar(s));                            // arrives once this thread's copies land
+        if (++s == STAGES) { s = 0; ph ^= 1u; }
+      }
+    }
   }
 
   tc_fence_before();
@@ -320,26 +379,36 @@ Params make_params(const GemmLaunch& g) {
   p.out = static_cast<__nv_bfloat16*>(g.out);
   p.row_scale = g.row_scale;
   p.row_src = g.row_src;
+  p.gather_src = static_cast<const uint8_t*>(g.gather_src);
+  p.k = g.k;
   return p;
 }
 
 }  // namespace
 
 cudaError_t gemm_kernels_init() {
-  cudaError_t e = cudaFuncSetAttribute(grouped_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       SMEM_BYTES);
+  cudaError_t e = cudaFuncSetAttribute(grouped_gemm_kernel<true, false>,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(grouped_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  e = cudaFuncSetAttribute(grouped_gemm_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(grouped_gemm_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               SMEM_BYTES);
 }
 
 cudaError_t launch_gateup_swiglu(const GemmLaunch& g, cudaStream_t st) {
-  grouped_gemm_kernel<true><<<g.num_sms, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_a, g.tm_b0, g.tm_b1, make_params(g));
+  if (g.gather_src != nullptr)
+    grouped_gemm_kernel<true, true><<<g.num_sms, NUM_THREADS + GATHER_THREADS, SMEM_BYTES, st>>>(
+        g.tm_act, g.tm_b0, g.tm_b1, make_params(g));
+  else
+    grouped_gemm_kernel<true, false><<<g.num_sms, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_act, g.tm_b0, g.tm_b1,
+                                                                                 make_params(g));
   return cudaGetLastError();
 }
 
 cudaError_t launch_down(const GemmLaunch& g, cudaStream_t st) {
-  grouped_gemm_kernel<false><<<g.num_sms, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_a, g.tm_b0, g.tm_b0, make_params(g));
+  grouped_gemm_kernel<false, false><<<g.num_sms, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_act, g.tm_b0, g.tm_b0,
+                                                                                  make_params(g));
   return cudaGetLastError();
 }
 
