@@ -8,7 +8,7 @@ from typing import Optional
 import torch
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libbg_moe.so")
+LIB_PATH = os.environ.get("BG_MOE_LIB") or os.path.join(HERE, "libbg_moe.so")
 
 BG_OK, BG_ERR_INVALID_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA, BG_ERR_NOMEM, BG_ERR_NO_WEIGHTS = 0, -1, -2, -3, -4, -5
 
