@@ -39,9 +39,6 @@ struct bg_moe_ctx {
   void* out_dev = nullptr;
   // weight tensor maps (encoded in set_weights)
   CUtensorMap tm_wg, tm_wu, tm_wd, tm_wr;
-  // activation tensor maps of the workspace x_perm / H (whole capacity: rows past T*k are never stored)
-  bg::ActMaps am_x, am_h;
-  bool fuse_gather = true;      // a6 inside a7 (BG_MOE_FUSE_GATHER=0 keeps the separate gather kernel)
   int64_t launches = 0;
   std::string last_error;
   // optional per-kernel timing of the fused chain
@@ -68,24 +65,17 @@ EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
-// [rows, K] bf16 row-major, box {64 k, box_rows rows}, 128B swizzle.
-bool encode_act_map(CUtensorMap* tm, const void* ptr, int64_t rows, int64_t K, int box_rows = 128) {
+// [rows, K] bf16 row-major, box {64 k, 128 rows}, 128B swizzle.
+bool encode_act_map(CUtensorMap* tm, const void* ptr, int64_t rows, int64_t K) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return false;
   cuuint64_t dims[2] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(rows)};
   cuuint64_t strides[1] = {static_cast<cuuint64_t>(K) * 2};
-  cuuint32_t box[2] = {64, static_cast<cuuint32_t>(box_rows)};
+  cuuint32_t box[2] = {64, 128};
   cuuint32_t estr[2] = {1, 1};
   return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
-// The five activation maps of the grouped GEMM (box rows 16, 32, 64, 128, 256).
-bool encode_act_maps(bg::ActMaps* am, const void* ptr, int64_t rows, int64_t K) {
-  for (int i = 0; i < 5; ++i)
-    if (!encode_act_map(&am->m[i], ptr, rows, K, 16 << i)) return false;
-  return true;
 }
 
 // [E, K, N] bf16 row-major (N contiguous), box {64 n, 64 k, 1 expert}, 128B swizzle.
@@ -170,39 +160,29 @@ int do_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits
   return BG_OK;
 }
 
-// x_perm == nullptr: fused gather, the gate/up GEMM reads its rows from `hidden` through row_src.
-int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const void* hidden, const int32_t* offsets, int32_t T, void* y,
+int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t T, void* y,
            const float* row_scale, const int32_t* row_src, cudaStream_t st, int mark_between = -1) {
   const bg_moe_config& c = ctx->cfg;
   const int64_t R = static_cast<int64_t>(T) * c.k;
   bg::GemmLaunch g1;
-  if (x_perm == nullptr || x_perm == ctx->x_perm) {
-    g1.tm_act = ctx->am_x;             // workspace maps, encoded once in bg_moe_create
-  } else if (!encode_act_maps(&g1.tm_act, x_perm, R, c.d)) {
-    ctx->last_error = "cuTensorMapEncodeTiled(x_perm) failed";
-    return BG_ERR_CUDA;
-  }
+  if (!encode_act_map(&g1.tm_a, x_perm, R, c.d)) { ctx->last_error = "cuTensorMapEncodeTiled(x_perm) failed"; return BG_ERR_CUDA; }
   g1.tm_b0 = ctx->tm_wg;
   g1.tm_b1 = ctx->tm_wu;
   g1.offsets = offsets;
   g1.E = c.E; g1.K = c.d; g1.N = c.f;
   g1.out = ctx->H;
-  g1.row_scale = nullptr;
-  g1.row_src = x_perm == nullptr ? row_src : nullptr;
-  g1.gather_src = x_perm == nullptr ? hidden : nullptr;
-  g1.k = c.k;
+  g1.row_scale = nullptr; g1.row_src = nullptr;
   g1.num_sms = ctx->num_sms;
   BG_LAUNCH(ctx, bg::launch_gateup_swiglu(g1, st), "gateup_swiglu");
   if (mark_between >= 0) mark(ctx, mark_between, st);
   bg::GemmLaunch g2;
-  g2.tm_act = ctx->am_h;
+  if (!encode_act_map(&g2.tm_a, ctx->H, R, c.f)) { ctx->last_error = "cuTensorMapEncodeTiled(H) failed"; return BG_ERR_CUDA; }
   g2.tm_b0 = ctx->tm_wd;
   g2.tm_b1 = ctx->tm_wd;
   g2.offsets = offsets;
   g2.E = c.E; g2.K = c.f; g2.N = c.d;
   g2.out = y;
   g2.row_scale = row_scale; g2.row_src = row_src;
-  g2.gather_src = nullptr; g2.k = c.k;
   g2.num_sms = ctx->num_sms;
   BG_LAUNCH(ctx, bg::launch_down(g2, st), "down");
   return BG_OK;
@@ -288,15 +268,6 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   ctx->Y = ctx->ws + o_y;
   ctx->hidden_dev = ctx->ws + o_hd;
   ctx->out_dev = ctx->ws + o_od;
-  if (!encode_act_maps(&ctx->am_x, ctx->x_perm, Rm, c.d) || !encode_act_maps(&ctx->am_h, ctx->H, Rm, c.f)) {
-    cudaFree(ctx->ws);
-    delete ctx;
-    return BG_ERR_CUDA;
-  }
-  {
-    const char* fg = std::getenv("BG_MOE_FUSE_GATHER");
-    if (fg != nullptr && fg[0] == '0') ctx->fuse_gather = false;
-  }
   *out = ctx;
   return BG_OK;
 }
@@ -394,7 +365,7 @@ int bg_moe_expert_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offset
   if (!x_perm || !offsets || !y_perm || !aligned16(x_perm) || !aligned16(y_perm)) return BG_ERR_INVALID_ARG;
   if (ctx->W_gate == nullptr) return BG_ERR_NO_WEIGHTS;
   DeviceGuard guard(ctx->cfg.device);
-  return do_ffn(ctx, x_perm, nullptr, offsets, T, y_perm, nullptr, nullptr, static_cast<cudaStream_t>(stream));
+  return do_ffn(ctx, x_perm, offsets, T, y_perm, nullptr, nullptr, static_cast<cudaStream_t>(stream));
 }
 
 int bg_moe_unpermute(bg_moe_ctx* ctx, const void* y_perm, const int32_t* inv_perm, const float* topk_w, int32_t T,
@@ -423,14 +394,9 @@ int bg_moe_combined_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void
   mark(ctx, 3, st);
   BG_LAUNCH(ctx, bg::launch_rank(ctx->topk_idx, ctx->block_base, T, c.E, c.k, ctx->row_src, ctx->inv_perm, st), "rank");
   mark(ctx, 4, st);
-  if (ctx->fuse_gather) {
-    mark(ctx, 5, st);   // a6 runs inside the gate/up GEMM: the "gather" stage has no kernel of its own
-    rc = do_ffn(ctx, nullptr, hidden, ctx->offsets, T, ctx->Y, ctx->topk_w, ctx->row_src, st, /*mark_between=*/6);
-  } else {
-    BG_LAUNCH(ctx, bg::launch_gather(hidden, ctx->row_src, T * c.k, c.k, c.d, ctx->x_perm, ctx->num_sms, st), "gather");
-    mark(ctx, 5, st);
-    rc = do_ffn(ctx, ctx->x_perm, nullptr, ctx->offsets, T, ctx->Y, ctx->topk_w, ctx->row_src, st, /*mark_between=*/6);
-  }
+  BG_LAUNCH(ctx, bg::launch_gather(hidden, ctx->row_src, T * c.k, c.k, c.d, ctx->x_perm, ctx->num_sms, st), "gather");
+  mark(ctx, 5, st);
+  rc = do_ffn(ctx, ctx->x_perm, ctx->offsets, T, ctx->Y, ctx->topk_w, ctx->row_src, st, /*mark_between=*/6);
   if (rc) return rc;
   mark(ctx, 7, st);
   BG_LAUNCH(ctx, bg::launch_unpermute(ctx->Y, ctx->inv_perm, nullptr, T, c.k, c.d, out, ctx->num_sms, st), "unpermute");

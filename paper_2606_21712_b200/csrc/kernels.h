@@ -48,24 +48,15 @@ cudaError_t launch_unpermute(const void* y_perm, const int32_t* inv_perm, const 
                              int d, void* out, int num_sms, cudaStream_t st);
 
 // ---- grouped GEMM (grouped_gemm.cu): steps a7 and a8
-// Activation tensor maps: the same [rows, K] bf16 matrix with TMA boxes of {64 k, 16 << i rows}.
-struct ActMaps {
-  CUtensorMap m[5];    // box rows 16, 32, 64, 128, 256
-};
 struct GemmLaunch {
-  ActMaps tm_act;      // activations [rows, K] bf16
+  CUtensorMap tm_a;    // activations [rows, K] bf16, box {64, 128}
   CUtensorMap tm_b0;   // weights [E, K, N] bf16, box {64, 64, 1}: W_gate (gate/up GEMM) or W_down
   CUtensorMap tm_b1;   // W_up (gate/up GEMM only)
   const int32_t* offsets;  // [E+1]
   int E, K, N;         // N = output columns (f for gate/up, d for down)
   void* out;           // bf16 [rows, N]
   const float* row_scale;   // down GEMM, fused path: topk_w flat [T*k] (else nullptr)
-  const int32_t* row_src;   // down GEMM, fused path: row -> flat index (gate weight lookup);
-                            // gate/up GEMM, fused path: row -> flat index (gather source, below)
-  // gate/up GEMM, fused path: when non-null the A rows are gathered straight from
-  // hidden[row_src[r] / k, :] (step a6 fused into a7's operand load); tm_act is then unused.
-  const void* gather_src;
-  int k;
+  const int32_t* row_src;   // down GEMM, fused path: row -> flat index
   int num_sms;
 };
 cudaError_t launch_gateup_swiglu(const GemmLaunch& g, cudaStream_t st);

@@ -185,7 +185,7 @@ def test_fused_forward_parity(cfg):
     n0 = layer.launch_count
     out = layer.combined_forward(g["hidden"])
     torch.cuda.synchronize()
-    assert layer.launch_count - n0 == 7          # router, topk, scan, rank, 2 GEMMs (gather fused), reduce
+    assert layer.launch_count - n0 == 8          # router, topk, scan, rank, gather, 2 GEMMs, reduce
     v = layer.debug_views(cfg.T)
     check_routing_against_oracle(v["logits"], v["idx"], v["w"], v["counts"], v["offsets"], v["row_src"],
                                  v["inv_perm"], cfg.E, cfg.k)
