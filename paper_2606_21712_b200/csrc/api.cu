@@ -39,6 +39,10 @@ struct bg_moe_ctx {
   void* out_dev = nullptr;
   // weight tensor maps (encoded in set_weights)
   CUtensorMap tm_wg, tm_wu, tm_wd, tm_wr;
+  CUtensorMap tm_wg4, tm_wu4, tm_wd4;   // 4-D block views (kernels.h GemmLaunch), valid when f % 64 == 0 / d % 64 == 0
+  // activation tensor maps of the workspace x_perm / H (whole capacity: rows past T*k are never stored)
+  bg::ActMaps am_x, am_h;
+  bool pair_gemm = true;        // CTA-pair grouped GEMM (BG_MOE_GEMM=tile selects the 1-CTA 128x256 kernel)
   int64_t launches = 0;
   std::string last_error;
   // optional per-kernel timing of the fused chain
@@ -65,15 +69,35 @@ EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
-// [rows, K] bf16 row-major, box {64 k, 128 rows}, 128B swizzle.
-bool encode_act_map(CUtensorMap* tm, const void* ptr, int64_t rows, int64_t K) {
+// [rows, K] bf16 row-major, box {64 k, box_rows rows}, 128B swizzle.
+bool encode_act_map(CUtensorMap* tm, const void* ptr, int64_t rows, int64_t K, int box_rows = 128) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return false;
   cuuint64_t dims[2] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(rows)};
   cuuint64_t strides[1] = {static_cast<cuuint64_t>(K) * 2};
-  cuuint32_t box[2] = {64, 128};
+  cuuint32_t box[2] = {64, static_cast<cuuint32_t>(box_rows)};
   cuuint32_t estr[2] = {1, 1};
   return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// The sixteen activation maps of the grouped GEMMs (box rows 8, 16, ..., 128).
+bool encode_act_maps(bg::ActMaps* am, const void* ptr, int64_t rows, int64_t K) {
+  for (int i = 0; i < 16; ++i)
+    if (!encode_act_map(&am->m[i], ptr, rows, K, 8 * (i + 1))) return false;
+  return true;
+}
+
+// [E, K, N] bf16 viewed as [E, N/64, K, 64] (N % 64 == 0), box {64 n, 64 k, nblk blocks, 1 expert}, 128B swizzle.
+bool encode_weight_map_4d(CUtensorMap* tm, const void* ptr, int64_t E, int64_t K, int64_t N, int nblk) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[4] = {64, static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(N / 64), static_cast<cuuint64_t>(E)};
+  cuuint64_t strides[3] = {static_cast<cuuint64_t>(N) * 2, 128, static_cast<cuuint64_t>(N) * K * 2};
+  cuuint32_t box[4] = {64, 64, static_cast<cuuint32_t>(nblk), 1};
+  cuuint32_t estr[4] = {1, 1, 1, 1};
+  return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(ptr), dims, strides, box, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
@@ -165,26 +189,38 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   const bg_moe_config& c = ctx->cfg;
   const int64_t R = static_cast<int64_t>(T) * c.k;
   bg::GemmLaunch g1;
-  if (!encode_act_map(&g1.tm_a, x_perm, R, c.d)) { ctx->last_error = "cuTensorMapEncodeTiled(x_perm) failed"; return BG_ERR_CUDA; }
+  if (x_perm == ctx->x_perm) {
+    g1.tm_act = ctx->am_x;             // workspace maps, encoded once in bg_moe_create
+  } else if (!encode_act_maps(&g1.tm_act, x_perm, R, c.d)) {
+    ctx->last_error = "cuTensorMapEncodeTiled(x_perm) failed";
+    return BG_ERR_CUDA;
+  }
   g1.tm_b0 = ctx->tm_wg;
   g1.tm_b1 = ctx->tm_wu;
+  g1.w4d = c.f % 64 == 0;
+  g1.tm_b0_4d = g1.w4d ? ctx->tm_wg4 : ctx->tm_wg;
+  g1.tm_b1_4d = g1.w4d ? ctx->tm_wu4 : ctx->tm_wu;
   g1.offsets = offsets;
   g1.E = c.E; g1.K = c.d; g1.N = c.f;
   g1.out = ctx->H;
   g1.row_scale = nullptr; g1.row_src = nullptr;
   g1.num_sms = ctx->num_sms;
-  BG_LAUNCH(ctx, bg::launch_gateup_swiglu(g1, st), "gateup_swiglu");
+  BG_LAUNCH(ctx, ctx->pair_gemm ? bg::launch_gateup_swiglu_pair(g1, st) : bg::launch_gateup_swiglu(g1, st),
+            "gateup_swiglu");
   if (mark_between >= 0) mark(ctx, mark_between, st);
   bg::GemmLaunch g2;
-  if (!encode_act_map(&g2.tm_a, ctx->H, R, c.f)) { ctx->last_error = "cuTensorMapEncodeTiled(H) failed"; return BG_ERR_CUDA; }
+  g2.tm_act = ctx->am_h;
   g2.tm_b0 = ctx->tm_wd;
   g2.tm_b1 = ctx->tm_wd;
+  g2.w4d = c.d % 64 == 0;
+  g2.tm_b0_4d = g2.w4d ? ctx->tm_wd4 : ctx->tm_wd;
+  g2.tm_b1_4d = g2.tm_b0_4d;
   g2.offsets = offsets;
   g2.E = c.E; g2.K = c.f; g2.N = c.d;
   g2.out = y;
   g2.row_scale = row_scale; g2.row_src = row_src;
   g2.num_sms = ctx->num_sms;
-  BG_LAUNCH(ctx, bg::launch_down(g2, st), "down");
+  BG_LAUNCH(ctx, ctx->pair_gemm ? bg::launch_down_pair(g2, st) : bg::launch_down(g2, st), "down");
   return BG_OK;
 }
 
@@ -224,7 +260,9 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   DeviceGuard guard(c.device);
   if (!guard.ok) return BG_ERR_CUDA;
   if (get_encode_fn() == nullptr) return BG_ERR_CUDA;
-  if (bg::gemm_kernels_init() != cudaSuccess || bg::router_kernels_init() != cudaSuccess) return BG_ERR_CUDA;
+  if (bg::gemm_kernels_init() != cudaSuccess || bg::router_kernels_init() != cudaSuccess ||
+      bg::pair_kernels_init() != cudaSuccess)
+    return BG_ERR_CUDA;
 
   bg_moe_ctx* ctx = new (std::nothrow) bg_moe_ctx();
   if (!ctx) return BG_ERR_NOMEM;
@@ -268,6 +306,15 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   ctx->Y = ctx->ws + o_y;
   ctx->hidden_dev = ctx->ws + o_hd;
   ctx->out_dev = ctx->ws + o_od;
+  if (!encode_act_maps(&ctx->am_x, ctx->x_perm, Rm, c.d) || !encode_act_maps(&ctx->am_h, ctx->H, Rm, c.f)) {
+    cudaFree(ctx->ws);
+    delete ctx;
+    return BG_ERR_CUDA;
+  }
+  {
+    const char* g = std::getenv("BG_MOE_GEMM");
+    if (g != nullptr && std::strcmp(g, "tile") == 0) ctx->pair_gemm = false;
+  }
   *out = ctx;
   return BG_OK;
 }
@@ -291,6 +338,16 @@ int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, cons
       !encode_weight_map(&ctx->tm_wd, W_down, c.E, c.f, c.d)) {
     ctx->last_error = "cuTensorMapEncodeTiled(weights) failed";
     return BG_ERR_CUDA;
+  }
+  {
+    // block views: pair kernel a7 = 1 block per map, a8 = 2; tile kernel a7 = 2, a8 = 4
+    const int nb_gu = ctx->pair_gemm ? 1 : 2, nb_d = ctx->pair_gemm ? 2 : 4;
+    if ((c.f % 64 == 0 && (!encode_weight_map_4d(&ctx->tm_wg4, W_gate, c.E, c.d, c.f, nb_gu) ||
+                           !encode_weight_map_4d(&ctx->tm_wu4, W_up, c.E, c.d, c.f, nb_gu))) ||
+        (c.d % 64 == 0 && !encode_weight_map_4d(&ctx->tm_wd4, W_down, c.E, c.f, c.d, nb_d))) {
+      ctx->last_error = "cuTensorMapEncodeTiled(weight block views) failed";
+      return BG_ERR_CUDA;
+    }
   }
   // exact bf16 hi/mid/lo split of W_r for the tensor-core router (router_gemm.cu); [3][d][E_ld]
   {

@@ -57,6 +57,7 @@ struct Params {
   __nv_bfloat16* out;
   const float* row_scale;
   const int32_t* row_src;
+  bool w4d;                    // tm_b0 / tm_b1 are the 4-D block views (kernels.h)
 };
 
 struct TileCoord {
@@ -189,7 +190,15 @@ grouped_gemm_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_const
           const uint32_t sb = sa + A_BYTES;
           mbar_expect_tx(full_bar(s), STAGE_BYTES);
           tma_load_2d(sa, &tm_a, full_bar(s), kb * BK, c.row0);
-          if (GATEUP) {
+          if (p.w4d) {
+            // one operation per weight tensor: 64-column blocks in [block][k][64 n] order (kernels.h)
+            if (GATEUP) {
+              tma_load_4d(sb, &tm_b0, full_bar(s), 0, kb * BK, n0 >> 6, c.e);
+              tma_load_4d(sb + 2 * B_BLK_BYTES, &tm_b1, full_bar(s), 0, kb * BK, n0 >> 6, c.e);
+            } else {
+              tma_load_4d(sb, &tm_b0, full_bar(s), 0, kb * BK, n0 >> 6, c.e);
+            }
+          } else if (GATEUP) {
             tma_load_3d(sb + 0 * B_BLK_BYTES, &tm_b0, full_bar(s), n0, kb * BK, c.e);
             tma_load_3d(sb + 1 * B_BLK_BYTES, &tm_b0, full_bar(s), n0 + 64, kb * BK, c.e);
             tma_load_3d(sb + 2 * B_BLK_BYTES, &tm_b1, full_bar(s), n0, kb * BK, c.e);
@@ -320,6 +329,7 @@ Params make_params(const GemmLaunch& g) {
   p.out = static_cast<__nv_bfloat16*>(g.out);
   p.row_scale = g.row_scale;
   p.row_src = g.row_src;
+  p.w4d = g.w4d;
   return p;
 }
 
@@ -334,12 +344,12 @@ cudaError_t gemm_kernels_init() {
 }
 
 cudaError_t launch_gateup_swiglu(const GemmLaunch& g, cudaStream_t st) {
-  grouped_gemm_kernel<true><<<g.num_sms, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_a, g.tm_b0, g.tm_b1, make_params(g));
+  grouped_gemm_kernel<true><<<g.num_sms, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_act.m[15], g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b1_4d : g.tm_b1, make_params(g));
   return cudaGetLastError();
 }
 
 cudaError_t launch_down(const GemmLaunch& g, cudaStream_t st) {
-  grouped_gemm_kernel<false><<<g.num_sms, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_a, g.tm_b0, g.tm_b0, make_params(g));
+  grouped_gemm_kernel<false><<<g.num_sms, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_act.m[15], g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b0_4d : g.tm_b0, make_params(g));
   return cudaGetLastError();
 }
 

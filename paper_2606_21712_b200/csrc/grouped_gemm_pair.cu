@@ -1,0 +1,432 @@
+// grouped_gemm_pair.cu -- steps a7 / a8 of the combined MoE layer on sm_100a tensor cores, CTA-pair form.
+//
+//   a7: H[r,:] = silu(x_perm[r,:] W_gate[e]) (.) (x_perm[r,:] W_up[e])      rows r of expert e
+//   a8: Y[r,:] = (w[row_src[r]]) * (H[r,:] W_down[e])
+// (BASELINE.json north_star "grouped SwiGLU expert FFN".)
+//
+// Orientation ("swap-AB"): the WEIGHTS sit on the UMMA M axis and the TOKENS on the UMMA N axis,
+// because N is the only tile dimension tcgen05 sizes finely (multiples of 16 up to 256).  Per-expert
+// row counts are whatever the router produced (a few rows for a cold expert, a ragged tail for every
+// expert); with tokens on N the tensor-core time of a tile follows the rows it really has instead of
+// a padded 128-row block.
+//
+// CTA pair (tcgen05 cta_group::2): two CTAs of a cluster run ONE MMA of M = 256.  Each CTA stages
+// 128 weight columns (its half of M) and HALF of the tile's tokens (its half of N) in its own shared
+// memory and owns 128 accumulator lanes x N columns in its own TMEM.  Per CTA and 64-wide k-block
+// that is 16 KB of weights + <= 16 KB of tokens for 128 x 256 x 64 MACs: two thirds of the L2->SM
+// traffic of the 1-CTA 128 x 256 tile (48 KB), which ncu showed running at 17 TB/s (profiles/r01).
+//
+//   A operand: weights [E, K, N_out] bf16, N_out contiguous -> MN-major, TMA boxes {64 n, 64 k, 1}
+//              a7: M rows 0..63 = 64 W_gate columns, rows 64..127 = the same 64 W_up columns (per CTA)
+//              a8: M rows 0..127 = 128 consecutive W_down columns (per CTA)
+//   B operand: activations [rows, K] bf16, K contiguous     -> K-major,  ONE TMA box {64 k, nt/2 rows}
+//              (sixteen tensor maps, one per multiple of 8 rows) -- the TMA unit costs ~40 ns per
+//              operation whatever its size, so a k-block is 2 (a8) or 3 (a7) operations per CTA
+//   D (TMEM) : [128 lanes = features] x [nt columns = tokens] fp32 per CTA, two stages of 256 columns
+// The weights are consumed in the layout the layer is given (reading S14): no transpose/prepack.
+//
+// Warp roles (persistent, one 256-thread CTA per SM, 74 clusters):
+//   warp 0 lane 0: TMA producer (both CTAs; transaction bytes of both land on the leader's barrier)
+//   warp 1 lane 0: tcgen05.mma issuer (leader CTA only); commits are multicast to both CTAs
+//   warp 2       : TMEM allocator
+//   warps 4-7    : epilogue (TMEM -> registers -> SwiGLU | gate weight -> bf16 -> smem transpose -> global)
+//
+// a7 epilogue: gate and up accumulators of one feature live in TMEM lanes f and 64+f, i.e. in
+// different warps.  Warp pairs (0,2) and (1,3) exchange 32-token chunks through shared memory: for
+// chunks (2i, 2i+1) the up-warp hands chunk 2i to the gate-warp and the gate-warp hands chunk 2i+1 to
+// the up-warp, so both warps do half of the SiLU work.
+//
+// Tile scheduler: token tiles never straddle experts.  Expert e with n_e rows owns
+// tt_e = ceil(n_e/256) token tiles of ceil16(ceil(n_e/tt_e)) rows (the last one shorter) times
+// ceil(N_out/OUT_FEATS) feature tiles, ordered feature-tile-major / token-tile-minor so that the
+// clusters running at the same time share weight strips through L2.  Tile t -> cluster (t mod #clusters).
+// Experts with no rows own no tiles and their weights are never touched.
+#include "kernels.h"
+#include "ptx_sm100.cuh"
+
+namespace bg {
+namespace {
+
+constexpr int BN_MAX = 256;        // UMMA N max: tokens per tile
+constexpr int BK = 64;             // k per pipeline stage = one 128-byte swizzle span of bf16
+constexpr int UK = 16;             // UMMA K for 16-bit inputs
+constexpr int STAGES = 6;
+constexpr int A_BLK_BYTES = 64 * BK * 2;            // 8 KB: one 64-feature block of weights
+constexpr int A_BYTES = 2 * A_BLK_BYTES;            // 16 KB: this CTA's 128 M rows
+constexpr int B_BYTES = (BN_MAX / 2) * BK * 2;      // 16 KB: this CTA's half of the tokens
+constexpr int STAGE_BYTES = A_BYTES + B_BYTES;      // 32 KB
+constexpr int RING_BYTES = STAGES * STAGE_BYTES;    // 192 KB
+constexpr int NUM_THREADS = 256;
+constexpr int MAX_E = 256;
+constexpr int XCH_PITCH = 36;                       // words per lane row of an exchange buffer (conflict-free v4)
+constexpr int XCH_BYTES = 32 * XCH_PITCH * 4;       // 4608 B
+constexpr int BAR_BYTES = 256;
+constexpr int TABLE_BYTES = 2064;                   // 2 x (MAX_E + 1) ints, 16-byte padded
+constexpr int STAGE_TILE_BYTES = 32 * 64;           // per-warp output staging: [32 tokens][32 features] bf16
+// epilogue scratch: [4 exchange buffers (a7) | 4 x 256 gate weights (a8)] then the 4 staging tiles
+constexpr int EPI_BYTES = 4 * XCH_BYTES + 4 * STAGE_TILE_BYTES;
+constexpr int SMEM_BYTES = RING_BYTES + 1024 /*align slack*/ + BAR_BYTES + TABLE_BYTES + EPI_BYTES;
+static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
+
+// M = 256 (pair), A MN-major (weights), B K-major (tokens); the N field is filled in per tile.
+constexpr uint32_t IDESC_BASE = umma_idesc_bf16(256, 0, /*A MN-major*/ 1, /*B K-major*/ 0);
+// A: MN-major SW128: 64-feature blocks A_BLK_BYTES apart (LBO); 8-k-row groups 1024 B apart (SBO).
+constexpr uint64_t ADESC_HI = umma_desc_sw128(A_BLK_BYTES, 1024);
+// B: K-major SW128: 8-token groups 1024 B apart (SBO); LBO unused inside one swizzle span.
+constexpr uint64_t BDESC_HI = umma_desc_sw128(16, 1024);
+
+struct Params {
+  const int32_t* offsets;
+  int E, K, N;                 // N = output features (f for a7, d for a8)
+  __nv_bfloat16* out;
+  const float* row_scale;
+  const int32_t* row_src;
+  bool w4d;                    // tm_w0 / tm_w1 are the 4-D block views (kernels.h)
+};
+
+__device__ __forceinline__ void named_bar_sync(int id, int threads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+
+struct TileCoord {
+  int e, row0, rows_valid, nt, f_tile;
+};
+
+// tile_start[e] = first linear tile index of expert e (tile_start[E] = total);
+// t_tiles[e] = token tiles of expert e.  Both live in shared memory.
+__device__ __forceinline__ TileCoord decode_tile(int t, const int* tile_start, const int* t_tiles,
+                                                 const int32_t* offsets, int E) {
+  int lo = 0, hi = E;              // largest e with tile_start[e] <= t
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (tile_start[mid] <= t) lo = mid; else hi = mid;
+  }
+  // experts with zero tiles share tile_start with their successor: the search above lands on the
+  // last expert whose start <= t, which is the one that owns t (its successors start later).
+  const int e = lo;
+  const int local = t - tile_start[e];
+  const int tt = t_tiles[e];
+  const int f_tile = local / tt;
+  const int t_tile = local - f_tile * tt;
+  const int beg = __ldg(offsets + e), end = __ldg(offsets + e + 1);
+  const int n_e = end - beg;
+  const int base = (((n_e + tt - 1) / tt) + 15) & ~15;      // rows per token tile, multiple of 16, <= 256
+  TileCoord c;
+  c.e = e;
+  c.row0 = beg + t_tile * base;
+  c.rows_valid = min(base, end - c.row0);
+  c.nt = (c.rows_valid + 15) & ~15;
+  c.f_tile = f_tile;
+  return c;
+}
+
+// silu(g) * u with silu(g) = g / (1 + exp(-g)) = h + h tanh(h), h = g/2 (the same function; one
+// MUFU instead of two; tanh.approx has 2^-11 relative error, far below the bf16 rounding of H).
+__device__ __forceinline__ float silu_mul(float g, float u) {
+  const float h = 0.5f * g;
+  float th;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(th) : "f"(h));
+  return fmaf(h, th, h) * u;
+}
+
+__device__ __forceinline__ void st_shared_bf16(uint32_t addr, float v) {
+  const __nv_bfloat16 b = __float2bfloat16_rn(v);
+  asm volatile("st.shared.b16 [%0], %1;" ::"r"(addr), "h"(*reinterpret_cast<const uint16_t*>(&b)) : "memory");
+}
+
+// GATEUP = true : a7 (per CTA A = [64 W_gate columns | 64 W_up columns], SwiGLU epilogue, 128 output features / pair tile)
+// GATEUP = false: a8 (per CTA A = 128 W_down columns, optional per-token scale, 256 output features / pair tile)
+template <bool GATEUP>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
+pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__ CUtensorMap tm_w0,
+                 const __grid_constant__ CUtensorMap tm_w1, const Params p) {
+  constexpr int CTA_FEATS = GATEUP ? 64 : 128;       // output features per CTA and tile
+  constexpr int OUT_FEATS = 2 * CTA_FEATS;           // output features per pair tile
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t raw = smem_u32(smem_raw);
+  const uint32_t base = (raw + 1023u) & ~1023u;       // SW128 tiles need 1024-byte alignment
+  uint8_t* smem = smem_raw + (base - raw);
+  const uint32_t bar_base = base + RING_BYTES;
+  // barriers: full[S] empty[S] tmem_full[2] tmem_empty[2]; then the TMEM address
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+  auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + a); };
+  auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + 2 + a); };
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + RING_BYTES + 8 * (2 * STAGES + 4));
+  int* tile_start = reinterpret_cast<int*>(smem + RING_BYTES + BAR_BYTES);
+  int* t_tiles = tile_start + (MAX_E + 1);
+  uint8_t* epi_smem = smem + RING_BYTES + BAR_BYTES + TABLE_BYTES;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();            // 0 = leader
+  const int cluster_id = blockIdx.x >> 1, num_clusters = gridDim.x >> 1;
+  const int E = p.E;
+  const int f_tiles = (p.N + OUT_FEATS - 1) / OUT_FEATS;
+  const int k_blocks = (p.K + BK - 1) / BK;
+
+  // ---- per-CTA tile table: inclusive scan of per-expert tile counts (E <= 256 = blockDim)
+  {
+    int tt = 0;
+    if (threadIdx.x < E) {
+      const int cnt = __ldg(p.offsets + threadIdx.x + 1) - __ldg(p.offsets + threadIdx.x);
+      tt = (cnt + BN_MAX - 1) / BN_MAX;
+      t_tiles[threadIdx.x] = tt;
+    }
+    int v = tt * f_tiles;
+    #pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int u = __shfl_up_sync(0xffffffffu, v, o);
+      if (lane >= o) v += u;
+    }
+    __shared__ int warp_tot[NUM_THREADS / 32];
+    if (lane == 31) warp_tot[warp] = v;
+    __syncthreads();
+    int add = 0;
+    for (int w = 0; w < warp; ++w) add += warp_tot[w];
+    v += add;                                   // inclusive prefix for thread's expert
+    if (threadIdx.x < E) tile_start[threadIdx.x + 1] = v;
+    if (threadIdx.x == 0) tile_start[0] = 0;
+  }
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tm_w0);
+    if (GATEUP) tma_prefetch_desc(&tm_w1);
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    // tmem_empty (used on the leader only): one arrival per epilogue warp of both CTAs
+    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 8); }
+    fence_barrier_init();
+  }
+  if (warp == 2) {
+    tmem_alloc_pair(smem_u32(tmem_slot), 512);
+    tmem_relinquish_pair();
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();                                 // the peer's barriers are initialised, its TMEM allocated
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+  const int total_tiles = tile_start[E];
+
+  if (warp == 0) {
+    // ===================== TMA producer (one thread per CTA) =====================
+    if (lane == 0) {
+      int s = 0;
+      uint32_t ph = 0;
+      for (int t = cluster_id; t < total_tiles; t += num_clusters) {
+        const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E);
+        const int n0 = c.f_tile * OUT_FEATS + static_cast<int>(rank) * CTA_FEATS;
+        const int half = c.nt >> 1;                    // this CTA's tokens (multiple of 8, <= 128)
+        const int brow0 = c.row0 + static_cast<int>(rank) * half;
+        const uint32_t tx_pair = 2u * (A_BYTES + static_cast<uint32_t>(half) * (BK * 2));
+        const CUtensorMap* tm_b = &tm_act.m[(half >> 3) - 1];
+        for (int kb = 0; kb < k_blocks; ++kb) {
+          mbar_wait(empty_bar(s), ph ^ 1u);            // this CTA's slot is free (multicast commit)
+          const uint32_t sa = base + s * STAGE_BYTES;
+          const uint32_t sb = sa + A_BYTES;
+          const uint32_t fb = leader_bar(full_bar(s));
+          if (rank == 0) mbar_expect_tx(full_bar(s), tx_pair);   // the bytes of both CTAs
+          if (p.w4d) {
+            // one operation per weight tensor: nblk 64-column blocks in [block][k][64 n] order
+            tma_load_4d_pair(sa, &tm_w0, fb, 0, kb * BK, n0 >> 6, c.e);
+            if (GATEUP) tma_load_4d_pair(sa + A_BLK_BYTES, &tm_w1, fb, 0, kb * BK, n0 >> 6, c.e);
+          } else if (GATEUP) {
+            tma_load_3d_pair(sa, &tm_w0, fb, n0, kb * BK, c.e);
+            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w1, fb, n0, kb * BK, c.e);
+          } else {
+            tma_load_3d_pair(sa, &tm_w0, fb, n0, kb * BK, c.e);
+            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w0, fb, n0 + 64, kb * BK, c.e);
+          }
+          // this CTA's half of the tokens: one box of exactly `half` rows
+          tma_load_2d_pair(sb, tm_b, fb, kb * BK, brow0);
+          if (++s == STAGES) { s = 0; ph ^= 1u; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (one thread of the leader CTA) =====================
+    if (lane == 0 && rank == 0) {
+      int s = 0;
+      uint32_t ph = 0;
+      int it = 0;
+      for (int t = cluster_id; t < total_tiles; t += num_clusters, ++it) {
+        const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E);
+        const uint32_t idesc = IDESC_BASE | (static_cast<uint32_t>(c.nt >> 3) << 17);
+        const int as = it & 1;
+        const uint32_t aph = (it >> 1) & 1u;
+        mbar_wait(tempty_bar(as), aph ^ 1u);          // both CTAs' epilogues have drained this accumulator
+        tc_fence_after();
+        const uint32_t d_tmem = tmem_base + as * BN_MAX;
+        for (int kb = 0; kb < k_blocks; ++kb) {
+          mbar_wait(full_bar(s), ph);
+          tc_fence_after();
+          const uint32_t a_addr = base + s * STAGE_BYTES;
+          const uint32_t b_addr = a_addr + A_BYTES;
+          const uint64_t ad = ADESC_HI | ((a_addr >> 4) & 0x3FFFu);
+          const uint64_t bd = BDESC_HI | ((b_addr >> 4) & 0x3FFFu);
+          #pragma unroll
+          for (int kk = 0; kk < BK / UK; ++kk) {
+            // A (MN-major): +16 k = two 8-row groups = +2048 bytes; B (K-major): +16 k = +32 bytes in the span
+            umma_f16_pair(d_tmem, ad + ((kk * UK * 128) >> 4), bd + ((kk * UK * 2) >> 4), idesc,
+                          (kb | kk) != 0 ? 1u : 0u);
+          }
+          umma_commit_pair(empty_bar(s));             // both CTAs' slots free once these MMAs retire
+          if (++s == STAGES) { s = 0; ph ^= 1u; }
+        }
+        umma_commit_pair(tfull_bar(as));              // accumulator complete -> both epilogues
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================== epilogue: TMEM -> registers -> shared (transpose) -> global ==========
+    // A thread owns one feature (TMEM lane) and reads 32 tokens (columns) at a time; the output is
+    // token-major, so each warp turns its 32 feature x 32 token block around in a private 2 KB
+    // staging tile ([token][32 features] bf16) and stores 16 bytes per lane, 64 contiguous bytes
+    // per token.
+    const int q = warp & 3;                            // TMEM lane quarter this warp may read
+    uint8_t* stage = epi_smem + 4 * XCH_BYTES + q * STAGE_TILE_BYTES;
+    const uint32_t stage_wr = smem_u32(stage) + lane * 2;                       // + token * 64
+    const uint32_t stage_rd = smem_u32(stage) + (lane >> 2) * 64 + (lane & 3) * 16;   // + i * 512
+    float* sc_smem = reinterpret_cast<float*>(epi_smem) + q * BN_MAX;           // a8: this warp's copy
+    const int feat0 = static_cast<int>(rank) * CTA_FEATS + (GATEUP ? (q & 1) : q) * 32;   // in the pair tile
+    int it = 0;
+    for (int t = cluster_id; t < total_tiles; t += num_clusters, ++it) {
+      const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E);
+      const int as = it & 1;
+      const uint32_t aph = (it >> 1) & 1u;
+      const int n_chunks = (c.nt + 31) >> 5;           // 32-token chunks (the last may be half used)
+      const int col = c.f_tile * OUT_FEATS + feat0 + (lane & 3) * 8;            // this lane's 8 output columns
+      const bool col_ok = col < p.N;                   // N is a multiple of 8
+      __nv_bfloat16* out_tile = p.out + static_cast<int64_t>(c.row0) * p.N + col;
+      if (!GATEUP) {
+        // gate weights of the tile's tokens -> shared memory, fetched before the accumulator is
+        // awaited so the two dependent loads hide behind the main loop
+        __syncwarp();
+        #pragma unroll
+        for (int i = 0; i < BN_MAX / 32; ++i) {
+          float sc = 1.0f;
+          if (p.row_scale != nullptr && i * 32 + lane < c.rows_valid)
+            sc = __ldg(p.row_scale + __ldg(p.row_src + c.row0 + i * 32 + lane));
+          sc_smem[i * 32 + lane] = sc;
+        }
+        __syncwarp();
+      }
+      mbar_wait(tfull_bar(as), aph);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + as * BN_MAX;
+      // token-major write-out of the staged 32 x 32 block of chunk cc
+      auto flush_chunk = [&](int cc) {
+        __syncwarp();
+        const int n_tok = c.rows_valid - cc * 32;
+        #pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int r = (lane >> 2) + 8 * i;
+          uint4 val;
+          asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                       : "=r"(val.x), "=r"(val.y), "=r"(val.z), "=r"(val.w) : "r"(stage_rd + i * 512));
+          if (col_ok && r < n_tok)
+            *reinterpret_cast<uint4*>(out_tile + static_cast<int64_t>(cc * 32 + r) * p.N) = val;
+        }
+        __syncwarp();
+      };
+      if (GATEUP) {
+        // pair (q&1): gate warp q in {0,1} and up warp q+2 hold the same 32 features
+        const bool is_up = q >= 2;
+        float* xch_g2u = reinterpret_cast<float*>(epi_smem + (q & 1) * 2 * XCH_BYTES);   // gate -> up warp
+        float* xch_u2g = xch_g2u + XCH_BYTES / 4;                                         // up -> gate warp
+        float* my_out = (is_up ? xch_u2g : xch_g2u) + lane * XCH_PITCH;
+        const float* my_in = (is_up ? xch_g2u : xch_u2g) + lane * XCH_PITCH;
+        const int bar_id = 1 + (q & 1);
+        #pragma unroll 1
+        for (int c0 = 0; c0 < n_chunks; c0 += 2) {
+          uint32_t v0[32], v1[32];
+          tmem_ld_32x32(taddr + c0 * 32, v0);
+          if (c0 + 1 < n_chunks) tmem_ld_32x32(taddr + (c0 + 1) * 32, v1);
+          tmem_ld_wait();
+          // hand over the chunk the partner finishes: up warp gives chunk c0, gate warp gives chunk c0+1
+          #pragma unroll
+          for (int j = 0; j < 32; j += 4)
+            *reinterpret_cast<uint4*>(my_out + j) =
+                is_up ? make_uint4(v0[j], v0[j + 1], v0[j + 2], v0[j + 3])
+                      : make_uint4(v1[j], v1[j + 1], v1[j + 2], v1[j + 3]);
+          named_bar_sync(bar_id, 64);
+          const int cc = is_up ? c0 + 1 : c0;            // the chunk this warp finishes
+          if (cc < n_chunks) {
+            #pragma unroll
+            for (int j = 0; j < 32; j += 4) {
+              const uint4 o = *reinterpret_cast<const uint4*>(my_in + j);
+              const uint32_t other[4] = {o.x, o.y, o.z, o.w};
+              #pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                const float g = __uint_as_float(is_up ? other[i] : v0[j + i]);
+                const float u = __uint_as_float(is_up ? v1[j + i] : other[i]);
+                st_shared_bf16(stage_wr + (j + i) * 64, silu_mul(g, u));
+              }
+            }
+            flush_chunk(cc);
+          }
+          named_bar_sync(bar_id, 64);                    // exchange buffers free for the next round
+        }
+      } else {
+        #pragma unroll 1
+        for (int cc = 0; cc < n_chunks; ++cc) {
+          uint32_t v[32];
+          tmem_ld_32x32(taddr + cc * 32, v);
+          tmem_ld_wait();
+          #pragma unroll
+          for (int j = 0; j < 32; j += 4) {
+            const float4 s4 = *reinterpret_cast<const float4*>(sc_smem + cc * 32 + j);   // broadcast
+            st_shared_bf16(stage_wr + (j + 0) * 64, __uint_as_float(v[j + 0]) * s4.x);
+            st_shared_bf16(stage_wr + (j + 1) * 64, __uint_as_float(v[j + 1]) * s4.y);
+            st_shared_bf16(stage_wr + (j + 2) * 64, __uint_as_float(v[j + 2]) * s4.z);
+            st_shared_bf16(stage_wr + (j + 3) * 64, __uint_as_float(v[j + 3]) * s4.w);
+          }
+          flush_chunk(cc);
+        }
+      }
+      // accumulator drained: one arrival per warp on the LEADER's tmem_empty barrier
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_cluster(tempty_bar(as), 0);
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();          // the peer may still read this CTA's shared memory / signal its barriers
+  if (warp == 2) {
+    tc_fence_after();
+    tmem_dealloc_pair(tmem_base, 512);
+  }
+}
+
+Params make_params(const GemmLaunch& g) {
+  Params p;
+  p.offsets = g.offsets;
+  p.E = g.E;
+  p.K = g.K;
+  p.N = g.N;
+  p.out = static_cast<__nv_bfloat16*>(g.out);
+  p.row_scale = g.row_scale;
+  p.row_src = g.row_src;
+  p.w4d = g.w4d;
+  return p;
+}
+
+}  // namespace
+
+cudaError_t pair_kernels_init() {
+  cudaError_t e = cudaFuncSetAttribute(pair_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(pair_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+}
+
+cudaError_t launch_gateup_swiglu_pair(const GemmLaunch& g, cudaStream_t st) {
+  pair_gemm_kernel<true><<<g.num_sms & ~1, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b1_4d : g.tm_b1, make_params(g));
+  return cudaGetLastError();
+}
+
+cudaError_t launch_down_pair(const GemmLaunch& g, cudaStream_t st) {
+  pair_gemm_kernel<false><<<g.num_sms & ~1, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b0_4d : g.tm_b0, make_params(g));
+  return cudaGetLastError();
+}
+
+}  // namespace bg

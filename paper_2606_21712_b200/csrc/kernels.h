@@ -48,10 +48,21 @@ cudaError_t launch_unpermute(const void* y_perm, const int32_t* inv_perm, const 
                              int d, void* out, int num_sms, cudaStream_t st);
 
 // ---- grouped GEMM (grouped_gemm.cu): steps a7 and a8
+// Activation tensor maps: the same [rows, K] bf16 matrix with TMA boxes of {64 k, 8 (i + 1) rows},
+// so that any token count that is a multiple of 8 (<= 128) is ONE TMA operation: the TMA unit's
+// per-operation cost (~40 ns), not its bandwidth, is what limits a 64-wide k-block.
+struct ActMaps {
+  CUtensorMap m[16];   // box rows 8, 16, ..., 128
+};
 struct GemmLaunch {
-  CUtensorMap tm_a;    // activations [rows, K] bf16, box {64, 128}
+  ActMaps tm_act;      // activations [rows, K] bf16
   CUtensorMap tm_b0;   // weights [E, K, N] bf16, box {64, 64, 1}: W_gate (gate/up GEMM) or W_down
   CUtensorMap tm_b1;   // W_up (gate/up GEMM only)
+  // The same weights viewed as [E, N/64, K, 64] with box {64 n, 64 k, nblk, 1}: one TMA operation
+  // brings nblk 64-column blocks in the [block][k][64 n] order the MN-major UMMA operand wants.
+  // Valid only when N % 64 == 0 (w4d); otherwise the kernels issue one 3-D box per block.
+  CUtensorMap tm_b0_4d, tm_b1_4d;
+  bool w4d;
   const int32_t* offsets;  // [E+1]
   int E, K, N;         // N = output columns (f for gate/up, d for down)
   void* out;           // bf16 [rows, N]
@@ -62,5 +73,9 @@ struct GemmLaunch {
 cudaError_t launch_gateup_swiglu(const GemmLaunch& g, cudaStream_t st);
 cudaError_t launch_down(const GemmLaunch& g, cudaStream_t st);
 cudaError_t gemm_kernels_init();   // sets the dynamic shared-memory attributes once
+// CTA-pair kernels (grouped_gemm_pair.cu): weights on UMMA M (256 per pair), tokens on UMMA N.
+cudaError_t launch_gateup_swiglu_pair(const GemmLaunch& g, cudaStream_t st);
+cudaError_t launch_down_pair(const GemmLaunch& g, cudaStream_t st);
+cudaError_t pair_kernels_init();
 
 }  // namespace bg
