@@ -1,5 +1,5 @@
 // gather_reduce.cu -- the two HBM-bound row movers of the combined MoE layer:
-//   a6 gather    x_perm[r,:] = hidden[row_src[r]/k,:]                        (16-byte vector copies)
+//   a6 gather    x_perm[r,:] = hidden[row_src[r]/k,:]   written as x_perm[inv_perm[i],:] = hidden[i/k,:]
 //   a9 reduce    out[t,:]    = sum_{s<k} (w[t,s]) * Y[inv_perm[t*k+s],:]     slot order, fp32, RNE->bf16
 // BASELINE.json north_star: "a gather kernel with 16-byte vectorised, coalesced row copies" and "a
 // gate-weighted un-permute that sums each token's top-k results", atomic-free.
@@ -22,24 +22,41 @@ __device__ __forceinline__ void st_stream(uint4* p, const uint4& v) {
                "r"(v.w) : "memory");
 }
 
+// a6 as a scatter: one warp per TOKEN reads its hidden row once (registers) and writes it to the k
+// expert-order rows inv_perm[t*k + s] -- x_perm[inv_perm[t*k+s]] = hidden[t] is the same assignment
+// as x_perm[r] = hidden[row_src[r]/k] (inv_perm is the inverse of row_src), with 1 load + k stores per
+// vector instead of k loads + k stores.
+template <int KMAX>
 __global__ void __launch_bounds__(256) gather_kernel(const uint4* __restrict__ hidden,
-                                                     const int32_t* __restrict__ row_src, int R, int k,
+                                                     const int32_t* __restrict__ inv_perm, int T, int k,
                                                      int vec_per_row, uint4* __restrict__ x_perm) {
   const int lane = threadIdx.x & 31;
   const int warps_total = gridDim.x * (blockDim.x >> 5);
-  for (int r = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); r < R; r += warps_total) {
-    const int t = __ldg(row_src + r) / k;
+  for (int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); t < T; t += warps_total) {
     const uint4* src = hidden + static_cast<int64_t>(t) * vec_per_row;
-    uint4* dst = x_perm + static_cast<int64_t>(r) * vec_per_row;
+    uint4* dst[KMAX];
+    #pragma unroll
+    for (int s = 0; s < KMAX; ++s)
+      dst[s] = x_perm + static_cast<int64_t>(s < k ? __ldg(inv_perm + static_cast<int64_t>(t) * k + s) : 0) * vec_per_row;
     int c = lane;
     for (; c + 96 < vec_per_row; c += 128) {
-      const uint4 a0 = __ldg(src + c), a1 = __ldg(src + c + 32), a2 = __ldg(src + c + 64), a3 = __ldg(src + c + 96);
-      st_stream(dst + c, a0);
-      st_stream(dst + c + 32, a1);
-      st_stream(dst + c + 64, a2);
-      st_stream(dst + c + 96, a3);
+      const uint4 a0 = ld_stream(src + c), a1 = ld_stream(src + c + 32), a2 = ld_stream(src + c + 64),
+                  a3 = ld_stream(src + c + 96);
+      #pragma unroll
+      for (int s = 0; s < KMAX; ++s)
+        if (s < k) {
+          st_stream(dst[s] + c, a0);
+          st_stream(dst[s] + c + 32, a1);
+          st_stream(dst[s] + c + 64, a2);
+          st_stream(dst[s] + c + 96, a3);
+        }
     }
-    for (; c < vec_per_row; c += 32) st_stream(dst + c, __ldg(src + c));
+    for (; c < vec_per_row; c += 32) {
+      const uint4 a = ld_stream(src + c);
+      #pragma unroll
+      for (int s = 0; s < KMAX; ++s)
+        if (s < k) st_stream(dst[s] + c, a);
+    }
   }
 }
 
@@ -103,11 +120,19 @@ inline int row_mover_grid(int rows, int num_sms) {
 
 }  // namespace
 
-cudaError_t launch_gather(const void* hidden, const int32_t* row_src, int R, int k, int d, void* x_perm,
+cudaError_t launch_gather(const void* hidden, const int32_t* inv_perm, int T, int k, int d, void* x_perm,
                           int num_sms, cudaStream_t st) {
-  if (R == 0) return cudaSuccess;
-  gather_kernel<<<row_mover_grid(R, num_sms), 256, 0, st>>>(static_cast<const uint4*>(hidden), row_src, R, k, d / 8,
-                                                            static_cast<uint4*>(x_perm));
+  if (T == 0) return cudaSuccess;
+  const int grid = row_mover_grid(T, num_sms);
+  if (k <= 2)
+    gather_kernel<2><<<grid, 256, 0, st>>>(static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
+                                           static_cast<uint4*>(x_perm));
+  else if (k <= 4)
+    gather_kernel<4><<<grid, 256, 0, st>>>(static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
+                                           static_cast<uint4*>(x_perm));
+  else
+    gather_kernel<8><<<grid, 256, 0, st>>>(static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
+                                           static_cast<uint4*>(x_perm));
   return cudaGetLastError();
 }
 

@@ -56,7 +56,7 @@ constexpr int A_BYTES = 2 * A_BLK_BYTES;            // 16 KB: this CTA's 128 M r
 constexpr int B_BYTES = (BN_MAX / 2) * BK * 2;      // 16 KB: this CTA's half of the tokens
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;      // 32 KB
 constexpr int RING_BYTES = STAGES * STAGE_BYTES;    // 192 KB
-constexpr int NUM_THREADS = 256;
+constexpr int MAX_THREADS = 384;             // 4 role warps + 4 (a7) or 8 (a8) epilogue warps
 constexpr int MAX_E = 256;
 constexpr int XCH_PITCH = 36;                       // words per lane row of an exchange buffer (conflict-free v4)
 constexpr int XCH_BYTES = 32 * XCH_PITCH * 4;       // 4608 B
@@ -64,7 +64,8 @@ constexpr int BAR_BYTES = 256;
 constexpr int TABLE_BYTES = 2064;                   // 2 x (MAX_E + 1) ints, 16-byte padded
 constexpr int STAGE_TILE_BYTES = 32 * 64;           // per-warp output staging: [32 tokens][32 features] bf16
 // epilogue scratch: [4 exchange buffers (a7) | 4 x 256 gate weights (a8)] then the 4 staging tiles
-constexpr int EPI_BYTES = 4 * XCH_BYTES + 4 * STAGE_TILE_BYTES;
+constexpr int EPI_BYTES = 4 * XCH_BYTES + 4 * STAGE_TILE_BYTES;   // a8: 8 KB of scales + 8 staging tiles = 24 KB
+static_assert(EPI_BYTES >= 8 * BN_MAX * 4 + 8 * STAGE_TILE_BYTES, "a8 epilogue scratch");
 constexpr int SMEM_BYTES = RING_BYTES + 1024 /*align slack*/ + BAR_BYTES + TABLE_BYTES + EPI_BYTES;
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
 
@@ -82,6 +83,7 @@ struct Params {
   const float* row_scale;
   const int32_t* row_src;
   bool w4d;                    // tm_w0 / tm_w1 are the 4-D block views (kernels.h)
+  int pf_groups;               // > 0: tm_pf0 / tm_pf1 are valid, L2-prefetch this many 4-k-block groups ahead
 };
 
 __device__ __forceinline__ void named_bar_sync(int id, int threads) {
@@ -89,7 +91,7 @@ __device__ __forceinline__ void named_bar_sync(int id, int threads) {
 }
 
 struct TileCoord {
-  int e, row0, rows_valid, nt, f_tile;
+  int e, row0, rows_valid, nt, f_tile, t_tile;
 };
 
 // tile_start[e] = first linear tile index of expert e (tile_start[E] = total);
@@ -117,6 +119,7 @@ __device__ __forceinline__ TileCoord decode_tile(int t, const int* tile_start, c
   c.rows_valid = min(base, end - c.row0);
   c.nt = (c.rows_valid + 15) & ~15;
   c.f_tile = f_tile;
+  c.t_tile = t_tile;
   return c;
 }
 
@@ -137,11 +140,15 @@ __device__ __forceinline__ void st_shared_bf16(uint32_t addr, float v) {
 // GATEUP = true : a7 (per CTA A = [64 W_gate columns | 64 W_up columns], SwiGLU epilogue, 128 output features / pair tile)
 // GATEUP = false: a8 (per CTA A = 128 W_down columns, optional per-token scale, 256 output features / pair tile)
 template <bool GATEUP>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GATEUP ? 256 : 384, 1)
 pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__ CUtensorMap tm_w0,
-                 const __grid_constant__ CUtensorMap tm_w1, const Params p) {
+                 const __grid_constant__ CUtensorMap tm_w1, const __grid_constant__ CUtensorMap tm_pf0,
+                 const __grid_constant__ CUtensorMap tm_pf1, const Params p) {
   constexpr int CTA_FEATS = GATEUP ? 64 : 128;       // output features per CTA and tile
   constexpr int OUT_FEATS = 2 * CTA_FEATS;           // output features per pair tile
+  // a8 has short k loops (K = f), so its epilogue gets two warps per TMEM lane quarter
+  constexpr int EPI_WARPS = GATEUP ? 4 : 8;
+  constexpr int STAGE_OFF = GATEUP ? 4 * XCH_BYTES : 8 * BN_MAX * 4;   // staging tiles follow the exchange / scale area
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;       // SW128 tiles need 1024-byte alignment
@@ -163,6 +170,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   const int E = p.E;
   const int f_tiles = (p.N + OUT_FEATS - 1) / OUT_FEATS;
   const int k_blocks = (p.K + BK - 1) / BK;
+  const int k_groups = (k_blocks + 3) >> 2;          // 4-k-block groups (L2 prefetch granularity)
 
   // ---- per-CTA tile table: inclusive scan of per-expert tile counts (E <= 256 = blockDim)
   {
@@ -178,7 +186,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       const int u = __shfl_up_sync(0xffffffffu, v, o);
       if (lane >= o) v += u;
     }
-    __shared__ int warp_tot[NUM_THREADS / 32];
+    __shared__ int warp_tot[MAX_THREADS / 32];
     if (lane == 31) warp_tot[warp] = v;
     __syncthreads();
     int add = 0;
@@ -193,7 +201,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     if (GATEUP) tma_prefetch_desc(&tm_w1);
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
     // tmem_empty (used on the leader only): one arrival per epilogue warp of both CTAs
-    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 8); }
+    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 2 * EPI_WARPS); }
     fence_barrier_init();
   }
   if (warp == 2) {
@@ -220,6 +228,23 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         const uint32_t tx_pair = 2u * (A_BYTES + static_cast<uint32_t>(half) * (BK * 2));
         const CUtensorMap* tm_b = &tm_act.m[(half >> 3) - 1];
         for (int kb = 0; kb < k_blocks; ++kb) {
+          // L2 prefetch of the weight stream pf_groups x 4 k-blocks ahead of the ring (one 4-k-block
+          // box per operation): HBM keeps streaming while the ring is full of landed data, and the
+          // ring's own loads then see L2 latency.  Only the first token tile of a strip prefetches
+          // it (the other token tiles run at the same time and hit L2).  The distance is bounded so
+          // that the prefetched-but-unused bytes of all CTAs stay well inside L2.
+          if (p.pf_groups > 0 && (kb & 3) == 0) {
+            int gg = (kb >> 2) + p.pf_groups, tt = t;
+            while (gg >= k_groups) { gg -= k_groups; tt += num_clusters; }
+            if (tt < total_tiles) {
+              const TileCoord c2 = (tt == t) ? c : decode_tile(tt, tile_start, t_tiles, p.offsets, E);
+              if (c2.t_tile == 0) {
+                const int pn = (c2.f_tile * OUT_FEATS + static_cast<int>(rank) * CTA_FEATS) >> 6;
+                tma_prefetch_l2_4d(&tm_pf0, 0, gg * 4 * BK, pn, c2.e);
+                if (GATEUP) tma_prefetch_l2_4d(&tm_pf1, 0, gg * 4 * BK, pn, c2.e);
+              }
+            }
+          }
           mbar_wait(empty_bar(s), ph ^ 1u);            // this CTA's slot is free (multicast commit)
           const uint32_t sa = base + s * STAGE_BYTES;
           const uint32_t sb = sa + A_BYTES;
@@ -282,10 +307,11 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     // staging tile ([token][32 features] bf16) and stores 16 bytes per lane, 64 contiguous bytes
     // per token.
     const int q = warp & 3;                            // TMEM lane quarter this warp may read
-    uint8_t* stage = epi_smem + 4 * XCH_BYTES + q * STAGE_TILE_BYTES;
+    const int ew = warp - 4, sub = ew >> 2;            // a8: warps 4-7 take even chunks, warps 8-11 odd chunks
+    uint8_t* stage = epi_smem + STAGE_OFF + ew * STAGE_TILE_BYTES;
     const uint32_t stage_wr = smem_u32(stage) + lane * 2;                       // + token * 64
     const uint32_t stage_rd = smem_u32(stage) + (lane >> 2) * 64 + (lane & 3) * 16;   // + i * 512
-    float* sc_smem = reinterpret_cast<float*>(epi_smem) + q * BN_MAX;           // a8: this warp's copy
+    float* sc_smem = reinterpret_cast<float*>(epi_smem) + ew * BN_MAX;          // a8: this warp's copy
     const int feat0 = static_cast<int>(rank) * CTA_FEATS + (GATEUP ? (q & 1) : q) * 32;   // in the pair tile
     int it = 0;
     for (int t = cluster_id; t < total_tiles; t += num_clusters, ++it) {
@@ -367,7 +393,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         }
       } else {
         #pragma unroll 1
-        for (int cc = 0; cc < n_chunks; ++cc) {
+        for (int cc = sub; cc < n_chunks; cc += 2) {
           uint32_t v[32];
           tmem_ld_32x32(taddr + cc * 32, v);
           tmem_ld_wait();
@@ -408,6 +434,7 @@ Params make_params(const GemmLaunch& g) {
   p.row_scale = g.row_scale;
   p.row_src = g.row_src;
   p.w4d = g.w4d;
+  p.pf_groups = g.w4d ? g.prefetch : 0;
   return p;
 }
 
@@ -420,12 +447,12 @@ cudaError_t pair_kernels_init() {
 }
 
 cudaError_t launch_gateup_swiglu_pair(const GemmLaunch& g, cudaStream_t st) {
-  pair_gemm_kernel<true><<<g.num_sms & ~1, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b1_4d : g.tm_b1, make_params(g));
+  pair_gemm_kernel<true><<<g.num_sms & ~1, 256, SMEM_BYTES, st>>>(g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b1_4d : g.tm_b1, g.tm_pf0, g.tm_pf1, make_params(g));
   return cudaGetLastError();
 }
 
 cudaError_t launch_down_pair(const GemmLaunch& g, cudaStream_t st) {
-  pair_gemm_kernel<false><<<g.num_sms & ~1, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b0_4d : g.tm_b0, make_params(g));
+  pair_gemm_kernel<false><<<g.num_sms & ~1, 384, SMEM_BYTES, st>>>(g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b0_4d : g.tm_b0, g.tm_pf0, g.tm_pf0, make_params(g));
   return cudaGetLastError();
 }
 

@@ -41,7 +41,7 @@ cudaError_t launch_rank(const int32_t* topk_idx, const int32_t* block_base, int 
                         int32_t* row_src, int32_t* inv_perm, cudaStream_t st);
 
 // ---- gather / reduce (gather_reduce.cu): steps a6 and a9
-cudaError_t launch_gather(const void* hidden, const int32_t* row_src, int R, int k, int d, void* x_perm,
+cudaError_t launch_gather(const void* hidden, const int32_t* inv_perm, int T, int k, int d, void* x_perm,
                           int num_sms, cudaStream_t st);
 // weights == nullptr: plain sum (fused path, Y already gate-weighted).
 cudaError_t launch_unpermute(const void* y_perm, const int32_t* inv_perm, const float* weights, int T, int k,
@@ -63,6 +63,9 @@ struct GemmLaunch {
   // Valid only when N % 64 == 0 (w4d); otherwise the kernels issue one 3-D box per block.
   CUtensorMap tm_b0_4d, tm_b1_4d;
   bool w4d;
+  // Pair kernel: the same view with box {64 n, 256 k, nblk, 1} for L2 prefetch of the next tile's strip.
+  CUtensorMap tm_pf0, tm_pf1;
+  int prefetch;        // prefetch distance in 4-k-block groups (0 = off)
   const int32_t* offsets;  // [E+1]
   int E, K, N;         // N = output columns (f for gate/up, d for down)
   void* out;           // bf16 [rows, N]
