@@ -32,6 +32,7 @@ struct bg_moe_ctx {
   int32_t* block_base = nullptr;
   int32_t* row_src = nullptr;
   int32_t* inv_perm = nullptr;
+  float* w_perm = nullptr;      // gate weights in expert order (fused path)
   void* x_perm = nullptr;
   void* H = nullptr;
   void* Y = nullptr;
@@ -208,7 +209,7 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g1.offsets = offsets;
   g1.E = c.E; g1.K = c.d; g1.N = c.f;
   g1.out = ctx->H;
-  g1.row_scale = nullptr; g1.row_src = nullptr;
+  g1.row_scale = nullptr; g1.row_src = nullptr; g1.row_scale_perm = nullptr;
   g1.num_sms = ctx->num_sms;
   BG_LAUNCH(ctx, ctx->pair_gemm ? bg::launch_gateup_swiglu_pair(g1, st) : bg::launch_gateup_swiglu(g1, st),
             "gateup_swiglu");
@@ -227,6 +228,7 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g2.E = c.E; g2.K = c.f; g2.N = c.d;
   g2.out = y;
   g2.row_scale = row_scale; g2.row_src = row_src;
+  g2.row_scale_perm = row_scale ? ctx->w_perm : nullptr;
   g2.num_sms = ctx->num_sms;
   BG_LAUNCH(ctx, ctx->pair_gemm ? bg::launch_down_pair(g2, st) : bg::launch_down(g2, st), "down");
   return BG_OK;
@@ -287,7 +289,7 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   const int64_t o_part = carve(part_rows * c.E * 4), o_pieces = carve(3LL * c.d * ((c.E + 15) & ~15) * 2);
   const int64_t o_counts = carve(c.E * 4), o_offsets = carve((c.E + 1) * 4);
   const int64_t o_bc = carve(nblk * c.E * 4), o_bb = carve(nblk * c.E * 4);
-  const int64_t o_rs = carve(Rm * 4), o_ip = carve(Rm * 4);
+  const int64_t o_rs = carve(Rm * 4), o_ip = carve(Rm * 4), o_wp = carve(Rm * 4);
   const int64_t o_x = carve(Rm * c.d * 2), o_h = carve(Rm * c.f * 2), o_y = carve(Rm * c.d * 2);
   const int64_t o_hd = carve(Tm * c.d * 2), o_od = carve(Tm * c.d * 2);
   ctx->ws_bytes = off;
@@ -309,6 +311,7 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   ctx->block_base = reinterpret_cast<int32_t*>(ctx->ws + o_bb);
   ctx->row_src = reinterpret_cast<int32_t*>(ctx->ws + o_rs);
   ctx->inv_perm = reinterpret_cast<int32_t*>(ctx->ws + o_ip);
+  ctx->w_perm = reinterpret_cast<float*>(ctx->ws + o_wp);
   ctx->x_perm = ctx->ws + o_x;
   ctx->H = ctx->ws + o_h;
   ctx->Y = ctx->ws + o_y;
@@ -425,7 +428,7 @@ int bg_moe_permute(bg_moe_ctx* ctx, const void* hidden, int32_t T, const int32_t
   BG_LAUNCH(ctx, bg::launch_block_hist(topk_idx, T, c.E, c.k, ctx->block_counts, st), "block_hist");
   BG_LAUNCH(ctx, bg::launch_scan(ctx->block_counts, bg::route_num_blocks(T, c.k), c.E, ctx->block_base, nullptr,
                                  nullptr, st), "scan");
-  BG_LAUNCH(ctx, bg::launch_rank(topk_idx, ctx->block_base, T, c.E, c.k, row_src, inv_perm, st), "rank");
+  BG_LAUNCH(ctx, bg::launch_rank(topk_idx, ctx->block_base, T, c.E, c.k, row_src, inv_perm, nullptr, nullptr, st), "rank");
   if (x_perm) BG_LAUNCH(ctx, bg::launch_gather(hidden, inv_perm, T, c.k, c.d, x_perm, ctx->num_sms, st), "gather");
   return BG_OK;
 }
@@ -465,7 +468,8 @@ int bg_moe_combined_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void
   rc = do_route(ctx, hidden, T, nullptr, ctx->logits, ctx->topk_idx, ctx->topk_w, ctx->counts, ctx->offsets, st);
   if (rc) return rc;
   mark(ctx, 3, st);
-  BG_LAUNCH(ctx, bg::launch_rank(ctx->topk_idx, ctx->block_base, T, c.E, c.k, ctx->row_src, ctx->inv_perm, st), "rank");
+  BG_LAUNCH(ctx, bg::launch_rank(ctx->topk_idx, ctx->block_base, T, c.E, c.k, ctx->row_src, ctx->inv_perm, ctx->topk_w,
+                                 ctx->w_perm, st), "rank");
   mark(ctx, 4, st);
   BG_LAUNCH(ctx, bg::launch_gather(hidden, ctx->inv_perm, T, c.k, c.d, ctx->x_perm, ctx->num_sms, st), "gather");
   mark(ctx, 5, st);

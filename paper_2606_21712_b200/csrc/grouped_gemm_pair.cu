@@ -64,8 +64,8 @@ constexpr int BAR_BYTES = 256;
 constexpr int TABLE_BYTES = 2064;                   // 2 x (MAX_E + 1) ints, 16-byte padded
 constexpr int STAGE_TILE_BYTES = 32 * 64;           // per-warp output staging: [32 tokens][32 features] bf16
 // epilogue scratch: [4 exchange buffers (a7) | 4 x 256 gate weights (a8)] then the 4 staging tiles
-constexpr int EPI_BYTES = 4 * XCH_BYTES + 4 * STAGE_TILE_BYTES;   // a8: 8 KB of scales + 8 staging tiles = 24 KB
-static_assert(EPI_BYTES >= 8 * BN_MAX * 4 + 8 * STAGE_TILE_BYTES, "a8 epilogue scratch");
+constexpr int EPI_BYTES = 4 * XCH_BYTES + 4 * STAGE_TILE_BYTES;   // a8: 2 KB of scales + 8 staging tiles = 18 KB
+static_assert(EPI_BYTES >= 2 * BN_MAX * 4 + 8 * STAGE_TILE_BYTES, "a8 epilogue scratch");
 constexpr int SMEM_BYTES = RING_BYTES + 1024 /*align slack*/ + BAR_BYTES + TABLE_BYTES + EPI_BYTES;
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
 
@@ -80,8 +80,7 @@ struct Params {
   const int32_t* offsets;
   int E, K, N;                 // N = output features (f for a7, d for a8)
   __nv_bfloat16* out;
-  const float* row_scale;
-  const int32_t* row_src;
+  const float* row_scale;      // a8, fused path: gate weight per expert-order row (w_perm[r]); nullptr = 1
   bool w4d;                    // tm_w0 / tm_w1 are the 4-D block views (kernels.h)
   int pf_groups;               // > 0: tm_pf0 / tm_pf1 are valid, L2-prefetch this many 4-k-block groups ahead
 };
@@ -148,7 +147,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   constexpr int OUT_FEATS = 2 * CTA_FEATS;           // output features per pair tile
   // a8 has short k loops (K = f), so its epilogue gets two warps per TMEM lane quarter
   constexpr int EPI_WARPS = GATEUP ? 4 : 8;
-  constexpr int STAGE_OFF = GATEUP ? 4 * XCH_BYTES : 8 * BN_MAX * 4;   // staging tiles follow the exchange / scale area
+  constexpr int STAGE_OFF = GATEUP ? 4 * XCH_BYTES : 2 * BN_MAX * 4;   // staging tiles follow the exchange / scale area
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;       // SW128 tiles need 1024-byte alignment
@@ -311,8 +310,14 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     uint8_t* stage = epi_smem + STAGE_OFF + ew * STAGE_TILE_BYTES;
     const uint32_t stage_wr = smem_u32(stage) + lane * 2;                       // + token * 64
     const uint32_t stage_rd = smem_u32(stage) + (lane >> 2) * 64 + (lane & 3) * 16;   // + i * 512
-    float* sc_smem = reinterpret_cast<float*>(epi_smem) + ew * BN_MAX;          // a8: this warp's copy
+    float* sc_smem = reinterpret_cast<float*>(epi_smem);                        // a8: [2][BN_MAX] gate weights, double-buffered
     const int feat0 = static_cast<int>(rank) * CTA_FEATS + (GATEUP ? (q & 1) : q) * 32;   // in the pair tile
+    if (!GATEUP && cluster_id < total_tiles) {       // gate weights of the first tile -> buffer 0
+      const TileCoord c0 = decode_tile(cluster_id, tile_start, t_tiles, p.offsets, E);
+      float sc = 1.0f;
+      if (p.row_scale != nullptr && ew * 32 + lane < c0.rows_valid) sc = __ldg(p.row_scale + c0.row0 + ew * 32 + lane);
+      sc_smem[ew * 32 + lane] = sc;
+    }
     int it = 0;
     for (int t = cluster_id; t < total_tiles; t += num_clusters, ++it) {
       const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E);
@@ -322,18 +327,18 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       const int col = c.f_tile * OUT_FEATS + feat0 + (lane & 3) * 8;            // this lane's 8 output columns
       const bool col_ok = col < p.N;                   // N is a multiple of 8
       __nv_bfloat16* out_tile = p.out + static_cast<int64_t>(c.row0) * p.N + col;
+      float sc_next = 1.0f;
       if (!GATEUP) {
-        // gate weights of the tile's tokens -> shared memory, fetched before the accumulator is
-        // awaited so the two dependent loads hide behind the main loop
-        __syncwarp();
-        #pragma unroll
-        for (int i = 0; i < BN_MAX / 32; ++i) {
-          float sc = 1.0f;
-          if (p.row_scale != nullptr && i * 32 + lane < c.rows_valid)
-            sc = __ldg(p.row_scale + __ldg(p.row_src + c.row0 + i * 32 + lane));
-          sc_smem[i * 32 + lane] = sc;
+        // Gate weights (already in expert order: w_perm[r]) of the NEXT tile: warp ew fetches tokens
+        // ew*32 .. +31 now and parks them in the other buffer after this tile's chunks, so the load
+        // latency never sits on the epilogue's critical path.  The barrier makes this tile's buffer
+        // (written by all eight warps at the end of the previous tile) visible.
+        const int tn = t + num_clusters;
+        if (tn < total_tiles && p.row_scale != nullptr) {
+          const TileCoord cn = decode_tile(tn, tile_start, t_tiles, p.offsets, E);
+          if (ew * 32 + lane < cn.rows_valid) sc_next = __ldg(p.row_scale + cn.row0 + ew * 32 + lane);
         }
-        __syncwarp();
+        named_bar_sync(3, 32 * EPI_WARPS);
       }
       mbar_wait(tfull_bar(as), aph);
       tc_fence_after();
@@ -407,7 +412,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
           tmem_ld_wait();
           #pragma unroll
           for (int j = 0; j < 32; j += 4) {
-            const float4 s4 = *reinterpret_cast<const float4*>(sc_smem + cc * 32 + j);   // broadcast
+            const float4 s4 = *reinterpret_cast<const float4*>(sc_smem + (it & 1) * BN_MAX + cc * 32 + j);   // broadcast
             st_shared_bf16(stage_wr + (j + 0) * 64, __uint_as_float(v[j + 0]) * s4.x);
             st_shared_bf16(stage_wr + (j + 1) * 64, __uint_as_float(v[j + 1]) * s4.y);
             st_shared_bf16(stage_wr + (j + 2) * 64, __uint_as_float(v[j + 2]) * s4.z);
@@ -416,6 +421,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
           flush_chunk(cc);
         }
       }
+      if (!GATEUP) sc_smem[((it + 1) & 1) * BN_MAX + ew * 32 + lane] = sc_next;
       // accumulator drained: one arrival per warp on the LEADER's tmem_empty barrier
       tc_fence_before();
       __syncwarp();
@@ -439,8 +445,7 @@ Params make_params(const GemmLaunch& g) {
   p.K = g.K;
   p.N = g.N;
   p.out = static_cast<__nv_bfloat16*>(g.out);
-  p.row_scale = g.row_scale;
-  p.row_src = g.row_src;
+  p.row_scale = g.row_scale_perm;
   p.w4d = g.w4d;
   p.pf_groups = g.w4d ? g.prefetch : 0;
   return p;

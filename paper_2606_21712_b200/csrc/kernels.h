@@ -37,8 +37,9 @@ cudaError_t launch_scan(const int32_t* block_counts, int nblk, int E, int32_t* b
 // topk_idx and offsets).
 cudaError_t launch_block_hist(const int32_t* topk_idx, int T, int E, int k, int32_t* block_counts,
                               cudaStream_t st);
+// topk_w / w_perm may be nullptr; otherwise w_perm[r] = topk_w[row_src[r]] (gate weights in expert order).
 cudaError_t launch_rank(const int32_t* topk_idx, const int32_t* block_base, int T, int E, int k,
-                        int32_t* row_src, int32_t* inv_perm, cudaStream_t st);
+                        int32_t* row_src, int32_t* inv_perm, const float* topk_w, float* w_perm, cudaStream_t st);
 
 // ---- gather / reduce (gather_reduce.cu): steps a6 and a9
 cudaError_t launch_gather(const void* hidden, const int32_t* inv_perm, int T, int k, int d, void* x_perm,
@@ -71,6 +72,7 @@ struct GemmLaunch {
   void* out;           // bf16 [rows, N]
   const float* row_scale;   // down GEMM, fused path: topk_w flat [T*k] (else nullptr)
   const int32_t* row_src;   // down GEMM, fused path: row -> flat index
+  const float* row_scale_perm;   // down GEMM, fused path: the same gate weights in expert order, w_perm[r] = topk_w[row_src[r]]
   int num_sms;
 };
 cudaError_t launch_gateup_swiglu(const GemmLaunch& g, cudaStream_t st);

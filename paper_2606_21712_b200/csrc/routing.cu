@@ -187,7 +187,8 @@ __global__ void __launch_bounds__(1024) scan_kernel(const int32_t* __restrict__ 
 __global__ void __launch_bounds__(RB) rank_kernel(const int32_t* __restrict__ topk_idx,
                                                    const int32_t* __restrict__ block_base, int T, int E, int k,
                                                    int tokens_per_block, int32_t* __restrict__ row_src,
-                                                   int32_t* __restrict__ inv_perm) {
+                                                   int32_t* __restrict__ inv_perm, const float* __restrict__ topk_w,
+                                                   float* __restrict__ w_perm) {
   __shared__ int wcnt[RB / 32][MAX_E];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   for (int i = threadIdx.x; i < (RB / 32) * MAX_E; i += RB) (&wcnt[0][0])[i] = 0;
@@ -209,6 +210,7 @@ __global__ void __launch_bounds__(RB) rank_kernel(const int32_t* __restrict__ to
     const int64_t i = i0 + threadIdx.x;
     row_src[r] = static_cast<int32_t>(i);
     inv_perm[i] = r;
+    if (w_perm != nullptr) w_perm[r] = __ldg(topk_w + i);
   }
 }
 
@@ -246,10 +248,11 @@ cudaError_t launch_scan(const int32_t* block_counts, int nblk, int E, int32_t* b
 }
 
 cudaError_t launch_rank(const int32_t* topk_idx, const int32_t* block_base, int T, int E, int k,
-                        int32_t* row_src, int32_t* inv_perm, cudaStream_t st) {
+                        int32_t* row_src, int32_t* inv_perm, const float* topk_w, float* w_perm,
+                        cudaStream_t st) {
   if (T == 0) return cudaSuccess;
   rank_kernel<<<route_num_blocks(T, k), RB, 0, st>>>(topk_idx, block_base, T, E, k, route_tokens_per_block(k),
-                                                      row_src, inv_perm);
+                                                      row_src, inv_perm, topk_w, w_perm);
   return cudaGetLastError();
 }
 
