@@ -40,8 +40,6 @@ struct bg_moe_ctx {
   void* out_dev = nullptr;
   // weight tensor maps (encoded in set_weights)
   CUtensorMap tm_wg, tm_wu, tm_wd, tm_wr;
-  CUtensorMap tm_wg_pf, tm_wu_pf, tm_wd_pf;   // L2-prefetch boxes (256 k) of the same views
-  int prefetch = 0;             // L2 prefetch distance of the weight stream in 4-k-block groups (BG_MOE_PREFETCH=n; 0 = off)
   CUtensorMap tm_wg4, tm_wu4, tm_wd4;   // 4-D block views (kernels.h GemmLaunch), valid when f % 64 == 0 / d % 64 == 0
   // activation tensor maps of the workspace x_perm / H (whole capacity: rows past T*k are never stored)
   bg::ActMaps am_x, am_h;
@@ -93,12 +91,12 @@ bool encode_act_maps(bg::ActMaps* am, const void* ptr, int64_t rows, int64_t K) 
 }
 
 // [E, K, N] bf16 viewed as [E, N/64, K, 64] (N % 64 == 0), box {64 n, 64 k, nblk blocks, 1 expert}, 128B swizzle.
-bool encode_weight_map_4d(CUtensorMap* tm, const void* ptr, int64_t E, int64_t K, int64_t N, int nblk, int box_k = 64) {
+bool encode_weight_map_4d(CUtensorMap* tm, const void* ptr, int64_t E, int64_t K, int64_t N, int nblk) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return false;
   cuuint64_t dims[4] = {64, static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(N / 64), static_cast<cuuint64_t>(E)};
   cuuint64_t strides[3] = {static_cast<cuuint64_t>(N) * 2, 128, static_cast<cuuint64_t>(N) * K * 2};
-  cuuint32_t box[4] = {64, static_cast<cuuint32_t>(box_k), static_cast<cuuint32_t>(nblk), 1};
+  cuuint32_t box[4] = {64, 64, static_cast<cuuint32_t>(nblk), 1};
   cuuint32_t estr[4] = {1, 1, 1, 1};
   return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(ptr), dims, strides, box, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -203,9 +201,6 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g1.w4d = c.f % 64 == 0;
   g1.tm_b0_4d = g1.w4d ? ctx->tm_wg4 : ctx->tm_wg;
   g1.tm_b1_4d = g1.w4d ? ctx->tm_wu4 : ctx->tm_wu;
-  g1.prefetch = g1.w4d ? ctx->prefetch : 0;
-  g1.tm_pf0 = g1.w4d ? ctx->tm_wg_pf : ctx->tm_wg;
-  g1.tm_pf1 = g1.w4d ? ctx->tm_wu_pf : ctx->tm_wu;
   g1.offsets = offsets;
   g1.E = c.E; g1.K = c.d; g1.N = c.f;
   g1.out = ctx->H;
@@ -221,9 +216,6 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g2.w4d = c.d % 64 == 0;
   g2.tm_b0_4d = g2.w4d ? ctx->tm_wd4 : ctx->tm_wd;
   g2.tm_b1_4d = g2.tm_b0_4d;
-  g2.prefetch = g2.w4d ? ctx->prefetch : 0;
-  g2.tm_pf0 = g2.w4d ? ctx->tm_wd_pf : ctx->tm_wd;
-  g2.tm_pf1 = g2.tm_pf0;
   g2.offsets = offsets;
   g2.E = c.E; g2.K = c.f; g2.N = c.d;
   g2.out = y;
@@ -325,8 +317,6 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   {
     const char* g = std::getenv("BG_MOE_GEMM");
     if (g != nullptr && std::strcmp(g, "tile") == 0) ctx->pair_gemm = false;
-    const char* pf = std::getenv("BG_MOE_PREFETCH");
-    if (pf != nullptr) ctx->prefetch = std::atoi(pf) < 0 ? 0 : std::atoi(pf);
   }
   *out = ctx;
   return BG_OK;
@@ -359,12 +349,6 @@ int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, cons
                            !encode_weight_map_4d(&ctx->tm_wu4, W_up, c.E, c.d, c.f, nb_gu))) ||
         (c.d % 64 == 0 && !encode_weight_map_4d(&ctx->tm_wd4, W_down, c.E, c.f, c.d, nb_d))) {
       ctx->last_error = "cuTensorMapEncodeTiled(weight block views) failed";
-      return BG_ERR_CUDA;
-    }
-    if ((c.f % 64 == 0 && (!encode_weight_map_4d(&ctx->tm_wg_pf, W_gate, c.E, c.d, c.f, nb_gu, 256) ||
-                           !encode_weight_map_4d(&ctx->tm_wu_pf, W_up, c.E, c.d, c.f, nb_gu, 256))) ||
-        (c.d % 64 == 0 && !encode_weight_map_4d(&ctx->tm_wd_pf, W_down, c.E, c.f, c.d, nb_d, 256))) {
-      ctx->last_error = "cuTensorMapEncodeTiled(weight prefetch views) failed";
       return BG_ERR_CUDA;
     }
   }

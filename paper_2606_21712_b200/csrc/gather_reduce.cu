@@ -6,6 +6,7 @@
 // One warp moves one row at a time; consecutive lanes touch consecutive 16-byte vectors, several
 // vectors in flight per lane.  Grid = a multiple of the SM count, warps stride over rows.
 #include "kernels.h"
+#include "ptx_sm100.cuh"
 #include <cuda_bf16.h>
 
 namespace bg {
@@ -30,6 +31,7 @@ template <int KMAX>
 __global__ void __launch_bounds__(256) gather_kernel(const uint4* __restrict__ hidden,
                                                      const int32_t* __restrict__ inv_perm, int T, int k,
                                                      int vec_per_row, uint4* __restrict__ x_perm) {
+  pdl_wait_then_trigger();
   const int lane = threadIdx.x & 31;
   const int warps_total = gridDim.x * (blockDim.x >> 5);
   for (int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); t < T; t += warps_total) {
@@ -75,6 +77,7 @@ __global__ void __launch_bounds__(256) unpermute_kernel(const uint4* __restrict_
                                                         const int32_t* __restrict__ inv_perm,
                                                         const float* __restrict__ weights, int T, int k,
                                                         int vec_per_row, uint4* __restrict__ out) {
+  pdl_wait_then_trigger();
   const int lane = threadIdx.x & 31;
   const int warps_total = gridDim.x * (blockDim.x >> 5);
   for (int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); t < T; t += warps_total) {
@@ -125,13 +128,13 @@ cudaError_t launch_gather(const void* hidden, const int32_t* inv_perm, int T, in
   if (T == 0) return cudaSuccess;
   const int grid = row_mover_grid(T, num_sms);
   if (k <= 2)
-    gather_kernel<2><<<grid, 256, 0, st>>>(static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
+    launch_pdl(gather_kernel<2>, grid, 256, 0, st, static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
                                            static_cast<uint4*>(x_perm));
   else if (k <= 4)
-    gather_kernel<4><<<grid, 256, 0, st>>>(static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
+    launch_pdl(gather_kernel<4>, grid, 256, 0, st, static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
                                            static_cast<uint4*>(x_perm));
   else
-    gather_kernel<8><<<grid, 256, 0, st>>>(static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
+    launch_pdl(gather_kernel<8>, grid, 256, 0, st, static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
                                            static_cast<uint4*>(x_perm));
   return cudaGetLastError();
 }
@@ -141,13 +144,13 @@ cudaError_t launch_unpermute(const void* y_perm, const int32_t* inv_perm, const 
   if (T == 0) return cudaSuccess;
   const int grid = row_mover_grid(T, num_sms);
   if (k <= 2)
-    unpermute_kernel<2><<<grid, 256, 0, st>>>(static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
+    launch_pdl(unpermute_kernel<2>, grid, 256, 0, st, static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
                                               static_cast<uint4*>(out));
   else if (k <= 4)
-    unpermute_kernel<4><<<grid, 256, 0, st>>>(static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
+    launch_pdl(unpermute_kernel<4>, grid, 256, 0, st, static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
                                               static_cast<uint4*>(out));
   else
-    unpermute_kernel<8><<<grid, 256, 0, st>>>(static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
+    launch_pdl(unpermute_kernel<8>, grid, 256, 0, st, static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
                                               static_cast<uint4*>(out));
   return cudaGetLastError();
 }

@@ -125,6 +125,7 @@ grouped_gemm_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_const
   const int n_tiles = (p.N + OUT_COLS - 1) / OUT_COLS;
   const int k_blocks = (p.K + BK - 1) / BK;
 
+  pdl_wait_then_trigger();
   // ---- per-CTA tile table: inclusive scan of per-expert tile counts (E <= 256 = blockDim)
   {
     int mt = 0;
@@ -344,12 +345,12 @@ cudaError_t gemm_kernels_init() {
 }
 
 cudaError_t launch_gateup_swiglu(const GemmLaunch& g, cudaStream_t st) {
-  grouped_gemm_kernel<true><<<g.num_sms, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_act.m[15], g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b1_4d : g.tm_b1, make_params(g));
+  launch_pdl(grouped_gemm_kernel<true>, g.num_sms, NUM_THREADS, SMEM_BYTES, st, g.tm_act.m[15], g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b1_4d : g.tm_b1, make_params(g));
   return cudaGetLastError();
 }
 
 cudaError_t launch_down(const GemmLaunch& g, cudaStream_t st) {
-  grouped_gemm_kernel<false><<<g.num_sms, NUM_THREADS, SMEM_BYTES, st>>>(g.tm_act.m[15], g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b0_4d : g.tm_b0, make_params(g));
+  launch_pdl(grouped_gemm_kernel<false>, g.num_sms, NUM_THREADS, SMEM_BYTES, st, g.tm_act.m[15], g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b0_4d : g.tm_b0, make_params(g));
   return cudaGetLastError();
 }
 

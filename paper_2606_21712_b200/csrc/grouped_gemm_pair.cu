@@ -82,7 +82,6 @@ struct Params {
   __nv_bfloat16* out;
   const float* row_scale;      // a8, fused path: gate weight per expert-order row (w_perm[r]); nullptr = 1
   bool w4d;                    // tm_w0 / tm_w1 are the 4-D block views (kernels.h)
-  int pf_groups;               // > 0: tm_pf0 / tm_pf1 are valid, L2-prefetch this many 4-k-block groups ahead
 };
 
 __device__ __forceinline__ void named_bar_sync(int id, int threads) {
@@ -141,8 +140,7 @@ __device__ __forceinline__ void st_shared_bf16(uint32_t addr, float v) {
 template <bool GATEUP>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GATEUP ? 256 : 384, 1)
 pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__ CUtensorMap tm_w0,
-                 const __grid_constant__ CUtensorMap tm_w1, const __grid_constant__ CUtensorMap tm_pf0,
-                 const __grid_constant__ CUtensorMap tm_pf1, const Params p) {
+                 const __grid_constant__ CUtensorMap tm_w1, const Params p) {
   constexpr int CTA_FEATS = GATEUP ? 64 : 128;       // output features per CTA and tile
   constexpr int OUT_FEATS = 2 * CTA_FEATS;           // output features per pair tile
   // a8 has short k loops (K = f), so its epilogue gets two warps per TMEM lane quarter
@@ -169,8 +167,22 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   const int E = p.E;
   const int f_tiles = (p.N + OUT_FEATS - 1) / OUT_FEATS;
   const int k_blocks = (p.K + BK - 1) / BK;
-  const int k_groups = (k_blocks + 3) >> 2;          // 4-k-block groups (L2 prefetch granularity)
 
+  // ---- independent of the previous kernel: barriers and TMEM
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tm_w0);
+    if (GATEUP) tma_prefetch_desc(&tm_w1);
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    // tmem_empty (used on the leader only): one arrival per epilogue warp of both CTAs
+    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 2 * EPI_WARPS); }
+    fence_barrier_init();
+  }
+  if (warp == 2) {
+    tmem_alloc_pair(smem_u32(tmem_slot), 512);
+    tmem_relinquish_pair();
+  }
+  // ---- everything below reads what the previous kernels wrote (offsets, activations)
+  pdl_wait_then_trigger();
   // ---- per-CTA tile table: inclusive scan of per-expert tile counts (E <= 256 = blockDim)
   {
     int tt = 0;
@@ -195,18 +207,6 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     if (threadIdx.x == 0) tile_start[0] = 0;
   }
 
-  if (warp == 0 && lane == 0) {
-    tma_prefetch_desc(&tm_w0);
-    if (GATEUP) tma_prefetch_desc(&tm_w1);
-    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    // tmem_empty (used on the leader only): one arrival per epilogue warp of both CTAs
-    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 2 * EPI_WARPS); }
-    fence_barrier_init();
-  }
-  if (warp == 2) {
-    tmem_alloc_pair(smem_u32(tmem_slot), 512);
-    tmem_relinquish_pair();
-  }
   tc_fence_before();
   __syncthreads();
   cluster_sync_all();                                 // the peer's barriers are initialised, its TMEM allocated
@@ -227,23 +227,6 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         const uint32_t tx_pair = 2u * (A_BYTES + static_cast<uint32_t>(half) * (BK * 2));
         const CUtensorMap* tm_b = &tm_act.m[(half >> 3) - 1];
         for (int kb = 0; kb < k_blocks; ++kb) {
-          // L2 prefetch of the weight stream pf_groups x 4 k-blocks ahead of the ring (one 4-k-block
-          // box per operation): HBM keeps streaming while the ring is full of landed data, and the
-          // ring's own loads then see L2 latency.  Only the first token tile of a strip prefetches
-          // it (the other token tiles run at the same time and hit L2).  The distance is bounded so
-          // that the prefetched-but-unused bytes of all CTAs stay well inside L2.
-          if (p.pf_groups > 0 && (kb & 3) == 0) {
-            int gg = (kb >> 2) + p.pf_groups, tt = t;
-            while (gg >= k_groups) { gg -= k_groups; tt += num_clusters; }
-            if (tt < total_tiles) {
-              const TileCoord c2 = (tt == t) ? c : decode_tile(tt, tile_start, t_tiles, p.offsets, E);
-              if (c2.t_tile == 0) {
-                const int pn = (c2.f_tile * OUT_FEATS + static_cast<int>(rank) * CTA_FEATS) >> 6;
-                tma_prefetch_l2_4d(&tm_pf0, 0, gg * 4 * BK, pn, c2.e);
-                if (GATEUP) tma_prefetch_l2_4d(&tm_pf1, 0, gg * 4 * BK, pn, c2.e);
-              }
-            }
-          }
           mbar_wait(empty_bar(s), ph ^ 1u);            // this CTA's slot is free (multicast commit)
           const uint32_t sa = base + s * STAGE_BYTES;
           const uint32_t sb = sa + A_BYTES;
@@ -447,7 +430,6 @@ Params make_params(const GemmLaunch& g) {
   p.out = static_cast<__nv_bfloat16*>(g.out);
   p.row_scale = g.row_scale_perm;
   p.w4d = g.w4d;
-  p.pf_groups = g.w4d ? g.prefetch : 0;
   return p;
 }
 
@@ -460,12 +442,12 @@ cudaError_t pair_kernels_init() {
 }
 
 cudaError_t launch_gateup_swiglu_pair(const GemmLaunch& g, cudaStream_t st) {
-  pair_gemm_kernel<true><<<g.num_sms & ~1, 256, SMEM_BYTES, st>>>(g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b1_4d : g.tm_b1, g.tm_pf0, g.tm_pf1, make_params(g));
+  launch_pdl(pair_gemm_kernel<true>, g.num_sms & ~1, 256, SMEM_BYTES, st, g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b1_4d : g.tm_b1, make_params(g));
   return cudaGetLastError();
 }
 
 cudaError_t launch_down_pair(const GemmLaunch& g, cudaStream_t st) {
-  pair_gemm_kernel<false><<<g.num_sms & ~1, 384, SMEM_BYTES, st>>>(g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b0_4d : g.tm_b0, g.tm_pf0, g.tm_pf0, make_params(g));
+  launch_pdl(pair_gemm_kernel<false>, g.num_sms & ~1, 384, SMEM_BYTES, st, g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b0_4d : g.tm_b0, make_params(g));
   return cudaGetLastError();
 }
 

@@ -7,6 +7,26 @@
 
 namespace bg {
 
+// Launch with programmatic stream serialization (PDL): the kernel may begin before the previous
+// kernel on the stream has finished; each kernel calls pdl_wait_then_trigger() (ptx_sm100.cuh)
+// before it touches anything its predecessor wrote.  Hides launch latency and prologues between
+// the eight kernels of the fused chain.
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                              Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 // ---- router logits on tensor cores (router_gemm.cu): step a1
 cudaError_t router_kernels_init();
 // pieces: bf16 [3][d][round_up(E,16)] = exact hi/mid/lo split of W_r (zero padded)
@@ -64,9 +84,6 @@ struct GemmLaunch {
   // Valid only when N % 64 == 0 (w4d); otherwise the kernels issue one 3-D box per block.
   CUtensorMap tm_b0_4d, tm_b1_4d;
   bool w4d;
-  // Pair kernel: the same view with box {64 n, 256 k, nblk, 1} for L2 prefetch of the next tile's strip.
-  CUtensorMap tm_pf0, tm_pf1;
-  int prefetch;        // prefetch distance in 4-k-block groups (0 = off)
   const int32_t* offsets;  // [E+1]
   int E, K, N;         // N = output columns (f for gate/up, d for down)
   void* out;           // bf16 [rows, N]

@@ -64,6 +64,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_consta
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int m_tile = blockIdx.x, ks = blockIdx.y;
+  pdl_wait_then_trigger();
   {  // zero the per-block expert histogram that the top-k kernel (next in the stream) accumulates into
     const int n_cta = gridDim.x * gridDim.y, cta = blockIdx.y * gridDim.x + blockIdx.x;
     const int per = (zero_n + n_cta - 1) / n_cta;
@@ -186,7 +187,7 @@ cudaError_t launch_router_gemm(const CUtensorMap& tm_h, const CUtensorMap& tm_w,
                                float* partial, int32_t* zero_buf, int zero_n, cudaStream_t st) {
   if (T == 0) return cudaSuccess;
   dim3 grid((T + BM - 1) / BM, ksplit);
-  router_gemm_kernel<<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tm_h, tm_w, T, d, E, ksplit, partial, zero_buf, zero_n);
+  launch_pdl(router_gemm_kernel, grid, NUM_THREADS, SMEM_BYTES, st, tm_h, tm_w, T, d, E, ksplit, partial, zero_buf, zero_n);
   return cudaGetLastError();
 }
 

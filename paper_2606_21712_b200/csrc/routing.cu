@@ -10,6 +10,7 @@
 // exclusive scan, a token permutation into expert-contiguous rows"; "ties broken by the lower
 // expert index"; routing artefacts bit-exact given the same fp32 logits.
 #include "kernels.h"
+#include "ptx_sm100.cuh"
 #include <cuda_bf16.h>
 #include <math_constants.h>
 
@@ -44,6 +45,7 @@ __global__ void __launch_bounds__(256) topk_hist_kernel(const float* __restrict_
                                                         int tokens_per_block, int32_t* __restrict__ topk_idx,
                                                         float* __restrict__ topk_w,
                                                         int32_t* __restrict__ block_counts) {
+  pdl_wait_then_trigger();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int t = blockIdx.x * 8 + warp;
   if (t >= T) return;
@@ -111,6 +113,7 @@ __global__ void __launch_bounds__(256) topk_hist_kernel(const float* __restrict_
 __global__ void __launch_bounds__(RB) block_hist_kernel(const int32_t* __restrict__ topk_idx, int T, int E, int k,
                                                          int tokens_per_block,
                                                          int32_t* __restrict__ block_counts) {
+  pdl_wait_then_trigger();
   __shared__ int hist[MAX_E];
   for (int e = threadIdx.x; e < E; e += RB) hist[e] = 0;
   __syncthreads();
@@ -131,6 +134,7 @@ __global__ void __launch_bounds__(RB) block_hist_kernel(const int32_t* __restric
 __global__ void __launch_bounds__(1024) scan_kernel(const int32_t* __restrict__ block_counts, int nblk, int E,
                                                     int32_t* __restrict__ block_base,
                                                     int32_t* __restrict__ counts, int32_t* __restrict__ offsets) {
+  pdl_wait_then_trigger();
   __shared__ int gtot[4][MAX_E];
   __shared__ int excl_e[MAX_E];
   __shared__ int warp_tot[8];
@@ -189,6 +193,7 @@ __global__ void __launch_bounds__(RB) rank_kernel(const int32_t* __restrict__ to
                                                    int tokens_per_block, int32_t* __restrict__ row_src,
                                                    int32_t* __restrict__ inv_perm, const float* __restrict__ topk_w,
                                                    float* __restrict__ w_perm) {
+  pdl_wait_then_trigger();
   __shared__ int wcnt[RB / 32][MAX_E];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   for (int i = threadIdx.x; i < (RB / 32) * MAX_E; i += RB) (&wcnt[0][0])[i] = 0;
@@ -221,7 +226,7 @@ cudaError_t launch_topk_hist(const float* src, int n_src, const float* b_r, floa
   if (T == 0) return cudaSuccess;
   const int tb = route_tokens_per_block(k);
   const int ne = (E + 31) / 32;
-#define BG_TOPK(NE_) topk_hist_kernel<NE_><<<(T + 7) / 8, 256, 0, st>>>(src, n_src, b_r, logits_out, T, E, k, tb, \
+#define BG_TOPK(NE_) launch_pdl(topk_hist_kernel<NE_>, (T + 7) / 8, 256, 0, st, src, n_src, b_r, logits_out, T, E, k, tb, \
                                                                        topk_idx, topk_w, block_counts)
   switch (ne) {
     case 1: BG_TOPK(1); break;
@@ -236,14 +241,14 @@ cudaError_t launch_topk_hist(const float* src, int n_src, const float* b_r, floa
 cudaError_t launch_block_hist(const int32_t* topk_idx, int T, int E, int k, int32_t* block_counts,
                               cudaStream_t st) {
   if (T == 0) return cudaSuccess;
-  block_hist_kernel<<<route_num_blocks(T, k), RB, 0, st>>>(topk_idx, T, E, k, route_tokens_per_block(k),
+  launch_pdl(block_hist_kernel, route_num_blocks(T, k), RB, 0, st, topk_idx, T, E, k, route_tokens_per_block(k),
                                                             block_counts);
   return cudaGetLastError();
 }
 
 cudaError_t launch_scan(const int32_t* block_counts, int nblk, int E, int32_t* block_base, int32_t* counts,
                         int32_t* offsets, cudaStream_t st) {
-  scan_kernel<<<1, 1024, 0, st>>>(block_counts, nblk, E, block_base, counts, offsets);
+  launch_pdl(scan_kernel, 1, 1024, 0, st, block_counts, nblk, E, block_base, counts, offsets);
   return cudaGetLastError();
 }
 
@@ -251,7 +256,7 @@ cudaError_t launch_rank(const int32_t* topk_idx, const int32_t* block_base, int 
                         int32_t* row_src, int32_t* inv_perm, const float* topk_w, float* w_perm,
                         cudaStream_t st) {
   if (T == 0) return cudaSuccess;
-  rank_kernel<<<route_num_blocks(T, k), RB, 0, st>>>(topk_idx, block_base, T, E, k, route_tokens_per_block(k),
+  launch_pdl(rank_kernel, route_num_blocks(T, k), RB, 0, st, topk_idx, block_base, T, E, k, route_tokens_per_block(k),
                                                       row_src, inv_perm, topk_w, w_perm);
   return cudaGetLastError();
 }
