@@ -43,6 +43,7 @@ struct bg_moe_ctx {
   CUtensorMap tm_wg4, tm_wu4, tm_wd4;   // 4-D block views (kernels.h GemmLaunch), valid when f % 64 == 0 / d % 64 == 0
   // activation tensor maps of the workspace x_perm / H (whole capacity: rows past T*k are never stored)
   bg::ActMaps am_x, am_h;
+  int sg_max = 0;               // BG_MOE_SG_TOKEN_TILES=n overrides the pair kernel's super-group size (tests)
   bool pair_gemm = true;        // CTA-pair grouped GEMM (BG_MOE_GEMM=tile selects the 1-CTA 128x256 kernel)
   int64_t launches = 0;
   std::string last_error;
@@ -198,6 +199,7 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   }
   g1.tm_b0 = ctx->tm_wg;
   g1.tm_b1 = ctx->tm_wu;
+  g1.sg_max = ctx->sg_max;
   g1.w4d = c.f % 64 == 0;
   g1.tm_b0_4d = g1.w4d ? ctx->tm_wg4 : ctx->tm_wg;
   g1.tm_b1_4d = g1.w4d ? ctx->tm_wu4 : ctx->tm_wu;
@@ -213,6 +215,7 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g2.tm_act = ctx->am_h;
   g2.tm_b0 = ctx->tm_wd;
   g2.tm_b1 = ctx->tm_wd;
+  g2.sg_max = ctx->sg_max;
   g2.w4d = c.d % 64 == 0;
   g2.tm_b0_4d = g2.w4d ? ctx->tm_wd4 : ctx->tm_wd;
   g2.tm_b1_4d = g2.tm_b0_4d;
@@ -317,6 +320,8 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   {
     const char* g = std::getenv("BG_MOE_GEMM");
     if (g != nullptr && std::strcmp(g, "tile") == 0) ctx->pair_gemm = false;
+    const char* sg = std::getenv("BG_MOE_SG_TOKEN_TILES");
+    if (sg != nullptr && std::atoi(sg) > 0) ctx->sg_max = std::atoi(sg);
   }
   *out = ctx;
   return BG_OK;

@@ -82,6 +82,7 @@ struct Params {
   __nv_bfloat16* out;
   const float* row_scale;      // a8, fused path: gate weight per expert-order row (w_perm[r]); nullptr = 1
   bool w4d;                    // tm_w0 / tm_w1 are the 4-D block views (kernels.h)
+  int sg_max;                  // 0 = derive the super-group size from K
 };
 
 __device__ __forceinline__ void named_bar_sync(int id, int threads) {
@@ -94,8 +95,14 @@ struct TileCoord {
 
 // tile_start[e] = first linear tile index of expert e (tile_start[E] = total);
 // t_tiles[e] = token tiles of expert e.  Both live in shared memory.
+// Inside an expert the order is feature-tile-major / token-tile-minor, so the token tiles that share a
+// weight strip run at the same time.  When an expert's token matrix is too large to stay in L2 between
+// two feature tiles (DeepSeek-shaped hot experts: thousands of rows x 14 KB), that order re-streams the
+// tokens from HBM once per feature tile; such experts are cut into super-groups of `sg_max` token tiles
+// (sized to ~48 MB of tokens) and each super-group runs through all feature tiles before the next starts:
+// the tokens stay in L2 and the expert's weights are streamed once per super-group instead.
 __device__ __forceinline__ TileCoord decode_tile(int t, const int* tile_start, const int* t_tiles,
-                                                 const int32_t* offsets, int E) {
+                                                 const int32_t* offsets, int E, int sg_max) {
   int lo = 0, hi = E;              // largest e with tile_start[e] <= t
   while (hi - lo > 1) {
     const int mid = (lo + hi) >> 1;
@@ -106,8 +113,21 @@ __device__ __forceinline__ TileCoord decode_tile(int t, const int* tile_start, c
   const int e = lo;
   const int local = t - tile_start[e];
   const int tt = t_tiles[e];
-  const int f_tile = local / tt;
-  const int t_tile = local - f_tile * tt;
+  int f_tile, t_tile;
+  if (tt <= sg_max) {
+    f_tile = local / tt;
+    t_tile = local - f_tile * tt;
+  } else {
+    const int f_tiles = (tile_start[e + 1] - tile_start[e]) / tt;
+    const int n_sg = (tt + sg_max - 1) / sg_max;
+    const int g = (tt + n_sg - 1) / n_sg;             // balanced super-group size; the last may be smaller
+    const int per_sg = g * f_tiles;
+    const int sg = local / per_sg;
+    const int r = local - sg * per_sg;
+    const int g_here = min(g, tt - sg * g);
+    f_tile = r / g_here;
+    t_tile = sg * g + (r - f_tile * g_here);
+  }
   const int beg = __ldg(offsets + e), end = __ldg(offsets + e + 1);
   const int n_e = end - beg;
   const int base = (((n_e + tt - 1) / tt) + 15) & ~15;      // rows per token tile, multiple of 16, <= 256
@@ -167,6 +187,8 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   const int E = p.E;
   const int f_tiles = (p.N + OUT_FEATS - 1) / OUT_FEATS;
   const int k_blocks = (p.K + BK - 1) / BK;
+  // token tiles whose rows fit ~48 MB of L2 (p.sg_max > 0: override, used by the tests to reach this path on small shapes)
+  const int sg_max = p.sg_max > 0 ? p.sg_max : max(1, (48 << 20) / (BN_MAX * 2 * p.K));
 
   // ---- independent of the previous kernel: barriers and TMEM
   if (warp == 0 && lane == 0) {
@@ -220,7 +242,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       int s = 0;
       uint32_t ph = 0;
       for (int t = cluster_id; t < total_tiles; t += num_clusters) {
-        const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E);
+        const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
         const int n0 = c.f_tile * OUT_FEATS + static_cast<int>(rank) * CTA_FEATS;
         const int half = c.nt >> 1;                    // this CTA's tokens (multiple of 8, <= 128)
         const int brow0 = c.row0 + static_cast<int>(rank) * half;
@@ -256,7 +278,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       uint32_t ph = 0;
       int it = 0;
       for (int t = cluster_id; t < total_tiles; t += num_clusters, ++it) {
-        const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E);
+        const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
         const uint32_t idesc = IDESC_BASE | (static_cast<uint32_t>(c.nt >> 3) << 17);
         const int as = it & 1;
         const uint32_t aph = (it >> 1) & 1u;
@@ -296,14 +318,14 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     float* sc_smem = reinterpret_cast<float*>(epi_smem);                        // a8: [2][BN_MAX] gate weights, double-buffered
     const int feat0 = static_cast<int>(rank) * CTA_FEATS + (GATEUP ? (q & 1) : q) * 32;   // in the pair tile
     if (!GATEUP && cluster_id < total_tiles) {       // gate weights of the first tile -> buffer 0
-      const TileCoord c0 = decode_tile(cluster_id, tile_start, t_tiles, p.offsets, E);
+      const TileCoord c0 = decode_tile(cluster_id, tile_start, t_tiles, p.offsets, E, sg_max);
       float sc = 1.0f;
       if (p.row_scale != nullptr && ew * 32 + lane < c0.rows_valid) sc = __ldg(p.row_scale + c0.row0 + ew * 32 + lane);
       sc_smem[ew * 32 + lane] = sc;
     }
     int it = 0;
     for (int t = cluster_id; t < total_tiles; t += num_clusters, ++it) {
-      const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E);
+      const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1u;
       const int n_chunks = (c.nt + 31) >> 5;           // 32-token chunks (the last may be half used)
@@ -318,7 +340,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         // (written by all eight warps at the end of the previous tile) visible.
         const int tn = t + num_clusters;
         if (tn < total_tiles && p.row_scale != nullptr) {
-          const TileCoord cn = decode_tile(tn, tile_start, t_tiles, p.offsets, E);
+          const TileCoord cn = decode_tile(tn, tile_start, t_tiles, p.offsets, E, sg_max);
           if (ew * 32 + lane < cn.rows_valid) sc_next = __ldg(p.row_scale + cn.row0 + ew * 32 + lane);
         }
         named_bar_sync(3, 32 * EPI_WARPS);
@@ -430,6 +452,7 @@ Params make_params(const GemmLaunch& g) {
   p.out = static_cast<__nv_bfloat16*>(g.out);
   p.row_scale = g.row_scale_perm;
   p.w4d = g.w4d;
+  p.sg_max = g.sg_max;
   return p;
 }
 

@@ -152,6 +152,29 @@ def test_expert_ffn_parity(rows, d, f):
             check_out(y[offsets[e]:offsets[e + 1]], ref[offsets[e]:offsets[e + 1]], f"expert {e}")
 
 
+@pytest.mark.parametrize("env", [{"BG_MOE_SG_TOKEN_TILES": "2"}, {"BG_MOE_SG_TOKEN_TILES": "1"}, {"BG_MOE_GEMM": "tile"}],
+                         ids=["supergroups-of-2", "supergroups-of-1", "tile-kernel"])
+def test_expert_ffn_scheduler_variants(env, monkeypatch):
+    """The same FFN through (i) the pair kernel's super-group tile order, which production shapes only
+    reach with experts of several thousand rows (forced here on experts of 3-5 token tiles), and (ii) the
+    1-CTA 128x256 kernel that BG_MOE_GEMM=tile selects."""
+    for k_, v in env.items():
+        monkeypatch.setenv(k_, v)              # read once, in bg_moe_create
+    rows = [1300, 0, 700, 257, 16, 1]
+    d, f = 192, 320
+    E, R = len(rows), sum(rows)
+    cfg = wl.MoEConfig("ffn-sched", 15, T=R, d=d, E=E, k=1, f=f)
+    lay, g, layer = make(cfg)
+    offsets = np.concatenate([[0], np.cumsum(rows)]).astype(np.int32)
+    y = layer.expert_ffn(g["hidden"], torch.from_numpy(offsets).cuda(), T=R)
+    torch.cuda.synchronize()
+    ref = oracle.expert_ffn(lay["hidden"], offsets, lay["W_gate"], lay["W_up"], lay["W_down"])
+    check_out(y, ref, f"expert_ffn {env}")
+    for e in range(E):
+        if rows[e]:
+            check_out(y[offsets[e]:offsets[e + 1]], ref[offsets[e]:offsets[e + 1]], f"expert {e} {env}")
+
+
 def test_unpermute_parity():
     T, k, d, E = 257, 3, 136, 7
     rng = np.random.default_rng(4)
