@@ -174,6 +174,52 @@ def whole_job_rate(units_per_rank: float, world: int, ms: float) -> float:
     return units_per_rank * world / (ms * 1e-3)
 
 
+# ----------------------------------------------------------------------------- C3 combine-size sweep
+C3_SWEEP_T = (64, 256, 1024, 4096, 16384, 32768)
+
+
+def run_c3_sweep(steps: int, peaks: dict, device_index: int):
+    """BASELINE.json configs[2]: the fine-grained layer at T in {64 .. 32768} combined tokens -- the
+    'throughput against combined-token count T' half of the metric.  Same fused chain, same timing
+    protocol as the headline line (CUDA events on the launching stream, warm-up, weights >> L2)."""
+    from paper_2606_21712_b200 import MoELayer
+    cfg_max = wl.CONFIGS["C3"].with_T(max(C3_SWEEP_T))
+    lay = wl.make_layer(cfg_max, "cuda")
+    layer = MoELayer(cfg_max.d, cfg_max.f, cfg_max.E, cfg_max.k, cfg_max.T, device=device_index)
+    layer.set_weights(lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"])
+    stream = torch.cuda.current_stream()
+    rows = []
+    for T in C3_SWEEP_T:
+        cfg = cfg_max.with_T(T)
+        hidden = lay["hidden"][:T].contiguous()
+        out = torch.empty_like(hidden)
+        # The part is power-managed: after a tensor-bound burst the clocks stay low for a few hundred
+        # ms (measured: the T=64 point reads 0.30 ms right after the C2 run, 0.225 ms after 1 s idle).
+        # The sweep points are independent workloads, so each starts from an idle GPU.
+        torch.cuda.synchronize()
+        time.sleep(1.0)
+        for _ in range(5):
+            layer.combined_forward(hidden, out, stream)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            layer.combined_forward(hidden, out, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        counts = layer.debug_views(T)["counts"].cpu().numpy()
+        E_act = int((counts > 0).sum())
+        F, B = cfg.flops(), cfg.min_bytes(E_act)
+        t_roof = max(F / (peaks["bf16_tflops"] * 1e12), B / (peaks["hbm_gbs"] * 1e9))
+        rows.append({"T": T, "ms_per_step": ms, "tflops": F / (ms * 1e-3) / 1e12, "tokens_per_s": T / (ms * 1e-3),
+                     "E_active": E_act, "bound": "tensor" if F / (peaks["bf16_tflops"] * 1e12) >= B / (peaks["hbm_gbs"] * 1e9)
+                     else "hbm", "frac_of_measured_burst": t_roof / (ms * 1e-3)})
+    del layer, lay
+    torch.cuda.empty_cache()
+    return rows
+
+
 # ----------------------------------------------------------------------------- our arm
 def run_ours(args):
     from paper_2606_21712_b200 import MoELayer
@@ -303,6 +349,8 @@ def run_ours(args):
         "clocks": clocks,
     }
 
+    if rank == 0 and world == 1 and not args.no_sweep:
+        line["sweep_c3"] = run_c3_sweep(args.steps, peaks, local)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
         cores = oracle.num_threads()
@@ -329,6 +377,7 @@ def main():
     ap.add_argument("--config", default="C2", choices=sorted(wl.CONFIGS))
     ap.add_argument("--T", type=int, default=0, help="override the combined-token count (C3 sweep)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the C3 combine-size sweep (sweep_c3 key)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
