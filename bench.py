@@ -46,6 +46,20 @@ def load_peaks():
     return dict(FALLBACK_PEAKS), "fallback"
 
 
+def load_traffic(cfg_key: str, kernel: str):
+    """DRAM bytes per launch of `kernel` from the committed `ncu --set full` capture of this configuration
+    (profiles/r01_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum), or None if there is none."""
+    p = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+    try:
+        for ln in open(p).read().splitlines()[1:]:
+            c, k, rd, wr = ln.split(",")
+            if c == cfg_key and k == kernel:
+                return float(rd) + float(wr)
+    except Exception:
+        pass
+    return None
+
+
 def get_config(args) -> wl.MoEConfig:
     cfg = wl.CONFIGS[args.config]
     if args.T:
@@ -323,7 +337,10 @@ def run_ours(args):
     else:
         achieved, peak, unit = work / dom_s / 1e12, 148 * 128 * 2 * 1.965e9 / 1e12, "TFLOP/s"
     roofline = {"kernel": dom, "bound": bound, "achieved": achieved, "peak": peak, "unit": unit,
-                "frac": achieved / peak, "traffic": None, "peak_source": f"{peak_src} (burst)",
+                "frac": achieved / peak,
+                "traffic": load_traffic(args.config + (f"@{args.T}" if args.T else ""), dom),
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01_traffic.csv)",
+                "algorithmic_work": work, "peak_source": f"{peak_src} (burst)",
                 "ms_per_launch": stage_ms[dom], "share_of_step": stage_ms[dom] / sum(stage_ms.values())}
 
     line = {
