@@ -39,7 +39,7 @@ struct bg_moe_ctx {
   void* hidden_dev = nullptr;   // staging for the host-pointer entry point
   void* out_dev = nullptr;
   // weight tensor maps (encoded in set_weights)
-  CUtensorMap tm_wg, tm_wu, tm_wd, tm_wr;
+  CUtensorMap tm_wg, tm_wu, tm_wd, tm_wr, tm_wr1;   // tm_wr1: one-piece box of the 4-D W_r view (E > 128)
   CUtensorMap tm_wg4, tm_wu4, tm_wd4;   // 4-D block views (kernels.h GemmLaunch), valid when f % 64 == 0 / d % 64 == 0
   // activation tensor maps of the workspace x_perm / H (whole capacity: rows past T*k are never stored)
   bg::ActMaps am_x, am_h;
@@ -169,7 +169,7 @@ int do_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits
     if (!encode_act_map(&tm_h, hidden, T, c.d)) { ctx->last_error = "cuTensorMapEncodeTiled(hidden) failed"; return BG_ERR_CUDA; }
     const int ks = bg::router_ksplit(T, c.d, ctx->num_sms);
     mark(ctx, 0, st);
-    BG_LAUNCH(ctx, bg::launch_router_gemm(tm_h, ctx->tm_wr, T, c.d, c.E, ks, ctx->partial, ctx->block_counts,
+    BG_LAUNCH(ctx, bg::launch_router_gemm(tm_h, ctx->tm_wr, ctx->tm_wr1, T, c.d, c.E, ks, ctx->partial, ctx->block_counts,
                                           bg::route_num_blocks(T, c.k) * c.E, st), "router_gemm");
     mark(ctx, 1, st);
     BG_LAUNCH(ctx, bg::launch_topk_hist(ctx->partial, ks, ctx->b_r, logits_buf, T, c.E, c.k, topk_idx, topk_w,
@@ -362,13 +362,33 @@ int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, cons
     DeviceGuard guard(c.device);
     const int64_t E_ld = (c.E + 15) & ~15;
     EncodeTiledFn fn = get_encode_fn();
-    cuuint64_t dims[3] = {static_cast<cuuint64_t>(E_ld), static_cast<cuuint64_t>(c.d), 3};
-    cuuint64_t strides[2] = {static_cast<cuuint64_t>(E_ld) * 2, static_cast<cuuint64_t>(E_ld) * c.d * 2};
-    cuuint32_t box[3] = {64, 64, 1};
-    cuuint32_t estr[3] = {1, 1, 1};
-    if (fn(&ctx->tm_wr, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, ctx->wr_pieces, dims, strides, box, estr,
-           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
+    CUresult res;
+    if (E_ld % 64 == 0) {
+      // [3][d][E_ld] viewed as [3][E_ld/64][d][64]: one box {64 e, 64 k, E_ld/64 blocks, 3 pieces} per
+      // k-block lands every piece and 64-expert block in the [piece][block][k][64 e] order of the MN-major operand
+      cuuint64_t dims[4] = {64, static_cast<cuuint64_t>(c.d), static_cast<cuuint64_t>(E_ld / 64), 3};
+      cuuint64_t strides[3] = {static_cast<cuuint64_t>(E_ld) * 2, 128, static_cast<cuuint64_t>(E_ld) * c.d * 2};
+      cuuint32_t box[4] = {64, 64, static_cast<cuuint32_t>(E_ld / 64), 3};
+      cuuint32_t estr[4] = {1, 1, 1, 1};
+      res = fn(&ctx->tm_wr, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, ctx->wr_pieces, dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      box[3] = 1;
+      if (res == CUDA_SUCCESS)
+        res = fn(&ctx->tm_wr1, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, ctx->wr_pieces, dims, strides, box, estr,
+                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    } else {
+      cuuint64_t dims[3] = {static_cast<cuuint64_t>(E_ld), static_cast<cuuint64_t>(c.d), 3};
+      cuuint64_t strides[2] = {static_cast<cuuint64_t>(E_ld) * 2, static_cast<cuuint64_t>(E_ld) * c.d * 2};
+      cuuint32_t box[3] = {64, 64, 1};
+      cuuint32_t estr[3] = {1, 1, 1};
+      res = fn(&ctx->tm_wr, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, ctx->wr_pieces, dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    }
+    if (E_ld % 64 != 0) ctx->tm_wr1 = ctx->tm_wr;
+    if (res != CUDA_SUCCESS) {
       ctx->last_error = "cuTensorMapEncodeTiled(W_r pieces) failed";
       return BG_ERR_CUDA;
     }

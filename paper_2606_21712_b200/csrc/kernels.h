@@ -33,7 +33,8 @@ cudaError_t router_kernels_init();
 cudaError_t launch_split_wr(const float* W_r, int d, int E, void* pieces, cudaStream_t st);
 int router_ksplit(int T, int d, int num_sms);
 // partial: fp32 [ksplit][T][E].  Also zeroes zero_buf[0..zero_n) (the histogram the top-k kernel fills).
-cudaError_t launch_router_gemm(const CUtensorMap& tm_h, const CUtensorMap& tm_w, int T, int d, int E, int ksplit,
+// tm_w: box of all three pieces (4-D view) or one 3-D block; tm_w1: the 4-D view with a one-piece box
+cudaError_t launch_router_gemm(const CUtensorMap& tm_h, const CUtensorMap& tm_w, const CUtensorMap& tm_w1, int T, int d, int E, int ksplit,
                                float* partial, int32_t* zero_buf, int zero_n, cudaStream_t st);
 
 // ---- routing (routing.cu): steps a1 (sum of partials + bias) - a5 of DESIGN.md §1

@@ -20,12 +20,15 @@
 namespace bg {
 namespace {
 
-constexpr int BM = 128, BK = 64, UK = 16, STAGES = 4;
+constexpr int BM = 128, BK = 64, UK = 16, MAX_STAGES = 6;
 constexpr int A_BYTES = BM * BK * 2;             // 16 KB
-constexpr int B_BLK_BYTES = 64 * BK * 2;         // 8 KB per 64 experts
-constexpr int B_BYTES = 4 * B_BLK_BYTES;         // up to 256 experts
-constexpr int STAGE_BYTES = A_BYTES + B_BYTES;   // 48 KB
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 + 256;
+constexpr int B_BLK_BYTES = 64 * BK * 2;         // 8 KB per 64 experts of one piece
+// A stage = one k-block: the hidden tile ONCE plus all three W_r pieces (3 x n_blk x 8 KB); the number
+// of stages is what fits in RING_BYTES (E <= 64: 5, E <= 128: 3, E <= 256: 2).  The hidden stream comes
+// from HBM, so what matters is k-blocks of hidden in flight (one stage per (k-block, piece) re-fetched
+// the hidden tile three times and kept 1.3 k-blocks in flight: 25 % of the HBM roofline on C5).
+constexpr int RING_BYTES = 224 * 1024;
+constexpr int SMEM_BYTES = RING_BYTES + 1024 + 256;
 constexpr int NUM_THREADS = 256;                 // warp 0 TMA, warp 1 MMA, warp 2 TMEM alloc, warps 4-7 epilogue
 
 constexpr uint64_t ADESC_HI = umma_desc_sw128(16, 1024);
@@ -50,17 +53,18 @@ __global__ void split_wr_kernel(const float* __restrict__ W_r, int d, int E, int
 }
 
 __global__ void __launch_bounds__(NUM_THREADS, 1)
-router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_constant__ CUtensorMap tm_w, int T, int d,
+router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_constant__ CUtensorMap tm_w,
+                   const __grid_constant__ CUtensorMap tm_w1, int T, int d,
                    int E, int ksplit, float* __restrict__ partial, int32_t* __restrict__ zero_buf, int zero_n) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (base - raw);
-  const uint32_t bar_base = base + STAGES * STAGE_BYTES;
+  const uint32_t bar_base = base + RING_BYTES;
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
-  auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
-  const uint32_t done_bar = bar_base + 8u * (2 * STAGES);
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + STAGES * STAGE_BYTES + 8 * (2 * STAGES + 1));
+  auto empty_bar = [&](int s) { return bar_base + 8u * (MAX_STAGES + s); };
+  const uint32_t done_bar = bar_base + 8u * (2 * MAX_STAGES);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + RING_BYTES + 8 * (2 * MAX_STAGES + 1));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int m_tile = blockIdx.x, ks = blockIdx.y;
@@ -74,15 +78,24 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_consta
   const int k_blocks = (d + BK - 1) / BK;
   const int kb_per = (k_blocks + ksplit - 1) / ksplit;
   const int kb0 = ks * kb_per, kb1 = min(k_blocks, kb0 + kb_per);
-  const int n_iter = max(0, kb1 - kb0) * 3;                  // (k-block, piece) pairs
+  const int n_kb = max(0, kb1 - kb0);                        // k-blocks of this CTA
   const int n_mma = (E + 15) & ~15;                          // UMMA N (multiple of 16 for M=128)
   const int n_blk = (E + 63) / 64;                           // 64-expert TMA boxes
+  const uint32_t piece_bytes = n_blk * B_BLK_BYTES;
+  // pieces per stage: all three when at least three such stages fit (E <= 128), else one (E <= 256:
+  // 4 stages of 48 KB, the hidden tile re-fetched per piece from L2)
+  const int pps = (3 * (A_BYTES + 3 * piece_bytes) <= RING_BYTES) ? 3 : 1;
+  const int ipk = 3 / pps;                                   // iterations (stages) per k-block
+  const int n_iter = n_kb * ipk;
+  const uint32_t stage_bytes = A_BYTES + pps * piece_bytes;
+  const int n_stages = min(MAX_STAGES, RING_BYTES / static_cast<int>(stage_bytes));
+  const bool w4d = (n_mma & 63) == 0;                        // 4-D block view of the pieces (api.cu)
   const uint32_t idesc = umma_idesc_bf16(BM, n_mma, 0, 1);
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tm_h);
     tma_prefetch_desc(&tm_w);
-    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    for (int s = 0; s < MAX_STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
     mbar_init(done_bar, 1);
     fence_barrier_init();
   }
@@ -94,32 +107,42 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_consta
 
   if (warp == 0) {
     if (lane == 0) {                              // ---- TMA producer
-      const uint32_t stage_tx = A_BYTES + n_blk * B_BLK_BYTES;
+      int s = 0;
+      uint32_t ph = 0;
       for (int it = 0; it < n_iter; ++it) {
-        const int s = it % STAGES;
-        const uint32_t ph = (it / STAGES) & 1u;
         mbar_wait(empty_bar(s), ph ^ 1u);
-        const int kb = kb0 + it / 3, piece = it % 3;
-        const uint32_t sa = base + s * STAGE_BYTES, sb = sa + A_BYTES;
-        mbar_expect_tx(full_bar(s), stage_tx);
+        const int kb = kb0 + it / ipk, pc0 = (it % ipk) * pps;
+        const uint32_t sa = base + s * stage_bytes, sb = sa + A_BYTES;
+        mbar_expect_tx(full_bar(s), stage_bytes);
         tma_load_2d(sa, &tm_h, full_bar(s), kb * BK, m_tile * BM);
-        for (int j = 0; j < n_blk; ++j) tma_load_3d(sb + j * B_BLK_BYTES, &tm_w, full_bar(s), 64 * j, kb * BK, piece);
+        if (w4d) {                                  // one operation: [piece][block][k][64 e]
+          tma_load_4d(sb, pps == 3 ? &tm_w : &tm_w1, full_bar(s), 0, kb * BK, 0, pc0);
+        } else {
+          for (int pc = 0; pc < pps; ++pc)
+            for (int j = 0; j < n_blk; ++j)
+              tma_load_3d(sb + pc * piece_bytes + j * B_BLK_BYTES, &tm_w, full_bar(s), 64 * j, kb * BK, pc0 + pc);
+        }
+        if (++s == n_stages) { s = 0; ph ^= 1u; }
       }
     }
   } else if (warp == 1) {
     if (lane == 0) {                              // ---- MMA issuer
+      int s = 0;
+      uint32_t ph = 0;
       for (int it = 0; it < n_iter; ++it) {
-        const int s = it % STAGES;
-        const uint32_t ph = (it / STAGES) & 1u;
         mbar_wait(full_bar(s), ph);
         tc_fence_after();
-        const uint32_t sa = base + s * STAGE_BYTES, sb = sa + A_BYTES;
+        const uint32_t sa = base + s * stage_bytes, sb = sa + A_BYTES;
         const uint64_t ad = ADESC_HI | ((sa >> 4) & 0x3FFFu);
-        const uint64_t bd = BDESC_HI | ((sb >> 4) & 0x3FFFu);
-        #pragma unroll
-        for (int kk = 0; kk < BK / UK; ++kk)
-          umma_f16(tmem_base, ad + ((kk * UK * 2) >> 4), bd + ((kk * UK * 128) >> 4), idesc, (it | kk) != 0 ? 1u : 0u);
+        for (int pc = 0; pc < pps; ++pc) {        // hidden * hi + hidden * mid + hidden * lo, one accumulator
+          const uint64_t bd = BDESC_HI | (((sb + pc * piece_bytes) >> 4) & 0x3FFFu);
+          #pragma unroll
+          for (int kk = 0; kk < BK / UK; ++kk)
+            umma_f16(tmem_base, ad + ((kk * UK * 2) >> 4), bd + ((kk * UK * 128) >> 4), idesc,
+                     (it | pc | kk) != 0 ? 1u : 0u);
+        }
         umma_commit(empty_bar(s));
+        if (++s == n_stages) { s = 0; ph ^= 1u; }
       }
       umma_commit(done_bar);
     }
@@ -127,7 +150,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_consta
     const int q = warp & 3;                       // TMEM lane quarter of this warp
     const int row = m_tile * BM + q * 32 + lane;
     float* dst = partial + (static_cast<int64_t>(ks) * T + row) * E;
-    if (n_iter == 0) {
+    if (n_kb == 0) {
       if (row < T) for (int e = 0; e < E; ++e) dst[e] = 0.0f;
     } else {
       mbar_wait(done_bar, 0);
@@ -183,11 +206,11 @@ int router_ksplit(int T, int d, int num_sms) {
   return ks;
 }
 
-cudaError_t launch_router_gemm(const CUtensorMap& tm_h, const CUtensorMap& tm_w, int T, int d, int E, int ksplit,
+cudaError_t launch_router_gemm(const CUtensorMap& tm_h, const CUtensorMap& tm_w, const CUtensorMap& tm_w1, int T, int d, int E, int ksplit,
                                float* partial, int32_t* zero_buf, int zero_n, cudaStream_t st) {
   if (T == 0) return cudaSuccess;
   dim3 grid((T + BM - 1) / BM, ksplit);
-  launch_pdl(router_gemm_kernel, grid, NUM_THREADS, SMEM_BYTES, st, tm_h, tm_w, T, d, E, ksplit, partial, zero_buf, zero_n);
+  launch_pdl(router_gemm_kernel, grid, NUM_THREADS, SMEM_BYTES, st, tm_h, tm_w, tm_w1, T, d, E, ksplit, partial, zero_buf, zero_n);
   return cudaGetLastError();
 }
 
