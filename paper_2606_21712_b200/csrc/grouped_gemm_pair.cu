@@ -358,11 +358,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
           uint4 val;
           asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
                        : "=r"(val.x), "=r"(val.y), "=r"(val.z), "=r"(val.w) : "r"(stage_rd + i * 512));
-#ifdef BG_DBG_NOSTORE
-          if (col_ok && r < n_tok && val.x == 0x12345678u)
-#else
           if (col_ok && r < n_tok)
-#endif
             *reinterpret_cast<uint4*>(out_tile + static_cast<int64_t>(cc * 32 + r) * p.N) = val;
         }
         __syncwarp();
@@ -407,11 +403,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         }
       } else {
         #pragma unroll 1
-#ifdef BG_DBG_NOEPI
-        for (int cc = sub; cc < 0; cc += 2) {
-#else
         for (int cc = sub; cc < n_chunks; cc += 2) {
-#endif
           uint32_t v[32];
           tmem_ld_32x32(taddr + cc * 32, v);
           tmem_ld_wait();

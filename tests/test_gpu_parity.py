@@ -131,6 +131,7 @@ FFN_SHAPES = [
     ([300], 64, 64),                   # minimum d, f; one expert
     ([5, 0, 0, 700, 2], 192, 200),     # f not a multiple of 128, K not a multiple of 64
     ([33, 90], 1024, 136),             # N tail of 8
+    ([256, 257, 512, 16, 17, 1, 0, 255, 513], 128, 256),   # token-tile boundaries: 1 / 2 / 3 tiles, 16-row steps
 ]
 
 
