@@ -368,6 +368,13 @@ def run_ours(args):
 
     if rank == 0 and world == 1 and not args.no_sweep:
         line["sweep_c3"] = run_c3_sweep(args.steps, peaks, local)
+        # module-level roofline fitted to the sweep and the B_moe it implies (include/bg_moe.h)
+        import paper_2606_21712_b200 as pk
+        c3 = wl.CONFIGS["C3"]
+        fit = pk.fit_roofline([r["T"] for r in line["sweep_c3"]], [r["ms_per_step"] for r in line["sweep_c3"]])
+        b_moe, reached = pk.choose_tokens(c3.d, c3.f, c3.E, c3.k, fit, 0.8, 8 << 30, 64)
+        line["plan_c3"] = {"fit": fit.as_dict(), "target_util": 0.8, "memory_budget_bytes": 8 << 30,
+                           "B_moe_tokens": b_moe, "target_reached": reached}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
         cores = oracle.num_threads()

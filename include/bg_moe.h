@@ -127,6 +127,43 @@ int64_t bg_moe_launch_count(const bg_moe_ctx* ctx);
 /* Bytes of device workspace owned by `ctx`. */
 int64_t bg_moe_workspace_bytes(const bg_moe_ctx* ctx);
 
+/* ---- Module-level roofline fit and B_moe choice (host only; no GPU work, no context needed) -------
+ * The paper plans the MoE batch statically: "a module-level roofline model enables static planning
+ * for batch accumulation ... we can select the largest feasible module batch size that remains
+ * within memory constraints" (§5.1); the model is fitted to profiled runtimes of the
+ * module "over multiple batch sizes" (§5.4).  Here the module is this library's fused
+ * chain, the profile is bench.py's combine-size sweep, and memory is the context's workspace.
+ *
+ * Model: t(T) = max(t_floor_ms, t0_ms + ms_per_token * T) -- flat while the expert weights bound
+ * the step (small combined batches), linear once the tensor cores do.  Utilisation of a batch of T
+ * tokens = its token rate relative to the asymptotic rate: u(T) = ms_per_token * T / t(T). */
+typedef struct {
+  double t_floor_ms;    /* weight-bound floor */
+  double t0_ms;         /* intercept of the compute-bound line */
+  double ms_per_token;  /* slope of the compute-bound line (> 0) */
+  double ridge_tokens;  /* where the two meet: (t_floor_ms - t0_ms) / ms_per_token */
+  double rms_rel_err;   /* root mean square of (model - measured) / measured over the fitted points */
+} bg_moe_fit;
+
+/* Least-squares fit of the model to n >= 3 measured points (tokens strictly increasing, ms > 0; HOST
+ * pointers): every split "first j points flat, the rest on a line" (1 <= j <= n-2) is tried, the flat
+ * level is the mean of its points and the line the ordinary least-squares line of its points; the
+ * split with the smallest sum of squared relative errors of max(flat, line) wins (lowest j on ties).
+ * BG_ERR_INVALID_ARG if no split has a positive slope. */
+int bg_moe_fit_roofline(const int32_t* tokens, const double* ms, int32_t n, bg_moe_fit* out);
+
+/* Bytes of device workspace a context with this config and max_tokens = tokens would allocate
+ * (what bg_moe_create allocates on a 148-SM B200; cfg->max_tokens and cfg->device are ignored). */
+int bg_moe_workspace_bytes_for(const bg_moe_config* cfg, int32_t tokens, int64_t* bytes_out);
+
+/* B_moe: *tokens_out = the SMALLEST multiple of `granularity` (>= 1) whose model utilisation reaches
+ * target_util (0 < target_util < 1), capped at the LARGEST multiple of `granularity` whose workspace
+ * fits in memory_budget_bytes; *reached_out (may be NULL) = 1 if the target was reached under the
+ * cap, 0 if the cap bound it.  BG_ERR_NOMEM if not even `granularity` tokens fit. */
+int bg_moe_choose_tokens(const bg_moe_config* cfg, const bg_moe_fit* fit, double target_util,
+                         int64_t memory_budget_bytes, int32_t granularity, int32_t* tokens_out,
+                         int32_t* reached_out);
+
 const char* bg_moe_strerror(int status);
 /* Text of the last CUDA error seen by `ctx` ("" if none).  Owned by the context. */
 const char* bg_moe_last_error(const bg_moe_ctx* ctx);

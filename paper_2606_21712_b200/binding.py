@@ -15,7 +15,7 @@ BG_OK, BG_ERR_INVALID_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA, BG_ERR_NOMEM, BG_ERR
 EXPORTS = ["bg_moe_create", "bg_moe_destroy", "bg_moe_set_weights", "bg_moe_route", "bg_moe_permute",
            "bg_moe_expert_ffn", "bg_moe_unpermute", "bg_moe_combined_forward", "bg_moe_combined_forward_host",
            "bg_moe_debug_views", "bg_moe_profile_enable", "bg_moe_profile_read", "bg_moe_launch_count", "bg_moe_workspace_bytes", "bg_moe_strerror",
-           "bg_moe_last_error"]
+           "bg_moe_last_error", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens"]
 
 
 class BgMoeConfig(ctypes.Structure):
@@ -218,3 +218,49 @@ class _DeviceArray:
     def __init__(self, ptr: int, shape, typestr: str):
         self.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": typestr, "data": (ptr, False),
                                          "version": 2, "strides": None}
+
+
+# ---------------------------------------------------------------------- planning (host only)
+class BgMoeFit(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_double) for n in ("t_floor_ms", "t0_ms", "ms_per_token", "ridge_tokens", "rms_rel_err")]
+
+    def as_dict(self) -> dict:
+        return {n: float(getattr(self, n)) for n, _ in self._fields_}
+
+
+def _plan_check(lib, rc: int):
+    if rc != BG_OK:
+        raise BgMoeError(rc, lib.bg_moe_strerror(rc).decode())
+
+
+def fit_roofline(tokens, ms) -> BgMoeFit:
+    """bg_moe_fit_roofline: module-level roofline t(T) = max(t_floor, t0 + s T) fitted to measured points."""
+    lib = load_library()
+    n = len(tokens)
+    tok = (ctypes.c_int32 * n)(*[int(t) for t in tokens])
+    y = (ctypes.c_double * n)(*[float(v) for v in ms])
+    fit = BgMoeFit()
+    lib.bg_moe_fit_roofline.restype = ctypes.c_int
+    _plan_check(lib, lib.bg_moe_fit_roofline(tok, y, ctypes.c_int32(n), ctypes.byref(fit)))
+    return fit
+
+
+def workspace_bytes_for(d: int, f: int, E: int, k: int, tokens: int) -> int:
+    """bg_moe_workspace_bytes_for: device workspace of a context with max_tokens = tokens."""
+    lib = load_library()
+    cfg = BgMoeConfig(d, f, E, k, 0, 0, 0)
+    out = ctypes.c_int64()
+    _plan_check(lib, lib.bg_moe_workspace_bytes_for(ctypes.byref(cfg), ctypes.c_int32(tokens), ctypes.byref(out)))
+    return int(out.value)
+
+
+def choose_tokens(d: int, f: int, E: int, k: int, fit: BgMoeFit, target_util: float, memory_budget_bytes: int,
+                  granularity: int = 1):
+    """bg_moe_choose_tokens: (B_moe, reached) -- see include/bg_moe.h."""
+    lib = load_library()
+    cfg = BgMoeConfig(d, f, E, k, 0, 0, 0)
+    tok, reached = ctypes.c_int32(), ctypes.c_int32()
+    _plan_check(lib, lib.bg_moe_choose_tokens(ctypes.byref(cfg), ctypes.byref(fit), ctypes.c_double(target_util),
+                                              ctypes.c_int64(memory_budget_bytes), ctypes.c_int32(granularity),
+                                              ctypes.byref(tok), ctypes.byref(reached)))
+    return int(tok.value), bool(reached.value)

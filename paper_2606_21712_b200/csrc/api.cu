@@ -275,18 +275,11 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   ctx->num_sms = prop.multiProcessorCount;
   const int64_t Tm = c.max_tokens > 0 ? c.max_tokens : 1;
   const int64_t Rm = Tm * c.k;
-  const int64_t nblk = bg::route_num_blocks(static_cast<int>(Tm), c.k);
-  int64_t off = 0;
-  auto carve = [&](int64_t bytes) { int64_t o = off; off = align_up(off + bytes, 1024); return o; };
-  const int64_t Tpad = align_up(Tm, 128);
-  const int64_t part_rows = Tpad > static_cast<int64_t>(ctx->num_sms) * 128 ? Tpad : static_cast<int64_t>(ctx->num_sms) * 128;
-  const int64_t o_logits = carve(Tm * c.E * 4), o_idx = carve(Rm * 4), o_w = carve(Rm * 4);
-  const int64_t o_part = carve(part_rows * c.E * 4), o_pieces = carve(3LL * c.d * ((c.E + 15) & ~15) * 2);
-  const int64_t o_counts = carve(c.E * 4), o_offsets = carve((c.E + 1) * 4);
-  const int64_t o_bc = carve(nblk * c.E * 4), o_bb = carve(nblk * c.E * 4);
-  const int64_t o_rs = carve(Rm * 4), o_ip = carve(Rm * 4), o_wp = carve(Rm * 4);
-  const int64_t o_x = carve(Rm * c.d * 2), o_h = carve(Rm * c.f * 2), o_y = carve(Rm * c.d * 2);
-  const int64_t o_hd = carve(Tm * c.d * 2), o_od = carve(Tm * c.d * 2);
+  const bg::WsLayout L = bg::ws_layout(c, Tm, ctx->num_sms);
+  const int64_t off = L.total;
+  const int64_t o_logits = L.logits, o_idx = L.idx, o_w = L.w, o_part = L.part, o_pieces = L.pieces;
+  const int64_t o_counts = L.counts, o_offsets = L.offsets, o_bc = L.bc, o_bb = L.bb;
+  const int64_t o_rs = L.rs, o_ip = L.ip, o_wp = L.wp, o_x = L.x, o_h = L.h, o_y = L.y, o_hd = L.hd, o_od = L.od;
   ctx->ws_bytes = off;
   void* p = nullptr;
   if (cudaMalloc(&p, static_cast<size_t>(off)) != cudaSuccess) {

@@ -4,6 +4,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include "../../include/bg_moe.h"
 
 namespace bg {
 
@@ -36,6 +37,12 @@ int router_ksplit(int T, int d, int num_sms);
 // tm_w: box of all three pieces (4-D view) or one 3-D block; tm_w1: the 4-D view with a one-piece box
 cudaError_t launch_router_gemm(const CUtensorMap& tm_h, const CUtensorMap& tm_w, const CUtensorMap& tm_w1, int T, int d, int E, int ksplit,
                                float* partial, int32_t* zero_buf, int zero_n, cudaStream_t st);
+
+// ---- workspace layout (plan.cu): byte offsets of every slab of the context's single allocation
+struct WsLayout {
+  int64_t logits, idx, w, part, pieces, counts, offsets, bc, bb, rs, ip, wp, x, h, y, hd, od, total;
+};
+WsLayout ws_layout(const bg_moe_config& c, int64_t max_tokens, int num_sms);
 
 // ---- routing (routing.cu): steps a1 (sum of partials + bias) - a5 of DESIGN.md §1
 // Tokens handled by one block of the top-k / rank kernels: chosen so that a block owns at most

@@ -291,3 +291,12 @@ def test_argument_errors():
     with pytest.raises(BgMoeError) as ei:
         layer.combined_forward(h)                # T > max_tokens
     assert ei.value.status == BG_ERR_INVALID_ARG
+
+
+def test_planned_workspace_equals_allocated_workspace():
+    """bg_moe_workspace_bytes_for (host-only planner) must predict what bg_moe_create allocates."""
+    import paper_2606_21712_b200 as pk
+    for (d, f, E, k, T) in [(512, 1024, 8, 2, 256), (2048, 768, 128, 8, 4096), (192, 200, 5, 5, 1000)]:
+        layer = pk.MoELayer(d, f, E, k, T)
+        assert layer.lib.bg_moe_workspace_bytes(layer._ctx) == pk.workspace_bytes_for(d, f, E, k, T)
+        layer.close()
