@@ -140,8 +140,6 @@ int cuda_fail(bg_moe_ctx* ctx, cudaError_t e, const char* where) {
     (ctx)->launches += 1;           \
   } while (0)
 
-int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
-
 struct DeviceGuard {
   int prev = -1;
   bool ok = true;
