@@ -102,6 +102,23 @@ int bg_moe_unpermute(bg_moe_ctx* ctx, const void* y_perm, const int32_t* inv_per
  * fp32, before the bf16 rounding of Y) and the final reduce only sums. */
 int bg_moe_combined_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void* out, void* stream);
 
+/* Zero-copy COMBINE (Algorithm 1 l.7; Table 2 "COMBINE without offloading: 0 (GPU
+ * resident)"): the combined batch given as the list of the yielded coroutines' own buffers instead of
+ * one concatenated tensor.  Segment s holds n_tokens rows of bf16 [n_tokens, d] at `hidden` (device,
+ * 16-byte aligned) and receives its rows of the result at `out`; the combined token order is the list
+ * order (token t of the batch = row t - sum_{s'<s} n_tokens_{s'} of segment s).  `segments` is a HOST
+ * array, copied to the device on `stream`; 0 <= n_segments <= max_tokens, sum of n_tokens <= max_tokens;
+ * empty segments are allowed.  The result is bit-identical to bg_moe_combined_forward on the
+ * concatenation: the router, the gather and the un-permute address rows through the segment table,
+ * every other kernel is the same. */
+typedef struct {
+  const void* hidden;   /* device, bf16 [n_tokens, d] */
+  void* out;            /* device, bf16 [n_tokens, d] */
+  int32_t n_tokens;
+} bg_moe_segment;
+int bg_moe_combined_forward_segments(bg_moe_ctx* ctx, const bg_moe_segment* segments,
+                                     int32_t n_segments, void* stream);
+
 /* Same, but `hidden_host` and `out_host` are HOST pointers (pinned memory recommended): copies
  * hidden host->device, runs the fused chain, copies out device->host, all on `stream`. */
 int bg_moe_combined_forward_host(bg_moe_ctx* ctx, const void* hidden_host, int32_t T,

@@ -15,11 +15,15 @@ BG_OK, BG_ERR_INVALID_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA, BG_ERR_NOMEM, BG_ERR
 EXPORTS = ["bg_moe_create", "bg_moe_destroy", "bg_moe_set_weights", "bg_moe_route", "bg_moe_permute",
            "bg_moe_expert_ffn", "bg_moe_unpermute", "bg_moe_combined_forward", "bg_moe_combined_forward_host",
            "bg_moe_debug_views", "bg_moe_profile_enable", "bg_moe_profile_read", "bg_moe_launch_count", "bg_moe_workspace_bytes", "bg_moe_strerror",
-           "bg_moe_last_error", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens"]
+           "bg_moe_last_error", "bg_moe_combined_forward_segments", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens"]
 
 
 class BgMoeConfig(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in ("d", "f", "E", "k", "max_tokens", "gate_fn", "device")]
+
+
+class BgMoeSegment(ctypes.Structure):
+    _fields_ = [("hidden", ctypes.c_void_p), ("out", ctypes.c_void_p), ("n_tokens", ctypes.c_int32)]
 
 
 class BgMoeError(RuntimeError):
@@ -177,6 +181,25 @@ class MoELayer:
         self._check(self.lib.bg_moe_combined_forward_host(self._ctx, _ptr(hidden_host), T, _ptr(out_host),
                                                           _stream(stream)))
         return out_host
+
+    def combined_forward_segments(self, hidden_segments, out_segments=None, stream=None):
+        """bg_moe_combined_forward_segments: zero-copy COMBINE.  hidden_segments: list of CUDA bf16 tensors
+        [n_s, d] (the yielded coroutines' buffers; n_s may be 0); returns the list of per-segment outputs."""
+        if out_segments is None:
+            out_segments = [torch.empty_like(h) for h in hidden_segments]
+        n = len(hidden_segments)
+        arr = (BgMoeSegment * max(n, 1))()
+        for i, (h, o) in enumerate(zip(hidden_segments, out_segments)):
+            assert h.dtype == torch.bfloat16 and h.is_cuda and h.is_contiguous() and h.shape[1] == self.d
+            assert o.dtype == torch.bfloat16 and o.is_cuda and o.is_contiguous() and o.shape == h.shape
+            arr[i].hidden = h.data_ptr() if h.shape[0] else None
+            arr[i].out = o.data_ptr() if o.shape[0] else None
+            arr[i].n_tokens = h.shape[0]
+        self.lib.bg_moe_combined_forward_segments.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32,
+                                                              ctypes.c_void_p]
+        self._check(self.lib.bg_moe_combined_forward_segments(self._ctx, ctypes.cast(arr, ctypes.c_void_p),
+                                                              ctypes.c_int32(n), _stream(stream)))
+        return out_segments
 
     STAGES = ("router", "topk_hist", "scan", "rank", "gather", "gateup_swiglu", "down", "unpermute")
 

@@ -8,6 +8,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 struct bg_moe_ctx {
   bg_moe_config cfg;
@@ -33,6 +34,13 @@ struct bg_moe_ctx {
   int32_t* row_src = nullptr;
   int32_t* inv_perm = nullptr;
   float* w_perm = nullptr;      // gate weights in expert order (fused path)
+  // segment table of bg_moe_combined_forward_segments (device arrays + pageable host staging)
+  int32_t max_segments = 0;
+  const void** seg_dev_hidden = nullptr;
+  void** seg_dev_out = nullptr;
+  int32_t* seg_dev_start = nullptr;
+  std::vector<const void*> seg_host_ptrs;
+  std::vector<int32_t> seg_host_start;
   void* x_perm = nullptr;
   void* H = nullptr;
   void* Y = nullptr;
@@ -160,15 +168,23 @@ int check_T(const bg_moe_ctx* ctx, int32_t T) {
 
 // a1-a4 on explicit buffers.
 int do_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits_in, float* logits_buf,
-             int32_t* topk_idx, float* topk_w, int32_t* counts, int32_t* offsets, cudaStream_t st) {
+             int32_t* topk_idx, float* topk_w, int32_t* counts, int32_t* offsets, cudaStream_t st,
+             const bg::SegTable* seg = nullptr) {
   const bg_moe_config& c = ctx->cfg;
   if (logits_in == nullptr) {
-    CUtensorMap tm_h;
-    if (!encode_act_map(&tm_h, hidden, T, c.d)) { ctx->last_error = "cuTensorMapEncodeTiled(hidden) failed"; return BG_ERR_CUDA; }
     const int ks = bg::router_ksplit(T, c.d, ctx->num_sms);
-    mark(ctx, 0, st);
-    BG_LAUNCH(ctx, bg::launch_router_gemm(tm_h, ctx->tm_wr, ctx->tm_wr1, T, c.d, c.E, ks, ctx->partial, ctx->block_counts,
-                                          bg::route_num_blocks(T, c.k) * c.E, st), "router_gemm");
+    if (seg != nullptr) {
+      mark(ctx, 0, st);
+      BG_LAUNCH(ctx, bg::launch_router_gemm_segments(*seg, ctx->tm_wr, ctx->tm_wr1, T, c.d, c.E, ks, ctx->partial,
+                                                     ctx->block_counts, bg::route_num_blocks(T, c.k) * c.E, st),
+                "router_gemm_segments");
+    } else {
+      CUtensorMap tm_h;
+      if (!encode_act_map(&tm_h, hidden, T, c.d)) { ctx->last_error = "cuTensorMapEncodeTiled(hidden) failed"; return BG_ERR_CUDA; }
+      mark(ctx, 0, st);
+      BG_LAUNCH(ctx, bg::launch_router_gemm(tm_h, ctx->tm_wr, ctx->tm_wr1, T, c.d, c.E, ks, ctx->partial, ctx->block_counts,
+                                            bg::route_num_blocks(T, c.k) * c.E, st), "router_gemm");
+    }
     mark(ctx, 1, st);
     BG_LAUNCH(ctx, bg::launch_topk_hist(ctx->partial, ks, ctx->b_r, logits_buf, T, c.E, c.k, topk_idx, topk_w,
                                         ctx->block_counts, st), "topk_hist");
@@ -298,6 +314,10 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   ctx->row_src = reinterpret_cast<int32_t*>(ctx->ws + o_rs);
   ctx->inv_perm = reinterpret_cast<int32_t*>(ctx->ws + o_ip);
   ctx->w_perm = reinterpret_cast<float*>(ctx->ws + o_wp);
+  ctx->max_segments = static_cast<int32_t>(Tm);
+  ctx->seg_dev_hidden = reinterpret_cast<const void**>(ctx->ws + L.seg_hidden);
+  ctx->seg_dev_out = reinterpret_cast<void**>(ctx->ws + L.seg_out);
+  ctx->seg_dev_start = reinterpret_cast<int32_t*>(ctx->ws + L.seg_start);
   ctx->x_perm = ctx->ws + o_x;
   ctx->H = ctx->ws + o_h;
   ctx->Y = ctx->ws + o_y;
@@ -456,6 +476,28 @@ int bg_moe_unpermute(bg_moe_ctx* ctx, const void* y_perm, const int32_t* inv_per
   return BG_OK;
 }
 
+// The fused chain a1-a9; seg != nullptr: token rows are read from / written to the segments' buffers.
+static int do_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void* out, cudaStream_t st,
+                      const bg::SegTable* seg) {
+  const bg_moe_config& c = ctx->cfg;
+  int rc = do_route(ctx, hidden, T, nullptr, ctx->logits, ctx->topk_idx, ctx->topk_w, ctx->counts, ctx->offsets, st, seg);
+  if (rc) return rc;
+  mark(ctx, 3, st);
+  BG_LAUNCH(ctx, bg::launch_rank(ctx->topk_idx, ctx->block_base, T, c.E, c.k, ctx->row_src, ctx->inv_perm, ctx->topk_w,
+                                 ctx->w_perm, st), "rank");
+  mark(ctx, 4, st);
+  BG_LAUNCH(ctx, bg::launch_gather(hidden, ctx->inv_perm, T, c.k, c.d, ctx->x_perm, ctx->num_sms, st, seg), "gather");
+  mark(ctx, 5, st);
+  rc = do_ffn(ctx, ctx->x_perm, ctx->offsets, T, ctx->Y, ctx->topk_w, ctx->row_src, st, /*mark_between=*/6);
+  if (rc) return rc;
+  mark(ctx, 7, st);
+  BG_LAUNCH(ctx, bg::launch_unpermute(ctx->Y, ctx->inv_perm, nullptr, T, c.k, c.d, out, ctx->num_sms, st, seg),
+            "unpermute");
+  mark(ctx, 8, st);
+  ctx->profile_valid = ctx->profile;
+  return BG_OK;
+}
+
 int bg_moe_combined_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void* out, void* stream) {
   int rc = check_T(ctx, T);
   if (rc) return rc;
@@ -463,23 +505,57 @@ int bg_moe_combined_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void
   if (!hidden || !out || !aligned16(hidden) || !aligned16(out)) return BG_ERR_INVALID_ARG;
   if (ctx->W_r == nullptr) return BG_ERR_NO_WEIGHTS;
   DeviceGuard guard(ctx->cfg.device);
+  return do_forward(ctx, hidden, T, out, static_cast<cudaStream_t>(stream), nullptr);
+}
+
+int bg_moe_combined_forward_segments(bg_moe_ctx* ctx, const bg_moe_segment* segments, int32_t n_segments,
+                                     void* stream) {
+  if (ctx == nullptr || n_segments < 0 || (n_segments > 0 && segments == nullptr)) return BG_ERR_INVALID_ARG;
+  if (n_segments > ctx->max_segments) return BG_ERR_INVALID_ARG;
+  int64_t T64 = 0;
+  for (int i = 0; i < n_segments; ++i) {
+    const bg_moe_segment& sg = segments[i];
+    if (sg.n_tokens < 0) return BG_ERR_INVALID_ARG;
+    if (sg.n_tokens > 0 && (!sg.hidden || !sg.out || !aligned16(sg.hidden) || !aligned16(sg.out)))
+      return BG_ERR_INVALID_ARG;
+    T64 += sg.n_tokens;
+  }
+  if (T64 > ctx->cfg.max_tokens) return BG_ERR_INVALID_ARG;
+  const int32_t T = static_cast<int32_t>(T64);
+  if (T == 0) return BG_OK;
+  if (ctx->W_r == nullptr) return BG_ERR_NO_WEIGHTS;
+  DeviceGuard guard(ctx->cfg.device);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  const bg_moe_config& c = ctx->cfg;
-  rc = do_route(ctx, hidden, T, nullptr, ctx->logits, ctx->topk_idx, ctx->topk_w, ctx->counts, ctx->offsets, st);
-  if (rc) return rc;
-  mark(ctx, 3, st);
-  BG_LAUNCH(ctx, bg::launch_rank(ctx->topk_idx, ctx->block_base, T, c.E, c.k, ctx->row_src, ctx->inv_perm, ctx->topk_w,
-                                 ctx->w_perm, st), "rank");
-  mark(ctx, 4, st);
-  BG_LAUNCH(ctx, bg::launch_gather(hidden, ctx->inv_perm, T, c.k, c.d, ctx->x_perm, ctx->num_sms, st), "gather");
-  mark(ctx, 5, st);
-  rc = do_ffn(ctx, ctx->x_perm, ctx->offsets, T, ctx->Y, ctx->topk_w, ctx->row_src, st, /*mark_between=*/6);
-  if (rc) return rc;
-  mark(ctx, 7, st);
-  BG_LAUNCH(ctx, bg::launch_unpermute(ctx->Y, ctx->inv_perm, nullptr, T, c.k, c.d, out, ctx->num_sms, st), "unpermute");
-  mark(ctx, 8, st);
-  ctx->profile_valid = ctx->profile;
-  return BG_OK;
+  // The segment table goes to the device through pageable host staging: cudaMemcpyAsync from pageable
+  // memory returns once the bytes are staged, so the vectors can be reused by the next call.
+  const int n = n_segments;
+  ctx->seg_host_ptrs.resize(2 * static_cast<size_t>(n));
+  ctx->seg_host_start.resize(static_cast<size_t>(n) + 1);
+  // an empty segment may carry null pointers (its rows are never looked up); the router uses hidden[0]
+  // as the source address of zero-filled copies, so every entry is made a valid address
+  const void* first_valid = nullptr;
+  for (int i = 0; i < n && first_valid == nullptr; ++i)
+    if (segments[i].n_tokens > 0) first_valid = segments[i].hidden;
+  int32_t acc = 0;
+  for (int i = 0; i < n; ++i) {
+    ctx->seg_host_ptrs[i] = segments[i].n_tokens > 0 ? segments[i].hidden : first_valid;
+    ctx->seg_host_ptrs[n + i] = segments[i].out;
+    ctx->seg_host_start[i] = acc;
+    acc += segments[i].n_tokens;
+  }
+  ctx->seg_host_start[n] = acc;
+  BG_CUDA(ctx, cudaMemcpyAsync(ctx->seg_dev_hidden, ctx->seg_host_ptrs.data(), sizeof(void*) * n, cudaMemcpyHostToDevice, st),
+          "H2D segment table (hidden)");
+  BG_CUDA(ctx, cudaMemcpyAsync(ctx->seg_dev_out, ctx->seg_host_ptrs.data() + n, sizeof(void*) * n, cudaMemcpyHostToDevice, st),
+          "H2D segment table (out)");
+  BG_CUDA(ctx, cudaMemcpyAsync(ctx->seg_dev_start, ctx->seg_host_start.data(), sizeof(int32_t) * (n + 1),
+                               cudaMemcpyHostToDevice, st), "H2D segment table (start)");
+  bg::SegTable seg;
+  seg.hidden = reinterpret_cast<const void* const*>(ctx->seg_dev_hidden);
+  seg.out = reinterpret_cast<void* const*>(ctx->seg_dev_out);
+  seg.start = ctx->seg_dev_start;
+  seg.n = n;
+  return do_forward(ctx, nullptr, T, nullptr, st, &seg);
 }
 
 int bg_moe_combined_forward_host(bg_moe_ctx* ctx, const void* hidden_host, int32_t T, void* out_host, void* stream) {

@@ -30,12 +30,18 @@ __device__ __forceinline__ void st_stream(uint4* p, const uint4& v) {
 template <int KMAX>
 __global__ void __launch_bounds__(256) gather_kernel(const uint4* __restrict__ hidden,
                                                      const int32_t* __restrict__ inv_perm, int T, int k,
-                                                     int vec_per_row, uint4* __restrict__ x_perm) {
+                                                     int vec_per_row, uint4* __restrict__ x_perm, const SegTable seg) {
   pdl_wait_then_trigger();
   const int lane = threadIdx.x & 31;
   const int warps_total = gridDim.x * (blockDim.x >> 5);
   for (int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); t < T; t += warps_total) {
-    const uint4* src = hidden + static_cast<int64_t>(t) * vec_per_row;
+    const uint4* src;
+    if (seg.n > 0) {               // zero-copy COMBINE: the token's row inside its coroutine's own buffer
+      const int sg = seg_of(seg.start, seg.n, t);
+      src = static_cast<const uint4*>(seg.hidden[sg]) + static_cast<int64_t>(t - __ldg(seg.start + sg)) * vec_per_row;
+    } else {
+      src = hidden + static_cast<int64_t>(t) * vec_per_row;
+    }
     uint4* dst[KMAX];
     #pragma unroll
     for (int s = 0; s < KMAX; ++s)
@@ -76,7 +82,7 @@ template <int KMAX>
 __global__ void __launch_bounds__(256) unpermute_kernel(const uint4* __restrict__ y_perm,
                                                         const int32_t* __restrict__ inv_perm,
                                                         const float* __restrict__ weights, int T, int k,
-                                                        int vec_per_row, uint4* __restrict__ out) {
+                                                        int vec_per_row, uint4* __restrict__ out, const SegTable seg) {
   pdl_wait_then_trigger();
   const int lane = threadIdx.x & 31;
   const int warps_total = gridDim.x * (blockDim.x >> 5);
@@ -92,7 +98,13 @@ __global__ void __launch_bounds__(256) unpermute_kernel(const uint4* __restrict_
         w[s] = weights ? __ldg(weights + static_cast<int64_t>(t) * k + s) : 1.0f;
       }
     }
-    uint4* dst = out + static_cast<int64_t>(t) * vec_per_row;
+    uint4* dst;
+    if (seg.n > 0) {               // zero-copy split: the result goes back to the token's coroutine
+      const int sg = seg_of(seg.start, seg.n, t);
+      dst = static_cast<uint4*>(seg.out[sg]) + static_cast<int64_t>(t - __ldg(seg.start + sg)) * vec_per_row;
+    } else {
+      dst = out + static_cast<int64_t>(t) * vec_per_row;
+    }
     for (int c = lane; c < vec_per_row; c += 32) {
       uint4 v[KMAX];
       #pragma unroll
@@ -124,34 +136,36 @@ inline int row_mover_grid(int rows, int num_sms) {
 }  // namespace
 
 cudaError_t launch_gather(const void* hidden, const int32_t* inv_perm, int T, int k, int d, void* x_perm,
-                          int num_sms, cudaStream_t st) {
+                          int num_sms, cudaStream_t st, const SegTable* segp) {
+  const SegTable seg = segp ? *segp : SegTable{nullptr, nullptr, nullptr, 0};
   if (T == 0) return cudaSuccess;
   const int grid = row_mover_grid(T, num_sms);
   if (k <= 2)
     launch_pdl(gather_kernel<2>, grid, 256, 0, st, static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
-                                           static_cast<uint4*>(x_perm));
+                                           static_cast<uint4*>(x_perm), seg);
   else if (k <= 4)
     launch_pdl(gather_kernel<4>, grid, 256, 0, st, static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
-                                           static_cast<uint4*>(x_perm));
+                                           static_cast<uint4*>(x_perm), seg);
   else
     launch_pdl(gather_kernel<8>, grid, 256, 0, st, static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
-                                           static_cast<uint4*>(x_perm));
+                                           static_cast<uint4*>(x_perm), seg);
   return cudaGetLastError();
 }
 
 cudaError_t launch_unpermute(const void* y_perm, const int32_t* inv_perm, const float* weights, int T, int k,
-                             int d, void* out, int num_sms, cudaStream_t st) {
+                             int d, void* out, int num_sms, cudaStream_t st, const SegTable* segp) {
+  const SegTable seg = segp ? *segp : SegTable{nullptr, nullptr, nullptr, 0};
   if (T == 0) return cudaSuccess;
   const int grid = row_mover_grid(T, num_sms);
   if (k <= 2)
     launch_pdl(unpermute_kernel<2>, grid, 256, 0, st, static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
-                                              static_cast<uint4*>(out));
+                                              static_cast<uint4*>(out), seg);
   else if (k <= 4)
     launch_pdl(unpermute_kernel<4>, grid, 256, 0, st, static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
-                                              static_cast<uint4*>(out));
+                                              static_cast<uint4*>(out), seg);
   else
     launch_pdl(unpermute_kernel<8>, grid, 256, 0, st, static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
-                                              static_cast<uint4*>(out));
+                                              static_cast<uint4*>(out), seg);
   return cudaGetLastError();
 }
 

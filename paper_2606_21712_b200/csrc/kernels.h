@@ -38,11 +38,26 @@ int router_ksplit(int T, int d, int num_sms);
 cudaError_t launch_router_gemm(const CUtensorMap& tm_h, const CUtensorMap& tm_w, const CUtensorMap& tm_w1, int T, int d, int E, int ksplit,
                                float* partial, int32_t* zero_buf, int zero_n, cudaStream_t st);
 
+// ---- segments (zero-copy COMBINE): the combined tokens given as a list
+// of per-coroutine buffers.  Token t lives in row (t - start[s]) of hidden[s] (and of out[s]), s = the segment
+// with start[s] <= t < start[s+1].  All three arrays are DEVICE arrays.
+struct SegTable {
+  const void* const* hidden;   // [n] bf16 [n_tokens_s, d]
+  void* const* out;            // [n] bf16 [n_tokens_s, d]
+  const int32_t* start;        // [n+1] exclusive prefix sum of the segment lengths
+  int n;
+};
+
 // ---- workspace layout (plan.cu): byte offsets of every slab of the context's single allocation
 struct WsLayout {
-  int64_t logits, idx, w, part, pieces, counts, offsets, bc, bb, rs, ip, wp, x, h, y, hd, od, total;
+  int64_t logits, idx, w, part, pieces, counts, offsets, bc, bb, rs, ip, wp, x, h, y, hd, od, seg_hidden, seg_out,
+      seg_start, total;
 };
 WsLayout ws_layout(const bg_moe_config& c, int64_t max_tokens, int num_sms);
+
+cudaError_t launch_router_gemm_segments(const SegTable& seg, const CUtensorMap& tm_w, const CUtensorMap& tm_w1, int T,
+                                        int d, int E, int ksplit, float* partial, int32_t* zero_buf, int zero_n,
+                                        cudaStream_t st);
 
 // ---- routing (routing.cu): steps a1 (sum of partials + bias) - a5 of DESIGN.md §1
 // Tokens handled by one block of the top-k / rank kernels: chosen so that a block owns at most
@@ -70,11 +85,12 @@ cudaError_t launch_rank(const int32_t* topk_idx, const int32_t* block_base, int 
                         int32_t* row_src, int32_t* inv_perm, const float* topk_w, float* w_perm, cudaStream_t st);
 
 // ---- gather / reduce (gather_reduce.cu): steps a6 and a9
+// seg != nullptr: token rows are read from / written to the segments' own buffers (hidden / out unused).
 cudaError_t launch_gather(const void* hidden, const int32_t* inv_perm, int T, int k, int d, void* x_perm,
-                          int num_sms, cudaStream_t st);
+                          int num_sms, cudaStream_t st, const SegTable* seg = nullptr);
 // weights == nullptr: plain sum (fused path, Y already gate-weighted).
 cudaError_t launch_unpermute(const void* y_perm, const int32_t* inv_perm, const float* weights, int T, int k,
-                             int d, void* out, int num_sms, cudaStream_t st);
+                             int d, void* out, int num_sms, cudaStream_t st, const SegTable* seg = nullptr);
 
 // ---- grouped GEMM (grouped_gemm.cu): steps a7 and a8
 // Activation tensor maps: the same [rows, K] bf16 matrix with TMA boxes of {64 k, 8 (i + 1) rows},

@@ -23,6 +23,18 @@ __device__ __forceinline__ void pdl_wait_then_trigger() {
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 
+// ------------------------------------------------------------------ segments (kernels.h SegTable)
+// The segment that holds combined token t: the largest s with start[s] <= t (empty segments share their
+// start with their successor, which is the one the search lands on).
+__device__ __forceinline__ int seg_of(const int32_t* start, int n, int t) {
+  int lo = 0, hi = n;
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (__ldg(start + mid) <= t) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+
 // ------------------------------------------------------------------ mbarrier
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");

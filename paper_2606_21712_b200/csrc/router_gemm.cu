@@ -52,10 +52,22 @@ __global__ void split_wr_kernel(const float* __restrict__ W_r, int d, int E, int
   pieces[2 * n + i] = lo;
 }
 
+__device__ __forceinline__ void cp_async_16(uint32_t dst, const void* src, uint32_t src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+
+// ROWS = false: A (hidden tile) by TMA from one contiguous [T, d] matrix (tm_h).
+// ROWS = true : A rows fetched through per-row pointers (segments) by the four epilogue warps with 16-byte
+//               cp.async copies into the 128B-swizzled layout TMA would have produced; cp.async writes
+//               through the generic proxy and tcgen05.mma reads through the async proxy, so every loader
+//               thread waits for its own copies (two stages behind the one it issues), fences the proxies,
+//               and only then arrives on the stage's full barrier.
+template <bool ROWS>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_constant__ CUtensorMap tm_w,
                    const __grid_constant__ CUtensorMap tm_w1, int T, int d,
-                   int E, int ksplit, float* __restrict__ partial, int32_t* __restrict__ zero_buf, int zero_n) {
+                   int E, int ksplit, float* __restrict__ partial, int32_t* __restrict__ zero_buf, int zero_n,
+                   const void* const* __restrict__ seg_hidden, const int32_t* __restrict__ seg_start, int n_segs) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;
@@ -93,9 +105,9 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_consta
   const uint32_t idesc = umma_idesc_bf16(BM, n_mma, 0, 1);
 
   if (warp == 0 && lane == 0) {
-    tma_prefetch_desc(&tm_h);
+    if (!ROWS) tma_prefetch_desc(&tm_h);
     tma_prefetch_desc(&tm_w);
-    for (int s = 0; s < MAX_STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    for (int s = 0; s < MAX_STAGES; ++s) { mbar_init(full_bar(s), ROWS ? 1 + 128 : 1); mbar_init(empty_bar(s), 1); }
     mbar_init(done_bar, 1);
     fence_barrier_init();
   }
@@ -113,8 +125,8 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_consta
         mbar_wait(empty_bar(s), ph ^ 1u);
         const int kb = kb0 + it / ipk, pc0 = (it % ipk) * pps;
         const uint32_t sa = base + s * stage_bytes, sb = sa + A_BYTES;
-        mbar_expect_tx(full_bar(s), stage_bytes);
-        tma_load_2d(sa, &tm_h, full_bar(s), kb * BK, m_tile * BM);
+        mbar_expect_tx(full_bar(s), ROWS ? stage_bytes - A_BYTES : stage_bytes);
+        if (!ROWS) tma_load_2d(sa, &tm_h, full_bar(s), kb * BK, m_tile * BM);
         if (w4d) {                                  // one operation: [piece][block][k][64 e]
           tma_load_4d(sb, pps == 3 ? &tm_w : &tm_w1, full_bar(s), 0, kb * BK, 0, pc0);
         } else {
@@ -147,6 +159,45 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_consta
       umma_commit(done_bar);
     }
   } else if (warp >= 4) {
+    if (ROWS) {                                   // ---- row loader (thread <-> one row of the 128-token tile)
+      constexpr int LAG = 2;                      // stages in flight per thread (n_stages >= 3 always)
+      const int row = threadIdx.x - 128;
+      const int t = m_tile * BM + row;
+      const uint8_t* rowp = nullptr;
+      if (t < T) {
+        const int sg = seg_of(seg_start, n_segs, t);
+        rowp = static_cast<const uint8_t*>(seg_hidden[sg]) + static_cast<int64_t>(t - __ldg(seg_start + sg)) * d * 2;
+      }
+      const uint8_t* dummy = static_cast<const uint8_t*>(seg_hidden[0]);
+      const uint32_t dst_row = row * 128, sw = row & 7;
+      int s = 0, pub_s = 0, issued = 0;
+      uint32_t ph = 0;
+      for (int it = 0; it < n_iter; ++it) {
+        if (issued >= LAG) {                      // publish the stage issued LAG iterations ago
+          asm volatile("cp.async.wait_group %0;" ::"n"(LAG - 1) : "memory");
+          fence_proxy_async();
+          mbar_arrive(full_bar(pub_s));
+          if (++pub_s == n_stages) pub_s = 0;
+        }
+        mbar_wait(empty_bar(s), ph ^ 1u);
+        const int kb = kb0 + it / ipk;
+        const uint32_t sa = base + s * stage_bytes + dst_row;
+        #pragma unroll
+        for (int c = 0; c < 8; ++c) {             // chunk c of row r lands at r*128 + ((c ^ (r & 7)) << 4)
+          const bool ok = rowp != nullptr && kb * BK + c * 8 < d;
+          cp_async_16(sa + ((c ^ sw) << 4), ok ? rowp + kb * (BK * 2) + c * 16 : dummy, ok ? 16u : 0u);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        ++issued;
+        if (++s == n_stages) { s = 0; ph ^= 1u; }
+      }
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      fence_proxy_async();
+      for (int i = issued > LAG ? LAG : issued; i > 0; --i) {
+        mbar_arrive(full_bar(pub_s));
+        if (++pub_s == n_stages) pub_s = 0;
+      }
+    }
     const int q = warp & 3;                       // TMEM lane quarter of this warp
     const int row = m_tile * BM + q * 32 + lane;
     float* dst = partial + (static_cast<int64_t>(ks) * T + row) * E;
@@ -185,7 +236,9 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_consta
 }  // namespace
 
 cudaError_t router_kernels_init() {
-  return cudaFuncSetAttribute(router_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaError_t e = cudaFuncSetAttribute(router_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(router_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
 }
 
 cudaError_t launch_split_wr(const float* W_r, int d, int E, void* pieces, cudaStream_t st) {
@@ -210,7 +263,18 @@ cudaError_t launch_router_gemm(const CUtensorMap& tm_h, const CUtensorMap& tm_w,
                                float* partial, int32_t* zero_buf, int zero_n, cudaStream_t st) {
   if (T == 0) return cudaSuccess;
   dim3 grid((T + BM - 1) / BM, ksplit);
-  launch_pdl(router_gemm_kernel, grid, NUM_THREADS, SMEM_BYTES, st, tm_h, tm_w, tm_w1, T, d, E, ksplit, partial, zero_buf, zero_n);
+  launch_pdl(router_gemm_kernel<false>, grid, NUM_THREADS, SMEM_BYTES, st, tm_h, tm_w, tm_w1, T, d, E, ksplit, partial,
+             zero_buf, zero_n, static_cast<const void* const*>(nullptr), static_cast<const int32_t*>(nullptr), 0);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_router_gemm_segments(const SegTable& seg, const CUtensorMap& tm_w, const CUtensorMap& tm_w1, int T,
+                                        int d, int E, int ksplit, float* partial, int32_t* zero_buf, int zero_n,
+                                        cudaStream_t st) {
+  if (T == 0) return cudaSuccess;
+  dim3 grid((T + BM - 1) / BM, ksplit);
+  launch_pdl(router_gemm_kernel<true>, grid, NUM_THREADS, SMEM_BYTES, st, tm_w, tm_w, tm_w1, T, d, E, ksplit, partial,
+             zero_buf, zero_n, seg.hidden, seg.start, seg.n);
   return cudaGetLastError();
 }
 

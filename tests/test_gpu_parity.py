@@ -300,3 +300,56 @@ def test_planned_workspace_equals_allocated_workspace():
         layer = pk.MoELayer(d, f, E, k, T)
         assert layer.lib.bg_moe_workspace_bytes(layer._ctx) == pk.workspace_bytes_for(d, f, E, k, T)
         layer.close()
+
+
+@pytest.mark.parametrize("lengths", [
+    [256],                                   # one segment = the contiguous case
+    [16] * 16,                               # C1's 16 coroutines x 16 tokens
+    [100, 0, 1, 1, 1, 57, 0, 96],            # ragged, single-token (decode) and empty segments
+    [1] * 256,                               # every token its own coroutine
+    [130, 126],                              # a boundary inside a 128-token router tile, off the 8-row grid
+], ids=["one", "16x16", "ragged", "all-decode", "straddle"])
+def test_zero_copy_segments_equal_the_concatenation(lengths):
+    """bg_moe_combined_forward_segments: COMBINE = concatenation, so the
+    segment path must give bit-identical routing artefacts and outputs to the fused call on the concatenated
+    tensor, and that result is checked against the oracle."""
+    cfg = wl.C1
+    assert sum(lengths) == cfg.T
+    lay, g, layer = make(cfg)
+    ref_out = layer.combined_forward(g["hidden"]).clone()
+    v0 = {k: x.clone() for k, x in layer.debug_views(cfg.T).items()}
+    torch.cuda.synchronize()
+    # every segment in its own allocation (not views of one buffer), in list order
+    segs, pos = [], 0
+    for n in lengths:
+        segs.append(g["hidden"][pos:pos + n].clone())
+        pos += n
+    n0 = layer.launch_count
+    outs = layer.combined_forward_segments(segs)
+    torch.cuda.synchronize()
+    assert layer.launch_count - n0 == 8
+    v1 = layer.debug_views(cfg.T)
+    for key in ("logits", "idx", "w", "counts", "offsets", "row_src", "inv_perm"):
+        assert torch.equal(v0[key], v1[key]), key
+    got = torch.cat(outs, dim=0)
+    assert torch.equal(got, ref_out), "segment path differs from the concatenated path"
+    L = v1["logits"].cpu().numpy()
+    ref = oracle.forward_batched(lay["hidden"], lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"],
+                                 cfg.k, logits_in=L)["out"]
+    check_out(got, ref, f"segments {lengths[:4]}...")
+
+
+def test_zero_copy_segments_argument_errors_and_empty_batch():
+    import ctypes
+    from paper_2606_21712_b200.binding import BgMoeSegment, BG_ERR_INVALID_ARG
+    cfg = wl.C1
+    lay, g, layer = make(cfg)
+    assert layer.combined_forward_segments([]) == []                      # no segments: BG_OK, nothing launched
+    empty = torch.empty(0, cfg.d, dtype=torch.bfloat16, device="cuda")
+    n0 = layer.launch_count
+    layer.combined_forward_segments([empty, empty])
+    assert layer.launch_count == n0
+    too_many = [g["hidden"], g["hidden"][:1].clone()]                     # T + 1 tokens > max_tokens
+    with pytest.raises(Exception) as e:
+        layer.combined_forward_segments(too_many)
+    assert getattr(e.value, "status", None) == BG_ERR_INVALID_ARG
