@@ -275,6 +275,61 @@ def run_c3_sweep(steps: int, peaks: dict, device_index: int):
     return rows
 
 
+# ----------------------------------------------------------------------------- zero-copy COMBINE on C5
+def run_c5_combine(steps: int, device_index: int):
+    """BASELINE.json configs[4]: 30 prefill coroutines x 512 tokens + 1024 decode coroutines x 1 token combined
+    at one MoE boundary.  Times (a) concatenating the coroutines' buffers (torch.cat, one copy kernel per
+    call) followed by the fused chain and splitting the result back, against (b) the zero-copy entry point
+    that reads and writes the coroutines' own buffers (bg_moe_combined_forward_segments)."""
+    from paper_2606_21712_b200 import MoELayer
+    cfg = wl.CONFIGS["C5"]
+    lay = wl.make_layer(cfg, "cuda")
+    layer = MoELayer(cfg.d, cfg.f, cfg.E, cfg.k, cfg.T, device=device_index)
+    layer.set_weights(lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"])
+    lengths = [512] * 30 + [1] * 1024
+    segs, pos = [], 0
+    for n in lengths:
+        segs.append(lay["hidden"][pos:pos + n].clone())
+        pos += n
+    outs = [torch.empty_like(h) for h in segs]
+    table = layer.build_segments(segs, outs)
+    stream = torch.cuda.current_stream()
+    out_cat = torch.empty_like(lay["hidden"])
+
+    h_cat = torch.cat(segs, dim=0)
+
+    def contiguous_path():                   # the combined tensor already exists: no COMBINE cost at all
+        layer.combined_forward(h_cat, out_cat, stream)
+
+    def concat_path():                       # COMBINE as a copy: torch.cat, then the fused chain; the
+        h = torch.cat(segs, dim=0)           # per-coroutine results are views of out_cat (no split copies)
+        layer.combined_forward(h, out_cat, stream)
+
+    def zero_copy_path():
+        layer.combined_forward_segments(segs, outs, stream, table=table)
+
+    res = {}
+    for name, fn in (("fused_on_contiguous_ms", contiguous_path), ("concat_then_fused_ms", concat_path),
+                     ("zero_copy_segments_ms", zero_copy_path)):
+        torch.cuda.synchronize()
+        time.sleep(1.0)
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        res[name] = e0.elapsed_time(e1) / steps
+    res["segments"] = len(lengths)
+    res["note"] = ("fused_on_contiguous = the chain on an already concatenated tensor; concat_then_fused = torch.cat of "
+                   "the 1054 buffers + the chain (results left as views); zero_copy_segments = one call, rows addressed "
+                   "through the segment table, results written into the coroutines' own buffers")
+    return res
+
+
 # ----------------------------------------------------------------------------- our arm
 def run_ours(args):
     from paper_2606_21712_b200 import MoELayer
@@ -416,6 +471,8 @@ def run_ours(args):
         b_moe, reached = pk.choose_tokens(c3.d, c3.f, c3.E, c3.k, fit, 0.8, 8 << 30, 64)
         line["plan_c3"] = {"fit": fit.as_dict(), "target_util": 0.8, "memory_budget_bytes": 8 << 30,
                            "B_moe_tokens": b_moe, "target_reached": reached}
+    if rank == 0 and world == 1 and not args.no_sweep:
+        line["combine_c5"] = run_c5_combine(args.steps, local)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
         cores = oracle.num_threads()

@@ -182,11 +182,8 @@ class MoELayer:
                                                           _stream(stream)))
         return out_host
 
-    def combined_forward_segments(self, hidden_segments, out_segments=None, stream=None):
-        """bg_moe_combined_forward_segments: zero-copy COMBINE.  hidden_segments: list of CUDA bf16 tensors
-        [n_s, d] (the yielded coroutines' buffers; n_s may be 0); returns the list of per-segment outputs."""
-        if out_segments is None:
-            out_segments = [torch.empty_like(h) for h in hidden_segments]
+    def build_segments(self, hidden_segments, out_segments):
+        """The bg_moe_segment array for a list of per-coroutine tensors (marshalling only; reusable)."""
         n = len(hidden_segments)
         arr = (BgMoeSegment * max(n, 1))()
         for i, (h, o) in enumerate(zip(hidden_segments, out_segments)):
@@ -195,6 +192,15 @@ class MoELayer:
             arr[i].hidden = h.data_ptr() if h.shape[0] else None
             arr[i].out = o.data_ptr() if o.shape[0] else None
             arr[i].n_tokens = h.shape[0]
+        return arr, n
+
+    def combined_forward_segments(self, hidden_segments, out_segments=None, stream=None, table=None):
+        """bg_moe_combined_forward_segments: zero-copy COMBINE.  hidden_segments: list of CUDA bf16 tensors
+        [n_s, d] (the yielded coroutines' buffers; n_s may be 0); returns the list of per-segment outputs.
+        `table` = a (array, n) pair from build_segments for the same tensors skips the marshalling."""
+        if out_segments is None:
+            out_segments = [torch.empty_like(h) for h in hidden_segments]
+        arr, n = table if table is not None else self.build_segments(hidden_segments, out_segments)
         self.lib.bg_moe_combined_forward_segments.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32,
                                                               ctypes.c_void_p]
         self._check(self.lib.bg_moe_combined_forward_segments(self._ctx, ctypes.cast(arr, ctypes.c_void_p),

@@ -160,32 +160,44 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_consta
     }
   } else if (warp >= 4) {
     if (ROWS) {                                   // ---- row loader (thread <-> one row of the 128-token tile)
-      constexpr int LAG = 2;                      // stages in flight per thread (n_stages >= 3 always)
-      const int row = threadIdx.x - 128;
-      const int t = m_tile * BM + row;
-      const uint8_t* rowp = nullptr;
-      if (t < T) {
-        const int sg = seg_of(seg_start, n_segs, t);
-        rowp = static_cast<const uint8_t*>(seg_hidden[sg]) + static_cast<int64_t>(t - __ldg(seg_start + sg)) * d * 2;
+      const int LAG = min(4, n_stages - 1);       // stages in flight per thread (n_stages >= 3 always)
+      // Eight consecutive lanes copy the eight 16-byte chunks of one row's 128-byte k-span (one full line
+      // per row); a warp instruction covers 4 rows, 8 instructions the warp's 32 rows.
+      const int lw = warp - 4, sub = lane >> 3, chunk = lane & 7;
+      const uint8_t* rowp[8];
+      uint32_t dst_off[8];
+      #pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int row = lw * 32 + j * 4 + sub;
+        const int t = m_tile * BM + row;
+        rowp[j] = nullptr;
+        if (t < T) {
+          const int sg = seg_of(seg_start, n_segs, t);
+          rowp[j] = static_cast<const uint8_t*>(seg_hidden[sg]) + static_cast<int64_t>(t - __ldg(seg_start + sg)) * d * 2 +
+                    chunk * 16;
+        }
+        dst_off[j] = row * 128 + ((chunk ^ (row & 7)) << 4);   // the 128B swizzle TMA applies
       }
       const uint8_t* dummy = static_cast<const uint8_t*>(seg_hidden[0]);
-      const uint32_t dst_row = row * 128, sw = row & 7;
       int s = 0, pub_s = 0, issued = 0;
       uint32_t ph = 0;
       for (int it = 0; it < n_iter; ++it) {
         if (issued >= LAG) {                      // publish the stage issued LAG iterations ago
-          asm volatile("cp.async.wait_group %0;" ::"n"(LAG - 1) : "memory");
+          if (LAG == 4) asm volatile("cp.async.wait_group 3;" ::: "memory");
+          else if (LAG == 3) asm volatile("cp.async.wait_group 2;" ::: "memory");
+          else asm volatile("cp.async.wait_group 1;" ::: "memory");
           fence_proxy_async();
           mbar_arrive(full_bar(pub_s));
           if (++pub_s == n_stages) pub_s = 0;
         }
         mbar_wait(empty_bar(s), ph ^ 1u);
         const int kb = kb0 + it / ipk;
-        const uint32_t sa = base + s * stage_bytes + dst_row;
+        const uint32_t sa = base + s * stage_bytes;
+        const bool k_ok = kb * BK + chunk * 8 < d;          // k past d must read as zero
         #pragma unroll
-        for (int c = 0; c < 8; ++c) {             // chunk c of row r lands at r*128 + ((c ^ (r & 7)) << 4)
-          const bool ok = rowp != nullptr && kb * BK + c * 8 < d;
-          cp_async_16(sa + ((c ^ sw) << 4), ok ? rowp + kb * (BK * 2) + c * 16 : dummy, ok ? 16u : 0u);
+        for (int j = 0; j < 8; ++j) {
+          const bool ok = k_ok && rowp[j] != nullptr;
+          cp_async_16(sa + dst_off[j], ok ? rowp[j] + kb * (BK * 2) : dummy, ok ? 16u : 0u);
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
         ++issued;
