@@ -353,3 +353,60 @@ def test_zero_copy_segments_argument_errors_and_empty_batch():
     with pytest.raises(Exception) as e:
         layer.combined_forward_segments(too_many)
     assert getattr(e.value, "status", None) == BG_ERR_INVALID_ARG
+
+
+def _guarded(rows, cols, dtype=torch.bfloat16, guard=8):
+    """A [rows, cols] view in the middle of a larger buffer whose other rows hold a sentinel."""
+    full = torch.full((rows + 2 * guard, cols), 123.0, dtype=dtype, device="cuda")
+    return full, full[guard:guard + rows], guard
+
+
+def _guards_intact(full, rows, guard):
+    return bool((full[:guard] == 123.0).all()) and bool((full[guard + rows:] == 123.0).all())
+
+
+def test_no_writes_outside_the_output_buffers():
+    """Bounds check of our own (compute-sanitizer is not available on the GPU pool): every caller-owned
+    output sits between sentinel rows; ragged experts, a ragged last router tile and a column count that is
+    not a multiple of 64 exercise the masked stores of both GEMM epilogues, the gather and the un-permute."""
+    import ctypes
+    from paper_2606_21712_b200.binding import _ptr, _stream
+    cfg = wl.small_config(T=333, d=200, E=7, k=3, f=136, index=21)
+    lay, g, layer = make(cfg)
+    T, R = cfg.T, cfg.T * cfg.k
+    # fused call
+    full_o, out, gd = _guarded(T, cfg.d)
+    layer.combined_forward(g["hidden"], out)
+    torch.cuda.synchronize()
+    assert _guards_intact(full_o, T, gd)
+    ref = layer.combined_forward(g["hidden"]).clone()
+    assert torch.equal(out, ref)
+    # split calls on guarded buffers
+    r = layer.route(g["hidden"])
+    full_x, x_perm, _ = _guarded(R, cfg.d)
+    full_rs = torch.full((R + 16,), -77, dtype=torch.int32, device="cuda")
+    full_ip = torch.full((R + 16,), -77, dtype=torch.int32, device="cuda")
+    layer._check(layer.lib.bg_moe_permute(layer._ctx, _ptr(g["hidden"]), T, _ptr(r["idx"]), _ptr(r["offsets"]),
+                                          _ptr(full_rs[8:8 + R]), _ptr(full_ip[8:8 + R]), _ptr(x_perm), _stream(None)))
+    full_y, y_perm, _ = _guarded(R, cfg.d)
+    layer._check(layer.lib.bg_moe_expert_ffn(layer._ctx, _ptr(x_perm), _ptr(r["offsets"]), T, _ptr(y_perm), _stream(None)))
+    full_o2, out2, _ = _guarded(T, cfg.d)
+    layer._check(layer.lib.bg_moe_unpermute(layer._ctx, _ptr(y_perm), _ptr(full_ip[8:8 + R]), _ptr(r["w"]), T,
+                                            _ptr(out2), _stream(None)))
+    torch.cuda.synchronize()
+    assert _guards_intact(full_x, R, gd) and _guards_intact(full_y, R, gd) and _guards_intact(full_o2, T, gd)
+    for t_ in (full_rs, full_ip):
+        assert bool((t_[:8] == -77).all()) and bool((t_[8 + R:] == -77).all())
+    # zero-copy segments: each coroutine's output between its own sentinels
+    lengths = [100, 1, 0, 232]
+    segs, outs, fulls, pos = [], [], [], 0
+    for n in lengths:
+        segs.append(g["hidden"][pos:pos + n].clone())
+        full, view, _ = _guarded(n, cfg.d)
+        fulls.append(full)
+        outs.append(view)
+        pos += n
+    layer.combined_forward_segments(segs, outs)
+    torch.cuda.synchronize()
+    assert all(_guards_intact(f_, n, gd) for f_, n in zip(fulls, lengths))
+    assert torch.equal(torch.cat(outs, 0), ref)
