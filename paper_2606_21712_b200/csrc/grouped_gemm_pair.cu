@@ -25,11 +25,12 @@
 //   D (TMEM) : [128 lanes = features] x [nt columns = tokens] fp32 per CTA, two stages of 256 columns
 // The weights are consumed in the layout the layer is given (reading S14): no transpose/prepack.
 //
-// Warp roles (persistent, one 256-thread CTA per SM, 74 clusters):
+// Warp roles (persistent, one CTA per SM, 74 clusters; every launch uses programmatic dependent launch):
 //   warp 0 lane 0: TMA producer (both CTAs; transaction bytes of both land on the leader's barrier)
 //   warp 1 lane 0: tcgen05.mma issuer (leader CTA only); commits are multicast to both CTAs
 //   warp 2       : TMEM allocator
-//   warps 4-7    : epilogue (TMEM -> registers -> SwiGLU | gate weight -> bf16 -> smem transpose -> global)
+//   warps 4-7    : epilogue (TMEM -> registers -> SwiGLU | gate weight -> bf16 -> smem transpose -> global);
+//                  a8 adds warps 8-11 (384 threads): its k loops are short, two warps serve each TMEM lane quarter
 //
 // a7 epilogue: gate and up accumulators of one feature live in TMEM lanes f and 64+f, i.e. in
 // different warps.  Warp pairs (0,2) and (1,3) exchange 32-token chunks through shared memory: for
