@@ -34,6 +34,8 @@ struct bg_moe_ctx {
   int32_t* row_src = nullptr;
   int32_t* inv_perm = nullptr;
   float* w_perm = nullptr;      // gate weights in expert order (fused path)
+  int32_t* tile_counters = nullptr;   // [4]: ticket / finished counters of the two pair GEMMs (self re-arming)
+  bool dyn_sched = true;        // dynamic tile feed of the pair GEMMs (BG_MOE_SCHED=static: tile t -> cluster t mod 74)
   // segment table of bg_moe_combined_forward_segments (device arrays + pageable host staging)
   int32_t max_segments = 0;
   const void** seg_dev_hidden = nullptr;
@@ -214,6 +216,7 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g1.tm_b0 = ctx->tm_wg;
   g1.tm_b1 = ctx->tm_wu;
   g1.sg_max = ctx->sg_max;
+  g1.tile_counter = ctx->dyn_sched ? ctx->tile_counters : nullptr;
   g1.w4d = c.f % 64 == 0;
   g1.tm_b0_4d = g1.w4d ? ctx->tm_wg4 : ctx->tm_wg;
   g1.tm_b1_4d = g1.w4d ? ctx->tm_wu4 : ctx->tm_wu;
@@ -230,6 +233,7 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g2.tm_b0 = ctx->tm_wd;
   g2.tm_b1 = ctx->tm_wd;
   g2.sg_max = ctx->sg_max;
+  g2.tile_counter = ctx->dyn_sched ? ctx->tile_counters + 2 : nullptr;
   g2.w4d = c.d % 64 == 0;
   g2.tm_b0_4d = g2.w4d ? ctx->tm_wd4 : ctx->tm_wd;
   g2.tm_b1_4d = g2.tm_b0_4d;
@@ -314,6 +318,12 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   ctx->row_src = reinterpret_cast<int32_t*>(ctx->ws + o_rs);
   ctx->inv_perm = reinterpret_cast<int32_t*>(ctx->ws + o_ip);
   ctx->w_perm = reinterpret_cast<float*>(ctx->ws + o_wp);
+  ctx->tile_counters = reinterpret_cast<int32_t*>(ctx->ws + L.tile_counters);
+  if (cudaMemset(ctx->tile_counters, 0, 16) != cudaSuccess) {
+    cudaFree(ctx->ws);
+    delete ctx;
+    return BG_ERR_CUDA;
+  }
   ctx->max_segments = static_cast<int32_t>(Tm);
   ctx->seg_dev_hidden = reinterpret_cast<const void**>(ctx->ws + L.seg_hidden);
   ctx->seg_dev_out = reinterpret_cast<void**>(ctx->ws + L.seg_out);
@@ -331,6 +341,8 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   {
     const char* g = std::getenv("BG_MOE_GEMM");
     if (g != nullptr && std::strcmp(g, "tile") == 0) ctx->pair_gemm = false;
+    const char* sc = std::getenv("BG_MOE_SCHED");
+    if (sc != nullptr && std::strcmp(sc, "static") == 0) ctx->dyn_sched = false;
     const char* sg = std::getenv("BG_MOE_SG_TOKEN_TILES");
     if (sg != nullptr && std::atoi(sg) > 0) ctx->sg_max = std::atoi(sg);
   }

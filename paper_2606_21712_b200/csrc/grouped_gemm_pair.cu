@@ -52,6 +52,7 @@ constexpr int BN_MAX = 256;        // UMMA N max: tokens per tile
 constexpr int BK = 64;             // k per pipeline stage = one 128-byte swizzle span of bf16
 constexpr int UK = 16;             // UMMA K for 16-bit inputs
 constexpr int STAGES = 6;
+constexpr int SCHED_SLOTS = 4;     // tile indices published ahead by the dynamic scheduler
 constexpr int A_BLK_BYTES = 64 * BK * 2;            // 8 KB: one 64-feature block of weights
 constexpr int A_BYTES = 2 * A_BLK_BYTES;            // 16 KB: this CTA's 128 M rows
 constexpr int B_BYTES = (BN_MAX / 2) * BK * 2;      // 16 KB: this CTA's half of the tokens
@@ -84,6 +85,7 @@ struct Params {
   const float* row_scale;      // a8, fused path: gate weight per expert-order row (w_perm[r]); nullptr = 1
   bool w4d;                    // tm_w0 / tm_w1 are the 4-D block views (kernels.h)
   int sg_max;                  // 0 = derive the super-group size from K
+  int* tile_counter;           // dynamic feed: [2] = ticket counter, clusters-finished counter (zero between launches); nullptr = static feed
 };
 
 __device__ __forceinline__ void named_bar_sync(int id, int threads) {
@@ -177,7 +179,14 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
   auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + a); };
   auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + 2 + a); };
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + RING_BYTES + 8 * (2 * STAGES + 4));
+  // tile feed (dynamic scheduler): sched_full[SCHED_SLOTS] per CTA, sched_empty[SCHED_SLOTS] on the leader
+  auto sfull_bar = [&](int i) { return bar_base + 8u * (2 * STAGES + 4 + i); };
+  auto sempty_bar = [&](int i) { return bar_base + 8u * (2 * STAGES + 4 + SCHED_SLOTS + i); };
+  constexpr int NBAR = 2 * STAGES + 4 + 2 * SCHED_SLOTS;
+  static_assert(8 * NBAR + 16 + 4 * SCHED_SLOTS <= BAR_BYTES, "barrier area");
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + RING_BYTES + 8 * NBAR);
+  volatile int* tile_slot = reinterpret_cast<volatile int*>(smem + RING_BYTES + 8 * NBAR + 16);
+  constexpr int N_CONSUMERS = 3 + 2 * EPI_WARPS;      // two producers, the MMA thread, every epilogue warp of the pair
   int* tile_start = reinterpret_cast<int*>(smem + RING_BYTES + BAR_BYTES);
   int* t_tiles = tile_start + (MAX_E + 1);
   uint8_t* epi_smem = smem + RING_BYTES + BAR_BYTES + TABLE_BYTES;
@@ -198,6 +207,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
     // tmem_empty (used on the leader only): one arrival per epilogue warp of both CTAs
     for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 2 * EPI_WARPS); }
+    for (int i = 0; i < SCHED_SLOTS; ++i) { mbar_init(sfull_bar(i), 1); mbar_init(sempty_bar(i), N_CONSUMERS); }
     fence_barrier_init();
   }
   if (warp == 2) {
@@ -237,12 +247,39 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   const uint32_t tmem_base = *tmem_slot;
   const int total_tiles = tile_start[E];
 
+  // ---- tile feed.  Static (tile_counter == nullptr): cluster c takes tiles c, c + 74, ...  Dynamic: tiles
+  // are handed out in linear order from a global ticket counter by one thread of the leader CTA (warp 3),
+  // written to a 4-slot ring in BOTH CTAs' shared memory and published through sched_full; every consumer
+  // (the two TMA producers, the MMA thread, each epilogue warp) reads the ticket and hands the slot back on
+  // the leader's sched_empty.  -1 ends the stream.  With tickets drawn in real time the token tiles that
+  // share a weight strip stay concurrent however unequal the tiles of a launch are.
+  const bool dyn = p.tile_counter != nullptr;
+  struct Feed { int slot; uint32_t ph; int t; };
+  auto feed_next = [&](Feed& f, bool warp_collective) -> int {
+    if (!dyn) {
+      f.t = (f.t < 0) ? cluster_id : f.t + num_clusters;
+      return f.t < total_tiles ? f.t : -1;
+    }
+    mbar_wait_cluster(sfull_bar(f.slot), f.ph);
+    const int t = tile_slot[f.slot];
+    // Hand the slot back with a RELAXED arrive whose address depends on the ticket just read (so it cannot
+    // pass the read): a releasing arrive is a fence that waits for the thread's outstanding work -- the
+    // epilogue's global stores, the MMA thread's in-flight tcgen05 operations -- once per tile.
+    uint32_t zero;
+    asm volatile("and.b32 %0, %1, 0;" : "=r"(zero) : "r"(t));
+    if (warp_collective) __syncwarp();                 // all 32 lanes have read; one lane arrives
+    if (!warp_collective || lane == 0) mbar_arrive_cluster_relaxed(sempty_bar(f.slot) + zero, 0);
+    if (++f.slot == SCHED_SLOTS) { f.slot = 0; f.ph ^= 1u; }
+    return t;
+  };
+
   if (warp == 0) {
     // ===================== TMA producer (one thread per CTA) =====================
     if (lane == 0) {
       int s = 0;
       uint32_t ph = 0;
-      for (int t = cluster_id; t < total_tiles; t += num_clusters) {
+      Feed feed = {0, 0, -1};
+      for (int t = feed_next(feed, false); t >= 0; t = feed_next(feed, false)) {
         const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
         const int n0 = c.f_tile * OUT_FEATS + static_cast<int>(rank) * CTA_FEATS;
         const int half = c.nt >> 1;                    // this CTA's tokens (multiple of 8, <= 128)
@@ -272,13 +309,37 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         }
       }
     }
+  } else if (warp == 3) {
+    // ===================== tile scheduler (dynamic feed only; one thread of the leader CTA) ==========
+    if (dyn && lane == 0 && rank == 0) {
+      int slot = 0;
+      uint32_t ph = 0;
+      while (true) {
+        mbar_wait(sempty_bar(slot), ph ^ 1u);          // every consumer has read this slot's previous ticket
+        int t = atomicAdd(p.tile_counter, 1);
+        if (t >= total_tiles) t = -1;
+        tile_slot[slot] = t;
+        st_shared_cluster_u32(smem_u32(const_cast<int*>(tile_slot + slot)), 1, static_cast<uint32_t>(t));
+        mbar_arrive(sfull_bar(slot));                  // release.cta: the local store above
+        mbar_arrive_cluster(sfull_bar(slot), 1);       // release.cluster: the remote store above
+        if (t < 0) break;
+        if (++slot == SCHED_SLOTS) { slot = 0; ph ^= 1u; }
+      }
+      // the last cluster to run dry re-arms the counters for the next launch
+      if (atomicAdd(p.tile_counter + 1, 1) == num_clusters - 1) {
+        p.tile_counter[0] = 0;
+        p.tile_counter[1] = 0;
+        __threadfence();
+      }
+    }
   } else if (warp == 1) {
     // ===================== MMA issuer (one thread of the leader CTA) =====================
     if (lane == 0 && rank == 0) {
       int s = 0;
       uint32_t ph = 0;
       int it = 0;
-      for (int t = cluster_id; t < total_tiles; t += num_clusters, ++it) {
+      Feed feed = {0, 0, -1};
+      for (int t = feed_next(feed, false); t >= 0; t = feed_next(feed, false), ++it) {
         const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
         const uint32_t idesc = IDESC_BASE | (static_cast<uint32_t>(c.nt >> 3) << 17);
         const int as = it & 1;
@@ -318,15 +379,18 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     const uint32_t stage_rd = smem_u32(stage) + (lane >> 2) * 64 + (lane & 3) * 16;   // + i * 512
     float* sc_smem = reinterpret_cast<float*>(epi_smem);                        // a8: [2][BN_MAX] gate weights, double-buffered
     const int feat0 = static_cast<int>(rank) * CTA_FEATS + (GATEUP ? (q & 1) : q) * 32;   // in the pair tile
-    if (!GATEUP && cluster_id < total_tiles) {       // gate weights of the first tile -> buffer 0
-      const TileCoord c0 = decode_tile(cluster_id, tile_start, t_tiles, p.offsets, E, sg_max);
+    Feed feed = {0, 0, -1};
+    int t = feed_next(feed, true);
+    if (!GATEUP && t >= 0) {                         // gate weights of the first tile -> buffer 0
+      const TileCoord c0 = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
       float sc = 1.0f;
       if (p.row_scale != nullptr && ew * 32 + lane < c0.rows_valid) sc = __ldg(p.row_scale + c0.row0 + ew * 32 + lane);
       sc_smem[ew * 32 + lane] = sc;
     }
     int it = 0;
-    for (int t = cluster_id; t < total_tiles; t += num_clusters, ++it) {
+    for (; t >= 0; ++it) {
       const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
+      const int tn = feed_next(feed, true);            // this cluster's next tile (-1: none)
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1u;
       const int n_chunks = (c.nt + 31) >> 5;           // 32-token chunks (the last may be half used)
@@ -339,8 +403,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         // ew*32 .. +31 now and parks them in the other buffer after this tile's chunks, so the load
         // latency never sits on the epilogue's critical path.  The barrier makes this tile's buffer
         // (written by all eight warps at the end of the previous tile) visible.
-        const int tn = t + num_clusters;
-        if (tn < total_tiles && p.row_scale != nullptr) {
+        if (tn >= 0 && p.row_scale != nullptr) {
           const TileCoord cn = decode_tile(tn, tile_start, t_tiles, p.offsets, E, sg_max);
           if (ew * 32 + lane < cn.rows_valid) sc_next = __ldg(p.row_scale + cn.row0 + ew * 32 + lane);
         }
@@ -424,6 +487,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive_cluster_relaxed(tempty_bar(as), 0);   // relaxed: must not wait for the stores
+      t = tn;
     }
   }
 
@@ -446,6 +510,7 @@ Params make_params(const GemmLaunch& g) {
   p.row_scale = g.row_scale_perm;
   p.w4d = g.w4d;
   p.sg_max = g.sg_max;
+  p.tile_counter = g.tile_counter;
   return p;
 }
 

@@ -51,7 +51,7 @@ struct SegTable {
 // ---- workspace layout (plan.cu): byte offsets of every slab of the context's single allocation
 struct WsLayout {
   int64_t logits, idx, w, part, pieces, counts, offsets, bc, bb, rs, ip, wp, x, h, y, hd, od, seg_hidden, seg_out,
-      seg_start, total;
+      seg_start, tile_counters, total;
 };
 WsLayout ws_layout(const bg_moe_config& c, int64_t max_tokens, int num_sms);
 
@@ -108,6 +108,7 @@ struct GemmLaunch {
   // Valid only when N % 64 == 0 (w4d); otherwise the kernels issue one 3-D box per block.
   CUtensorMap tm_b0_4d, tm_b1_4d;
   bool w4d;
+  int* tile_counter;   // pair kernel, dynamic tile feed: two ints (tickets, clusters finished), zero between launches; nullptr = static
   int sg_max;          // pair kernel: token tiles per super-group (0 = sized from K to ~48 MB of tokens)
   const int32_t* offsets;  // [E+1]
   int E, K, N;         // N = output columns (f for gate/up, d for down)

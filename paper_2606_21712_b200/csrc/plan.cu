@@ -40,6 +40,7 @@ WsLayout ws_layout(const bg_moe_config& c, int64_t max_tokens, int num_sms) {
   L.seg_hidden = carve(Tm * 8);      // segment table: at most max_tokens segments
   L.seg_out = carve(Tm * 8);
   L.seg_start = carve((Tm + 1) * 4);
+  L.tile_counters = carve(16);
   L.total = off;
   return L;
 }

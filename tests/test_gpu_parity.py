@@ -153,12 +153,15 @@ def test_expert_ffn_parity(rows, d, f):
             check_out(y[offsets[e]:offsets[e + 1]], ref[offsets[e]:offsets[e + 1]], f"expert {e}")
 
 
-@pytest.mark.parametrize("env", [{"BG_MOE_SG_TOKEN_TILES": "2"}, {"BG_MOE_SG_TOKEN_TILES": "1"}, {"BG_MOE_GEMM": "tile"}],
-                         ids=["supergroups-of-2", "supergroups-of-1", "tile-kernel"])
+@pytest.mark.parametrize("env", [{"BG_MOE_SG_TOKEN_TILES": "2"}, {"BG_MOE_SG_TOKEN_TILES": "1"}, {"BG_MOE_GEMM": "tile"},
+                                 {"BG_MOE_SCHED": "static"}, {"BG_MOE_SCHED": "static", "BG_MOE_SG_TOKEN_TILES": "2"}],
+                         ids=["supergroups-of-2", "supergroups-of-1", "tile-kernel", "static-feed",
+                              "static-feed-supergroups"])
 def test_expert_ffn_scheduler_variants(env, monkeypatch):
     """The same FFN through (i) the pair kernel's super-group tile order, which production shapes only
-    reach with experts of several thousand rows (forced here on experts of 3-5 token tiles), and (ii) the
-    1-CTA 128x256 kernel that BG_MOE_GEMM=tile selects."""
+    reach with experts of several thousand rows (forced here on experts of 3-5 token tiles), (ii) the
+    1-CTA 128x256 kernel that BG_MOE_GEMM=tile selects, and (iii) the static tile feed (BG_MOE_SCHED=static;
+    the default is the dynamic ticket feed)."""
     for k_, v in env.items():
         monkeypatch.setenv(k_, v)              # read once, in bg_moe_create
     rows = [1300, 0, 700, 257, 16, 1]
