@@ -29,6 +29,7 @@
 //   warp 0 lane 0: TMA producer (both CTAs; transaction bytes of both land on the leader's barrier)
 //   warp 1 lane 0: tcgen05.mma issuer (leader CTA only); commits are multicast to both CTAs
 //   warp 2       : TMEM allocator
+//   warp 3 lane 0: tile scheduler (leader only): ticket counter -> 4-slot ring in both CTAs' shared memory
 //   warps 4-7    : epilogue (TMEM -> registers -> SwiGLU | gate weight -> bf16 -> smem transpose -> global);
 //                  a8 adds warps 8-11 (384 threads): its k loops are short, two warps serve each TMEM lane quarter
 //
@@ -40,7 +41,9 @@
 // Tile scheduler: token tiles never straddle experts.  Expert e with n_e rows owns
 // tt_e = ceil(n_e/256) token tiles of ceil16(ceil(n_e/tt_e)) rows (the last one shorter) times
 // ceil(N_out/OUT_FEATS) feature tiles, ordered feature-tile-major / token-tile-minor so that the
-// clusters running at the same time share weight strips through L2.  Tile t -> cluster (t mod #clusters).
+// clusters running at the same time share weight strips through L2.  Tiles are drawn in that order from a
+// global ticket counter (dynamic feed, see `feed_next`), so the neighbours really run concurrently and a strip
+// is read from HBM once; BG_MOE_SCHED=static keeps the fixed map tile t -> cluster (t mod #clusters).
 // Experts with no rows own no tiles and their weights are never touched.
 #include "kernels.h"
 #include "ptx_sm100.cuh"
