@@ -413,3 +413,30 @@ def test_no_writes_outside_the_output_buffers():
     torch.cuda.synchronize()
     assert all(_guards_intact(f_, n, gd) for f_, n in zip(fulls, lengths))
     assert torch.equal(torch.cat(outs, 0), ref)
+
+
+def test_dynamic_tile_feed_rearms_across_many_launches():
+    """The pair GEMMs draw tiles from ticket counters that the last cluster of a launch re-arms.  Many
+    back-to-back launches with changing token counts (hence changing tile counts, including fewer tiles than
+    clusters) must neither hang nor change results: every call is compared bit for bit with the first result
+    for that token count."""
+    cfg = wl.small_config(T=700, d=256, E=16, k=4, f=192, index=31)
+    lay, g, layer = make(cfg)
+    first = {}
+    rng = np.random.default_rng(0)
+    for it in range(120):
+        T = int(rng.choice([1, 3, 64, 129, 300, 700]))
+        out = layer.combined_forward(g["hidden"][:T].contiguous())
+        if it % 10 == 9:
+            torch.cuda.synchronize()
+        if T in first:
+            assert torch.equal(out, first[T]), f"launch {it}, T={T}: result changed"
+        else:
+            first[T] = out.clone()
+    last = layer.combined_forward(g["hidden"])            # T = 700 once more: its logits feed the oracle
+    torch.cuda.synchronize()
+    assert torch.equal(last, first[700])
+    L = layer.debug_views(700)["logits"].cpu().numpy()
+    ref = oracle.forward_batched(lay["hidden"], lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"],
+                                 cfg.k, logits_in=L)["out"]
+    check_out(first[700], ref, "T=700 after 120 launches")
