@@ -187,7 +187,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_consta
           else if (LAG == 3) asm volatile("cp.async.wait_group 2;" ::: "memory");
           else asm volatile("cp.async.wait_group 1;" ::: "memory");
           fence_proxy_async();
-          mbar_arrive(full_bar(pub_s));
+          mbar_arrive_relaxed(full_bar(pub_s));
           if (++pub_s == n_stages) pub_s = 0;
         }
         mbar_wait(empty_bar(s), ph ^ 1u);
@@ -206,7 +206,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_consta
       asm volatile("cp.async.wait_group 0;" ::: "memory");
       fence_proxy_async();
       for (int i = issued > LAG ? LAG : issued; i > 0; --i) {
-        mbar_arrive(full_bar(pub_s));
+        mbar_arrive_relaxed(full_bar(pub_s));
         if (++pub_s == n_stages) pub_s = 0;
       }
     }
