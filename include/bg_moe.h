@@ -22,7 +22,9 @@
  *    T = combined tokens, d = hidden, E = experts, k = top-k, f = expert intermediate, R = T*k.
  *  - Indices are int32 (R <= 2^31-1); byte offsets are computed in 64 bits.
  *  - Return value: BG_OK (0) or a negative bg_moe_status.  Nothing aborts or throws across the
- *    ABI.  T == 0 is BG_OK and a no-op.  A context is not thread-safe: one call at a time.
+ *    ABI.  T == 0 is BG_OK and a no-op.  A context is not thread-safe: one call at a time, and the
+ *    calls made on one context must be STREAM-ORDERED with respect to each other (same stream, or
+ *    streams the caller orders with events): they share the context's workspace and tile counters.
  *  - Supported ranges: 1 <= E <= 256, 1 <= k <= min(E, 8), d and f multiples of 8 (d >= 64,
  *    f >= 64), 0 <= T <= max_tokens.  Device must be sm_100 (B200).  There is no CPU fallback.
  */
@@ -65,8 +67,16 @@ int bg_moe_destroy(bg_moe_ctx* ctx);
 /* Borrows (does not copy) the layer's parameters.  W_r fp32 [d,E]; b_r fp32 [E] or NULL (reading
  * S7: added to the logits in fp32, used for selection and gates); W_gate, W_up bf16 [E,d,f];
  * W_down bf16 [E,f,d].  Consumed in these layouts as given (reading S14). */
+/* Asynchronous on `stream` like every other call: the only device work is the exact bf16 three-way
+ * split of W_r (read on `stream`, so a W_r produced on that stream is ordered before it). */
 int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, const void* W_gate,
-                       const void* W_up, const void* W_down);
+                       const void* W_up, const void* W_down, void* stream);
+
+/* Debug / test switches of the grouped-GEMM tile scheduler; production never calls this.
+ *   static_tile_feed != 0     tile t -> cluster (t mod #clusters) instead of the dynamic ticket feed
+ *   supergroup_token_tiles    > 0: token tiles per super-group (forces the super-group order on small
+ *                             shapes); 0: sized from K so that a super-group's tokens fit ~48 MB of L2 */
+int bg_moe_set_debug(bg_moe_ctx* ctx, int32_t static_tile_feed, int32_t supergroup_token_tiles);
 
 /* Steps a1-a4: router logits, top-k + gates, histogram, exclusive scan.
  *   hidden     bf16 [T,d]
@@ -119,8 +129,13 @@ typedef struct {
 int bg_moe_combined_forward_segments(bg_moe_ctx* ctx, const bg_moe_segment* segments,
                                      int32_t n_segments, void* stream);
 
-/* Same, but `hidden_host` and `out_host` are HOST pointers (pinned memory recommended): copies
- * hidden host->device, runs the fused chain, copies out device->host, all on `stream`. */
+/* Same, but `hidden_host` and `out_host` are HOST pointers (pinned memory, or the copies are not
+ * asynchronous): hidden host->device, the fused chain, out device->host.  The three run on streams the
+ * context owns, over two staging slots, so that consecutive calls overlap the upload of call i+1 and the
+ * download of call i-1 with the GEMMs of call i.  Ordering: hidden_host must hold its data when the call is
+ * made (host memory is not stream-ordered); the call is ordered after every earlier call on the context;
+ * `stream` is made to wait for the download, so work enqueued on `stream` afterwards -- or a synchronize
+ * on it -- sees out_host complete. */
 int bg_moe_combined_forward_host(bg_moe_ctx* ctx, const void* hidden_host, int32_t T,
                                  void* out_host, void* stream);
 
@@ -132,10 +147,11 @@ int bg_moe_debug_views(bg_moe_ctx* ctx, const float** logits, const int32_t** to
 
 /* Per-kernel timing of the fused chain.  While enabled, bg_moe_combined_forward records a CUDA
  * event on `stream` before and after each of its BG_MOE_NUM_STAGES kernels (in launch order:
- * router, top-k+histogram, scan, rank, gather, gate/up GEMM+SwiGLU, down GEMM, un-permute reduce).
+ * fused router (logits, top-k, histogram, scan, tile ranks), gather (+ permutation), gate/up
+ * GEMM+SwiGLU, down GEMM, un-permute reduce).
  * bg_moe_profile_read waits for the last recorded call and writes that call's per-kernel
  * durations in milliseconds to ms_out[BG_MOE_NUM_STAGES] (HOST pointer). */
-#define BG_MOE_NUM_STAGES 8
+#define BG_MOE_NUM_STAGES 5
 int bg_moe_profile_enable(bg_moe_ctx* ctx, int enable);
 int bg_moe_profile_read(bg_moe_ctx* ctx, float* ms_out);
 

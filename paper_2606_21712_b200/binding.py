@@ -15,7 +15,7 @@ BG_OK, BG_ERR_INVALID_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA, BG_ERR_NOMEM, BG_ERR
 EXPORTS = ["bg_moe_create", "bg_moe_destroy", "bg_moe_set_weights", "bg_moe_route", "bg_moe_permute",
            "bg_moe_expert_ffn", "bg_moe_unpermute", "bg_moe_combined_forward", "bg_moe_combined_forward_host",
            "bg_moe_debug_views", "bg_moe_profile_enable", "bg_moe_profile_read", "bg_moe_launch_count", "bg_moe_workspace_bytes", "bg_moe_strerror",
-           "bg_moe_last_error", "bg_moe_combined_forward_segments", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens"]
+           "bg_moe_last_error", "bg_moe_set_debug", "bg_moe_combined_forward_segments", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens"]
 
 
 class BgMoeConfig(ctypes.Structure):
@@ -46,7 +46,8 @@ def load_library() -> ctypes.CDLL:
         vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
         lib.bg_moe_create.argtypes = [ctypes.POINTER(BgMoeConfig), ctypes.POINTER(vp)]
         lib.bg_moe_destroy.argtypes = [vp]
-        lib.bg_moe_set_weights.argtypes = [vp] * 6
+        lib.bg_moe_set_weights.argtypes = [vp] * 7
+        lib.bg_moe_set_debug.argtypes = [vp, i32, i32]
         lib.bg_moe_route.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
         lib.bg_moe_permute.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp]
         lib.bg_moe_expert_ffn.argtypes = [vp, vp, vp, i32, vp, vp]
@@ -119,15 +120,20 @@ class MoELayer:
         return int(self.lib.bg_moe_workspace_bytes(self._ctx))
 
     # ------------------------------------------------------------------ C ABI mirrors
-    def set_weights(self, W_r, b_r, W_gate, W_up, W_down):
-        assert W_r.dtype == torch.float32 and W_r.shape == (self.d, self.E) and W_r.is_contiguous()
-        assert b_r is None or (b_r.dtype == torch.float32 and b_r.shape == (self.E,))
+    def set_debug(self, static_tile_feed: bool = False, supergroup_token_tiles: int = 0):
+        """bg_moe_set_debug: scheduler switches used by the tests only."""
+        self._check(self.lib.bg_moe_set_debug(self._ctx, int(static_tile_feed), int(supergroup_token_tiles)))
+
+    def set_weights(self, W_r, b_r, W_gate, W_up, W_down, stream=None):
+        assert W_r.dtype == torch.float32 and W_r.shape == (self.d, self.E) and W_r.is_contiguous() and W_r.is_cuda
+        assert b_r is None or (b_r.dtype == torch.float32 and b_r.shape == (self.E,) and b_r.is_contiguous()
+                               and b_r.is_cuda)
         for w, shp in ((W_gate, (self.E, self.d, self.f)), (W_up, (self.E, self.d, self.f)),
                        (W_down, (self.E, self.f, self.d))):
             assert w.dtype == torch.bfloat16 and tuple(w.shape) == shp and w.is_contiguous() and w.is_cuda
         self._weights = (W_r, b_r, W_gate, W_up, W_down)          # keep the borrowed tensors alive
         self._check(self.lib.bg_moe_set_weights(self._ctx, _ptr(W_r), _ptr(b_r), _ptr(W_gate), _ptr(W_up),
-                                                _ptr(W_down)))
+                                                _ptr(W_down), _stream(stream)))
 
     def route(self, hidden, logits_in=None, want_logits=True, stream=None):
         T = hidden.shape[0] if hidden is not None else logits_in.shape[0]
@@ -207,7 +213,7 @@ class MoELayer:
                                                               ctypes.c_int32(n), _stream(stream)))
         return out_segments
 
-    STAGES = ("router", "topk_hist", "scan", "rank", "gather", "gateup_swiglu", "down", "unpermute")
+    STAGES = ("router", "gather", "gateup_swiglu", "down", "unpermute")
 
     def profile_enable(self, on: bool = True):
         self._check(self.lib.bg_moe_profile_enable(self._ctx, int(on)))

@@ -4,7 +4,6 @@
 #include "kernels.h"
 
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -23,38 +22,45 @@ struct bg_moe_ctx {
   uint8_t* ws = nullptr;
   int64_t ws_bytes = 0;
   float* logits = nullptr;
-  float* partial = nullptr;     // router split-K partials [ksplit][T][E]
   void* wr_pieces = nullptr;    // bf16 [3][d][round_up(E,16)]: exact hi/mid/lo split of W_r
   int32_t* topk_idx = nullptr;
   float* topk_w = nullptr;
   int32_t* counts = nullptr;
   int32_t* offsets = nullptr;
-  int32_t* block_counts = nullptr;
-  int32_t* block_base = nullptr;
+  int32_t* tile_counts = nullptr;   // [n_tiles][E] per-128-token-tile expert histograms
+  int32_t* tile_base = nullptr;     // [n_tiles][E] first row of tile's entries inside each expert
+  int32_t* tile_rank = nullptr;     // [R] stable rank of an entry among its tile's entries of the same expert
   int32_t* row_src = nullptr;
   int32_t* inv_perm = nullptr;
   float* w_perm = nullptr;      // gate weights in expert order (fused path)
-  int32_t* tile_counters = nullptr;   // [4]: ticket / finished counters of the two pair GEMMs (self re-arming)
-  bool dyn_sched = true;        // dynamic tile feed of the pair GEMMs (BG_MOE_SCHED=static: tile t -> cluster t mod 74)
+  int32_t* tile_counters = nullptr;   // [0..3]: ticket / finished counters of the two pair GEMMs; [4]: router tiles done
+  bool counters_dirty = false;  // a call failed after launching: re-zero the counters before the next launch
+  bool dyn_sched = true;        // dynamic tile feed of the pair GEMMs (bg_moe_set_debug: static = tile t -> cluster t mod 74)
   // segment table of bg_moe_combined_forward_segments (device arrays + pageable host staging)
   int32_t max_segments = 0;
   const void** seg_dev_hidden = nullptr;
   void** seg_dev_out = nullptr;
   int32_t* seg_dev_start = nullptr;
-  std::vector<const void*> seg_host_ptrs;
-  std::vector<int32_t> seg_host_start;
+  std::vector<uint8_t> seg_host_img;     // packed host image of the three device arrays
   void* x_perm = nullptr;
   void* H = nullptr;
   void* Y = nullptr;
-  void* hidden_dev = nullptr;   // staging for the host-pointer entry point
-  void* out_dev = nullptr;
+  // host-pointer entry point: two staging slots and the context's own copy / compute streams
+  void* hidden_dev[2] = {nullptr, nullptr};
+  void* out_dev[2] = {nullptr, nullptr};
+  cudaStream_t st_in = nullptr, st_compute = nullptr, st_out = nullptr;
+  cudaEvent_t ev_h2d[2] = {}, ev_compute[2] = {}, ev_d2h[2] = {};
+  cudaEvent_t ev_device_call = nullptr;   // recorded after every device-pointer call (orders host calls after them)
+  bool device_call_pending = false;       // a device-pointer call was made since the last host call
+  bool host_call_pending = false;         // a host call was made since the last device-pointer call
+  int host_slot = 0;
+  int64_t host_calls = 0;
   // weight tensor maps (encoded in set_weights)
   CUtensorMap tm_wg, tm_wu, tm_wd, tm_wr, tm_wr1;   // tm_wr1: one-piece box of the 4-D W_r view (E > 128)
   CUtensorMap tm_wg4, tm_wu4, tm_wd4;   // 4-D block views (kernels.h GemmLaunch), valid when f % 64 == 0 / d % 64 == 0
   // activation tensor maps of the workspace x_perm / H (whole capacity: rows past T*k are never stored)
   bg::ActMaps am_x, am_h;
-  int sg_max = 0;               // BG_MOE_SG_TOKEN_TILES=n overrides the pair kernel's super-group size (tests)
-  bool pair_gemm = true;        // CTA-pair grouped GEMM (BG_MOE_GEMM=tile selects the 1-CTA 128x256 kernel)
+  int sg_max = 0;               // bg_moe_set_debug: overrides the pair kernel's super-group size (tests)
   int64_t launches = 0;
   std::string last_error;
   // optional per-kernel timing of the fused chain
@@ -134,7 +140,10 @@ inline void mark(bg_moe_ctx* ctx, int i, cudaStream_t st) {
 }
 
 int cuda_fail(bg_moe_ctx* ctx, cudaError_t e, const char* where) {
-  if (ctx) ctx->last_error = std::string(where) + ": " + cudaGetErrorString(e);
+  if (ctx) {
+    ctx->last_error = std::string(where) + ": " + cudaGetErrorString(e);
+    ctx->counters_dirty = true;     // a chain may have stopped half-way: the ticket / done counters are suspect
+  }
   return BG_ERR_CUDA;
 }
 
@@ -168,42 +177,61 @@ int check_T(const bg_moe_ctx* ctx, int32_t T) {
   return BG_OK;
 }
 
+// Start of every device-pointer call that launches kernels on `st`:
+//  * counters left non-zero by a call that failed half-way are re-zeroed (stream-ordered);
+//  * work the host-pointer entry point still has in flight on the context's own streams is waited for.
+int begin_call(bg_moe_ctx* ctx, cudaStream_t st) {
+  if (ctx->counters_dirty) {
+    BG_CUDA(ctx, cudaMemsetAsync(ctx->tile_counters, 0, 64, st), "memset counters");
+    ctx->counters_dirty = false;
+  }
+  if (ctx->host_call_pending) {
+    BG_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_compute[ctx->host_slot ^ 1], 0), "wait for host-path compute");
+    ctx->host_call_pending = false;
+  }
+  return BG_OK;
+}
+// End of every device-pointer call: remember where the context's work ends on the caller's stream.
+int end_call(bg_moe_ctx* ctx, cudaStream_t st, bool internal) {
+  if (!internal) {
+    BG_CUDA(ctx, cudaEventRecord(ctx->ev_device_call, st), "record device call");
+    ctx->device_call_pending = true;
+  }
+  return BG_OK;
+}
+
 // a1-a4 on explicit buffers.
 int do_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits_in, float* logits_buf,
              int32_t* topk_idx, float* topk_w, int32_t* counts, int32_t* offsets, cudaStream_t st,
              const bg::SegTable* seg = nullptr) {
   const bg_moe_config& c = ctx->cfg;
   if (logits_in == nullptr) {
-    const int ks = bg::router_ksplit(T, c.d, ctx->num_sms);
-    if (seg != nullptr) {
-      mark(ctx, 0, st);
-      BG_LAUNCH(ctx, bg::launch_router_gemm_segments(*seg, ctx->tm_wr, ctx->tm_wr1, T, c.d, c.E, ks, ctx->partial,
-                                                     ctx->block_counts, bg::route_num_blocks(T, c.k) * c.E, st),
-                "router_gemm_segments");
-    } else {
-      CUtensorMap tm_h;
-      if (!encode_act_map(&tm_h, hidden, T, c.d)) { ctx->last_error = "cuTensorMapEncodeTiled(hidden) failed"; return BG_ERR_CUDA; }
-      mark(ctx, 0, st);
-      BG_LAUNCH(ctx, bg::launch_router_gemm(tm_h, ctx->tm_wr, ctx->tm_wr1, T, c.d, c.E, ks, ctx->partial, ctx->block_counts,
-                                            bg::route_num_blocks(T, c.k) * c.E, st), "router_gemm");
+    bg::RouterLaunch r;
+    r.T = T; r.d = c.d; r.E = c.E; r.k = c.k;
+    r.b_r = ctx->b_r;
+    r.logits_out = logits_buf;
+    r.topk_idx = topk_idx; r.topk_w = topk_w;
+    r.tile_rank = ctx->tile_rank; r.tile_counts = ctx->tile_counts; r.tile_base = ctx->tile_base;
+    r.counts = counts; r.offsets = offsets;
+    r.done_counter = ctx->tile_counters + 4;
+    r.gemm_counters = ctx->tile_counters;
+    CUtensorMap tm_h;
+    if (seg == nullptr && !encode_act_map(&tm_h, hidden, T, c.d)) {
+      ctx->last_error = "cuTensorMapEncodeTiled(hidden) failed";
+      return BG_ERR_CUDA;
     }
-    mark(ctx, 1, st);
-    BG_LAUNCH(ctx, bg::launch_topk_hist(ctx->partial, ks, ctx->b_r, logits_buf, T, c.E, c.k, topk_idx, topk_w,
-                                        ctx->block_counts, st), "topk_hist");
+    BG_LAUNCH(ctx, bg::launch_router_fused(seg ? nullptr : &tm_h, ctx->tm_wr, ctx->tm_wr1, r, seg, st), "router_fused");
   } else {
-    BG_CUDA(ctx, cudaMemsetAsync(ctx->block_counts, 0, sizeof(int32_t) * bg::route_num_blocks(T, c.k) * c.E, st),
-            "memset block_counts");
-    BG_LAUNCH(ctx, bg::launch_topk_hist(logits_in, 1, nullptr, nullptr, T, c.E, c.k, topk_idx, topk_w,
-                                        ctx->block_counts, st), "topk_hist");
+    BG_LAUNCH(ctx, bg::launch_topk_tile(logits_in, T, c.E, c.k, topk_idx, topk_w, ctx->tile_rank, ctx->tile_counts, st),
+              "topk_tile");
+    BG_LAUNCH(ctx, bg::launch_scan(ctx->tile_counts, bg::route_num_tiles(T), c.E, ctx->tile_base, counts, offsets, st),
+              "scan");
   }
-  mark(ctx, 2, st);
-  BG_LAUNCH(ctx, bg::launch_scan(ctx->block_counts, bg::route_num_blocks(T, c.k), c.E, ctx->block_base, counts,
-                                 offsets, st), "scan");
   return BG_OK;
 }
 
 int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t T, void* y,
-           const float* row_scale, const int32_t* row_src, cudaStream_t st, int mark_between = -1) {
+           const float* row_scale_perm, cudaStream_t st, int mark_between = -1) {
   const bg_moe_config& c = ctx->cfg;
   const int64_t R = static_cast<int64_t>(T) * c.k;
   bg::GemmLaunch g1;
@@ -223,10 +251,9 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g1.offsets = offsets;
   g1.E = c.E; g1.K = c.d; g1.N = c.f;
   g1.out = ctx->H;
-  g1.row_scale = nullptr; g1.row_src = nullptr; g1.row_scale_perm = nullptr;
+  g1.row_scale_perm = nullptr;
   g1.num_sms = ctx->num_sms;
-  BG_LAUNCH(ctx, ctx->pair_gemm ? bg::launch_gateup_swiglu_pair(g1, st) : bg::launch_gateup_swiglu(g1, st),
-            "gateup_swiglu");
+  BG_LAUNCH(ctx, bg::launch_gateup_swiglu_pair(g1, st), "gateup_swiglu");
   if (mark_between >= 0) mark(ctx, mark_between, st);
   bg::GemmLaunch g2;
   g2.tm_act = ctx->am_h;
@@ -240,11 +267,47 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g2.offsets = offsets;
   g2.E = c.E; g2.K = c.f; g2.N = c.d;
   g2.out = y;
-  g2.row_scale = row_scale; g2.row_src = row_src;
-  g2.row_scale_perm = row_scale ? ctx->w_perm : nullptr;
+  g2.row_scale_perm = row_scale_perm;
   g2.num_sms = ctx->num_sms;
-  BG_LAUNCH(ctx, ctx->pair_gemm ? bg::launch_down_pair(g2, st) : bg::launch_down(g2, st), "down");
+  BG_LAUNCH(ctx, bg::launch_down_pair(g2, st), "down");
   return BG_OK;
+}
+
+// The fused chain a1-a9; seg != nullptr: token rows are read from / written to the segments' buffers.
+int do_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void* out, cudaStream_t st, const bg::SegTable* seg) {
+  const bg_moe_config& c = ctx->cfg;
+  mark(ctx, 0, st);
+  int rc = do_route(ctx, hidden, T, nullptr, ctx->logits, ctx->topk_idx, ctx->topk_w, ctx->counts, ctx->offsets, st, seg);
+  if (rc) return rc;
+  mark(ctx, 1, st);
+  bg::PermLaunch pl = {ctx->topk_idx, ctx->tile_rank, ctx->tile_base, ctx->topk_w, ctx->row_src, ctx->inv_perm,
+                       ctx->w_perm};
+  BG_LAUNCH(ctx, bg::launch_gather(hidden, pl, T, c.E, c.k, c.d, ctx->x_perm, ctx->num_sms, st, seg), "gather");
+  mark(ctx, 2, st);
+  rc = do_ffn(ctx, ctx->x_perm, ctx->offsets, T, ctx->Y, ctx->w_perm, st, /*mark_between=*/3);
+  if (rc) return rc;
+  mark(ctx, 4, st);
+  BG_LAUNCH(ctx, bg::launch_unpermute(ctx->Y, ctx->inv_perm, nullptr, T, c.k, c.d, out, ctx->num_sms, st, seg),
+            "unpermute");
+  mark(ctx, 5, st);
+  ctx->profile_valid = ctx->profile;
+  return BG_OK;
+}
+
+void destroy_ctx(bg_moe_ctx* ctx) {
+  for (cudaEvent_t e : ctx->ev)
+    if (e) cudaEventDestroy(e);
+  for (int i = 0; i < 2; ++i) {
+    if (ctx->ev_h2d[i]) cudaEventDestroy(ctx->ev_h2d[i]);
+    if (ctx->ev_compute[i]) cudaEventDestroy(ctx->ev_compute[i]);
+    if (ctx->ev_d2h[i]) cudaEventDestroy(ctx->ev_d2h[i]);
+  }
+  if (ctx->ev_device_call) cudaEventDestroy(ctx->ev_device_call);
+  if (ctx->st_in) cudaStreamDestroy(ctx->st_in);
+  if (ctx->st_compute) cudaStreamDestroy(ctx->st_compute);
+  if (ctx->st_out) cudaStreamDestroy(ctx->st_out);
+  if (ctx->ws) cudaFree(ctx->ws);
+  delete ctx;
 }
 
 }  // namespace
@@ -283,9 +346,7 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   DeviceGuard guard(c.device);
   if (!guard.ok) return BG_ERR_CUDA;
   if (get_encode_fn() == nullptr) return BG_ERR_CUDA;
-  if (bg::gemm_kernels_init() != cudaSuccess || bg::router_kernels_init() != cudaSuccess ||
-      bg::pair_kernels_init() != cudaSuccess)
-    return BG_ERR_CUDA;
+  if (bg::router_kernels_init() != cudaSuccess || bg::pair_kernels_init() != cudaSuccess) return BG_ERR_CUDA;
 
   bg_moe_ctx* ctx = new (std::nothrow) bg_moe_ctx();
   if (!ctx) return BG_ERR_NOMEM;
@@ -294,57 +355,53 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
   const int64_t Tm = c.max_tokens > 0 ? c.max_tokens : 1;
   const int64_t Rm = Tm * c.k;
   const bg::WsLayout L = bg::ws_layout(c, Tm, ctx->num_sms);
-  const int64_t off = L.total;
-  const int64_t o_logits = L.logits, o_idx = L.idx, o_w = L.w, o_part = L.part, o_pieces = L.pieces;
-  const int64_t o_counts = L.counts, o_offsets = L.offsets, o_bc = L.bc, o_bb = L.bb;
-  const int64_t o_rs = L.rs, o_ip = L.ip, o_wp = L.wp, o_x = L.x, o_h = L.h, o_y = L.y, o_hd = L.hd, o_od = L.od;
-  ctx->ws_bytes = off;
+  ctx->ws_bytes = L.total;
   void* p = nullptr;
-  if (cudaMalloc(&p, static_cast<size_t>(off)) != cudaSuccess) {
+  if (cudaMalloc(&p, static_cast<size_t>(L.total)) != cudaSuccess) {
     cudaGetLastError();
     delete ctx;
     return BG_ERR_NOMEM;
   }
   ctx->ws = static_cast<uint8_t*>(p);
-  ctx->logits = reinterpret_cast<float*>(ctx->ws + o_logits);
-  ctx->partial = reinterpret_cast<float*>(ctx->ws + o_part);
-  ctx->wr_pieces = ctx->ws + o_pieces;
-  ctx->topk_idx = reinterpret_cast<int32_t*>(ctx->ws + o_idx);
-  ctx->topk_w = reinterpret_cast<float*>(ctx->ws + o_w);
-  ctx->counts = reinterpret_cast<int32_t*>(ctx->ws + o_counts);
-  ctx->offsets = reinterpret_cast<int32_t*>(ctx->ws + o_offsets);
-  ctx->block_counts = reinterpret_cast<int32_t*>(ctx->ws + o_bc);
-  ctx->block_base = reinterpret_cast<int32_t*>(ctx->ws + o_bb);
-  ctx->row_src = reinterpret_cast<int32_t*>(ctx->ws + o_rs);
-  ctx->inv_perm = reinterpret_cast<int32_t*>(ctx->ws + o_ip);
-  ctx->w_perm = reinterpret_cast<float*>(ctx->ws + o_wp);
+  ctx->logits = reinterpret_cast<float*>(ctx->ws + L.logits);
+  ctx->wr_pieces = ctx->ws + L.pieces;
+  ctx->topk_idx = reinterpret_cast<int32_t*>(ctx->ws + L.idx);
+  ctx->topk_w = reinterpret_cast<float*>(ctx->ws + L.w);
+  ctx->counts = reinterpret_cast<int32_t*>(ctx->ws + L.counts);
+  ctx->offsets = reinterpret_cast<int32_t*>(ctx->ws + L.offsets);
+  ctx->tile_counts = reinterpret_cast<int32_t*>(ctx->ws + L.tc);
+  ctx->tile_base = reinterpret_cast<int32_t*>(ctx->ws + L.tb);
+  ctx->tile_rank = reinterpret_cast<int32_t*>(ctx->ws + L.tr);
+  ctx->row_src = reinterpret_cast<int32_t*>(ctx->ws + L.rs);
+  ctx->inv_perm = reinterpret_cast<int32_t*>(ctx->ws + L.ip);
+  ctx->w_perm = reinterpret_cast<float*>(ctx->ws + L.wp);
   ctx->tile_counters = reinterpret_cast<int32_t*>(ctx->ws + L.tile_counters);
-  if (cudaMemset(ctx->tile_counters, 0, 16) != cudaSuccess) {
-    cudaFree(ctx->ws);
-    delete ctx;
-    return BG_ERR_CUDA;
-  }
   ctx->max_segments = static_cast<int32_t>(Tm);
   ctx->seg_dev_hidden = reinterpret_cast<const void**>(ctx->ws + L.seg_hidden);
   ctx->seg_dev_out = reinterpret_cast<void**>(ctx->ws + L.seg_out);
   ctx->seg_dev_start = reinterpret_cast<int32_t*>(ctx->ws + L.seg_start);
-  ctx->x_perm = ctx->ws + o_x;
-  ctx->H = ctx->ws + o_h;
-  ctx->Y = ctx->ws + o_y;
-  ctx->hidden_dev = ctx->ws + o_hd;
-  ctx->out_dev = ctx->ws + o_od;
-  if (!encode_act_maps(&ctx->am_x, ctx->x_perm, Rm, c.d) || !encode_act_maps(&ctx->am_h, ctx->H, Rm, c.f)) {
-    cudaFree(ctx->ws);
-    delete ctx;
-    return BG_ERR_CUDA;
+  ctx->x_perm = ctx->ws + L.x;
+  ctx->H = ctx->ws + L.h;
+  ctx->Y = ctx->ws + L.y;
+  const int64_t stage_bytes = Tm * c.d * 2;
+  for (int i = 0; i < 2; ++i) {
+    ctx->hidden_dev[i] = ctx->ws + L.hd + i * stage_bytes;
+    ctx->out_dev[i] = ctx->ws + L.od + i * stage_bytes;
   }
-  {
-    const char* g = std::getenv("BG_MOE_GEMM");
-    if (g != nullptr && std::strcmp(g, "tile") == 0) ctx->pair_gemm = false;
-    const char* sc = std::getenv("BG_MOE_SCHED");
-    if (sc != nullptr && std::strcmp(sc, "static") == 0) ctx->dyn_sched = false;
-    const char* sg = std::getenv("BG_MOE_SG_TOKEN_TILES");
-    if (sg != nullptr && std::atoi(sg) > 0) ctx->sg_max = std::atoi(sg);
+  bool ok = cudaMemset(ctx->tile_counters, 0, 64) == cudaSuccess;
+  ok = ok && encode_act_maps(&ctx->am_x, ctx->x_perm, Rm, c.d) && encode_act_maps(&ctx->am_h, ctx->H, Rm, c.f);
+  ok = ok && cudaStreamCreateWithFlags(&ctx->st_in, cudaStreamNonBlocking) == cudaSuccess &&
+       cudaStreamCreateWithFlags(&ctx->st_compute, cudaStreamNonBlocking) == cudaSuccess &&
+       cudaStreamCreateWithFlags(&ctx->st_out, cudaStreamNonBlocking) == cudaSuccess;
+  for (int i = 0; i < 2 && ok; ++i)
+    ok = cudaEventCreateWithFlags(&ctx->ev_h2d[i], cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&ctx->ev_compute[i], cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&ctx->ev_d2h[i], cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaEventCreateWithFlags(&ctx->ev_device_call, cudaEventDisableTiming) == cudaSuccess;
+  if (!ok) {
+    cudaGetLastError();
+    destroy_ctx(ctx);
+    return BG_ERR_CUDA;
   }
   *out = ctx;
   return BG_OK;
@@ -353,15 +410,23 @@ int bg_moe_create(const bg_moe_config* cfg, bg_moe_ctx** out) {
 int bg_moe_destroy(bg_moe_ctx* ctx) {
   if (ctx == nullptr) return BG_OK;
   DeviceGuard guard(ctx->cfg.device);
-  for (cudaEvent_t e : ctx->ev)
-    if (e) cudaEventDestroy(e);
-  if (ctx->ws) cudaFree(ctx->ws);
-  delete ctx;
+  // the context's own streams may still hold host-path work that touches the workspace
+  if (ctx->st_in) cudaStreamSynchronize(ctx->st_in);
+  if (ctx->st_compute) cudaStreamSynchronize(ctx->st_compute);
+  if (ctx->st_out) cudaStreamSynchronize(ctx->st_out);
+  destroy_ctx(ctx);
+  return BG_OK;
+}
+
+int bg_moe_set_debug(bg_moe_ctx* ctx, int32_t static_tile_feed, int32_t supergroup_token_tiles) {
+  if (ctx == nullptr || supergroup_token_tiles < 0) return BG_ERR_INVALID_ARG;
+  ctx->dyn_sched = static_tile_feed == 0;
+  ctx->sg_max = supergroup_token_tiles;
   return BG_OK;
 }
 
 int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, const void* W_gate, const void* W_up,
-                       const void* W_down) {
+                       const void* W_down, void* stream) {
   if (!ctx || !W_r || !W_gate || !W_up || !W_down) return BG_ERR_INVALID_ARG;
   if (!aligned16(W_r) || !aligned16(W_gate) || !aligned16(W_up) || !aligned16(W_down)) return BG_ERR_INVALID_ARG;
   const bg_moe_config& c = ctx->cfg;
@@ -370,19 +435,17 @@ int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, cons
     ctx->last_error = "cuTensorMapEncodeTiled(weights) failed";
     return BG_ERR_CUDA;
   }
-  {
-    // block views: pair kernel a7 = 1 block per map, a8 = 2; tile kernel a7 = 2, a8 = 4
-    const int nb_gu = ctx->pair_gemm ? 1 : 2, nb_d = ctx->pair_gemm ? 2 : 4;
-    if ((c.f % 64 == 0 && (!encode_weight_map_4d(&ctx->tm_wg4, W_gate, c.E, c.d, c.f, nb_gu) ||
-                           !encode_weight_map_4d(&ctx->tm_wu4, W_up, c.E, c.d, c.f, nb_gu))) ||
-        (c.d % 64 == 0 && !encode_weight_map_4d(&ctx->tm_wd4, W_down, c.E, c.f, c.d, nb_d))) {
-      ctx->last_error = "cuTensorMapEncodeTiled(weight block views) failed";
-      return BG_ERR_CUDA;
-    }
+  // block views for the pair kernel: a7 = 1 block of 64 columns per map, a8 = 2
+  if ((c.f % 64 == 0 && (!encode_weight_map_4d(&ctx->tm_wg4, W_gate, c.E, c.d, c.f, 1) ||
+                         !encode_weight_map_4d(&ctx->tm_wu4, W_up, c.E, c.d, c.f, 1))) ||
+      (c.d % 64 == 0 && !encode_weight_map_4d(&ctx->tm_wd4, W_down, c.E, c.f, c.d, 2))) {
+    ctx->last_error = "cuTensorMapEncodeTiled(weight block views) failed";
+    return BG_ERR_CUDA;
   }
-  // exact bf16 hi/mid/lo split of W_r for the tensor-core router (router_gemm.cu); [3][d][E_ld]
+  // exact bf16 hi/mid/lo split of W_r for the tensor-core router (router_fused.cu); [3][d][E_ld]
   {
     DeviceGuard guard(c.device);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
     const int64_t E_ld = (c.E + 15) & ~15;
     EncodeTiledFn fn = get_encode_fn();
     CUresult res;
@@ -415,8 +478,11 @@ int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, cons
       ctx->last_error = "cuTensorMapEncodeTiled(W_r pieces) failed";
       return BG_ERR_CUDA;
     }
-    BG_LAUNCH(ctx, bg::launch_split_wr(W_r, c.d, c.E, ctx->wr_pieces, nullptr), "split_wr");
-    BG_CUDA(ctx, cudaStreamSynchronize(nullptr), "split_wr sync");   // set_weights is the one synchronous call
+    int rc = begin_call(ctx, st);      // also orders the split after host-path work that still reads the old pieces
+    if (rc) return rc;
+    BG_LAUNCH(ctx, bg::launch_split_wr(W_r, c.d, c.E, ctx->wr_pieces, st), "split_wr");
+    rc = end_call(ctx, st, false);
+    if (rc) return rc;
   }
   ctx->W_r = W_r; ctx->b_r = b_r; ctx->W_gate = W_gate; ctx->W_up = W_up; ctx->W_down = W_down;
   return BG_OK;
@@ -427,24 +493,25 @@ int bg_moe_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* lo
   int rc = check_T(ctx, T);
   if (rc) return rc;
   if (!counts || !offsets) return BG_ERR_INVALID_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
   if (T == 0) {   // nothing routed: counts and offsets are all zero
     DeviceGuard guard0(ctx->cfg.device);
-    BG_LAUNCH(ctx, bg::launch_scan(ctx->block_counts, 0, ctx->cfg.E, ctx->block_base, counts, offsets,
-                                   static_cast<cudaStream_t>(stream)), "scan");
-    return BG_OK;
+    if ((rc = begin_call(ctx, st))) return rc;
+    BG_LAUNCH(ctx, bg::launch_scan(ctx->tile_counts, 0, ctx->cfg.E, ctx->tile_base, counts, offsets, st), "scan");
+    return end_call(ctx, st, false);
   }
   if (!topk_idx || !topk_w) return BG_ERR_INVALID_ARG;
   if (logits_in == nullptr && (hidden == nullptr || !aligned16(hidden))) return BG_ERR_INVALID_ARG;
   if (logits_in == nullptr && ctx->W_r == nullptr) return BG_ERR_NO_WEIGHTS;
   DeviceGuard guard(ctx->cfg.device);
-  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if ((rc = begin_call(ctx, st))) return rc;
   float* lbuf = logits_out ? logits_out : ctx->logits;
   rc = do_route(ctx, hidden, T, logits_in, lbuf, topk_idx, topk_w, counts, offsets, st);
   if (rc) return rc;
-  if (logits_in && logits_out && logits_in != logits_out && T > 0)
+  if (logits_in && logits_out && logits_in != logits_out)
     BG_CUDA(ctx, cudaMemcpyAsync(logits_out, logits_in, sizeof(float) * T * ctx->cfg.E, cudaMemcpyDeviceToDevice, st),
             "copy logits");
-  return BG_OK;
+  return end_call(ctx, st, false);
 }
 
 int bg_moe_permute(bg_moe_ctx* ctx, const void* hidden, int32_t T, const int32_t* topk_idx, const int32_t* offsets,
@@ -457,12 +524,14 @@ int bg_moe_permute(bg_moe_ctx* ctx, const void* hidden, int32_t T, const int32_t
   DeviceGuard guard(ctx->cfg.device);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const bg_moe_config& c = ctx->cfg;
-  BG_LAUNCH(ctx, bg::launch_block_hist(topk_idx, T, c.E, c.k, ctx->block_counts, st), "block_hist");
-  BG_LAUNCH(ctx, bg::launch_scan(ctx->block_counts, bg::route_num_blocks(T, c.k), c.E, ctx->block_base, nullptr,
-                                 nullptr, st), "scan");
-  BG_LAUNCH(ctx, bg::launch_rank(topk_idx, ctx->block_base, T, c.E, c.k, row_src, inv_perm, nullptr, nullptr, st), "rank");
-  if (x_perm) BG_LAUNCH(ctx, bg::launch_gather(hidden, inv_perm, T, c.k, c.d, x_perm, ctx->num_sms, st), "gather");
-  return BG_OK;
+  if ((rc = begin_call(ctx, st))) return rc;
+  // the permutation is rebuilt from topk_idx alone (offsets = the exclusive scan of its histogram)
+  BG_LAUNCH(ctx, bg::launch_tile_rank(topk_idx, T, c.E, c.k, ctx->tile_rank, ctx->tile_counts, st), "tile_rank");
+  BG_LAUNCH(ctx, bg::launch_scan(ctx->tile_counts, bg::route_num_tiles(T), c.E, ctx->tile_base, nullptr, nullptr, st),
+            "scan");
+  bg::PermLaunch pl = {topk_idx, ctx->tile_rank, ctx->tile_base, nullptr, row_src, inv_perm, nullptr};
+  BG_LAUNCH(ctx, bg::launch_gather(hidden, pl, T, c.E, c.k, c.d, x_perm, ctx->num_sms, st), "gather");
+  return end_call(ctx, st, false);
 }
 
 int bg_moe_expert_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t T, void* y_perm,
@@ -473,7 +542,13 @@ int bg_moe_expert_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offset
   if (!x_perm || !offsets || !y_perm || !aligned16(x_perm) || !aligned16(y_perm)) return BG_ERR_INVALID_ARG;
   if (ctx->W_gate == nullptr) return BG_ERR_NO_WEIGHTS;
   DeviceGuard guard(ctx->cfg.device);
-  return do_ffn(ctx, x_perm, offsets, T, y_perm, nullptr, nullptr, static_cast<cudaStream_t>(stream));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if ((rc = begin_call(ctx, st))) return rc;
+  // no router kernel precedes the GEMMs here: zero their ticket counters on the stream
+  BG_CUDA(ctx, cudaMemsetAsync(ctx->tile_counters, 0, 16, st), "memset ticket counters");
+  rc = do_ffn(ctx, x_perm, offsets, T, y_perm, nullptr, st);
+  if (rc) return rc;
+  return end_call(ctx, st, false);
 }
 
 int bg_moe_unpermute(bg_moe_ctx* ctx, const void* y_perm, const int32_t* inv_perm, const float* topk_w, int32_t T,
@@ -483,31 +558,11 @@ int bg_moe_unpermute(bg_moe_ctx* ctx, const void* y_perm, const int32_t* inv_per
   if (T == 0) return BG_OK;
   if (!y_perm || !inv_perm || !topk_w || !out || !aligned16(y_perm) || !aligned16(out)) return BG_ERR_INVALID_ARG;
   DeviceGuard guard(ctx->cfg.device);
-  BG_LAUNCH(ctx, bg::launch_unpermute(y_perm, inv_perm, topk_w, T, ctx->cfg.k, ctx->cfg.d, out, ctx->num_sms,
-                                      static_cast<cudaStream_t>(stream)), "unpermute");
-  return BG_OK;
-}
-
-// The fused chain a1-a9; seg != nullptr: token rows are read from / written to the segments' buffers.
-static int do_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void* out, cudaStream_t st,
-                      const bg::SegTable* seg) {
-  const bg_moe_config& c = ctx->cfg;
-  int rc = do_route(ctx, hidden, T, nullptr, ctx->logits, ctx->topk_idx, ctx->topk_w, ctx->counts, ctx->offsets, st, seg);
-  if (rc) return rc;
-  mark(ctx, 3, st);
-  BG_LAUNCH(ctx, bg::launch_rank(ctx->topk_idx, ctx->block_base, T, c.E, c.k, ctx->row_src, ctx->inv_perm, ctx->topk_w,
-                                 ctx->w_perm, st), "rank");
-  mark(ctx, 4, st);
-  BG_LAUNCH(ctx, bg::launch_gather(hidden, ctx->inv_perm, T, c.k, c.d, ctx->x_perm, ctx->num_sms, st, seg), "gather");
-  mark(ctx, 5, st);
-  rc = do_ffn(ctx, ctx->x_perm, ctx->offsets, T, ctx->Y, ctx->topk_w, ctx->row_src, st, /*mark_between=*/6);
-  if (rc) return rc;
-  mark(ctx, 7, st);
-  BG_LAUNCH(ctx, bg::launch_unpermute(ctx->Y, ctx->inv_perm, nullptr, T, c.k, c.d, out, ctx->num_sms, st, seg),
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if ((rc = begin_call(ctx, st))) return rc;
+  BG_LAUNCH(ctx, bg::launch_unpermute(y_perm, inv_perm, topk_w, T, ctx->cfg.k, ctx->cfg.d, out, ctx->num_sms, st),
             "unpermute");
-  mark(ctx, 8, st);
-  ctx->profile_valid = ctx->profile;
-  return BG_OK;
+  return end_call(ctx, st, false);
 }
 
 int bg_moe_combined_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void* out, void* stream) {
@@ -517,7 +572,11 @@ int bg_moe_combined_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void
   if (!hidden || !out || !aligned16(hidden) || !aligned16(out)) return BG_ERR_INVALID_ARG;
   if (ctx->W_r == nullptr) return BG_ERR_NO_WEIGHTS;
   DeviceGuard guard(ctx->cfg.device);
-  return do_forward(ctx, hidden, T, out, static_cast<cudaStream_t>(stream), nullptr);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if ((rc = begin_call(ctx, st))) return rc;
+  rc = do_forward(ctx, hidden, T, out, st, nullptr);
+  if (rc) return rc;
+  return end_call(ctx, st, false);
 }
 
 int bg_moe_combined_forward_segments(bg_moe_ctx* ctx, const bg_moe_segment* segments, int32_t n_segments,
@@ -538,11 +597,19 @@ int bg_moe_combined_forward_segments(bg_moe_ctx* ctx, const bg_moe_segment* segm
   if (ctx->W_r == nullptr) return BG_ERR_NO_WEIGHTS;
   DeviceGuard guard(ctx->cfg.device);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  // The segment table goes to the device through pageable host staging: cudaMemcpyAsync from pageable
-  // memory returns once the bytes are staged, so the vectors can be reused by the next call.
+  int rc = begin_call(ctx, st);
+  if (rc) return rc;
+  // The segment table goes to the device in ONE copy through pageable host staging (cudaMemcpyAsync from
+  // pageable memory returns once the bytes are staged, so the vector can be reused by the next call).
+  // Device layout (one slab): hidden[max_segments] | out[max_segments] | start[max_segments + 1]; the host
+  // image is packed the same way so a single contiguous copy serves the three arrays.
   const int n = n_segments;
-  ctx->seg_host_ptrs.resize(2 * static_cast<size_t>(n));
-  ctx->seg_host_start.resize(static_cast<size_t>(n) + 1);
+  const size_t cap = static_cast<size_t>(ctx->max_segments);
+  const size_t img_bytes = 16 * cap + 4 * (cap + 1);
+  ctx->seg_host_img.resize(img_bytes);
+  const void** h_hidden = reinterpret_cast<const void**>(ctx->seg_host_img.data());
+  void** h_out = reinterpret_cast<void**>(ctx->seg_host_img.data() + 8 * cap);
+  int32_t* h_start = reinterpret_cast<int32_t*>(ctx->seg_host_img.data() + 16 * cap);
   // an empty segment may carry null pointers (its rows are never looked up); the router uses hidden[0]
   // as the source address of zero-filled copies, so every entry is made a valid address
   const void* first_valid = nullptr;
@@ -550,38 +617,76 @@ int bg_moe_combined_forward_segments(bg_moe_ctx* ctx, const bg_moe_segment* segm
     if (segments[i].n_tokens > 0) first_valid = segments[i].hidden;
   int32_t acc = 0;
   for (int i = 0; i < n; ++i) {
-    ctx->seg_host_ptrs[i] = segments[i].n_tokens > 0 ? segments[i].hidden : first_valid;
-    ctx->seg_host_ptrs[n + i] = segments[i].out;
-    ctx->seg_host_start[i] = acc;
+    h_hidden[i] = segments[i].n_tokens > 0 ? segments[i].hidden : first_valid;
+    h_out[i] = segments[i].out;
+    h_start[i] = acc;
     acc += segments[i].n_tokens;
   }
-  ctx->seg_host_start[n] = acc;
-  BG_CUDA(ctx, cudaMemcpyAsync(ctx->seg_dev_hidden, ctx->seg_host_ptrs.data(), sizeof(void*) * n, cudaMemcpyHostToDevice, st),
-          "H2D segment table (hidden)");
-  BG_CUDA(ctx, cudaMemcpyAsync(ctx->seg_dev_out, ctx->seg_host_ptrs.data() + n, sizeof(void*) * n, cudaMemcpyHostToDevice, st),
-          "H2D segment table (out)");
-  BG_CUDA(ctx, cudaMemcpyAsync(ctx->seg_dev_start, ctx->seg_host_start.data(), sizeof(int32_t) * (n + 1),
-                               cudaMemcpyHostToDevice, st), "H2D segment table (start)");
+  h_start[n] = acc;
+  if (static_cast<size_t>(n) * 4 >= cap) {
+    // long tables: one copy of the whole image
+    BG_CUDA(ctx, cudaMemcpyAsync(ctx->seg_dev_hidden, ctx->seg_host_img.data(), img_bytes, cudaMemcpyHostToDevice, st),
+            "H2D segment table");
+  } else {
+    // short tables in a large context: three short copies beat one of 20 bytes x max_tokens
+    BG_CUDA(ctx, cudaMemcpyAsync(ctx->seg_dev_hidden, h_hidden, sizeof(void*) * n, cudaMemcpyHostToDevice, st),
+            "H2D segment table (hidden)");
+    BG_CUDA(ctx, cudaMemcpyAsync(ctx->seg_dev_out, h_out, sizeof(void*) * n, cudaMemcpyHostToDevice, st),
+            "H2D segment table (out)");
+    BG_CUDA(ctx, cudaMemcpyAsync(ctx->seg_dev_start, h_start, sizeof(int32_t) * (n + 1), cudaMemcpyHostToDevice, st),
+            "H2D segment table (start)");
+  }
   bg::SegTable seg;
   seg.hidden = reinterpret_cast<const void* const*>(ctx->seg_dev_hidden);
   seg.out = reinterpret_cast<void* const*>(ctx->seg_dev_out);
   seg.start = ctx->seg_dev_start;
   seg.n = n;
-  return do_forward(ctx, nullptr, T, nullptr, st, &seg);
+  rc = do_forward(ctx, nullptr, T, nullptr, st, &seg);
+  if (rc) return rc;
+  return end_call(ctx, st, false);
 }
 
+// Host-pointer entry point, pipelined over the context's own streams (two staging slots):
+//   st_in:      H2D of call i           (after the chain of call i-2 has released the slot's input buffer)
+//   st_compute: the fused chain of call i (after its H2D; after the D2H of call i-2 has released the output buffer)
+//   st_out:     D2H of call i           (after its chain)
+// so the upload of call i+1 and the download of call i-1 overlap the GEMMs of call i.  `stream` only WAITS for
+// the download: work the caller enqueues on `stream` afterwards (and a synchronize on it) sees out_host complete.
+// The host buffers are not stream-ordered objects: hidden_host must hold its data when the call is made.
 int bg_moe_combined_forward_host(bg_moe_ctx* ctx, const void* hidden_host, int32_t T, void* out_host, void* stream) {
   int rc = check_T(ctx, T);
   if (rc) return rc;
   if (T == 0) return BG_OK;
   if (!hidden_host || !out_host) return BG_ERR_INVALID_ARG;
+  if (ctx->W_r == nullptr) return BG_ERR_NO_WEIGHTS;
   DeviceGuard guard(ctx->cfg.device);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int slot = ctx->host_slot;
   const size_t bytes = static_cast<size_t>(T) * ctx->cfg.d * 2;
-  BG_CUDA(ctx, cudaMemcpyAsync(ctx->hidden_dev, hidden_host, bytes, cudaMemcpyHostToDevice, st), "H2D hidden");
-  rc = bg_moe_combined_forward(ctx, ctx->hidden_dev, T, ctx->out_dev, stream);
+  if (ctx->counters_dirty) {
+    BG_CUDA(ctx, cudaMemsetAsync(ctx->tile_counters, 0, 64, ctx->st_compute), "memset counters");
+    ctx->counters_dirty = false;
+  }
+  // ordered after every earlier device-pointer call on this context (weights, workspace)
+  if (ctx->device_call_pending) {
+    BG_CUDA(ctx, cudaStreamWaitEvent(ctx->st_compute, ctx->ev_device_call, 0), "order after device calls");
+    ctx->device_call_pending = false;
+  }
+  if (ctx->host_calls >= 2) BG_CUDA(ctx, cudaStreamWaitEvent(ctx->st_in, ctx->ev_compute[slot], 0), "slot input free");
+  BG_CUDA(ctx, cudaMemcpyAsync(ctx->hidden_dev[slot], hidden_host, bytes, cudaMemcpyHostToDevice, ctx->st_in), "H2D hidden");
+  BG_CUDA(ctx, cudaEventRecord(ctx->ev_h2d[slot], ctx->st_in), "record H2D");
+  BG_CUDA(ctx, cudaStreamWaitEvent(ctx->st_compute, ctx->ev_h2d[slot], 0), "wait H2D");
+  if (ctx->host_calls >= 2) BG_CUDA(ctx, cudaStreamWaitEvent(ctx->st_compute, ctx->ev_d2h[slot], 0), "slot output free");
+  rc = do_forward(ctx, ctx->hidden_dev[slot], T, ctx->out_dev[slot], ctx->st_compute, nullptr);
   if (rc) return rc;
-  BG_CUDA(ctx, cudaMemcpyAsync(out_host, ctx->out_dev, bytes, cudaMemcpyDeviceToHost, st), "D2H out");
+  BG_CUDA(ctx, cudaEventRecord(ctx->ev_compute[slot], ctx->st_compute), "record chain");
+  BG_CUDA(ctx, cudaStreamWaitEvent(ctx->st_out, ctx->ev_compute[slot], 0), "wait chain");
+  BG_CUDA(ctx, cudaMemcpyAsync(out_host, ctx->out_dev[slot], bytes, cudaMemcpyDeviceToHost, ctx->st_out), "D2H out");
+  BG_CUDA(ctx, cudaEventRecord(ctx->ev_d2h[slot], ctx->st_out), "record D2H");
+  BG_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_d2h[slot], 0), "caller's stream waits for the result");
+  ctx->host_slot ^= 1;
+  ctx->host_calls += 1;
+  ctx->host_call_pending = true;
   return BG_OK;
 }
 

@@ -1,5 +1,6 @@
 // gather_reduce.cu -- the two HBM-bound row movers of the combined MoE layer:
-//   a6 gather    x_perm[r,:] = hidden[row_src[r]/k,:]   written as x_perm[inv_perm[i],:] = hidden[i/k,:]
+//   a5'' + a6    row r of entry i = t*k+s from the tile bases and tile-local ranks (inv_perm, row_src, w_perm),
+//                x_perm[r,:] = hidden[row_src[r]/k,:]   written as x_perm[inv_perm[i],:] = hidden[i/k,:]
 //   a9 reduce    out[t,:]    = sum_{s<k} (w[t,s]) * Y[inv_perm[t*k+s],:]     slot order, fp32, RNE->bf16
 // BASELINE.json north_star: "a gather kernel with 16-byte vectorised, coalesced row copies" and "a
 // gate-weighted un-permute that sums each token's top-k results", atomic-free.
@@ -23,18 +24,41 @@ __device__ __forceinline__ void st_stream(uint4* p, const uint4& v) {
                "r"(v.w) : "memory");
 }
 
-// a6 as a scatter: one warp per TOKEN reads its hidden row once (registers) and writes it to the k
-// expert-order rows inv_perm[t*k + s] -- x_perm[inv_perm[t*k+s]] = hidden[t] is the same assignment
-// as x_perm[r] = hidden[row_src[r]/k] (inv_perm is the inverse of row_src), with 1 load + k stores per
-// vector instead of k loads + k stores.
+// a5 (second half) + a6 as a scatter: one warp per TOKEN.  Lane s < k finishes the permutation of entry
+// i = t*k + s -- row r = tile_base[t/128][idx] + tile_rank[i] (routing_common.cuh), inv_perm[i] = r,
+// row_src[r] = i, w_perm[r] = topk_w[i] -- then the warp reads the token's hidden row once (registers) and writes
+// it to its k expert-order rows: x_perm[inv_perm[t*k+s]] = hidden[t] is the same assignment as
+// x_perm[r] = hidden[row_src[r]/k], with 1 load + k stores per vector instead of k loads + k stores.
+struct PermArgs {
+  const int32_t* topk_idx;    // [T,k]
+  const int32_t* tile_rank;   // [T,k]
+  const int32_t* tile_base;   // [n_tiles,E]
+  const float* topk_w;        // [T,k] or nullptr
+  int32_t* row_src;           // [T*k]
+  int32_t* inv_perm;          // [T*k]
+  float* w_perm;              // [T*k] or nullptr
+  int E;
+};
+
 template <int KMAX>
-__global__ void __launch_bounds__(256) gather_kernel(const uint4* __restrict__ hidden,
-                                                     const int32_t* __restrict__ inv_perm, int T, int k,
+__global__ void __launch_bounds__(256) gather_kernel(const uint4* __restrict__ hidden, const PermArgs pa, int T, int k,
                                                      int vec_per_row, uint4* __restrict__ x_perm, const SegTable seg) {
   pdl_wait_then_trigger();
   const int lane = threadIdx.x & 31;
   const int warps_total = gridDim.x * (blockDim.x >> 5);
   for (int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); t < T; t += warps_total) {
+    int r = -1;
+    if (lane < k) {
+      const int64_t i = static_cast<int64_t>(t) * k + lane;
+      const int e = __ldg(pa.topk_idx + i);
+      if (e >= 0 && e < pa.E) {
+        r = __ldg(pa.tile_base + static_cast<int64_t>(t >> 7) * pa.E + e) + __ldg(pa.tile_rank + i);
+        pa.inv_perm[i] = r;
+        pa.row_src[r] = static_cast<int32_t>(i);
+        if (pa.w_perm != nullptr) pa.w_perm[r] = __ldg(pa.topk_w + i);
+      }
+    }
+    if (x_perm == nullptr) continue;
     const uint4* src;
     if (seg.n > 0) {               // zero-copy COMBINE: the token's row inside its coroutine's own buffer
       const int sg = seg_of(seg.start, seg.n, t);
@@ -43,16 +67,20 @@ __global__ void __launch_bounds__(256) gather_kernel(const uint4* __restrict__ h
       src = hidden + static_cast<int64_t>(t) * vec_per_row;
     }
     uint4* dst[KMAX];
+    bool ok[KMAX];
     #pragma unroll
-    for (int s = 0; s < KMAX; ++s)
-      dst[s] = x_perm + static_cast<int64_t>(s < k ? __ldg(inv_perm + static_cast<int64_t>(t) * k + s) : 0) * vec_per_row;
+    for (int s = 0; s < KMAX; ++s) {
+      const int rs = __shfl_sync(0xffffffffu, r, s);
+      ok[s] = s < k && rs >= 0;
+      dst[s] = x_perm + static_cast<int64_t>(ok[s] ? rs : 0) * vec_per_row;
+    }
     int c = lane;
     for (; c + 96 < vec_per_row; c += 128) {
       const uint4 a0 = ld_stream(src + c), a1 = ld_stream(src + c + 32), a2 = ld_stream(src + c + 64),
                   a3 = ld_stream(src + c + 96);
       #pragma unroll
       for (int s = 0; s < KMAX; ++s)
-        if (s < k) {
+        if (ok[s]) {
           st_stream(dst[s] + c, a0);
           st_stream(dst[s] + c + 32, a1);
           st_stream(dst[s] + c + 64, a2);
@@ -63,7 +91,7 @@ __global__ void __launch_bounds__(256) gather_kernel(const uint4* __restrict__ h
       const uint4 a = ld_stream(src + c);
       #pragma unroll
       for (int s = 0; s < KMAX; ++s)
-        if (s < k) st_stream(dst[s] + c, a);
+        if (ok[s]) st_stream(dst[s] + c, a);
     }
   }
 }
@@ -135,19 +163,22 @@ inline int row_mover_grid(int rows, int num_sms) {
 
 }  // namespace
 
-cudaError_t launch_gather(const void* hidden, const int32_t* inv_perm, int T, int k, int d, void* x_perm,
+cudaError_t launch_gather(const void* hidden, const PermLaunch& pl, int T, int E, int k, int d, void* x_perm,
                           int num_sms, cudaStream_t st, const SegTable* segp) {
   const SegTable seg = segp ? *segp : SegTable{nullptr, nullptr, nullptr, 0};
   if (T == 0) return cudaSuccess;
+  PermArgs pa;
+  pa.topk_idx = pl.topk_idx; pa.tile_rank = pl.tile_rank; pa.tile_base = pl.tile_base; pa.topk_w = pl.topk_w;
+  pa.row_src = pl.row_src; pa.inv_perm = pl.inv_perm; pa.w_perm = pl.w_perm; pa.E = E;
   const int grid = row_mover_grid(T, num_sms);
   if (k <= 2)
-    launch_pdl(gather_kernel<2>, grid, 256, 0, st, static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
+    launch_pdl(gather_kernel<2>, grid, 256, 0, st, static_cast<const uint4*>(hidden), pa, T, k, d / 8,
                                            static_cast<uint4*>(x_perm), seg);
   else if (k <= 4)
-    launch_pdl(gather_kernel<4>, grid, 256, 0, st, static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
+    launch_pdl(gather_kernel<4>, grid, 256, 0, st, static_cast<const uint4*>(hidden), pa, T, k, d / 8,
                                            static_cast<uint4*>(x_perm), seg);
   else
-    launch_pdl(gather_kernel<8>, grid, 256, 0, st, static_cast<const uint4*>(hidden), inv_perm, T, k, d / 8,
+    launch_pdl(gather_kernel<8>, grid, 256, 0, st, static_cast<const uint4*>(hidden), pa, T, k, d / 8,
                                            static_cast<uint4*>(x_perm), seg);
   return cudaGetLastError();
 }

@@ -10,37 +10,38 @@ namespace bg {
 WsLayout ws_layout(const bg_moe_config& c, int64_t max_tokens, int num_sms) {
   const int64_t Tm = max_tokens > 0 ? max_tokens : 1;
   const int64_t Rm = Tm * c.k;
-  const int64_t nblk = route_num_blocks(static_cast<int>(Tm), c.k);
+  const int64_t ntile = route_num_tiles(static_cast<int>(Tm));
   int64_t off = 0;
   auto carve = [&](int64_t bytes) {
     const int64_t o = off;
     off = (off + bytes + 1023) / 1024 * 1024;
     return o;
   };
-  const int64_t Tpad = (Tm + 127) / 128 * 128;
-  const int64_t part_rows = Tpad > static_cast<int64_t>(num_sms) * 128 ? Tpad : static_cast<int64_t>(num_sms) * 128;
+  (void)num_sms;
   WsLayout L;
   L.logits = carve(Tm * c.E * 4);
   L.idx = carve(Rm * 4);
   L.w = carve(Rm * 4);
-  L.part = carve(part_rows * c.E * 4);
   L.pieces = carve(3LL * c.d * ((c.E + 15) & ~15) * 2);
   L.counts = carve(c.E * 4);
   L.offsets = carve((c.E + 1) * 4);
-  L.bc = carve(nblk * c.E * 4);
-  L.bb = carve(nblk * c.E * 4);
+  L.tc = carve(ntile * c.E * 4);     // per-tile expert histograms
+  L.tb = carve(ntile * c.E * 4);     // per-tile base rows
+  L.tr = carve(Rm * 4);              // tile-local ranks
   L.rs = carve(Rm * 4);
   L.ip = carve(Rm * 4);
   L.wp = carve(Rm * 4);
   L.x = carve(Rm * c.d * 2);
   L.h = carve(Rm * c.f * 2);
   L.y = carve(Rm * c.d * 2);
-  L.hd = carve(Tm * c.d * 2);
-  L.od = carve(Tm * c.d * 2);
-  L.seg_hidden = carve(Tm * 8);      // segment table: at most max_tokens segments
-  L.seg_out = carve(Tm * 8);
-  L.seg_start = carve((Tm + 1) * 4);
-  L.tile_counters = carve(16);
+  L.hd = carve(2 * Tm * c.d * 2);    // host entry point: two staging slots each way
+  L.od = carve(2 * Tm * c.d * 2);
+  // segment table (at most max_tokens segments), ONE slab so that one copy can fill it:
+  // hidden[Tm] pointers | out[Tm] pointers | start[Tm + 1] ints
+  L.seg_hidden = carve(16 * Tm + 4 * (Tm + 1));
+  L.seg_out = L.seg_hidden + 8 * Tm;
+  L.seg_start = L.seg_hidden + 16 * Tm;
+  L.tile_counters = carve(64);       // [0..3] GEMM ticket counters, [4] router tiles-done counter
   L.total = off;
   return L;
 }

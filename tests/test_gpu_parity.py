@@ -153,22 +153,19 @@ def test_expert_ffn_parity(rows, d, f):
             check_out(y[offsets[e]:offsets[e + 1]], ref[offsets[e]:offsets[e + 1]], f"expert {e}")
 
 
-@pytest.mark.parametrize("env", [{"BG_MOE_SG_TOKEN_TILES": "2"}, {"BG_MOE_SG_TOKEN_TILES": "1"}, {"BG_MOE_GEMM": "tile"},
-                                 {"BG_MOE_SCHED": "static"}, {"BG_MOE_SCHED": "static", "BG_MOE_SG_TOKEN_TILES": "2"}],
-                         ids=["supergroups-of-2", "supergroups-of-1", "tile-kernel", "static-feed",
-                              "static-feed-supergroups"])
-def test_expert_ffn_scheduler_variants(env, monkeypatch):
+@pytest.mark.parametrize("env", [dict(supergroup_token_tiles=2), dict(supergroup_token_tiles=1),
+                                 dict(static_tile_feed=True), dict(static_tile_feed=True, supergroup_token_tiles=2)],
+                         ids=["supergroups-of-2", "supergroups-of-1", "static-feed", "static-feed-supergroups"])
+def test_expert_ffn_scheduler_variants(env):
     """The same FFN through (i) the pair kernel's super-group tile order, which production shapes only
-    reach with experts of several thousand rows (forced here on experts of 3-5 token tiles), (ii) the
-    1-CTA 128x256 kernel that BG_MOE_GEMM=tile selects, and (iii) the static tile feed (BG_MOE_SCHED=static;
-    the default is the dynamic ticket feed)."""
-    for k_, v in env.items():
-        monkeypatch.setenv(k_, v)              # read once, in bg_moe_create
+    reach with experts of several thousand rows (forced here on experts of 3-5 token tiles) and (ii) the
+    static tile feed (the default is the dynamic ticket feed); both selected through bg_moe_set_debug."""
     rows = [1300, 0, 700, 257, 16, 1]
     d, f = 192, 320
     E, R = len(rows), sum(rows)
     cfg = wl.MoEConfig("ffn-sched", 15, T=R, d=d, E=E, k=1, f=f)
     lay, g, layer = make(cfg)
+    layer.set_debug(**env)
     offsets = np.concatenate([[0], np.cumsum(rows)]).astype(np.int32)
     y = layer.expert_ffn(g["hidden"], torch.from_numpy(offsets).cuda(), T=R)
     torch.cuda.synchronize()
@@ -212,7 +209,7 @@ def test_fused_forward_parity(cfg):
     n0 = layer.launch_count
     out = layer.combined_forward(g["hidden"])
     torch.cuda.synchronize()
-    assert layer.launch_count - n0 == 8          # router, topk, scan, rank, gather, 2 GEMMs, reduce
+    assert layer.launch_count - n0 == 5          # fused router, gather (+ permutation), 2 GEMMs, reduce
     v = layer.debug_views(cfg.T)
     check_routing_against_oracle(v["logits"], v["idx"], v["w"], v["counts"], v["offsets"], v["row_src"],
                                  v["inv_perm"], cfg.E, cfg.k)
@@ -259,6 +256,31 @@ def test_combine_invariance_on_gpu():
     assert torch.equal(shuf, full[perm])
 
 
+@pytest.mark.parametrize("d,E,k", [(2048, 128, 8), (4096, 16, 2), (7168, 256, 8)], ids=["d2048", "d4096", "d7168"])
+def test_combine_invariance_large_d(d, E, k):
+    """the router's K partition (cluster of router_nch(d) CTAs, partials added in chunk order) is a
+    function of d only, so the fp32 logits of a row -- and everything downstream -- cannot depend on how many
+    tokens it was combined with.  T=4096 against its two halves and against single 128-token tiles, at the d of
+    C3 / C2,C5 / C4 (4 / 4 / 8 K chunks)."""
+    cfg = wl.small_config(T=4096, d=d, E=E, k=k, f=128, index=33)
+    lay, g, layer = make(cfg)
+    h = g["hidden"]
+    full = layer.combined_forward(h).clone()
+    L_full = layer.debug_views(4096)["logits"].clone()
+    outs, Ls = [], []
+    for lo, hi in ((0, 2048), (2048, 4096)):
+        outs.append(layer.combined_forward(h[lo:hi].contiguous()).clone())
+        Ls.append(layer.debug_views(hi - lo)["logits"].clone())
+    assert torch.equal(torch.cat(Ls), L_full), "router logits depend on the combined-batch size"
+    assert torch.equal(torch.cat(outs), full), "outputs depend on the combined-batch size"
+    for lo, hi in ((0, 1), (130, 257), (4000, 4096)):
+        o = layer.combined_forward(h[lo:hi].contiguous())
+        assert torch.equal(layer.debug_views(hi - lo)["logits"], L_full[lo:hi])
+        assert torch.equal(o, full[lo:hi])
+    own = oracle.router_logits(lay["hidden"], lay["W_r"], lay["b_r"])
+    assert np.all(np.abs(L_full.cpu().numpy() - own) <= 1e-4 * np.maximum(1.0, np.abs(own)))
+
+
 def test_host_entry_point_and_zero_tokens():
     cfg = wl.small_config(T=200, d=128, E=8, k=2, f=128, index=29)
     lay, g, layer = make(cfg)
@@ -266,6 +288,26 @@ def test_host_entry_point_and_zero_tokens():
     host_out = layer.combined_forward_host(lay["hidden"].pin_memory())
     torch.cuda.synchronize()
     assert torch.equal(host_out, dev_out.cpu())
+    # pipelined back-to-back host calls with different inputs and sizes (two staging slots, the context's own
+    # copy / compute streams): every result must equal the device-pointer path on the same rows
+    gen = torch.Generator().manual_seed(5)
+    ins, outs, refs = [], [], []
+    for i in range(7):
+        T = [200, 64, 200, 1, 129, 200, 37][i]
+        hi = (torch.randn(T, cfg.d, generator=gen) * (1 + i)).to(torch.bfloat16).pin_memory()
+        ins.append(hi)
+        outs.append(layer.combined_forward_host(hi))
+    torch.cuda.current_stream().synchronize()          # the caller's stream waited for every download
+    for hi, ho in zip(ins, outs):
+        refs.append(layer.combined_forward(hi.cuda()).cpu())
+    for i, (ho, r) in enumerate(zip(outs, refs)):
+        assert torch.equal(ho, r), f"host call {i} differs from the device-pointer path"
+    # a device-pointer call right after host calls (and the reverse) is ordered correctly
+    a = layer.combined_forward_host(ins[0])
+    b = layer.combined_forward(g["hidden"])
+    c = layer.combined_forward_host(ins[2])
+    torch.cuda.synchronize()
+    assert torch.equal(a, refs[0]) and torch.equal(b, dev_out) and torch.equal(c, refs[2])
     empty = torch.empty(0, cfg.d, dtype=torch.bfloat16, device="cuda")
     assert layer.combined_forward(empty).shape == (0, cfg.d)          # T == 0: BG_OK, no-op
     r = layer.route(empty)
@@ -294,6 +336,59 @@ def test_argument_errors():
     with pytest.raises(BgMoeError) as ei:
         layer.combined_forward(h)                # T > max_tokens
     assert ei.value.status == BG_ERR_INVALID_ARG
+
+
+def test_context_survives_failed_and_degenerate_calls():
+    """the tile-feed and tiles-done counters must be zero at every launch whatever the
+    previous calls did.  The fused router's last tile zeroes the GEMM ticket counters, the split FFN zeroes
+    them on the stream, and a CUDA failure marks the context so that the next call re-zeroes everything.  Here:
+    rejected calls (T > max_tokens, misaligned pointer), a split FFN that draws zero tiles (all experts empty) and
+    one with fewer tiles than clusters, interleaved with fused calls that must stay bit-identical."""
+    from paper_2606_21712_b200 import BgMoeError
+    cfg = wl.small_config(T=300, d=256, E=12, k=3, f=192, index=34)
+    lay, g, layer = make(cfg)
+    first = layer.combined_forward(g["hidden"]).clone()
+    x = torch.zeros(cfg.T * cfg.k + 8, cfg.d, dtype=torch.bfloat16, device="cuda")
+    empty_off = torch.zeros(cfg.E + 1, dtype=torch.int32, device="cuda")     # all experts empty: zero tiles drawn
+    layer.expert_ffn(x[:cfg.T * cfg.k], empty_off, T=cfg.T)
+    assert torch.equal(layer.combined_forward(g["hidden"]), first)
+    with pytest.raises(BgMoeError):
+        layer.combined_forward(torch.zeros(cfg.T + 1, cfg.d, dtype=torch.bfloat16, device="cuda"))   # T > max_tokens
+    with pytest.raises(BgMoeError):
+        layer.expert_ffn(x.view(-1)[4:4 + cfg.T * cfg.k * cfg.d].view(cfg.T * cfg.k, cfg.d), empty_off, T=cfg.T)  # 8-byte aligned
+    one_off = torch.zeros(cfg.E + 1, dtype=torch.int32, device="cuda")
+    one_off[3:] = 5                                                          # one expert, 5 rows: 1-2 tiles
+    layer.expert_ffn(x[:cfg.T * cfg.k], one_off, T=cfg.T)
+    for _ in range(3):
+        assert torch.equal(layer.combined_forward(g["hidden"]), first)
+    torch.cuda.synchronize()
+
+
+def test_non_finite_logits_are_memory_safe():
+    """Reading S4: non-finite logits are out of contract; the routing kernels must still produce in-range, distinct
+    expert indices and a valid permutation (memory safety), whatever the values."""
+    T, E, k = 257, 40, 4
+    rng = np.random.default_rng(8)
+    L = rng.standard_normal((T, E)).astype(np.float32)
+    L[0, :] = -np.inf
+    L[1, ::3] = np.inf
+    L[2, 5] = np.nan
+    L[3, :] = np.nan
+    L[4, :10] = -np.inf
+    cfg = wl.small_config(T=T, d=64, E=E, k=k, f=64, index=35)
+    lay, g, layer = make(cfg)
+    r = layer.route(None, logits_in=torch.from_numpy(L).cuda())
+    idx = r["idx"].cpu().numpy()
+    assert idx.min() >= 0 and idx.max() < E
+    assert all(len(set(row)) == k for row in idx.tolist())
+    p = layer.permute(g["hidden"], r["idx"], r["offsets"])
+    rs = p["row_src"].cpu().numpy()
+    assert np.array_equal(np.sort(rs), np.arange(T * k))
+    assert r["counts"].sum().item() == T * k
+    # rows without non-finite entries still match the oracle bit for bit
+    fin = np.isfinite(L).all(axis=1)
+    o_idx, _ = oracle.topk_gate(L[fin], k)
+    assert np.array_equal(idx[fin], o_idx)
 
 
 def test_planned_workspace_equals_allocated_workspace():
@@ -330,7 +425,7 @@ def test_zero_copy_segments_equal_the_concatenation(lengths):
     n0 = layer.launch_count
     outs = layer.combined_forward_segments(segs)
     torch.cuda.synchronize()
-    assert layer.launch_count - n0 == 8
+    assert layer.launch_count - n0 == 5
     v1 = layer.debug_views(cfg.T)
     for key in ("logits", "idx", "w", "counts", "offsets", "row_src", "inv_perm"):
         assert torch.equal(v0[key], v1[key]), key
