@@ -61,6 +61,7 @@ struct bg_moe_ctx {
   // activation tensor maps of the workspace x_perm / H (whole capacity: rows past T*k are never stored)
   bg::ActMaps am_x, am_h;
   int sg_max = 0;               // bg_moe_set_debug: overrides the pair kernel's super-group size (tests)
+  int router_form = 0;          // bg_moe_set_debug: 0 = by T, 1 = sequential, 2 = cluster
   int64_t launches = 0;
   std::string last_error;
   // optional per-kernel timing of the fused chain
@@ -215,6 +216,8 @@ int do_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits
     r.counts = counts; r.offsets = offsets;
     r.done_counter = ctx->tile_counters + 4;
     r.gemm_counters = ctx->tile_counters;
+    r.num_sms = ctx->num_sms;
+    r.force_form = ctx->router_form;
     CUtensorMap tm_h;
     if (seg == nullptr && !encode_act_map(&tm_h, hidden, T, c.d)) {
       ctx->last_error = "cuTensorMapEncodeTiled(hidden) failed";
@@ -418,10 +421,11 @@ int bg_moe_destroy(bg_moe_ctx* ctx) {
   return BG_OK;
 }
 
-int bg_moe_set_debug(bg_moe_ctx* ctx, int32_t static_tile_feed, int32_t supergroup_token_tiles) {
-  if (ctx == nullptr || supergroup_token_tiles < 0) return BG_ERR_INVALID_ARG;
+int bg_moe_set_debug(bg_moe_ctx* ctx, int32_t static_tile_feed, int32_t supergroup_token_tiles, int32_t router_form) {
+  if (ctx == nullptr || supergroup_token_tiles < 0 || router_form < 0 || router_form > 2) return BG_ERR_INVALID_ARG;
   ctx->dyn_sched = static_tile_feed == 0;
   ctx->sg_max = supergroup_token_tiles;
+  ctx->router_form = router_form;
   return BG_OK;
 }
 

@@ -50,6 +50,8 @@ struct RouterLaunch {
   int32_t* offsets;         // [E+1]
   int32_t* done_counter;    // one int, zero between launches (re-armed by the kernel)
   int32_t* gemm_counters;   // four ints zeroed by the kernel's last tile (or nullptr)
+  int num_sms;
+  int force_form;           // 0 = choose from T (router_sequential); 1 = sequential form; 2 = cluster form (tests)
 };
 
 // ---- segments (zero-copy COMBINE): the combined tokens given as a list

@@ -28,6 +28,14 @@
 //   4. the last tile to finish (a global counter) scans the tile histograms into counts / offsets / per-tile
 //      bases and re-arms the counters.
 // No partial logits, no per-block histogram and no separate top-k / scan / rank launches touch HBM.
+//
+// Two forms of the same arithmetic (SEQ template flag), chosen on the host from T:
+//   cluster form (above): nch CTAs per tile; used while the grid fits about one wave (small / mid T, where the
+//     layer is latency-bound and K must be spread over SMs) and whenever nch accumulators do not fit in TMEM;
+//   sequential form: ONE CTA per tile runs the nch chunks one after the other into nch separate TMEM
+//     accumulators (nch * round_up(E,16) <= 512 columns) and adds them in the same ascending order in its
+//     epilogue -- the same partial sums, hence bit-identical logits, with no cluster traffic and a quarter of
+//     the CTAs; its epilogue thread owns a token and scans all E logits straight out of TMEM.
 #include "kernels.h"
 #include "ptx_sm100.cuh"
 #include "routing_common.cuh"
@@ -50,7 +58,9 @@ constexpr int NUM_THREADS = 256;                 // warp 0 TMA, warp 1 MMA, warp
 constexpr int RECV_BYTES = BM * (ROUTE_MAX_E + 4) * 4;   // [nch][128/nch][n_mma + 4] fp32 partial rows
 constexpr int LIST_BYTES = BM * ROUTE_MAX_K * 8;         // per-thread k-lists (key, expert)
 constexpr int SCAN_BYTES = (2 * 256 + 8) * 4;
-static_assert(RECV_BYTES + LIST_BYTES + SCAN_BYTES <= RING_BYTES, "epilogue scratch must fit in the ring");
+constexpr int XPOSE_PITCH = 36;                          // floats per row of a warp's 32 x 32 transposition tile
+constexpr int XPOSE_BYTES = 4 * 32 * XPOSE_PITCH * 4;    // one tile per epilogue warp
+static_assert(RECV_BYTES + LIST_BYTES + SCAN_BYTES + XPOSE_BYTES <= RING_BYTES, "epilogue scratch must fit in the ring");
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
 
 constexpr uint64_t ADESC_HI = umma_desc_sw128(16, 1024);
@@ -118,13 +128,39 @@ __device__ __forceinline__ void klist_insert(uint32_t (&bk)[KMAX], int (&be)[KMA
   }
 }
 
+// Gates (reading S2: softmax over the k selected logits, slot 0 holds the maximum), the token's rows of
+// topk_idx / topk_w, and its selected experts into the tile table `dst` (this CTA's or the leader's).
+template <int KMAX, typename Store>
+__device__ __forceinline__ void finish_token(const uint32_t (&bk)[KMAX], const int (&be)[KMAX], int k, int t, int T,
+                                             const RouterParams& p, Store store_idx) {
+  const float v0 = ordered_to_float(bk[0]);
+  float ex[KMAX];
+  float denom = 0.0f;
+  #pragma unroll
+  for (int s = 0; s < KMAX; ++s) {
+    ex[s] = (s < k) ? expf(ordered_to_float(bk[s]) - v0) : 0.0f;
+    denom += ex[s];                                // slot order
+  }
+  #pragma unroll
+  for (int s = 0; s < KMAX; ++s)
+    if (s < k) {
+      if (t < T) {
+        p.topk_idx[static_cast<int64_t>(t) * k + s] = be[s];
+        p.topk_w[static_cast<int64_t>(t) * k + s] = ex[s] / denom;
+      }
+      store_idx(s, t < T ? be[s] : -1);
+    }
+}
+
 // ROWS = false: A (hidden tile) by TMA from one contiguous [T, d] matrix (tm_h).
 // ROWS = true : A rows fetched through per-row pointers (segments, zero-copy COMBINE) by the four epilogue
 //               warps with 16-byte cp.async copies into the 128B-swizzled layout TMA would have produced;
 //               cp.async writes through the generic proxy and tcgen05.mma reads through the async proxy, so
 //               every loader thread waits for its own copies, fences the proxies, and only then arrives on
 //               the stage's full barrier.
-template <bool ROWS, int KMAX>
+// SEQ = false : cluster form, one K chunk per CTA (cluster size = p.nch), partials reduced through DSMEM.
+// SEQ = true  : sequential form, one CTA per tile, chunk c accumulates in TMEM columns [c * n_mma, (c+1) * n_mma).
+template <bool ROWS, bool SEQ, int KMAX>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_constant__ CUtensorMap tm_w,
                     const __grid_constant__ CUtensorMap tm_w1, const RouterParams p) {
@@ -145,17 +181,20 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
   uint32_t* list_k = reinterpret_cast<uint32_t*>(smem + RECV_BYTES);                 // [128][KMAX]
   int* list_e = reinterpret_cast<int*>(smem + RECV_BYTES + BM * ROUTE_MAX_K * 4);    // [128][KMAX]
   int* scan_scratch = reinterpret_cast<int*>(smem + RECV_BYTES + LIST_BYTES);
+  float* xpose = reinterpret_cast<float*>(smem + RECV_BYTES + LIST_BYTES + SCAN_BYTES);   // [4][32][XPOSE_PITCH]
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int T = p.T, d = p.d, E = p.E, k = p.k;
-  const int cs = p.nch;                                      // cluster size = K chunks
-  const uint32_t crank = cluster_ctarank();
+  const int cs = SEQ ? 1 : p.nch;                            // cluster size
+  const int nch = p.nch;                                     // K chunks (a function of d only)
+  const uint32_t crank = SEQ ? 0u : cluster_ctarank();
   const int m_tile = blockIdx.x / cs;
   const int n_tiles = gridDim.x / cs;
   const int k_blocks = (d + BK - 1) / BK;
-  const int kb_per = (k_blocks + cs - 1) / cs;
-  const int kb0 = static_cast<int>(crank) * kb_per, kb1 = min(k_blocks, kb0 + kb_per);
-  const int n_kb = max(0, kb1 - kb0);                        // k-blocks of this CTA (>= 1 for every rank, see router_nch)
+  const int kb_per = (k_blocks + nch - 1) / nch;             // k-blocks per chunk (every chunk has >= 1, see router_nch)
+  const int kb0 = SEQ ? 0 : static_cast<int>(crank) * kb_per;
+  const int kb1 = SEQ ? k_blocks : min(k_blocks, kb0 + kb_per);
+  const int n_kb = max(0, kb1 - kb0);                        // k-blocks of this CTA
   const int n_mma = (E + 15) & ~15;                          // UMMA N (multiple of 16 for M=128)
   const int n_blk = (E + 63) / 64;                           // 64-expert TMA boxes
   const uint32_t piece_bytes = n_blk * B_BLK_BYTES;
@@ -166,6 +205,7 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
   const int n_stages = min(MAX_STAGES, RING_BYTES / static_cast<int>(stage_bytes));
   const bool w4d = (n_mma & 63) == 0;                        // 4-D block view of the pieces (api.cu)
   const uint32_t idesc = umma_idesc_bf16(BM, n_mma, 0, 1);
+  const uint32_t tmem_cols = (SEQ && nch * n_mma > 256) ? 512u : 256u;
 
   // ---- independent of the previous kernel: barriers, TMEM
   if (warp == 0 && lane == 0) {
@@ -175,7 +215,7 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
     mbar_init(done_bar, 1);
     fence_barrier_init();
   }
-  if (warp == 2) { tmem_alloc(smem_u32(tmem_slot), 256); tmem_relinquish(); }
+  if (warp == 2) { tmem_alloc(smem_u32(tmem_slot), tmem_cols); tmem_relinquish(); }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -211,12 +251,17 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
         tc_fence_after();
         const uint32_t sa = base + s * stage_bytes, sb = sa + A_BYTES;
         const uint64_t ad = ADESC_HI | ((sa >> 4) & 0x3FFFu);
+        // sequential form: chunk c = kb / kb_per owns its own accumulator, restarted at the chunk's first k-block
+        const int kbl = it / ipk;                                   // k-block of this CTA
+        const int chunk = SEQ ? kbl / kb_per : 0;
+        const bool first = SEQ ? (kbl - chunk * kb_per == 0 && it % ipk == 0) : (it == 0);
+        const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(chunk * n_mma);
         for (int pc = 0; pc < pps; ++pc) {        // hidden * hi + hidden * mid + hidden * lo, one accumulator
           const uint64_t bd = BDESC_HI | (((sb + pc * piece_bytes) >> 4) & 0x3FFFu);
           #pragma unroll
           for (int kk = 0; kk < BK / UK; ++kk)
-            umma_f16(tmem_base, ad + ((kk * UK * 2) >> 4), bd + ((kk * UK * 128) >> 4), idesc,
-                     (it | pc | kk) != 0 ? 1u : 0u);
+            umma_f16(d_tmem, ad + ((kk * UK * 2) >> 4), bd + ((kk * UK * 128) >> 4), idesc,
+                     (first && pc == 0 && kk == 0) ? 0u : 1u);
         }
         umma_commit(empty_bar(s));
         if (++s == n_stages) { s = 0; ph ^= 1u; }
@@ -275,114 +320,163 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
         if (++pub_s == n_stages) pub_s = 0;
       }
     }
-    mbar_wait(done_bar, 0);                       // this CTA's accumulator is complete
+    mbar_wait(done_bar, 0);                       // this CTA's accumulator(s) are complete
     tc_fence_after();
   }
 
-  // ===================== epilogue over the cluster =====================
-  const int tpc = BM / cs;                        // token rows owned by each CTA after the reduce-scatter
-  const int EP = n_mma + 4;                       // row pitch (floats) of the received partial rows
   const int tid = threadIdx.x - 128;              // epilogue thread 0..127 (warps 4-7)
-
-  // (A) every CTA of the cluster has retired its MMAs: the rings may be overwritten by peers
-  __syncthreads();
-  cluster_sync_all();
-
-  // ---- 1. reduce-scatter of the partial tiles through distributed shared memory
-  if (warp >= 4) {
-    const int q = warp & 3;                       // TMEM lane quarter of this warp
-    const int row = q * 32 + lane;
-    const int owner = row / tpc, tl = row - owner * tpc;
-    const uint32_t dst = mapa_shared(base + static_cast<uint32_t>((static_cast<int>(crank) * tpc + tl) * EP) * 4u,
-                                     static_cast<uint32_t>(owner));
-    const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16);
-    for (int c0 = 0; c0 < n_mma; c0 += 32) {
-      uint32_t v[32];
-      tmem_ld_32x32(taddr + c0, v);               // columns past n_mma are allocated but unused
-      tmem_ld_wait();
-      #pragma unroll
-      for (int j = 0; j < 32; j += 4)
-        if (c0 + j < n_mma) {
-          if (n_kb > 0) st_shared_cluster_v4(dst + (c0 + j) * 4, v[j], v[j + 1], v[j + 2], v[j + 3]);
-          else st_shared_cluster_v4(dst + (c0 + j) * 4, 0u, 0u, 0u, 0u);
-        }
-    }
-    tc_fence_before();
-  }
-  // (B) all partial rows have arrived
-  __syncthreads();
-  cluster_sync_all();
-
-  const int t_cta0 = m_tile * BM + static_cast<int>(crank) * tpc;     // first token owned by this CTA
-  if (warp >= 4) {
-    // ---- logits of this CTA's tokens: partials added in ascending chunk order, then the bias
-    for (int i = tid; i < tpc * E; i += 128) {
-      const int tl = i / E, e = i - tl * E;
-      float v = recv[tl * EP + e];
-      for (int c = 1; c < cs; ++c) v += recv[(c * tpc + tl) * EP + e];
-      if (p.b_r != nullptr) v += __ldg(p.b_r + e);
-      recv[tl * EP + e] = v;
-      if (t_cta0 + tl < T) p.logits_out[static_cast<int64_t>(t_cta0 + tl) * E + e] = v;
-    }
-    if (crank == 0)
+  if (SEQ) {
+    // ===================== sequential form: thread <-> token row, all E logits straight from TMEM =====
+    if (warp >= 4) {
+      const int q = warp & 3;
+      const int row = q * 32 + lane, t = m_tile * BM + row;
+      const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16);
       for (int i = tid; i < ROUTE_MAX_E * 4; i += 128) mask[i] = 0u;
-    named_bar_sync(1, 128);
-
-    // ---- 2. top-k: thread (part, tl) scans experts part, part + cs, ... of token tl
-    const int part = tid / tpc, tl = tid - part * tpc;
-    uint32_t bk[KMAX];
-    int be[KMAX];
-    #pragma unroll
-    for (int s = 0; s < KMAX; ++s) { bk[s] = 0u; be[s] = 0x7fffffff; }
-    {
-      const float* rowp = recv + tl * EP;
-      for (int e = part; e < E; e += cs) klist_insert<KMAX, false>(bk, be, float_to_ordered(rowp[e]), e);
-    }
-    if (cs > 1) {
+      uint32_t bk[KMAX];
+      int be[KMAX];
       #pragma unroll
-      for (int s = 0; s < KMAX; ++s) { list_k[tid * KMAX + s] = bk[s]; list_e[tid * KMAX + s] = be[s]; }
-      named_bar_sync(1, 128);
-      if (part == 0)
-        for (int pp = 1; pp < cs; ++pp) {
-          const int o = (pp * tpc + tl) * KMAX;
+      for (int s = 0; s < KMAX; ++s) { bk[s] = 0u; be[s] = 0x7fffffff; }
+      float* lrow = p.logits_out + static_cast<int64_t>(t) * E;
+      for (int c0 = 0; c0 < n_mma; c0 += 32) {
+        uint32_t v[32];
+        tmem_ld_32x32(taddr + c0, v);             // chunk 0
+        tmem_ld_wait();
+        for (int c = 1; c < nch; ++c) {           // + chunk c, ascending: the cluster form's summation order
+          uint32_t u[32];
+          tmem_ld_32x32(taddr + c * n_mma + c0, u);
+          tmem_ld_wait();
           #pragma unroll
-          for (int s = 0; s < KMAX; ++s) {
-            const uint32_t x = list_k[o + s];
-            if (x != 0u) klist_insert<KMAX, true>(bk, be, x, list_e[o + s]);
+          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(u[j]));
+        }
+        #pragma unroll
+        for (int j = 0; j < 32; ++j) {
+          const int e = c0 + j;
+          if (e < E) {
+            float x = __uint_as_float(v[j]);
+            if (p.b_r != nullptr) x += __ldg(p.b_r + e);
+            v[j] = __float_as_uint(x);
+            klist_insert<KMAX, false>(bk, be, float_to_ordered(x), e);
           }
         }
-    }
-    if (part == 0) {
-      // gates: softmax over the k selected logits; slot 0 holds the maximum (reading S2)
-      const int t = t_cta0 + tl;
-      const int row = static_cast<int>(crank) * tpc + tl;
-      const float v0 = ordered_to_float(bk[0]);
-      float ex[KMAX];
-      float denom = 0.0f;
-      #pragma unroll
-      for (int s = 0; s < KMAX; ++s) {
-        ex[s] = (s < k) ? expf(ordered_to_float(bk[s]) - v0) : 0.0f;
-        denom += ex[s];                            // slot order
+        if (t < T) {
+          if ((E & 3) == 0) {
+            #pragma unroll
+            for (int j = 0; j < 32; j += 4)
+              if (c0 + j + 4 <= E)
+                *reinterpret_cast<uint4*>(lrow + c0 + j) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
+          } else {
+            #pragma unroll
+            for (int j = 0; j < 32; ++j)
+              if (c0 + j < E) lrow[c0 + j] = __uint_as_float(v[j]);
+          }
+        }
       }
-      const uint32_t lead = mapa_shared(smem_u32(idx_tile) + static_cast<uint32_t>(row * ROUTE_MAX_K) * 4u, 0u);
-      #pragma unroll
-      for (int s = 0; s < KMAX; ++s)
-        if (s < k) {
-          if (t < T) {
-            p.topk_idx[static_cast<int64_t>(t) * k + s] = be[s];
-            p.topk_w[static_cast<int64_t>(t) * k + s] = ex[s] / denom;
-          }
-          st_shared_cluster_u32_addr(lead + s * 4, static_cast<uint32_t>(t < T ? be[s] : -1));
-        }
+      finish_token<KMAX>(bk, be, k, t, T, p, [&](int s, int e) { idx_tile[row * ROUTE_MAX_K + s] = e; });
+      tc_fence_before();
     }
+    __syncthreads();
+  } else {
+    // ===================== cluster form: reduce-scatter over the cluster =====================
+    const int tpc = BM / cs;                      // token rows owned by each CTA after the reduce-scatter
+    const int EP = n_mma + 4;                     // row pitch (floats) of the received partial rows
+
+    // (A) every CTA of the cluster has retired its MMAs: the rings may be overwritten by peers
+    __syncthreads();
+    cluster_sync_all();
+
+    // ---- 1. partial rows to their owners through distributed shared memory.  A thread owns a token row in
+    // TMEM, but remote stores must be coalesced (scattered 16-byte stores run at a few percent of the DSMEM
+    // bandwidth): each warp turns 32 rows x 32 columns around in a private tile and sends 128-byte row pieces.
+    if (warp >= 4) {
+      const int q = warp & 3;                     // TMEM lane quarter of this warp
+      float* tile = xpose + q * 32 * XPOSE_PITCH;
+      const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16);
+      const int sub = lane >> 3, cc = (lane & 7) * 4;
+      for (int c0 = 0; c0 < n_mma; c0 += 32) {
+        uint32_t v[32];
+        tmem_ld_32x32(taddr + c0, v);             // columns past n_mma are allocated but unused
+        tmem_ld_wait();
+        #pragma unroll
+        for (int j = 0; j < 32; j += 4)
+          *reinterpret_cast<uint4*>(tile + lane * XPOSE_PITCH + j) =
+              n_kb > 0 ? make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]) : make_uint4(0u, 0u, 0u, 0u);
+        __syncwarp();
+        if (c0 + cc < n_mma) {
+          #pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int r = i * 4 + sub, row = q * 32 + r;
+            const int owner = row / tpc, tl = row - owner * tpc;
+            const uint4 x = *reinterpret_cast<const uint4*>(tile + r * XPOSE_PITCH + cc);
+            const uint32_t dst = mapa_shared(
+                base + static_cast<uint32_t>((static_cast<int>(crank) * tpc + tl) * EP + c0 + cc) * 4u,
+                static_cast<uint32_t>(owner));
+            st_shared_cluster_v4(dst, x.x, x.y, x.z, x.w);
+          }
+        }
+        __syncwarp();
+      }
+      tc_fence_before();
+    }
+    // (B) all partial rows have arrived
+    __syncthreads();
+    cluster_sync_all();
+
+    const int t_cta0 = m_tile * BM + static_cast<int>(crank) * tpc;     // first token owned by this CTA
+    if (warp >= 4) {
+      // ---- logits of this CTA's tokens: partials added in ascending chunk order, then the bias
+      for (int tl = 0; tl < tpc; ++tl) {
+        const bool live = t_cta0 + tl < T;
+        for (int e = tid; e < E; e += 128) {
+          float v = recv[tl * EP + e];
+          for (int c = 1; c < cs; ++c) v += recv[(c * tpc + tl) * EP + e];
+          if (p.b_r != nullptr) v += __ldg(p.b_r + e);
+          recv[tl * EP + e] = v;
+          if (live) p.logits_out[static_cast<int64_t>(t_cta0 + tl) * E + e] = v;
+        }
+      }
+      if (crank == 0)
+        for (int i = tid; i < ROUTE_MAX_E * 4; i += 128) mask[i] = 0u;
+      named_bar_sync(1, 128);
+
+      // ---- 2. top-k: thread (part, tl) scans experts part, part + cs, ... of token tl
+      const int part = tid / tpc, tl = tid - part * tpc;
+      uint32_t bk[KMAX];
+      int be[KMAX];
+      #pragma unroll
+      for (int s = 0; s < KMAX; ++s) { bk[s] = 0u; be[s] = 0x7fffffff; }
+      {
+        const float* rowp = recv + tl * EP;
+        for (int e = part; e < E; e += cs) klist_insert<KMAX, false>(bk, be, float_to_ordered(rowp[e]), e);
+      }
+      if (cs > 1) {
+        #pragma unroll
+        for (int s = 0; s < KMAX; ++s) { list_k[tid * KMAX + s] = bk[s]; list_e[tid * KMAX + s] = be[s]; }
+        named_bar_sync(1, 128);
+        if (part == 0)
+          for (int pp = 1; pp < cs; ++pp) {
+            const int o = (pp * tpc + tl) * KMAX;
+            #pragma unroll
+            for (int s = 0; s < KMAX; ++s) {
+              const uint32_t x = list_k[o + s];
+              if (x != 0u) klist_insert<KMAX, true>(bk, be, x, list_e[o + s]);
+            }
+          }
+      }
+      if (part == 0) {
+        const int row = static_cast<int>(crank) * tpc + tl;
+        const uint32_t lead = mapa_shared(smem_u32(idx_tile) + static_cast<uint32_t>(row * ROUTE_MAX_K) * 4u, 0u);
+        finish_token<KMAX>(bk, be, k, t_cta0 + tl, T, p,
+                           [&](int s, int e) { st_shared_cluster_u32_addr(lead + s * 4, static_cast<uint32_t>(e)); });
+      }
+    }
+    // (C) the leader holds the tile's selected experts
+    __syncthreads();
+    cluster_sync_all();
   }
-  // (C) the leader holds the tile's selected experts
-  __syncthreads();
-  cluster_sync_all();
 
   if (crank == 0) {
     if (warp >= 4) {
-      // ---- 3. tile-local stable rank + histogram (leader; thread <-> token row)
+      // ---- 3. tile-local stable rank + histogram (thread <-> token row)
       const int row = tid, t = m_tile * BM + row;
       int e[ROUTE_MAX_K], rk[ROUTE_MAX_K];
       #pragma unroll
@@ -409,22 +503,17 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 2) { tc_fence_after(); tmem_dealloc(tmem_base, 256); }
+  if (warp == 2) { tc_fence_after(); tmem_dealloc(tmem_base, tmem_cols); }
 }
 
-template <bool ROWS, int KMAX>
+template <bool ROWS, bool SEQ, int KMAX>
 cudaError_t launch_one(const CUtensorMap& tm_h, const CUtensorMap& tm_w, const CUtensorMap& tm_w1,
                        const RouterParams& p, cudaStream_t st) {
-  static bool attr_set = false;      // per instantiation; bg_moe_create calls router_kernels_init first
-  auto* kern = router_fused_kernel<ROWS, KMAX>;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  auto* kern = router_fused_kernel<ROWS, SEQ, KMAX>;
   const int n_tiles = (p.T + BM - 1) / BM;
+  const int cs = SEQ ? 1 : p.nch;
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(static_cast<unsigned>(n_tiles) * p.nch);
+  cfg.gridDim = dim3(static_cast<unsigned>(n_tiles) * cs);
   cfg.blockDim = dim3(NUM_THREADS);
   cfg.dynamicSmemBytes = SMEM_BYTES;
   cfg.stream = st;
@@ -432,37 +521,43 @@ cudaError_t launch_one(const CUtensorMap& tm_h, const CUtensorMap& tm_w, const C
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   attr[1].id = cudaLaunchAttributeClusterDimension;
-  attr[1].val.clusterDim.x = p.nch;
+  attr[1].val.clusterDim.x = cs;
   attr[1].val.clusterDim.y = 1;
   attr[1].val.clusterDim.z = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = 2;
+  cfg.numAttrs = SEQ ? 1 : 2;
   return cudaLaunchKernelEx(&cfg, kern, tm_h, tm_w, tm_w1, p);
 }
 
-template <bool ROWS>
+template <bool ROWS, bool SEQ>
 cudaError_t launch_k(const CUtensorMap& tm_h, const CUtensorMap& tm_w, const CUtensorMap& tm_w1,
                      const RouterParams& p, cudaStream_t st) {
-  if (p.k <= 2) return launch_one<ROWS, 2>(tm_h, tm_w, tm_w1, p, st);
-  if (p.k <= 4) return launch_one<ROWS, 4>(tm_h, tm_w, tm_w1, p, st);
-  return launch_one<ROWS, 8>(tm_h, tm_w, tm_w1, p, st);
+  if (p.k <= 2) return launch_one<ROWS, SEQ, 2>(tm_h, tm_w, tm_w1, p, st);
+  if (p.k <= 4) return launch_one<ROWS, SEQ, 4>(tm_h, tm_w, tm_w1, p, st);
+  return launch_one<ROWS, SEQ, 8>(tm_h, tm_w, tm_w1, p, st);
 }
 
-template <bool ROWS, int KMAX>
+template <bool ROWS, bool SEQ, int KMAX>
 cudaError_t init_one() {
-  return cudaFuncSetAttribute(router_fused_kernel<ROWS, KMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  return cudaFuncSetAttribute(router_fused_kernel<ROWS, SEQ, KMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              SMEM_BYTES);
+}
+template <bool ROWS, bool SEQ>
+cudaError_t init_k() {
+  cudaError_t e;
+  if ((e = init_one<ROWS, SEQ, 2>()) != cudaSuccess) return e;
+  if ((e = init_one<ROWS, SEQ, 4>()) != cudaSuccess) return e;
+  return init_one<ROWS, SEQ, 8>();
 }
 
 }  // namespace
 
 cudaError_t router_kernels_init() {
   cudaError_t e;
-  if ((e = init_one<false, 2>()) != cudaSuccess) return e;
-  if ((e = init_one<false, 4>()) != cudaSuccess) return e;
-  if ((e = init_one<false, 8>()) != cudaSuccess) return e;
-  if ((e = init_one<true, 2>()) != cudaSuccess) return e;
-  if ((e = init_one<true, 4>()) != cudaSuccess) return e;
-  return init_one<true, 8>();
+  if ((e = init_k<false, false>()) != cudaSuccess) return e;
+  if ((e = init_k<false, true>()) != cudaSuccess) return e;
+  if ((e = init_k<true, false>()) != cudaSuccess) return e;
+  return init_k<true, true>();
 }
 
 cudaError_t launch_split_wr(const float* W_r, int d, int E, void* pieces, cudaStream_t st) {
@@ -483,6 +578,18 @@ int router_nch(int d) {
   return 1;
 }
 
+// Which form runs (both give the same bits): the sequential form needs nch accumulators in TMEM; it is used when
+// there is only one chunk anyway, or when the cluster form's grid would exceed about one wave of the machine
+// (then K need not be spread over SMs and a quarter of the CTAs do without the cluster traffic).
+bool router_sequential(int T, int d, int E, int num_sms) {
+  const int nch = router_nch(d);
+  if (nch == 1) return true;
+  const int n_mma = (E + 15) & ~15;
+  if (nch * n_mma > 512) return false;
+  const int n_tiles = (T + BM - 1) / BM;
+  return n_tiles * nch > num_sms + num_sms / 4;
+}
+
 cudaError_t launch_router_fused(const CUtensorMap* tm_h, const CUtensorMap& tm_w, const CUtensorMap& tm_w1,
                                 const RouterLaunch& r, const SegTable* seg, cudaStream_t st) {
   if (r.T == 0) return cudaSuccess;
@@ -497,8 +604,10 @@ cudaError_t launch_router_fused(const CUtensorMap* tm_h, const CUtensorMap& tm_w
   p.seg_hidden = seg ? seg->hidden : nullptr;
   p.seg_start = seg ? seg->start : nullptr;
   p.n_segs = seg ? seg->n : 0;
-  if (seg != nullptr) return launch_k<true>(tm_w, tm_w, tm_w1, p, st);
-  return launch_k<false>(*tm_h, tm_w, tm_w1, p, st);
+  const bool seq = r.force_form == 0 ? router_sequential(r.T, r.d, r.E, r.num_sms)
+                                     : (r.force_form == 1 && (p.nch * ((r.E + 15) & ~15) <= 512 || p.nch == 1));
+  if (seg != nullptr) return seq ? launch_k<true, true>(tm_w, tm_w, tm_w1, p, st) : launch_k<true, false>(tm_w, tm_w, tm_w1, p, st);
+  return seq ? launch_k<false, true>(*tm_h, tm_w, tm_w1, p, st) : launch_k<false, false>(*tm_h, tm_w, tm_w1, p, st);
 }
 
 }  // namespace bg
