@@ -21,8 +21,9 @@
 // TMEM.  Then, through distributed shared memory:
 //   1. reduce-scatter: CTA c sends rows [r*128/nch, (r+1)*128/nch) of its partial tile to CTA r; CTA r adds the
 //      nch partials in ascending chunk order (+ bias) -> the logits of its 128/nch tokens (written to HBM once);
-//   2. top-k of those tokens in registers: nch threads per token scan interleaved expert subsets keeping a
-//      sorted k-list (branch-free insertion on sortable uint32 keys), merged by one thread per token;
+//   2. top-k of those tokens in registers: 256 / (128/nch) adjacent lanes per token scan interleaved groups of four
+//      experts keeping a sorted k-list (branch-free insertion on sortable uint32 keys); the lists are merged by k
+//      rounds of a shuffle tournament;
 //   3. the selected experts go to the cluster's leader, which builds the tile's [E] x 128-bit selection mask
 //      (integer OR), from it every entry's stable rank inside the tile and the tile's histogram;
 //   4. the last tile to finish (a global counter) scans the tile histograms into counts / offsets / per-tile
@@ -35,7 +36,7 @@
 //   sequential form: ONE CTA per tile runs the nch chunks one after the other into nch separate TMEM
 //     accumulators (nch * round_up(E,16) <= 512 columns) and adds them in the same ascending order in its
 //     epilogue -- the same partial sums, hence bit-identical logits, with no cluster traffic and a quarter of
-//     the CTAs; its epilogue thread owns a token and scans all E logits straight out of TMEM.
+//     the CTAs; the summed rows go to shared memory and through the same top-k code (two lanes per token).
 #include "kernels.h"
 #include "ptx_sm100.cuh"
 #include "routing_common.cuh"
@@ -56,11 +57,10 @@ constexpr int SMEM_BYTES = RING_BYTES + 1024 + BAR_BYTES + IDX_TILE_BYTES + MASK
 constexpr int NUM_THREADS = 256;                 // warp 0 TMA, warp 1 MMA, warp 2 TMEM alloc, warps 4-7 epilogue
 // epilogue scratch that reuses the ring once every MMA of the cluster has retired
 constexpr int RECV_BYTES = BM * (ROUTE_MAX_E + 4) * 4;   // [nch][128/nch][n_mma + 4] fp32 partial rows
-constexpr int LIST_BYTES = BM * ROUTE_MAX_K * 8;         // per-thread k-lists (key, expert)
 constexpr int SCAN_BYTES = (2 * 256 + 8) * 4;
 constexpr int XPOSE_PITCH = 36;                          // floats per row of a warp's 32 x 32 transposition tile
-constexpr int XPOSE_BYTES = 4 * 32 * XPOSE_PITCH * 4;    // one tile per epilogue warp
-static_assert(RECV_BYTES + LIST_BYTES + SCAN_BYTES + XPOSE_BYTES <= RING_BYTES, "epilogue scratch must fit in the ring");
+constexpr int XPOSE_BYTES = 8 * 32 * XPOSE_PITCH * 4;    // one tile per warp
+static_assert(RECV_BYTES + SCAN_BYTES + XPOSE_BYTES <= RING_BYTES, "epilogue scratch must fit in the ring");
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
 
 constexpr uint64_t ADESC_HI = umma_desc_sw128(16, 1024);
@@ -108,6 +108,10 @@ struct RouterParams {
   const int32_t* seg_start;
   int n_segs;
 };
+
+#ifdef BG_ROUTER_TRACE
+__device__ unsigned long long g_router_trace[8 * 16];   // development builds only: globaltimer stamps of CTAs 0..7
+#endif
 
 // Sorted insertion of (x, xe) into the descending list (bk, be): after every entry that `wins` against it.
 // TIE_BY_INDEX = false: entries arrive in ascending expert order, so an equal key already in the list has the
@@ -178,13 +182,23 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
   uint32_t* mask = reinterpret_cast<uint32_t*>(smem + RING_BYTES + BAR_BYTES + IDX_TILE_BYTES);   // [E][4]
   // ring reuse after the main loop
   float* recv = reinterpret_cast<float*>(smem);
-  uint32_t* list_k = reinterpret_cast<uint32_t*>(smem + RECV_BYTES);                 // [128][KMAX]
-  int* list_e = reinterpret_cast<int*>(smem + RECV_BYTES + BM * ROUTE_MAX_K * 4);    // [128][KMAX]
-  int* scan_scratch = reinterpret_cast<int*>(smem + RECV_BYTES + LIST_BYTES);
-  float* xpose = reinterpret_cast<float*>(smem + RECV_BYTES + LIST_BYTES + SCAN_BYTES);   // [4][32][XPOSE_PITCH]
+  int* scan_scratch = reinterpret_cast<int*>(smem + RECV_BYTES);
+  float* xpose = reinterpret_cast<float*>(smem + RECV_BYTES + SCAN_BYTES);           // [8 warps][32][XPOSE_PITCH]
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int T = p.T, d = p.d, E = p.E, k = p.k;
+#ifdef BG_ROUTER_TRACE
+  auto trace = [&](int slot) {
+    if (threadIdx.x == 128 && blockIdx.x < 8) {
+      unsigned long long t;
+      asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+      g_router_trace[blockIdx.x * 16 + slot] = t;
+    }
+  };
+#else
+  auto trace = [](int) {};
+#endif
+  trace(0);
   const int cs = SEQ ? 1 : p.nch;                            // cluster size
   const int nch = p.nch;                                     // K chunks (a function of d only)
   const uint32_t crank = SEQ ? 0u : cluster_ctarank();
@@ -221,6 +235,7 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   pdl_wait_then_trigger();
+  trace(1);
 
   if (warp == 0) {
     if (lane == 0) {                              // ---- TMA producer
@@ -320,79 +335,55 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
         if (++pub_s == n_stages) pub_s = 0;
       }
     }
-    mbar_wait(done_bar, 0);                       // this CTA's accumulator(s) are complete
-    tc_fence_after();
   }
+  // Every warp takes part in the epilogue (the TMA / MMA / allocator warps are idle by now): two warps share
+  // each TMEM lane quarter.
+  __syncwarp();
+  mbar_wait(done_bar, 0);                         // this CTA's accumulator(s) are complete
+  tc_fence_after();
+  trace(2);
 
-  const int tid = threadIdx.x - 128;              // epilogue thread 0..127 (warps 4-7)
+  const int tid = threadIdx.x - 128;              // epilogue-group thread 0..127 (warps 4-7), used by the rank step
+  const int q = warp & 3, half = warp >> 2;       // TMEM lane quarter; which half of the 32-column chunks
+  const int EP = n_mma + 4;                       // row pitch (floats) of the partial / logit rows in shared memory
+  const int tpc = BM / cs;                        // token rows this CTA finishes (128 in the sequential form)
+  const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16);
   if (SEQ) {
-    // ===================== sequential form: thread <-> token row, all E logits straight from TMEM =====
-    if (warp >= 4) {
-      const int q = warp & 3;
-      const int row = q * 32 + lane, t = m_tile * BM + row;
-      const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16);
-      for (int i = tid; i < ROUTE_MAX_E * 4; i += 128) mask[i] = 0u;
-      uint32_t bk[KMAX];
-      int be[KMAX];
-      #pragma unroll
-      for (int s = 0; s < KMAX; ++s) { bk[s] = 0u; be[s] = 0x7fffffff; }
-      float* lrow = p.logits_out + static_cast<int64_t>(t) * E;
-      for (int c0 = 0; c0 < n_mma; c0 += 32) {
-        uint32_t v[32];
-        tmem_ld_32x32(taddr + c0, v);             // chunk 0
+    // ===================== sequential form: the nch accumulators added in chunk order, rows to shared memory ====
+    const int row = q * 32 + lane;                // (every warp has seen done_bar: the ring is free)
+    for (int c0 = half * 32; c0 < n_mma; c0 += 64) {
+      uint32_t v[32];
+      tmem_ld_32x32(taddr + c0, v);               // chunk 0
+      tmem_ld_wait();
+      for (int c = 1; c < nch; ++c) {             // + chunk c, ascending: the cluster form's summation order
+        uint32_t u[32];
+        tmem_ld_32x32(taddr + c * n_mma + c0, u);
         tmem_ld_wait();
-        for (int c = 1; c < nch; ++c) {           // + chunk c, ascending: the cluster form's summation order
-          uint32_t u[32];
-          tmem_ld_32x32(taddr + c * n_mma + c0, u);
-          tmem_ld_wait();
-          #pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(u[j]));
-        }
         #pragma unroll
-        for (int j = 0; j < 32; ++j) {
-          const int e = c0 + j;
-          if (e < E) {
-            float x = __uint_as_float(v[j]);
-            if (p.b_r != nullptr) x += __ldg(p.b_r + e);
-            v[j] = __float_as_uint(x);
-            klist_insert<KMAX, false>(bk, be, float_to_ordered(x), e);
-          }
-        }
-        if (t < T) {
-          if ((E & 3) == 0) {
-            #pragma unroll
-            for (int j = 0; j < 32; j += 4)
-              if (c0 + j + 4 <= E)
-                *reinterpret_cast<uint4*>(lrow + c0 + j) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
-          } else {
-            #pragma unroll
-            for (int j = 0; j < 32; ++j)
-              if (c0 + j < E) lrow[c0 + j] = __uint_as_float(v[j]);
-          }
-        }
+        for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(u[j]));
       }
-      finish_token<KMAX>(bk, be, k, t, T, p, [&](int s, int e) { idx_tile[row * ROUTE_MAX_K + s] = e; });
-      tc_fence_before();
+      #pragma unroll
+      for (int j = 0; j < 32; j += 4)
+        if (c0 + j < n_mma)
+          *reinterpret_cast<uint4*>(recv + row * EP + c0 + j) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
     }
+    tc_fence_before();
+    for (int i = threadIdx.x; i < ROUTE_MAX_E * 4; i += NUM_THREADS) mask[i] = 0u;
     __syncthreads();
   } else {
     // ===================== cluster form: reduce-scatter over the cluster =====================
-    const int tpc = BM / cs;                      // token rows owned by each CTA after the reduce-scatter
-    const int EP = n_mma + 4;                     // row pitch (floats) of the received partial rows
-
     // (A) every CTA of the cluster has retired its MMAs: the rings may be overwritten by peers
     __syncthreads();
     cluster_sync_all();
+    trace(3);
 
     // ---- 1. partial rows to their owners through distributed shared memory.  A thread owns a token row in
     // TMEM, but remote stores must be coalesced (scattered 16-byte stores run at a few percent of the DSMEM
     // bandwidth): each warp turns 32 rows x 32 columns around in a private tile and sends 128-byte row pieces.
-    if (warp >= 4) {
-      const int q = warp & 3;                     // TMEM lane quarter of this warp
-      float* tile = xpose + q * 32 * XPOSE_PITCH;
-      const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16);
+    {
+      float* tile = xpose + warp * 32 * XPOSE_PITCH;
       const int sub = lane >> 3, cc = (lane & 7) * 4;
-      for (int c0 = 0; c0 < n_mma; c0 += 32) {
+      for (int c0 = half * 32; c0 < n_mma; c0 += 64) {
         uint32_t v[32];
         tmem_ld_32x32(taddr + c0, v);             // columns past n_mma are allocated but unused
         tmem_ld_wait();
@@ -416,63 +407,94 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
         __syncwarp();
       }
       tc_fence_before();
+      trace(4);
     }
+    if (crank == 0)
+      for (int i = threadIdx.x; i < ROUTE_MAX_E * 4; i += NUM_THREADS) mask[i] = 0u;
     // (B) all partial rows have arrived
     __syncthreads();
     cluster_sync_all();
+    trace(5);
+  }
 
-    const int t_cta0 = m_tile * BM + static_cast<int>(crank) * tpc;     // first token owned by this CTA
-    if (warp >= 4) {
-      // ---- logits of this CTA's tokens: partials added in ascending chunk order, then the bias
-      for (int tl = 0; tl < tpc; ++tl) {
-        const bool live = t_cta0 + tl < T;
-        for (int e = tid; e < E; e += 128) {
-          float v = recv[tl * EP + e];
-          for (int c = 1; c < cs; ++c) v += recv[(c * tpc + tl) * EP + e];
-          if (p.b_r != nullptr) v += __ldg(p.b_r + e);
-          recv[tl * EP + e] = v;
-          if (live) p.logits_out[static_cast<int64_t>(t_cta0 + tl) * E + e] = v;
+  // ===================== logits + top-k of this CTA's tpc tokens, P = 256 / tpc threads per token ==========
+  // Thread (tl, part): lanes of one token are adjacent.  It adds the partial rows of experts 4g .. 4g+3,
+  // g = part, part + P, ... in ascending chunk order (+ bias), writes those logits, and keeps a sorted k-list
+  // (branch-free insertion, ascending expert order inside the thread).  The P lists of a token are then merged
+  // by k rounds of a shuffle tournament under the order of reading S3 (key desc, expert index asc).
+  {
+    const int P = NUM_THREADS / tpc;              // 2 (sequential form) .. 16 (cluster of 8): a power of two
+    const int tl = threadIdx.x / P, part = threadIdx.x - tl * P;
+    const int row = static_cast<int>(crank) * tpc + tl;        // row of the 128-token tile
+    const int t = m_tile * BM + row;
+    const int n_sum = SEQ ? 1 : cs;               // partial rows to add (the sequential form added in registers)
+    uint32_t bk[KMAX];
+    int be[KMAX];
+    #pragma unroll
+    for (int s = 0; s < KMAX; ++s) { bk[s] = 0u; be[s] = 0x7fffffff; }
+    const bool vec_ok = (E & 3) == 0;
+    for (int e0 = part * 4; e0 < E; e0 += P * 4) {
+      float4 v = *reinterpret_cast<const float4*>(recv + tl * EP + e0);
+      for (int c = 1; c < n_sum; ++c) {
+        const float4 u = *reinterpret_cast<const float4*>(recv + (c * tpc + tl) * EP + e0);
+        v.x += u.x; v.y += u.y; v.z += u.z; v.w += u.w;
+      }
+      float x[4] = {v.x, v.y, v.z, v.w};
+      #pragma unroll
+      for (int j = 0; j < 4; ++j)
+        if (e0 + j < E) {
+          if (p.b_r != nullptr) x[j] += __ldg(p.b_r + e0 + j);
+          klist_insert<KMAX, false>(bk, be, float_to_ordered(x[j]), e0 + j);
+        }
+      if (t < T) {
+        float* lrow = p.logits_out + static_cast<int64_t>(t) * E + e0;
+        if (vec_ok) {
+          *reinterpret_cast<float4*>(lrow) = make_float4(x[0], x[1], x[2], x[3]);
+        } else {
+          #pragma unroll
+          for (int j = 0; j < 4; ++j)
+            if (e0 + j < E) lrow[j] = x[j];
         }
       }
-      if (crank == 0)
-        for (int i = tid; i < ROUTE_MAX_E * 4; i += 128) mask[i] = 0u;
-      named_bar_sync(1, 128);
-
-      // ---- 2. top-k: thread (part, tl) scans experts part, part + cs, ... of token tl
-      const int part = tid / tpc, tl = tid - part * tpc;
-      uint32_t bk[KMAX];
-      int be[KMAX];
-      #pragma unroll
-      for (int s = 0; s < KMAX; ++s) { bk[s] = 0u; be[s] = 0x7fffffff; }
-      {
-        const float* rowp = recv + tl * EP;
-        for (int e = part; e < E; e += cs) klist_insert<KMAX, false>(bk, be, float_to_ordered(rowp[e]), e);
+    }
+    trace(6);
+    // tournament: each round every lane offers the head of its list; the winner's owner pops it
+    uint32_t rk[KMAX];
+    int re[KMAX];
+    #pragma unroll
+    for (int s = 0; s < KMAX; ++s) {
+      uint32_t hk = bk[0];
+      int he = be[0];
+      for (int o = 1; o < P; o <<= 1) {
+        const uint32_t ok = __shfl_xor_sync(0xffffffffu, hk, o);
+        const int oe = __shfl_xor_sync(0xffffffffu, he, o);
+        if (ok > hk || (ok == hk && oe < he)) { hk = ok; he = oe; }
       }
-      if (cs > 1) {
+      rk[s] = hk;
+      re[s] = he;
+      if (he == be[0]) {                           // expert indices are unique: this lane owns the winner
         #pragma unroll
-        for (int s = 0; s < KMAX; ++s) { list_k[tid * KMAX + s] = bk[s]; list_e[tid * KMAX + s] = be[s]; }
-        named_bar_sync(1, 128);
-        if (part == 0)
-          for (int pp = 1; pp < cs; ++pp) {
-            const int o = (pp * tpc + tl) * KMAX;
-            #pragma unroll
-            for (int s = 0; s < KMAX; ++s) {
-              const uint32_t x = list_k[o + s];
-              if (x != 0u) klist_insert<KMAX, true>(bk, be, x, list_e[o + s]);
-            }
-          }
+        for (int i = 0; i + 1 < KMAX; ++i) { bk[i] = bk[i + 1]; be[i] = be[i + 1]; }
+        bk[KMAX - 1] = 0u;
+        be[KMAX - 1] = 0x7fffffff;
       }
-      if (part == 0) {
-        const int row = static_cast<int>(crank) * tpc + tl;
+    }
+    trace(7);
+    if (part == 0) {
+      if (SEQ) {
+        finish_token<KMAX>(rk, re, k, t, T, p, [&](int s, int e) { idx_tile[row * ROUTE_MAX_K + s] = e; });
+      } else {
         const uint32_t lead = mapa_shared(smem_u32(idx_tile) + static_cast<uint32_t>(row * ROUTE_MAX_K) * 4u, 0u);
-        finish_token<KMAX>(bk, be, k, t_cta0 + tl, T, p,
+        finish_token<KMAX>(rk, re, k, t, T, p,
                            [&](int s, int e) { st_shared_cluster_u32_addr(lead + s * 4, static_cast<uint32_t>(e)); });
       }
     }
-    // (C) the leader holds the tile's selected experts
-    __syncthreads();
-    cluster_sync_all();
+    trace(8);
   }
+  // (C) the tile's selected experts are in idx_tile (of the leader, in the cluster form)
+  __syncthreads();
+  if (!SEQ) cluster_sync_all();
+  trace(9);
 
   if (crank == 0) {
     if (warp >= 4) {
@@ -487,6 +509,7 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
       for (int s = 0; s < ROUTE_MAX_K; ++s)
         if (s < k && e[s] >= 0) p.tile_rank[static_cast<int64_t>(t) * k + s] = rk[s];
       __threadfence();
+      trace(10);
     }
     __syncthreads();
     if (threadIdx.x == 0) *last_flag = (atomicAdd(p.done_counter, 1) == n_tiles - 1) ? 1 : 0;
@@ -501,6 +524,7 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
       }
     }
   }
+  trace(11);
   tc_fence_before();
   __syncthreads();
   if (warp == 2) { tc_fence_after(); tmem_dealloc(tmem_base, tmem_cols); }
@@ -559,6 +583,12 @@ cudaError_t router_kernels_init() {
   if ((e = init_k<true, false>()) != cudaSuccess) return e;
   return init_k<true, true>();
 }
+
+#ifdef BG_ROUTER_TRACE
+extern "C" int bg_moe_debug_router_trace(unsigned long long* out) {
+  return cudaMemcpyFromSymbol(out, g_router_trace, sizeof(g_router_trace)) == cudaSuccess ? 0 : -3;
+}
+#endif
 
 cudaError_t launch_split_wr(const float* W_r, int d, int E, void* pieces, cudaStream_t st) {
   const int E_ld = (E + 15) & ~15;
