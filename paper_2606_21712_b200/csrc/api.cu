@@ -33,7 +33,7 @@ struct bg_moe_ctx {
   int32_t* row_src = nullptr;
   int32_t* inv_perm = nullptr;
   float* w_perm = nullptr;      // gate weights in expert order (fused path)
-  int32_t* tile_counters = nullptr;   // [0..3]: ticket / finished counters of the two pair GEMMs; [4]: router tiles done
+  int32_t* tile_counters = nullptr;   // [0..3], [4..7]: hot tickets / cold tickets / clusters finished of the two pair GEMMs; [8]: router tiles done
   bool counters_dirty = false;  // a call failed after launching: re-zero the counters before the next launch
   bool dyn_sched = true;        // dynamic tile feed of the pair GEMMs (bg_moe_set_debug: static = tile t -> cluster t mod 74)
   // segment table of bg_moe_combined_forward_segments (device arrays + pageable host staging)
@@ -214,7 +214,7 @@ int do_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits
     r.topk_idx = topk_idx; r.topk_w = topk_w;
     r.tile_rank = ctx->tile_rank; r.tile_counts = ctx->tile_counts; r.tile_base = ctx->tile_base;
     r.counts = counts; r.offsets = offsets;
-    r.done_counter = ctx->tile_counters + 4;
+    r.done_counter = ctx->tile_counters + 8;
     r.gemm_counters = ctx->tile_counters;
     r.num_sms = ctx->num_sms;
     r.force_form = ctx->router_form;
@@ -263,7 +263,7 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g2.tm_b0 = ctx->tm_wd;
   g2.tm_b1 = ctx->tm_wd;
   g2.sg_max = ctx->sg_max;
-  g2.tile_counter = ctx->dyn_sched ? ctx->tile_counters + 2 : nullptr;
+  g2.tile_counter = ctx->dyn_sched ? ctx->tile_counters + 4 : nullptr;
   g2.w4d = c.d % 64 == 0;
   g2.tm_b0_4d = g2.w4d ? ctx->tm_wd4 : ctx->tm_wd;
   g2.tm_b1_4d = g2.tm_b0_4d;
@@ -549,7 +549,7 @@ int bg_moe_expert_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offset
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   if ((rc = begin_call(ctx, st))) return rc;
   // no router kernel precedes the GEMMs here: zero their ticket counters on the stream
-  BG_CUDA(ctx, cudaMemsetAsync(ctx->tile_counters, 0, 16, st), "memset ticket counters");
+  BG_CUDA(ctx, cudaMemsetAsync(ctx->tile_counters, 0, 32, st), "memset ticket counters");
   rc = do_ffn(ctx, x_perm, offsets, T, y_perm, nullptr, st);
   if (rc) return rc;
   return end_call(ctx, st, false);

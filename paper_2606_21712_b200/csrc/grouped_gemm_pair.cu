@@ -43,7 +43,9 @@
 // ceil(N_out/OUT_FEATS) feature tiles, ordered feature-tile-major / token-tile-minor so that the
 // clusters running at the same time share weight strips through L2.  Tiles are drawn in that order from a
 // global ticket counter (dynamic feed, see `feed_next`), so the neighbours really run concurrently and a strip
-// is read from HBM once; BG_MOE_SCHED=static keeps the fixed map tile t -> cluster (t mod #clusters).
+// is read from HBM once; bg_moe_set_debug(static_tile_feed) keeps the fixed map tile t -> cluster (t mod #clusters).
+// Launches that mix experts of many rows with many experts of <= 32 rows run two tile lists side by side
+// ("bimodal", see the tile tables in the kernel).
 // Experts with no rows own no tiles and their weights are never touched.
 #include "kernels.h"
 #include "ptx_sm100.cuh"
@@ -61,12 +63,20 @@ constexpr int A_BYTES = 2 * A_BLK_BYTES;            // 16 KB: this CTA's 128 M r
 constexpr int B_BYTES = (BN_MAX / 2) * BK * 2;      // 16 KB: this CTA's half of the tokens
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;      // 32 KB
 constexpr int RING_BYTES = STAGES * STAGE_BYTES;    // 192 KB
+// Cold class (bimodal launches only, see the tile scheduler below): experts with 1..COLD_ROWS rows.  Their tiles
+// are pure weight streaming (16 KB of weights per CTA and k-block against <= 2 KB of tokens), so the same ring
+// memory is cut into more, smaller stages: 10 x 18 KB keep 160 KB of weights in flight per SM instead of 96 KB.
+constexpr int COLD_ROWS = 32;
+constexpr int COLD_STAGES = 10;
+constexpr int COLD_B_BYTES = (COLD_ROWS / 2) * BK * 2;        // 2 KB: this CTA's half of <= 32 tokens
+constexpr int COLD_STAGE_BYTES = A_BYTES + COLD_B_BYTES;      // 18 KB (a multiple of 1024: SW128 alignment holds)
+static_assert(COLD_STAGES * COLD_STAGE_BYTES <= RING_BYTES, "cold ring must fit in the ring memory");
 constexpr int MAX_THREADS = 384;             // 4 role warps + 4 (a7) or 8 (a8) epilogue warps
 constexpr int MAX_E = 256;
 constexpr int XCH_PITCH = 36;                       // words per lane row of an exchange buffer (conflict-free v4)
 constexpr int XCH_BYTES = 32 * XCH_PITCH * 4;       // 4608 B
-constexpr int BAR_BYTES = 256;
-constexpr int TABLE_BYTES = 2064;                   // 2 x (MAX_E + 1) ints, 16-byte padded
+constexpr int BAR_BYTES = 512;
+constexpr int TABLE_BYTES = 3136;                   // 3 x (MAX_E + 1) ints + the launch's class totals, 16-byte padded
 constexpr int STAGE_TILE_BYTES = 32 * 64;           // per-warp output staging: [32 tokens][32 features] bf16
 // epilogue scratch: [4 exchange buffers (a7) | 4 x 256 gate weights (a8)] then the 4 staging tiles
 constexpr int EPI_BYTES = 4 * XCH_BYTES + 4 * STAGE_TILE_BYTES;   // a8: 2 KB of scales + 8 staging tiles = 18 KB
@@ -88,7 +98,8 @@ struct Params {
   const float* row_scale;      // a8, fused path: gate weight per expert-order row (w_perm[r]); nullptr = 1
   bool w4d;                    // tm_w0 / tm_w1 are the 4-D block views (kernels.h)
   int sg_max;                  // 0 = derive the super-group size from K
-  int* tile_counter;           // dynamic feed: [2] = ticket counter, clusters-finished counter (zero between launches); nullptr = static feed
+  int* tile_counter;           // dynamic feed: [3] = hot tickets, cold tickets, clusters finished (zero between launches); nullptr = static feed
+  int num_sms;
 };
 
 __device__ __forceinline__ void named_bar_sync(int id, int threads) {
@@ -96,19 +107,28 @@ __device__ __forceinline__ void named_bar_sync(int id, int threads) {
 }
 
 struct TileCoord {
-  int e, row0, rows_valid, nt, f_tile, t_tile;
+  int e, row0, rows_valid, nt, f_tile, t_tile, cold;
 };
 
-// tile_start[e] = first linear tile index of expert e (tile_start[E] = total);
-// t_tiles[e] = token tiles of expert e.  Both live in shared memory.
-// Inside an expert the order is feature-tile-major / token-tile-minor, so the token tiles that share a
-// weight strip run at the same time.  When an expert's token matrix is too large to stay in L2 between
-// two feature tiles (DeepSeek-shaped hot experts: thousands of rows x 14 KB), that order re-streams the
-// tokens from HBM once per feature tile; such experts are cut into super-groups of `sg_max` token tiles
-// (sized to ~48 MB of tokens) and each super-group runs through all feature tiles before the next starts:
-// the tokens stay in L2 and the expert's weights are streamed once per super-group instead.
-__device__ __forceinline__ TileCoord decode_tile(int t, const int* tile_start, const int* t_tiles,
-                                                 const int32_t* offsets, int E, int sg_max) {
+// Tile tables (shared memory).  A launch has up to two tile lists:
+//   hot list : tile_start_hot[e] = first linear tile index of expert e (tile_start_hot[E] = total); t_tiles[e] =
+//              token tiles of expert e.  Inside an expert the order is feature-tile-major / token-tile-minor, so
+//              the token tiles that share a weight strip run at the same time.  When an expert's token matrix is
+//              too large to stay in L2 between two feature tiles (DeepSeek-shaped hot experts: thousands of rows x
+//              14 KB), that order re-streams the tokens from HBM once per feature tile; such experts are cut into
+//              super-groups of `sg_max` token tiles (sized to ~48 MB of tokens) and each super-group runs through
+//              all feature tiles before the next starts: the tokens stay in L2 and the expert's weights are
+//              streamed once per super-group instead.
+//   cold list: (bimodal launches only) the experts with 1..COLD_ROWS rows, one token tile each, feature tiles in
+//              order.  In every other launch all experts are in the hot list and the cold list is empty.
+// A ticket is the linear index in its list, with bit 30 set for the cold list.
+constexpr int COLD_BIT = 1 << 30;
+
+__device__ __forceinline__ TileCoord decode_tile(int ticket, const int* tile_start_hot, const int* tile_start_cold,
+                                                 const int* t_tiles, const int32_t* offsets, int E, int sg_max) {
+  const int cold = (ticket & COLD_BIT) != 0;
+  const int t = ticket & (COLD_BIT - 1);
+  const int* tile_start = cold ? tile_start_cold : tile_start_hot;
   int lo = 0, hi = E;              // largest e with tile_start[e] <= t
   while (hi - lo > 1) {
     const int mid = (lo + hi) >> 1;
@@ -118,7 +138,7 @@ __device__ __forceinline__ TileCoord decode_tile(int t, const int* tile_start, c
   // last expert whose start <= t, which is the one that owns t (its successors start later).
   const int e = lo;
   const int local = t - tile_start[e];
-  const int tt = t_tiles[e];
+  const int tt = cold ? 1 : t_tiles[e];
   int f_tile, t_tile;
   if (tt <= sg_max) {
     f_tile = local / tt;
@@ -144,6 +164,7 @@ __device__ __forceinline__ TileCoord decode_tile(int t, const int* tile_start, c
   c.nt = (c.rows_valid + 15) & ~15;
   c.f_tile = f_tile;
   c.t_tile = t_tile;
+  c.cold = cold;
   return c;
 }
 
@@ -177,21 +198,24 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   const uint32_t base = (raw + 1023u) & ~1023u;       // SW128 tiles need 1024-byte alignment
   uint8_t* smem = smem_raw + (base - raw);
   const uint32_t bar_base = base + RING_BYTES;
-  // barriers: full[S] empty[S] tmem_full[2] tmem_empty[2]; then the TMEM address
-  auto full_bar = [&](int s) { return bar_base + 8u * s; };
-  auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
-  auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + a); };
-  auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + 2 + a); };
+  // barriers: hot ring full[S] empty[S], cold ring full[CS] empty[CS], tmem_full[2] tmem_empty[2]; then the TMEM address
+  auto full_bar = [&](int cold, int s) { return bar_base + 8u * ((cold ? 2 * STAGES : 0) + s); };
+  auto empty_bar = [&](int cold, int s) { return bar_base + 8u * ((cold ? 2 * STAGES + COLD_STAGES : STAGES) + s); };
+  constexpr int RING_BARS = 2 * STAGES + 2 * COLD_STAGES;
+  auto tfull_bar = [&](int a) { return bar_base + 8u * (RING_BARS + a); };
+  auto tempty_bar = [&](int a) { return bar_base + 8u * (RING_BARS + 2 + a); };
   // tile feed (dynamic scheduler): sched_full[SCHED_SLOTS] per CTA, sched_empty[SCHED_SLOTS] on the leader
-  auto sfull_bar = [&](int i) { return bar_base + 8u * (2 * STAGES + 4 + i); };
-  auto sempty_bar = [&](int i) { return bar_base + 8u * (2 * STAGES + 4 + SCHED_SLOTS + i); };
-  constexpr int NBAR = 2 * STAGES + 4 + 2 * SCHED_SLOTS;
+  auto sfull_bar = [&](int i) { return bar_base + 8u * (RING_BARS + 4 + i); };
+  auto sempty_bar = [&](int i) { return bar_base + 8u * (RING_BARS + 4 + SCHED_SLOTS + i); };
+  constexpr int NBAR = RING_BARS + 4 + 2 * SCHED_SLOTS;
   static_assert(8 * NBAR + 16 + 4 * SCHED_SLOTS <= BAR_BYTES, "barrier area");
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + RING_BYTES + 8 * NBAR);
   volatile int* tile_slot = reinterpret_cast<volatile int*>(smem + RING_BYTES + 8 * NBAR + 16);
   constexpr int N_CONSUMERS = 3 + 2 * EPI_WARPS;      // two producers, the MMA thread, every epilogue warp of the pair
-  int* tile_start = reinterpret_cast<int*>(smem + RING_BYTES + BAR_BYTES);
-  int* t_tiles = tile_start + (MAX_E + 1);
+  int* tile_start = reinterpret_cast<int*>(smem + RING_BYTES + BAR_BYTES);     // hot list
+  int* tile_start_cold = tile_start + (MAX_E + 1);
+  int* t_tiles = tile_start_cold + (MAX_E + 1);
+  int* launch_info = t_tiles + (MAX_E + 1);            // [0] clusters that start on the cold list (0 = not bimodal)
   uint8_t* epi_smem = smem + RING_BYTES + BAR_BYTES + TABLE_BYTES;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -207,7 +231,8 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tm_w0);
     if (GATEUP) tma_prefetch_desc(&tm_w1);
-    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(0, s), 1); mbar_init(empty_bar(0, s), 1); }
+    for (int s = 0; s < COLD_STAGES; ++s) { mbar_init(full_bar(1, s), 1); mbar_init(empty_bar(1, s), 1); }
     // tmem_empty (used on the leader only): one arrival per epilogue warp of both CTAs
     for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 2 * EPI_WARPS); }
     for (int i = 0; i < SCHED_SLOTS; ++i) { mbar_init(sfull_bar(i), 1); mbar_init(sempty_bar(i), N_CONSUMERS); }
@@ -219,28 +244,69 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   }
   // ---- everything below reads what the previous kernels wrote (offsets, activations)
   pdl_wait_then_trigger();
-  // ---- per-CTA tile table: inclusive scan of per-expert tile counts (E <= 256 = blockDim)
+  // ---- per-CTA tile tables: inclusive scans of per-expert tile counts (E <= 256 <= blockDim).
+  // Bimodal launches: when a launch has both experts of many rows (tensor-bound tiles whose weight
+  // strips are reused from L2) and many experts of a few rows (tiles that only stream weights from HBM), running
+  // them one after the other leaves HBM idle during the first and the tensor cores idle during the second.  The
+  // experts with 1..COLD_ROWS rows then go to a second (cold) tile list with its own ticket counter, a fixed
+  // share of the clusters starts on that list and the rest on the hot list, so both resources are busy at the
+  // same time; a cluster that runs its list dry moves to the other one.  Cold tiles use the deeper cold ring.
   {
-    int tt = 0;
+    const bool dyn_feed = p.tile_counter != nullptr;
+    int cnt = 0, tt = 0;
     if (threadIdx.x < E) {
-      const int cnt = __ldg(p.offsets + threadIdx.x + 1) - __ldg(p.offsets + threadIdx.x);
+      cnt = __ldg(p.offsets + threadIdx.x + 1) - __ldg(p.offsets + threadIdx.x);
       tt = (cnt + BN_MAX - 1) / BN_MAX;
       t_tiles[threadIdx.x] = tt;
     }
-    int v = tt * f_tiles;
+    const bool is_cold = cnt >= 1 && cnt <= COLD_ROWS;
+    // pass 1: totals of each class -> is the launch bimodal, and how many clusters start on the cold list
+    unsigned long long v = (static_cast<unsigned long long>(is_cold ? f_tiles : 0) << 32) |
+                           static_cast<unsigned>(is_cold ? 0 : tt * f_tiles);
+    int hot_rows = is_cold ? 0 : cnt;
+    #pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      v += __shfl_xor_sync(0xffffffffu, v, o);
+      hot_rows += __shfl_xor_sync(0xffffffffu, hot_rows, o);
+    }
+    __shared__ unsigned long long warp_tot[MAX_THREADS / 32];
+    __shared__ int warp_rows[MAX_THREADS / 32];
+    if (lane == 0) { warp_tot[warp] = v; warp_rows[warp] = hot_rows; }
+    __syncthreads();
+    unsigned long long tot = 0;
+    long long rows_tot = 0;
+    for (int w = 0; w < static_cast<int>(blockDim.x >> 5); ++w) { tot += warp_tot[w]; rows_tot += warp_rows[w]; }
+    const long long cold_total = static_cast<long long>(tot >> 32), hot_total = static_cast<long long>(tot & 0xffffffffu);
+    const int num_clusters_ = gridDim.x >> 1;
+    int n_cold_clusters = 0;
+    if (dyn_feed && cold_total >= 2 * num_clusters_ && hot_total >= 2 * num_clusters_) {
+      // time shares if every cluster worked on one class: a cold k-block is ~0.22 us of weight streaming per CTA,
+      // a hot k-block ~0.30 us of MMA per 256 token rows
+      const long long cold_w = cold_total * 22, hot_w = rows_tot * f_tiles * 30 / BN_MAX;
+      long long n = (num_clusters_ * cold_w + (cold_w + hot_w) / 2) / (cold_w + hot_w);
+      n_cold_clusters = static_cast<int>(n < 1 ? 1 : (n > num_clusters_ - 1 ? num_clusters_ - 1 : n));
+    }
+    const bool bimodal = n_cold_clusters > 0;
+    // pass 2: the two inclusive scans (one list when the launch is not bimodal)
+    const bool to_cold = bimodal && is_cold;
+    unsigned long long x = (static_cast<unsigned long long>(to_cold ? f_tiles : 0) << 32) |
+                           static_cast<unsigned>(to_cold ? 0 : tt * f_tiles);
     #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const int u = __shfl_up_sync(0xffffffffu, v, o);
-      if (lane >= o) v += u;
+      const unsigned long long u = __shfl_up_sync(0xffffffffu, x, o);
+      if (lane >= o) x += u;
     }
-    __shared__ int warp_tot[MAX_THREADS / 32];
-    if (lane == 31) warp_tot[warp] = v;
+    __syncthreads();                                // warp_tot is reused
+    if (lane == 31) warp_tot[warp] = x;
     __syncthreads();
-    int add = 0;
+    unsigned long long add = 0;
     for (int w = 0; w < warp; ++w) add += warp_tot[w];
-    v += add;                                   // inclusive prefix for thread's expert
-    if (threadIdx.x < E) tile_start[threadIdx.x + 1] = v;
-    if (threadIdx.x == 0) tile_start[0] = 0;
+    x += add;                                       // inclusive prefixes for this thread's expert
+    if (threadIdx.x < E) {
+      tile_start[threadIdx.x + 1] = static_cast<int>(x & 0xffffffffu);
+      tile_start_cold[threadIdx.x + 1] = static_cast<int>(x >> 32);
+    }
+    if (threadIdx.x == 0) { tile_start[0] = 0; tile_start_cold[0] = 0; launch_info[0] = n_cold_clusters; }
   }
 
   tc_fence_before();
@@ -248,7 +314,8 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   cluster_sync_all();                                 // the peer's barriers are initialised, its TMEM allocated
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
-  const int total_tiles = tile_start[E];
+  const int total_tiles = tile_start[E], total_cold = tile_start_cold[E];
+  const int n_cold_clusters = launch_info[0];
 
   // ---- tile feed.  Static (tile_counter == nullptr): cluster c takes tiles c, c + 74, ...  Dynamic: tiles
   // are handed out in linear order from a global ticket counter by one thread of the leader CTA (warp 3),
@@ -279,22 +346,38 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   if (warp == 0) {
     // ===================== TMA producer (one thread per CTA) =====================
     if (lane == 0) {
-      int s = 0;
-      uint32_t ph = 0;
+      int rs[2] = {0, 0};                              // next stage of the hot / cold ring
+      uint32_t rph[2] = {0, 0};
+      int cur = -1;                                    // class of the ring in use
       Feed feed = {0, 0, -1};
       for (int t = feed_next(feed, false); t >= 0; t = feed_next(feed, false)) {
-        const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
+        const TileCoord c = decode_tile(t, tile_start, tile_start_cold, t_tiles, p.offsets, E, sg_max);
+        const int cls = c.cold;
+        const int n_st = cls ? COLD_STAGES : STAGES;
+        const uint32_t st_bytes = cls ? COLD_STAGE_BYTES : STAGE_BYTES;
+        if (cur >= 0 && cur != cls) {
+          // The two rings share the same memory: before the first load of the new class, every stage of the old
+          // ring must have been consumed (wait, without taking it, for each slot's next "empty" phase).
+          const int n_old = cur ? COLD_STAGES : STAGES;
+          for (int j = 0; j < n_old; ++j) {
+            const int sj = rs[cur] + j;
+            mbar_wait(empty_bar(cur, sj < n_old ? sj : sj - n_old), (rph[cur] ^ (sj >= n_old ? 1u : 0u)) ^ 1u);
+          }
+        }
+        cur = cls;
+        int s = rs[cls];
+        uint32_t ph = rph[cls];
         const int n0 = c.f_tile * OUT_FEATS + static_cast<int>(rank) * CTA_FEATS;
-        const int half = c.nt >> 1;                    // this CTA's tokens (multiple of 8, <= 128)
+        const int half = c.nt >> 1;                    // this CTA's tokens (multiple of 8, <= 128; <= 16 in a cold tile)
         const int brow0 = c.row0 + static_cast<int>(rank) * half;
         const uint32_t tx_pair = 2u * (A_BYTES + static_cast<uint32_t>(half) * (BK * 2));
         const CUtensorMap* tm_b = &tm_act.m[(half >> 3) - 1];
         for (int kb = 0; kb < k_blocks; ++kb) {
-          mbar_wait(empty_bar(s), ph ^ 1u);            // this CTA's slot is free (multicast commit)
-          const uint32_t sa = base + s * STAGE_BYTES;
+          mbar_wait(empty_bar(cls, s), ph ^ 1u);       // this CTA's slot is free (multicast commit)
+          const uint32_t sa = base + s * st_bytes;
           const uint32_t sb = sa + A_BYTES;
-          const uint32_t fb = leader_bar(full_bar(s));
-          if (rank == 0) mbar_expect_tx(full_bar(s), tx_pair);   // the bytes of both CTAs
+          const uint32_t fb = leader_bar(full_bar(cls, s));
+          if (rank == 0) mbar_expect_tx(full_bar(cls, s), tx_pair);   // the bytes of both CTAs
           if (p.w4d) {
             // one operation per weight tensor: nblk 64-column blocks in [block][k][64 n] order
             tma_load_4d_pair(sa, &tm_w0, fb, 0, kb * BK, n0 >> 6, c.e);
@@ -308,8 +391,10 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
           }
           // this CTA's half of the tokens: one box of exactly `half` rows
           tma_load_2d_pair(sb, tm_b, fb, kb * BK, brow0);
-          if (++s == STAGES) { s = 0; ph ^= 1u; }
+          if (++s == n_st) { s = 0; ph ^= 1u; }
         }
+        rs[cls] = s;
+        rph[cls] = ph;
       }
     }
   } else if (warp == 3) {
@@ -317,10 +402,23 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     if (dyn && lane == 0 && rank == 0) {
       int slot = 0;
       uint32_t ph = 0;
+      // bimodal launch: clusters [0, n_cold_clusters) start on the cold list, the others on the hot list; a
+      // cluster whose list has run dry moves to the other list (once)
+      int list = (n_cold_clusters > 0 && cluster_id < n_cold_clusters) ? 1 : 0;
+      bool moved = n_cold_clusters == 0;
       while (true) {
         mbar_wait(sempty_bar(slot), ph ^ 1u);          // every consumer has read this slot's previous ticket
-        int t = atomicAdd(p.tile_counter, 1);
-        if (t >= total_tiles) t = -1;
+        int t = atomicAdd(p.tile_counter + list, 1);
+        if (t >= (list ? total_cold : total_tiles)) {
+          t = -1;
+          if (!moved) {
+            moved = true;
+            list ^= 1;
+            t = atomicAdd(p.tile_counter + list, 1);
+            if (t >= (list ? total_cold : total_tiles)) t = -1;
+          }
+        }
+        if (t >= 0 && list) t |= COLD_BIT;
         tile_slot[slot] = t;
         st_shared_cluster_u32(smem_u32(const_cast<int*>(tile_slot + slot)), 1, static_cast<uint32_t>(t));
         mbar_arrive(sfull_bar(slot));                  // release.cta: the local store above
@@ -329,21 +427,27 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         if (++slot == SCHED_SLOTS) { slot = 0; ph ^= 1u; }
       }
       // the last cluster to run dry re-arms the counters for the next launch
-      if (atomicAdd(p.tile_counter + 1, 1) == num_clusters - 1) {
+      if (atomicAdd(p.tile_counter + 2, 1) == num_clusters - 1) {
         p.tile_counter[0] = 0;
         p.tile_counter[1] = 0;
+        p.tile_counter[2] = 0;
         __threadfence();
       }
     }
   } else if (warp == 1) {
     // ===================== MMA issuer (one thread of the leader CTA) =====================
     if (lane == 0 && rank == 0) {
-      int s = 0;
-      uint32_t ph = 0;
+      int rs[2] = {0, 0};                              // next stage of the hot / cold ring
+      uint32_t rph[2] = {0, 0};
       int it = 0;
       Feed feed = {0, 0, -1};
       for (int t = feed_next(feed, false); t >= 0; t = feed_next(feed, false), ++it) {
-        const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
+        const TileCoord c = decode_tile(t, tile_start, tile_start_cold, t_tiles, p.offsets, E, sg_max);
+        const int cls = c.cold;
+        const int n_st = cls ? COLD_STAGES : STAGES;
+        const uint32_t st_bytes = cls ? COLD_STAGE_BYTES : STAGE_BYTES;
+        int s = rs[cls];
+        uint32_t ph = rph[cls];
         const uint32_t idesc = IDESC_BASE | (static_cast<uint32_t>(c.nt >> 3) << 17);
         const int as = it & 1;
         const uint32_t aph = (it >> 1) & 1u;
@@ -351,9 +455,9 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * BN_MAX;
         for (int kb = 0; kb < k_blocks; ++kb) {
-          mbar_wait(full_bar(s), ph);
+          mbar_wait(full_bar(cls, s), ph);
           tc_fence_after();
-          const uint32_t a_addr = base + s * STAGE_BYTES;
+          const uint32_t a_addr = base + s * st_bytes;
           const uint32_t b_addr = a_addr + A_BYTES;
           const uint64_t ad = ADESC_HI | ((a_addr >> 4) & 0x3FFFu);
           const uint64_t bd = BDESC_HI | ((b_addr >> 4) & 0x3FFFu);
@@ -363,9 +467,11 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
             umma_f16_pair(d_tmem, ad + ((kk * UK * 128) >> 4), bd + ((kk * UK * 2) >> 4), idesc,
                           (kb | kk) != 0 ? 1u : 0u);
           }
-          umma_commit_pair(empty_bar(s));             // both CTAs' slots free once these MMAs retire
-          if (++s == STAGES) { s = 0; ph ^= 1u; }
+          umma_commit_pair(empty_bar(cls, s));        // both CTAs' slots free once these MMAs retire
+          if (++s == n_st) { s = 0; ph ^= 1u; }
         }
+        rs[cls] = s;
+        rph[cls] = ph;
         umma_commit_pair(tfull_bar(as));              // accumulator complete -> both epilogues
       }
     }
@@ -385,14 +491,14 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     Feed feed = {0, 0, -1};
     int t = feed_next(feed, true);
     if (!GATEUP && t >= 0) {                         // gate weights of the first tile -> buffer 0
-      const TileCoord c0 = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
+      const TileCoord c0 = decode_tile(t, tile_start, tile_start_cold, t_tiles, p.offsets, E, sg_max);
       float sc = 1.0f;
       if (p.row_scale != nullptr && ew * 32 + lane < c0.rows_valid) sc = __ldg(p.row_scale + c0.row0 + ew * 32 + lane);
       sc_smem[ew * 32 + lane] = sc;
     }
     int it = 0;
     for (; t >= 0; ++it) {
-      const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
+      const TileCoord c = decode_tile(t, tile_start, tile_start_cold, t_tiles, p.offsets, E, sg_max);
       const int tn = feed_next(feed, true);            // this cluster's next tile (-1: none)
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1u;
@@ -407,7 +513,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         // latency never sits on the epilogue's critical path.  The barrier makes this tile's buffer
         // (written by all eight warps at the end of the previous tile) visible.
         if (tn >= 0 && p.row_scale != nullptr) {
-          const TileCoord cn = decode_tile(tn, tile_start, t_tiles, p.offsets, E, sg_max);
+          const TileCoord cn = decode_tile(tn, tile_start, tile_start_cold, t_tiles, p.offsets, E, sg_max);
           if (ew * 32 + lane < cn.rows_valid) sc_next = __ldg(p.row_scale + cn.row0 + ew * 32 + lane);
         }
         named_bar_sync(3, 32 * EPI_WARPS);
@@ -514,6 +620,7 @@ Params make_params(const GemmLaunch& g) {
   p.w4d = g.w4d;
   p.sg_max = g.sg_max;
   p.tile_counter = g.tile_counter;
+  p.num_sms = g.num_sms;
   return p;
 }
 

@@ -49,7 +49,7 @@ struct RouterLaunch {
   int32_t* counts;          // [E]
   int32_t* offsets;         // [E+1]
   int32_t* done_counter;    // one int, zero between launches (re-armed by the kernel)
-  int32_t* gemm_counters;   // four ints zeroed by the kernel's last tile (or nullptr)
+  int32_t* gemm_counters;   // eight ints zeroed by the kernel's last tile (or nullptr)
   int num_sms;
   int force_form;           // 0 = choose from T (router_sequential); 1 = sequential form; 2 = cluster form (tests)
 };
@@ -123,7 +123,7 @@ struct GemmLaunch {
   // Valid only when N % 64 == 0 (w4d); otherwise the kernels issue one 3-D box per block.
   CUtensorMap tm_b0_4d, tm_b1_4d;
   bool w4d;
-  int* tile_counter;   // pair kernel, dynamic tile feed: two ints (tickets, clusters finished), zero between launches; nullptr = static
+  int* tile_counter;   // pair kernel, dynamic tile feed: three ints (hot tickets, cold tickets, clusters finished), zero between launches; nullptr = static
   int sg_max;          // pair kernel: token tiles per super-group (0 = sized from K to ~48 MB of tokens)
   const int32_t* offsets;  // [E+1]
   int E, K, N;         // N = output columns (f for gate/up, d for down)

@@ -41,7 +41,7 @@ WsLayout ws_layout(const bg_moe_config& c, int64_t max_tokens, int num_sms) {
   L.seg_hidden = carve(16 * Tm + 4 * (Tm + 1));
   L.seg_out = L.seg_hidden + 8 * Tm;
   L.seg_start = L.seg_hidden + 16 * Tm;
-  L.tile_counters = carve(64);       // [0..3] GEMM ticket counters, [4] router tiles-done counter
+  L.tile_counters = carve(64);       // [0..7] GEMM ticket counters, [8] router tiles-done counter
   L.total = off;
   return L;
 }

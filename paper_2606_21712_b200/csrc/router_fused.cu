@@ -103,7 +103,7 @@ struct RouterParams {
   int32_t* counts;          // [E]
   int32_t* offsets;         // [E+1]
   int32_t* done_counter;    // zero on entry; the last tile re-arms it
-  int32_t* gemm_counters;   // 4 ints (ticket counters of the two grouped GEMMs) zeroed by the last tile; may be null
+  int32_t* gemm_counters;   // 8 ints (ticket counters of the two grouped GEMMs) zeroed by the last tile; may be null
   const void* const* seg_hidden;
   const int32_t* seg_start;
   int n_segs;
@@ -520,7 +520,8 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
       scan_tiles_block256(p.tile_counts, n_tiles, E, p.tile_base, p.counts, p.offsets, scan_scratch);
       if (threadIdx.x == 0) {
         *p.done_counter = 0;
-        if (p.gemm_counters != nullptr) { p.gemm_counters[0] = 0; p.gemm_counters[1] = 0; p.gemm_counters[2] = 0; p.gemm_counters[3] = 0; }
+        if (p.gemm_counters != nullptr)
+          for (int i = 0; i < 8; ++i) p.gemm_counters[i] = 0;
       }
     }
   }

@@ -176,6 +176,41 @@ def test_expert_ffn_scheduler_variants(env):
             check_out(y[offsets[e]:offsets[e + 1]], ref[offsets[e]:offsets[e + 1]], f"expert {e} {env}")
 
 
+def test_expert_ffn_bimodal_load():
+    """A launch that mixes experts of many rows with many experts of 1..32 rows runs the grouped GEMMs' two tile
+    lists side by side (hot list + cold list on the deeper cold ring): >= 148 tiles of each class
+    in both GEMMs here, cold experts of every row count 1..32, empty experts, and mid-size experts that stay hot."""
+    rng = np.random.default_rng(11)
+    rows = [0] * 256
+    for e in range(0, 200):
+        rows[e] = int(rng.integers(1, 33))           # cold class
+    rows[3] = 1; rows[4] = 32; rows[5] = 16; rows[6] = 17
+    for e in range(200, 212):
+        rows[e] = int(rng.integers(1500, 2600))      # hot, several token tiles each
+    for e in range(212, 230):
+        rows[e] = int(rng.integers(33, 257))         # one token tile, not cold
+    order = rng.permutation(256)
+    rows = [rows[i] for i in order]                  # classes interleaved by expert index
+    d, f = 512, 256
+    E, R = len(rows), sum(rows)
+    cfg = wl.MoEConfig("ffn-bimodal", 16, T=R, d=d, E=E, k=1, f=f)
+    lay, g, layer = make(cfg)
+    offsets = np.concatenate([[0], np.cumsum(rows)]).astype(np.int32)
+    outs = []
+    for _ in range(3):                               # the cluster -> list assignment is dynamic: repeat
+        outs.append(layer.expert_ffn(g["hidden"], torch.from_numpy(offsets).cuda(), T=R))
+    torch.cuda.synchronize()
+    assert torch.equal(outs[0], outs[1]) and torch.equal(outs[0], outs[2])
+    ref = oracle.expert_ffn(lay["hidden"], offsets, lay["W_gate"], lay["W_up"], lay["W_down"])
+    check_out(outs[0], ref, "expert_ffn bimodal")
+    for e in range(E):
+        if rows[e]:
+            check_out(outs[0][offsets[e]:offsets[e + 1]], ref[offsets[e]:offsets[e + 1]], f"expert {e} ({rows[e]} rows)")
+    layer.set_debug(static_tile_feed=True)           # the static feed never splits the lists: same bits
+    y_static = layer.expert_ffn(g["hidden"], torch.from_numpy(offsets).cuda(), T=R)
+    assert torch.equal(y_static, outs[0])
+
+
 def test_unpermute_parity():
     T, k, d, E = 257, 3, 136, 7
     rng = np.random.default_rng(4)
