@@ -177,14 +177,15 @@ def test_expert_ffn_scheduler_variants(env):
 
 
 def test_expert_ffn_bimodal_load():
-    """A launch that mixes experts of many rows with many experts of 1..32 rows runs the grouped GEMMs' two tile
-    lists side by side (hot list + cold list on the deeper cold ring): >= 148 tiles of each class
-    in both GEMMs here, cold experts of every row count 1..32, empty experts, and mid-size experts that stay hot."""
+    """A launch that mixes experts of many rows with many experts of <= 16 rows runs two tile streams in every CTA
+    pair at once (hot stream + cold stream with its own ring, accumulators and ticket counter).
+    Cold experts of every row count 1..16, experts of 17..32 rows (hot, one tile), empty experts, mid-size experts
+    and experts of several token tiles (capped at 240 rows in such a launch), classes interleaved by expert index."""
     rng = np.random.default_rng(11)
     rows = [0] * 256
     for e in range(0, 200):
         rows[e] = int(rng.integers(1, 33))           # cold class
-    rows[3] = 1; rows[4] = 32; rows[5] = 16; rows[6] = 17
+    rows[3] = 1; rows[4] = 32; rows[5] = 16; rows[6] = 17; rows[7] = 8; rows[8] = 9; rows[9] = 15
     for e in range(200, 212):
         rows[e] = int(rng.integers(1500, 2600))      # hot, several token tiles each
     for e in range(212, 230):
@@ -206,9 +207,12 @@ def test_expert_ffn_bimodal_load():
     for e in range(E):
         if rows[e]:
             check_out(outs[0][offsets[e]:offsets[e + 1]], ref[offsets[e]:offsets[e + 1]], f"expert {e} ({rows[e]} rows)")
-    layer.set_debug(static_tile_feed=True)           # the static feed never splits the lists: same bits
-    y_static = layer.expert_ffn(g["hidden"], torch.from_numpy(offsets).cuda(), T=R)
-    assert torch.equal(y_static, outs[0])
+    # the static feed and bimodal_mode = -1 never run a cold stream (256-row token tiles): same bits, since an
+    # output element's fp32 accumulation order depends on the k loop only
+    for dbg in (dict(static_tile_feed=True), dict(bimodal_mode=-1), dict(bimodal_mode=1)):
+        layer.set_debug(**dbg)
+        y2 = layer.expert_ffn(g["hidden"], torch.from_numpy(offsets).cuda(), T=R)
+        assert torch.equal(y2, outs[0]), dbg
 
 
 def test_unpermute_parity():
