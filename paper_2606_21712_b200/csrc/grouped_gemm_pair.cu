@@ -370,59 +370,68 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     return cold ? base + COLD_RING_OFF + s * COLD_STAGE_BYTES : base + s * STAGE_BYTES;
   };
 
+  // The TMA and MMA roles run WARP-WIDE with one elected lane issuing (elect.sync): inside `if (lane == 0)` ptxas
+  // cannot tell that a single lane is active and wraps every asm statement in an elect / branch loop; the issue
+  // loop of the MMA thread is instruction-bound (measured: ~0.25 us of issue work per 0.30 us k-block), so those
+  // extra instructions cost tensor time.
   if (warp == 0) {
-    // ===================== TMA producer (one thread per CTA): hot and cold stream, whichever has a free stage =====
-    if (lane == 0) {
-      struct Str { int t; TileCoord c; int kb, s; uint32_t ph; int n_st; Feed feed; };
-      Str st[2];
-      for (int c = 0; c < 2; ++c) {
-        st[c].feed = {0, 0, -1};
-        st[c].kb = 0; st[c].s = 0; st[c].ph = 0;
-        st[c].n_st = c ? COLD_STAGES : hot_stages;
-        st[c].t = feed_next(st[c].feed, c, false);
-        if (st[c].t >= 0) st[c].c = decode(st[c].t, c);
+    // ===================== TMA producer (one warp per CTA): hot and cold stream, whichever has a free stage =====
+    struct Str { int t, e, n0, brow0, kb, s, n_st; uint32_t ph, tx; const CUtensorMap* tm_b; Feed feed; };
+    Str st[2];
+    auto next_tile = [&](Str& q, int cls) {
+      q.t = feed_next(q.feed, cls, true);
+      if (q.t >= 0) {
+        const TileCoord c = decode(q.t, cls);
+        const int half = c.nt >> 1;                    // this CTA's tokens (multiple of 8, <= 128; 8 in a cold tile)
+        q.e = c.e;
+        q.n0 = c.f_tile * OUT_FEATS + static_cast<int>(rank) * CTA_FEATS;
+        q.brow0 = c.row0 + static_cast<int>(rank) * half;
+        q.tx = 2u * (A_BYTES + static_cast<uint32_t>(half) * (BK * 2));   // the bytes of both CTAs
+        q.tm_b = &tm_act.m[(half >> 3) - 1];
       }
-      while (st[0].t >= 0 || st[1].t >= 0) {
-        #pragma unroll
-        for (int cls = 0; cls < 2; ++cls) {
-          Str& q = st[cls];
-          if (q.t < 0) continue;
-          // a stream that is alone may block on its barrier; two live streams are polled in turn
-          if (st[cls ^ 1].t >= 0) {
-            if (!mbar_test(empty_bar(cls, q.s), q.ph ^ 1u)) continue;
-          } else {
-            mbar_wait(empty_bar(cls, q.s), q.ph ^ 1u);   // this CTA's slot is free (multicast commit)
-          }
-          const TileCoord& c = q.c;
-          const int n0 = c.f_tile * OUT_FEATS + static_cast<int>(rank) * CTA_FEATS;
-          const int half = c.nt >> 1;                    // this CTA's tokens (multiple of 8, <= 128; 8 in a cold tile)
-          const int brow0 = c.row0 + static_cast<int>(rank) * half;
-          const uint32_t tx_pair = 2u * (A_BYTES + static_cast<uint32_t>(half) * (BK * 2));
-          const CUtensorMap* tm_b = &tm_act.m[(half >> 3) - 1];
+    };
+    for (int c = 0; c < 2; ++c) {
+      st[c].feed = {0, 0, -1};
+      st[c].kb = 0; st[c].s = 0; st[c].ph = 0;
+      st[c].n_st = c ? COLD_STAGES : hot_stages;
+      next_tile(st[c], c);
+    }
+    while (st[0].t >= 0 || st[1].t >= 0) {
+      #pragma unroll
+      for (int cls = 0; cls < 2; ++cls) {
+        Str& q = st[cls];
+        if (q.t < 0) continue;
+        // a stream that is alone may block on its barrier; two live streams are polled in turn
+        if (st[cls ^ 1].t >= 0) {
+          if (!__shfl_sync(0xffffffffu, mbar_test(empty_bar(cls, q.s), q.ph ^ 1u) ? 1 : 0, 0)) continue;
+        } else {
+          mbar_wait(empty_bar(cls, q.s), q.ph ^ 1u);   // this CTA's slot is free (multicast commit)
+        }
+        if (elect_one()) {
           const int kb = q.kb;
           const uint32_t sa = stage_addr(cls, q.s);
           const uint32_t sb = sa + A_BYTES;
           const uint32_t fb = leader_bar(full_bar(cls, q.s));
-          if (rank == 0) mbar_expect_tx(full_bar(cls, q.s), tx_pair);   // the bytes of both CTAs
+          if (rank == 0) mbar_expect_tx(full_bar(cls, q.s), q.tx);
           if (p.w4d) {
             // one operation per weight tensor: nblk 64-column blocks in [block][k][64 n] order
-            tma_load_4d_pair(sa, &tm_w0, fb, 0, kb * BK, n0 >> 6, c.e);
-            if (GATEUP) tma_load_4d_pair(sa + A_BLK_BYTES, &tm_w1, fb, 0, kb * BK, n0 >> 6, c.e);
+            tma_load_4d_pair(sa, &tm_w0, fb, 0, kb * BK, q.n0 >> 6, q.e);
+            if (GATEUP) tma_load_4d_pair(sa + A_BLK_BYTES, &tm_w1, fb, 0, kb * BK, q.n0 >> 6, q.e);
           } else if (GATEUP) {
-            tma_load_3d_pair(sa, &tm_w0, fb, n0, kb * BK, c.e);
-            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w1, fb, n0, kb * BK, c.e);
+            tma_load_3d_pair(sa, &tm_w0, fb, q.n0, kb * BK, q.e);
+            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w1, fb, q.n0, kb * BK, q.e);
           } else {
-            tma_load_3d_pair(sa, &tm_w0, fb, n0, kb * BK, c.e);
-            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w0, fb, n0 + 64, kb * BK, c.e);
+            tma_load_3d_pair(sa, &tm_w0, fb, q.n0, kb * BK, q.e);
+            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w0, fb, q.n0 + 64, kb * BK, q.e);
           }
           // this CTA's half of the tokens: one box of exactly `half` rows
-          tma_load_2d_pair(sb, tm_b, fb, kb * BK, brow0);
-          if (++q.s == q.n_st) { q.s = 0; q.ph ^= 1u; }
-          if (++q.kb == k_blocks) {
-            q.kb = 0;
-            q.t = feed_next(q.feed, cls, false);
-            if (q.t >= 0) q.c = decode(q.t, cls);
-          }
+          tma_load_2d_pair(sb, q.tm_b, fb, kb * BK, q.brow0);
+        }
+        __syncwarp();
+        if (++q.s == q.n_st) { q.s = 0; q.ph ^= 1u; }
+        if (++q.kb == k_blocks) {
+          q.kb = 0;
+          next_tile(q, cls);
         }
       }
     }
@@ -433,16 +442,19 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     // ===================== tile scheduler of the hot list =====================
     if (dyn && lane == 0 && rank == 0) run_scheduler(0);
   } else if (warp == 1) {
-    // ===================== MMA issuer (one thread of the leader CTA): both streams ====================
-    if (lane == 0 && rank == 0) {
-      struct Str { int t; TileCoord c; int kb, s, it; uint32_t ph; int n_st; bool acc_ok; Feed feed; };
+    // ===================== MMA issuer (one warp of the leader CTA, one elected lane issues): both streams =====
+    if (rank == 0) {
+      struct Str { int t, kb, s, it, n_st; uint32_t ph, idesc; bool acc_ok; Feed feed; };
       Str st[2];
+      auto next_tile = [&](Str& q, int cls) {
+        q.t = feed_next(q.feed, cls, true);
+        if (q.t >= 0) q.idesc = IDESC_BASE | (static_cast<uint32_t>(decode(q.t, cls).nt >> 3) << 17);
+      };
       for (int c = 0; c < 2; ++c) {
         st[c].feed = {0, 0, -1};
         st[c].kb = 0; st[c].s = 0; st[c].ph = 0; st[c].it = 0; st[c].acc_ok = false;
         st[c].n_st = c ? COLD_STAGES : hot_stages;
-        st[c].t = feed_next(st[c].feed, c, false);
-        if (st[c].t >= 0) st[c].c = decode(st[c].t, c);
+        next_tile(st[c], c);
       }
       while (st[0].t >= 0 || st[1].t >= 0) {
         #pragma unroll
@@ -454,33 +466,37 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
           if (!q.acc_ok) {                             // both CTAs' epilogues have drained this accumulator
             const uint32_t aph = (q.it >> 1) & 1u;
             if (alone) mbar_wait(tempty_bar(cls, as), aph ^ 1u);
-            else if (!mbar_test(tempty_bar(cls, as), aph ^ 1u)) continue;
+            else if (!__shfl_sync(0xffffffffu, mbar_test(tempty_bar(cls, as), aph ^ 1u) ? 1 : 0, 0)) continue;
             q.acc_ok = true;
           }
           if (alone) mbar_wait(full_bar(cls, q.s), q.ph);
-          else if (!mbar_test(full_bar(cls, q.s), q.ph)) continue;
+          else if (!__shfl_sync(0xffffffffu, mbar_test(full_bar(cls, q.s), q.ph) ? 1 : 0, 0)) continue;
           tc_fence_after();
-          const uint32_t idesc = IDESC_BASE | (static_cast<uint32_t>(q.c.nt >> 3) << 17);
-          const uint32_t d_tmem = tmem_base + (cls ? cold_tmem_col(as) : as * BN_MAX);
-          const uint32_t a_addr = stage_addr(cls, q.s);
-          const uint32_t b_addr = a_addr + A_BYTES;
-          const uint64_t ad = ADESC_HI | ((a_addr >> 4) & 0x3FFFu);
-          const uint64_t bd = BDESC_HI | ((b_addr >> 4) & 0x3FFFu);
-          #pragma unroll
-          for (int kk = 0; kk < BK / UK; ++kk) {
-            // A (MN-major): +16 k = two 8-row groups = +2048 bytes; B (K-major): +16 k = +32 bytes in the span
-            umma_f16_pair(d_tmem, ad + ((kk * UK * 128) >> 4), bd + ((kk * UK * 2) >> 4), idesc,
-                          (q.kb | kk) != 0 ? 1u : 0u);
+          const bool last = q.kb + 1 == k_blocks;
+          if (elect_one()) {
+            const uint32_t d_tmem = tmem_base + (cls ? cold_tmem_col(as) : as * BN_MAX);
+            const uint32_t a_addr = stage_addr(cls, q.s);
+            const uint32_t b_addr = a_addr + A_BYTES;
+            const uint64_t ad = ADESC_HI | ((a_addr >> 4) & 0x3FFFu);
+            const uint64_t bd = BDESC_HI | ((b_addr >> 4) & 0x3FFFu);
+            #pragma unroll
+            for (int kk = 0; kk < BK / UK; ++kk) {
+              // A (MN-major): +16 k = two 8-row groups = +2048 bytes; B (K-major): +16 k = +32 bytes in the span
+              umma_f16_pair(d_tmem, ad + ((kk * UK * 128) >> 4), bd + ((kk * UK * 2) >> 4), q.idesc,
+                            (q.kb | kk) != 0 ? 1u : 0u);
+            }
+            umma_commit_pair(empty_bar(cls, q.s));    // both CTAs' slots free once these MMAs retire
+            if (last) umma_commit_pair(tfull_bar(cls, as));   // accumulator complete -> both epilogues
           }
-          umma_commit_pair(empty_bar(cls, q.s));      // both CTAs' slots free once these MMAs retire
+          __syncwarp();
           if (++q.s == q.n_st) { q.s = 0; q.ph ^= 1u; }
-          if (++q.kb == k_blocks) {
-            umma_commit_pair(tfull_bar(cls, as));     // accumulator complete -> both epilogues
+          if (last) {
             q.kb = 0;
             q.it += 1;
             q.acc_ok = false;
-            q.t = feed_next(q.feed, cls, false);
-            if (q.t >= 0) q.c = decode(q.t, cls);
+            next_tile(q, cls);
+          } else {
+            q.kb += 1;
           }
         }
       }

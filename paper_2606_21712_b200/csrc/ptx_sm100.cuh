@@ -35,6 +35,18 @@ __device__ __forceinline__ int seg_of(const int32_t* start, int n, int t) {
   return lo;
 }
 
+// True in exactly one lane of a converged warp.  Code issued under it (tcgen05.mma, TMA) is known to ptxas to run
+// in a single lane; under `if (lane == 0)` it is not, and every asm statement gets wrapped in an elect loop.
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "elect.sync _|p, 0xffffffff;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(pred));
+  return pred != 0;
+}
+
 // ------------------------------------------------------------------ mbarrier
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
