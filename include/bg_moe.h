@@ -77,12 +77,9 @@ int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, cons
  *   supergroup_token_tiles    > 0: token tiles per super-group (forces the super-group order on small
  *                             shapes); 0: sized from K so that a super-group's tokens fit ~48 MB of L2
  *   router_form               0: the router picks its form from T; 1: sequential form (one CTA per 128-token
- *                             tile) wherever it exists; 2: cluster form.  Both forms give the same bits.
- *   bimodal_mode              grouped GEMMs: 0 = a launch that mixes experts of many rows with many experts of
- *                             <= 16 rows runs the latter as a concurrent cold stream; -1 = never;
- *                             1 = whenever the launch has an expert of <= 16 rows */
+ *                             tile) wherever it exists; 2: cluster form.  Both forms give the same bits. */
 int bg_moe_set_debug(bg_moe_ctx* ctx, int32_t static_tile_feed, int32_t supergroup_token_tiles,
-                     int32_t router_form, int32_t bimodal_mode);
+                     int32_t router_form);
 
 /* Steps a1-a4: router logits, top-k + gates, histogram, exclusive scan.
  *   hidden     bf16 [T,d]

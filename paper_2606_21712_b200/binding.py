@@ -47,7 +47,7 @@ def load_library() -> ctypes.CDLL:
         lib.bg_moe_create.argtypes = [ctypes.POINTER(BgMoeConfig), ctypes.POINTER(vp)]
         lib.bg_moe_destroy.argtypes = [vp]
         lib.bg_moe_set_weights.argtypes = [vp] * 7
-        lib.bg_moe_set_debug.argtypes = [vp, i32, i32, i32, i32]
+        lib.bg_moe_set_debug.argtypes = [vp, i32, i32, i32]
         lib.bg_moe_route.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
         lib.bg_moe_permute.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp]
         lib.bg_moe_expert_ffn.argtypes = [vp, vp, vp, i32, vp, vp]
@@ -120,11 +120,10 @@ class MoELayer:
         return int(self.lib.bg_moe_workspace_bytes(self._ctx))
 
     # ------------------------------------------------------------------ C ABI mirrors
-    def set_debug(self, static_tile_feed: bool = False, supergroup_token_tiles: int = 0, router_form: int = 0,
-                  bimodal_mode: int = 0):
+    def set_debug(self, static_tile_feed: bool = False, supergroup_token_tiles: int = 0, router_form: int = 0):
         """bg_moe_set_debug: scheduler / router-form switches used by the tests only."""
         self._check(self.lib.bg_moe_set_debug(self._ctx, int(static_tile_feed), int(supergroup_token_tiles),
-                                              int(router_form), int(bimodal_mode)))
+                                              int(router_form)))
 
     def set_weights(self, W_r, b_r, W_gate, W_up, W_down, stream=None):
         assert W_r.dtype == torch.float32 and W_r.shape == (self.d, self.E) and W_r.is_contiguous() and W_r.is_cuda

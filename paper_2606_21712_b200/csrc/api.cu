@@ -62,7 +62,6 @@ struct bg_moe_ctx {
   bg::ActMaps am_x, am_h;
   int sg_max = 0;               // bg_moe_set_debug: overrides the pair kernel's super-group size (tests)
   int router_form = 0;          // bg_moe_set_debug: 0 = by T, 1 = sequential, 2 = cluster
-  int bimodal_mode = 0;         // bg_moe_set_debug: cold-stream override (see kernels.h GemmLaunch)
   int64_t launches = 0;
   std::string last_error;
   // optional per-kernel timing of the fused chain
@@ -248,7 +247,6 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g1.tm_b0 = ctx->tm_wg;
   g1.tm_b1 = ctx->tm_wu;
   g1.sg_max = ctx->sg_max;
-  g1.bimodal_mode = ctx->bimodal_mode;
   g1.tile_counter = ctx->dyn_sched ? ctx->tile_counters : nullptr;
   g1.w4d = c.f % 64 == 0;
   g1.tm_b0_4d = g1.w4d ? ctx->tm_wg4 : ctx->tm_wg;
@@ -265,7 +263,6 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g2.tm_b0 = ctx->tm_wd;
   g2.tm_b1 = ctx->tm_wd;
   g2.sg_max = ctx->sg_max;
-  g2.bimodal_mode = ctx->bimodal_mode;
   g2.tile_counter = ctx->dyn_sched ? ctx->tile_counters + 4 : nullptr;
   g2.w4d = c.d % 64 == 0;
   g2.tm_b0_4d = g2.w4d ? ctx->tm_wd4 : ctx->tm_wd;
@@ -424,12 +421,9 @@ int bg_moe_destroy(bg_moe_ctx* ctx) {
   return BG_OK;
 }
 
-int bg_moe_set_debug(bg_moe_ctx* ctx, int32_t static_tile_feed, int32_t supergroup_token_tiles, int32_t router_form,
-                     int32_t bimodal_mode) {
-  if (ctx == nullptr || supergroup_token_tiles < 0 || router_form < 0 || router_form > 2 || bimodal_mode < -1 ||
-      bimodal_mode > 1)
+int bg_moe_set_debug(bg_moe_ctx* ctx, int32_t static_tile_feed, int32_t supergroup_token_tiles, int32_t router_form) {
+  if (ctx == nullptr || supergroup_token_tiles < 0 || router_form < 0 || router_form > 2)
     return BG_ERR_INVALID_ARG;
-  ctx->bimodal_mode = bimodal_mode;
   ctx->dyn_sched = static_tile_feed == 0;
   ctx->sg_max = supergroup_token_tiles;
   ctx->router_form = router_form;

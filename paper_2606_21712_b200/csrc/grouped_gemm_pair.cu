@@ -26,9 +26,9 @@
 // The weights are consumed in the layout the layer is given (reading S14): no transpose/prepack.
 //
 // Warp roles (persistent, one CTA per SM, 74 clusters; every launch uses programmatic dependent launch):
-//   warp 0 lane 0: TMA producer (both CTAs; transaction bytes of both land on the leader's barrier)
-//   warp 1 lane 0: tcgen05.mma issuer (leader CTA only); commits are multicast to both CTAs
-//   warp 2       : TMEM allocator; lane 0 (leader only): tile scheduler of the cold stream
+//   warp 0       : TMA producer, one elected lane issues (both CTAs; transaction bytes of both land on the leader's barrier)
+//   warp 1       : tcgen05.mma issuer, one elected lane issues (leader CTA only); commits are multicast to both CTAs
+//   warp 2       : TMEM allocator
 //   warp 3 lane 0: tile scheduler (leader only): ticket counter -> 4-slot ring in both CTAs' shared memory
 //   warps 4-7    : epilogue (TMEM -> registers -> SwiGLU | gate weight -> bf16 -> smem transpose -> global);
 //                  a8 adds warps 8-11 (384 threads): its k loops are short, two warps serve each TMEM lane quarter
@@ -44,9 +44,6 @@
 // clusters running at the same time share weight strips through L2.  Tiles are drawn in that order from a
 // global ticket counter (dynamic feed, see `feed_next`), so the neighbours really run concurrently and a strip
 // is read from HBM once; bg_moe_set_debug(static_tile_feed) keeps the fixed map tile t -> cluster (t mod #clusters).
-// Bimodal launches -- experts of many rows next to many experts of <= 16 rows -- run TWO tile streams in every
-// CTA pair at the same time: the hot stream as above, and a cold stream (own ticket counter, own small ring, own
-// 16-column accumulators) whose tiles only stream weights from HBM; see "bimodal" in the kernel.
 // Experts with no rows own no tiles and their weights are never touched.
 #include "kernels.h"
 #include "ptx_sm100.cuh"
@@ -63,27 +60,13 @@ constexpr int A_BLK_BYTES = 64 * BK * 2;            // 8 KB: one 64-feature bloc
 constexpr int A_BYTES = 2 * A_BLK_BYTES;            // 16 KB: this CTA's 128 M rows
 constexpr int B_BYTES = (BN_MAX / 2) * BK * 2;      // 16 KB: this CTA's half of the tokens
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;      // 32 KB
-// Bimodal launches (see the kernel): the hot stream keeps BI_HOT_STAGES stages of the ring and caps its token
-// tiles at BI_HOT_CAP rows; the cold stream (experts of 1..COLD_ROWS rows) owns COLD_STAGES small stages behind
-// them and two COLD_ROWS-column accumulators in the TMEM columns the cap frees (columns 240..255 and 496..511).
-constexpr int BI_HOT_STAGES = 4;
-constexpr int BI_HOT_CAP = 240;
-constexpr int COLD_ROWS = 16;
-constexpr int COLD_STAGES = 4;
-constexpr int COLD_B_BYTES = (COLD_ROWS / 2) * BK * 2;        // 1 KB: this CTA's half of <= 16 tokens
-constexpr int COLD_STAGE_BYTES = A_BYTES + COLD_B_BYTES;      // 17 KB (a multiple of 1024: SW128 alignment holds)
-constexpr int COLD_RING_OFF = BI_HOT_STAGES * STAGE_BYTES;    // 128 KB
-constexpr int RING_BYTES = COLD_RING_OFF + COLD_STAGES * COLD_STAGE_BYTES;   // 196 KB (>= the 6 x 32 KB of other launches)
-static_assert(RING_BYTES >= STAGES * STAGE_BYTES, "ring memory");
-static_assert(BI_HOT_CAP + COLD_ROWS <= BN_MAX, "TMEM columns");
-// TMEM columns: hot accumulators at 0 and 256 as in every launch (<= 240 used), cold ones in the gaps behind them
-__host__ __device__ constexpr int cold_tmem_col(int as) { return as ? BN_MAX + BI_HOT_CAP : BI_HOT_CAP; }
+constexpr int RING_BYTES = STAGES * STAGE_BYTES;    // 192 KB
 constexpr int MAX_THREADS = 384;             // 4 role warps + 4 (a7) or 8 (a8) epilogue warps
 constexpr int MAX_E = 256;
 constexpr int XCH_PITCH = 36;                       // words per lane row of an exchange buffer (conflict-free v4)
 constexpr int XCH_BYTES = 32 * XCH_PITCH * 4;       // 4608 B
-constexpr int BAR_BYTES = 512;
-constexpr int TABLE_BYTES = 3136;                   // 3 x (MAX_E + 1) ints + the launch's flags, 16-byte padded
+constexpr int BAR_BYTES = 256;
+constexpr int TABLE_BYTES = 2064;                   // 2 x (MAX_E + 1) ints, 16-byte padded
 constexpr int STAGE_TILE_BYTES = 32 * 64;           // per-warp output staging: [32 tokens][32 features] bf16
 // epilogue scratch: [4 exchange buffers (a7) | 4 x 256 gate weights (a8)] then the 4 staging tiles
 constexpr int EPI_BYTES = 4 * XCH_BYTES + 4 * STAGE_TILE_BYTES;   // a8: 2 KB of scales + 8 staging tiles = 18 KB
@@ -105,8 +88,7 @@ struct Params {
   const float* row_scale;      // a8, fused path: gate weight per expert-order row (w_perm[r]); nullptr = 1
   bool w4d;                    // tm_w0 / tm_w1 are the 4-D block views (kernels.h)
   int sg_max;                  // 0 = derive the super-group size from K
-  int* tile_counter;           // dynamic feed: [3] = hot tickets, cold tickets, schedulers finished (zero between launches); nullptr = static feed
-  int bimodal_mode;            // 0 = decide from the load; -1 = never run a cold stream; 1 = whenever the launch has cold experts (tests)
+  int* tile_counter;           // dynamic feed: [2] = ticket counter, clusters-finished counter (zero between launches); nullptr = static feed
 };
 
 __device__ __forceinline__ void named_bar_sync(int id, int threads) {
@@ -117,19 +99,15 @@ struct TileCoord {
   int e, row0, rows_valid, nt, f_tile, t_tile;
 };
 
-// Tile tables (shared memory).  A launch has up to two tile lists:
-//   hot list : tile_start_hot[e] = first linear tile index of expert e (tile_start_hot[E] = total); t_tiles[e] =
-//              token tiles of expert e.  Inside an expert the order is feature-tile-major / token-tile-minor, so
-//              the token tiles that share a weight strip run at the same time.  When an expert's token matrix is
-//              too large to stay in L2 between two feature tiles (DeepSeek-shaped hot experts: thousands of rows x
-//              14 KB), that order re-streams the tokens from HBM once per feature tile; such experts are cut into
-//              super-groups of `sg_max` token tiles (sized to ~48 MB of tokens) and each super-group runs through
-//              all feature tiles before the next starts: the tokens stay in L2 and the expert's weights are
-//              streamed once per super-group instead.
-//   cold list: (bimodal launches only) the experts with 1..COLD_ROWS rows, one token tile each, feature tiles in
-//              order.  In every other launch all experts are in the hot list and the cold list is empty.
-// `cap` = rows a token tile may hold (256; BI_HOT_CAP for the hot list of a bimodal launch).
-__device__ __forceinline__ TileCoord decode_tile(int t, bool cold, const int* tile_start, const int* t_tiles,
+// tile_start[e] = first linear tile index of expert e (tile_start[E] = total);
+// t_tiles[e] = token tiles of expert e.  Both live in shared memory.
+// Inside an expert the order is feature-tile-major / token-tile-minor, so the token tiles that share a
+// weight strip run at the same time.  When an expert's token matrix is too large to stay in L2 between
+// two feature tiles (DeepSeek-shaped hot experts: thousands of rows x 14 KB), that order re-streams the
+// tokens from HBM once per feature tile; such experts are cut into super-groups of `sg_max` token tiles
+// (sized to ~48 MB of tokens) and each super-group runs through all feature tiles before the next starts:
+// the tokens stay in L2 and the expert's weights are streamed once per super-group instead.
+__device__ __forceinline__ TileCoord decode_tile(int t, const int* tile_start, const int* t_tiles,
                                                  const int32_t* offsets, int E, int sg_max) {
   int lo = 0, hi = E;              // largest e with tile_start[e] <= t
   while (hi - lo > 1) {
@@ -140,7 +118,7 @@ __device__ __forceinline__ TileCoord decode_tile(int t, bool cold, const int* ti
   // last expert whose start <= t, which is the one that owns t (its successors start later).
   const int e = lo;
   const int local = t - tile_start[e];
-  const int tt = cold ? 1 : t_tiles[e];
+  const int tt = t_tiles[e];
   int f_tile, t_tile;
   if (tt <= sg_max) {
     f_tile = local / tt;
@@ -158,7 +136,7 @@ __device__ __forceinline__ TileCoord decode_tile(int t, bool cold, const int* ti
   }
   const int beg = __ldg(offsets + e), end = __ldg(offsets + e + 1);
   const int n_e = end - beg;
-  const int base = (((n_e + tt - 1) / tt) + 15) & ~15;      // rows per token tile, multiple of 16, <= cap
+  const int base = (((n_e + tt - 1) / tt) + 15) & ~15;      // rows per token tile, multiple of 16, <= 256
   TileCoord c;
   c.e = e;
   c.row0 = beg + t_tile * base;
@@ -199,25 +177,21 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   const uint32_t base = (raw + 1023u) & ~1023u;       // SW128 tiles need 1024-byte alignment
   uint8_t* smem = smem_raw + (base - raw);
   const uint32_t bar_base = base + RING_BYTES;
-  // barriers, per stream (0 = hot, 1 = cold): ring full / empty, accumulator full / empty, ticket-slot full / empty
-  auto full_bar = [&](int cold, int s) { return bar_base + 8u * ((cold ? 2 * STAGES : 0) + s); };
-  auto empty_bar = [&](int cold, int s) { return bar_base + 8u * ((cold ? 2 * STAGES + COLD_STAGES : STAGES) + s); };
-  constexpr int RING_BARS = 2 * STAGES + 2 * COLD_STAGES;
-  auto tfull_bar = [&](int cold, int a) { return bar_base + 8u * (RING_BARS + 4 * cold + a); };
-  auto tempty_bar = [&](int cold, int a) { return bar_base + 8u * (RING_BARS + 4 * cold + 2 + a); };
-  // tile feeds (dynamic scheduler): sched_full[SCHED_SLOTS] per CTA, sched_empty[SCHED_SLOTS] on the leader
-  auto sfull_bar = [&](int cold, int i) { return bar_base + 8u * (RING_BARS + 8 + 2 * SCHED_SLOTS * cold + i); };
-  auto sempty_bar = [&](int cold, int i) { return bar_base + 8u * (RING_BARS + 8 + 2 * SCHED_SLOTS * cold + SCHED_SLOTS + i); };
-  constexpr int NBAR = RING_BARS + 8 + 4 * SCHED_SLOTS;
-  static_assert(8 * NBAR + 16 + 8 * SCHED_SLOTS + 16 <= BAR_BYTES, "barrier area");
+  // barriers: full[S] empty[S] tmem_full[2] tmem_empty[2]; then the TMEM address
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+  auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + a); };
+  auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + 2 + a); };
+  // tile feed (dynamic scheduler): sched_full[SCHED_SLOTS] per CTA, sched_empty[SCHED_SLOTS] on the leader
+  auto sfull_bar = [&](int i) { return bar_base + 8u * (2 * STAGES + 4 + i); };
+  auto sempty_bar = [&](int i) { return bar_base + 8u * (2 * STAGES + 4 + SCHED_SLOTS + i); };
+  constexpr int NBAR = 2 * STAGES + 4 + 2 * SCHED_SLOTS;
+  static_assert(8 * NBAR + 16 + 4 * SCHED_SLOTS <= BAR_BYTES, "barrier area");
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + RING_BYTES + 8 * NBAR);
-  volatile int* tile_slot = reinterpret_cast<volatile int*>(smem + RING_BYTES + 8 * NBAR + 16);   // [2][SCHED_SLOTS]
-  volatile int* epi_vote = tile_slot + 2 * SCHED_SLOTS;                                            // [2]
+  volatile int* tile_slot = reinterpret_cast<volatile int*>(smem + RING_BYTES + 8 * NBAR + 16);
   constexpr int N_CONSUMERS = 3 + 2 * EPI_WARPS;      // two producers, the MMA thread, every epilogue warp of the pair
-  int* tile_start = reinterpret_cast<int*>(smem + RING_BYTES + BAR_BYTES);     // hot list
-  int* tile_start_cold = tile_start + (MAX_E + 1);
-  int* t_tiles = tile_start_cold + (MAX_E + 1);
-  int* launch_info = t_tiles + (MAX_E + 1);            // [0] != 0: bimodal launch
+  int* tile_start = reinterpret_cast<int*>(smem + RING_BYTES + BAR_BYTES);
+  int* t_tiles = tile_start + (MAX_E + 1);
   uint8_t* epi_smem = smem + RING_BYTES + BAR_BYTES + TABLE_BYTES;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -226,19 +200,17 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   const int E = p.E;
   const int f_tiles = (p.N + OUT_FEATS - 1) / OUT_FEATS;
   const int k_blocks = (p.K + BK - 1) / BK;
-  const bool dyn = p.tile_counter != nullptr;
+  // token tiles whose rows fit ~48 MB of L2 (p.sg_max > 0: override, used by the tests to reach this path on small shapes)
+  const int sg_max = p.sg_max > 0 ? p.sg_max : max(1, (48 << 20) / (BN_MAX * 2 * p.K));
 
   // ---- independent of the previous kernel: barriers and TMEM
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tm_w0);
     if (GATEUP) tma_prefetch_desc(&tm_w1);
-    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(0, s), 1); mbar_init(empty_bar(0, s), 1); }
-    for (int s = 0; s < COLD_STAGES; ++s) { mbar_init(full_bar(1, s), 1); mbar_init(empty_bar(1, s), 1); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
     // tmem_empty (used on the leader only): one arrival per epilogue warp of both CTAs
-    for (int c = 0; c < 2; ++c) {
-      for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(c, a), 1); mbar_init(tempty_bar(c, a), 2 * EPI_WARPS); }
-      for (int i = 0; i < SCHED_SLOTS; ++i) { mbar_init(sfull_bar(c, i), 1); mbar_init(sempty_bar(c, i), N_CONSUMERS); }
-    }
+    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 2 * EPI_WARPS); }
+    for (int i = 0; i < SCHED_SLOTS; ++i) { mbar_init(sfull_bar(i), 1); mbar_init(sempty_bar(i), N_CONSUMERS); }
     fence_barrier_init();
   }
   if (warp == 2) {
@@ -247,59 +219,28 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   }
   // ---- everything below reads what the previous kernels wrote (offsets, activations)
   pdl_wait_then_trigger();
-  // ---- per-CTA tile tables: inclusive scans of per-expert tile counts (E <= 256 <= blockDim).
-  // Bimodal launches: when a launch has both experts of many rows (tensor-bound tiles whose weight
-  // strips are reused from L2) and many experts of a few rows (tiles that only stream weights from HBM), running
-  // them one after the other leaves HBM idle during the first and the tensor cores idle during the second -- and
-  // a CTA cannot pull more than ~50-70 GB/s from HBM (measured: the limit is outstanding requests per SM, not the
-  // ring depth), so giving the cold tiles to a few clusters does not work either: HBM is only saturated when EVERY
-  // SM streams.  So every CTA pair runs both kinds at once: the experts with 1..COLD_ROWS rows form a second (cold)
-  // tile list with its own ticket counter; its tiles flow through a small side ring (4 x 17 KB) and accumulate
-  // in 2 x 16 TMEM columns, issued by the same TMA and MMA threads whenever one of its stages is ready, while the
-  // hot stream keeps the tensor pipe busy; the epilogue warps drain cold accumulators between two hot tiles.
+  // ---- per-CTA tile table: inclusive scan of per-expert tile counts (E <= 256 = blockDim)
   {
-    int cnt = 0;
-    if (threadIdx.x < E) cnt = __ldg(p.offsets + threadIdx.x + 1) - __ldg(p.offsets + threadIdx.x);
-    const bool is_cold = cnt >= 1 && cnt <= COLD_ROWS;
-    // pass 1: class totals -> is the launch bimodal
-    int n_cold = is_cold ? 1 : 0, n_big = cnt > 2 * BN_MAX ? 1 : 0;
-    #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      n_cold += __shfl_xor_sync(0xffffffffu, n_cold, o);
-      n_big += __shfl_xor_sync(0xffffffffu, n_big, o);
+    int tt = 0;
+    if (threadIdx.x < E) {
+      const int cnt = __ldg(p.offsets + threadIdx.x + 1) - __ldg(p.offsets + threadIdx.x);
+      tt = (cnt + BN_MAX - 1) / BN_MAX;
+      t_tiles[threadIdx.x] = tt;
     }
-    __shared__ int warp_a[MAX_THREADS / 32], warp_b[MAX_THREADS / 32];
-    __shared__ unsigned long long warp_tot[MAX_THREADS / 32];
-    if (lane == 0) { warp_a[warp] = n_cold; warp_b[warp] = n_big; }
-    __syncthreads();
-    int cold_experts = 0, big_experts = 0;
-    for (int w = 0; w < static_cast<int>(blockDim.x >> 5); ++w) { cold_experts += warp_a[w]; big_experts += warp_b[w]; }
-    // bimodal: enough cold experts that their weight stream matters, and experts with several token tiles whose
-    // MMAs can hide it
-    bool bimodal = dyn && p.bimodal_mode >= 0 &&
-                   (p.bimodal_mode > 0 ? cold_experts > 0 : (cold_experts >= 8 && big_experts >= 2));
-    const int cap = bimodal ? BI_HOT_CAP : BN_MAX;
-    const bool to_cold = bimodal && is_cold;
-    const int tt = to_cold ? 0 : (cnt + cap - 1) / cap;
-    if (threadIdx.x < E) t_tiles[threadIdx.x] = tt;
-    // pass 2: the two inclusive scans (hot in the low word, cold in the high word)
-    unsigned long long x = (static_cast<unsigned long long>(to_cold ? f_tiles : 0) << 32) |
-                           static_cast<unsigned>(tt * f_tiles);
+    int v = tt * f_tiles;
     #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const unsigned long long u = __shfl_up_sync(0xffffffffu, x, o);
-      if (lane >= o) x += u;
+      const int u = __shfl_up_sync(0xffffffffu, v, o);
+      if (lane >= o) v += u;
     }
-    if (lane == 31) warp_tot[warp] = x;
+    __shared__ int warp_tot[MAX_THREADS / 32];
+    if (lane == 31) warp_tot[warp] = v;
     __syncthreads();
-    unsigned long long add = 0;
+    int add = 0;
     for (int w = 0; w < warp; ++w) add += warp_tot[w];
-    x += add;                                       // inclusive prefixes for this thread's expert
-    if (threadIdx.x < E) {
-      tile_start[threadIdx.x + 1] = static_cast<int>(x & 0xffffffffu);
-      tile_start_cold[threadIdx.x + 1] = static_cast<int>(x >> 32);
-    }
-    if (threadIdx.x == 0) { tile_start[0] = 0; tile_start_cold[0] = 0; launch_info[0] = bimodal ? 1 : 0; }
+    v += add;                                   // inclusive prefix for thread's expert
+    if (threadIdx.x < E) tile_start[threadIdx.x + 1] = v;
+    if (threadIdx.x == 0) tile_start[0] = 0;
   }
 
   tc_fence_before();
@@ -307,197 +248,131 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   cluster_sync_all();                                 // the peer's barriers are initialised, its TMEM allocated
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
-  const int total_tiles = tile_start[E], total_cold = tile_start_cold[E];
-  const bool bimodal = launch_info[0] != 0;
-  const int hot_stages = bimodal ? BI_HOT_STAGES : STAGES;
-  // token tiles whose rows fit ~48 MB of L2 (p.sg_max > 0: override, used by the tests to reach this path on small shapes)
-  const int sg_max = p.sg_max > 0 ? p.sg_max : max(1, (48 << 20) / (BN_MAX * 2 * p.K));
-  auto decode = [&](int t, int cold) {
-    return decode_tile(t, cold != 0, cold ? tile_start_cold : tile_start, t_tiles, p.offsets, E, sg_max);
-  };
+  const int total_tiles = tile_start[E];
 
-  // ---- tile feeds.  Static (tile_counter == nullptr): cluster c takes hot tiles c, c + 74, ... (no cold stream).
-  // Dynamic: tiles of a list are handed out in linear order from a global ticket counter by one thread of the
-  // leader CTA (warp 3: hot list, warp 2: cold list), written to a 4-slot ring in BOTH CTAs' shared memory and
-  // published through sched_full; every consumer (the two TMA producers, the MMA thread, each epilogue warp)
-  // reads the ticket and hands the slot back on the leader's sched_empty.  -1 ends the stream.  With tickets drawn
-  // in real time the token tiles that share a weight strip stay concurrent however unequal the tiles of a launch are.
+  // ---- tile feed.  Static (tile_counter == nullptr): cluster c takes tiles c, c + 74, ...  Dynamic: tiles
+  // are handed out in linear order from a global ticket counter by one thread of the leader CTA (warp 3),
+  // written to a 4-slot ring in BOTH CTAs' shared memory and published through sched_full; every consumer
+  // (the two TMA producers, the MMA thread, each epilogue warp) reads the ticket and hands the slot back on
+  // the leader's sched_empty.  -1 ends the stream.  With tickets drawn in real time the token tiles that
+  // share a weight strip stay concurrent however unequal the tiles of a launch are.
+  const bool dyn = p.tile_counter != nullptr;
   struct Feed { int slot; uint32_t ph; int t; };
-  auto feed_next = [&](Feed& f, int cold, bool warp_collective) -> int {
+  auto feed_next = [&](Feed& f, bool warp_collective) -> int {
     if (!dyn) {
-      if (cold) return -1;
       f.t = (f.t < 0) ? cluster_id : f.t + num_clusters;
       return f.t < total_tiles ? f.t : -1;
     }
-    mbar_wait_cluster(sfull_bar(cold, f.slot), f.ph);
-    const int t = tile_slot[cold * SCHED_SLOTS + f.slot];
+    mbar_wait_cluster(sfull_bar(f.slot), f.ph);
+    const int t = tile_slot[f.slot];
     // Hand the slot back with a RELAXED arrive whose address depends on the ticket just read (so it cannot
     // pass the read): a releasing arrive is a fence that waits for the thread's outstanding work -- the
     // epilogue's global stores, the MMA thread's in-flight tcgen05 operations -- once per tile.
     uint32_t zero;
     asm volatile("and.b32 %0, %1, 0;" : "=r"(zero) : "r"(t));
     if (warp_collective) __syncwarp();                 // all 32 lanes have read; one lane arrives
-    if (!warp_collective || lane == 0) mbar_arrive_cluster_relaxed(sempty_bar(cold, f.slot) + zero, 0);
+    if (!warp_collective || lane == 0) mbar_arrive_cluster_relaxed(sempty_bar(f.slot) + zero, 0);
     if (++f.slot == SCHED_SLOTS) { f.slot = 0; f.ph ^= 1u; }
     return t;
   };
-  auto run_scheduler = [&](int cold) {
-    const int total = cold ? total_cold : total_tiles;
-    int slot = 0;
-    uint32_t ph = 0;
-    while (true) {
-      mbar_wait(sempty_bar(cold, slot), ph ^ 1u);      // every consumer has read this slot's previous ticket
-      int t = atomicAdd(p.tile_counter + cold, 1);
-      if (t >= total) t = -1;
-      tile_slot[cold * SCHED_SLOTS + slot] = t;
-      st_shared_cluster_u32(smem_u32(const_cast<int*>(tile_slot + cold * SCHED_SLOTS + slot)), 1, static_cast<uint32_t>(t));
-      mbar_arrive(sfull_bar(cold, slot));              // release.cta: the local store above
-      mbar_arrive_cluster(sfull_bar(cold, slot), 1);   // release.cluster: the remote store above
-      if (t < 0) break;
-      if (++slot == SCHED_SLOTS) { slot = 0; ph ^= 1u; }
-    }
-    // the last scheduler (two per cluster) to run dry re-arms the counters for the next launch
-    if (atomicAdd(p.tile_counter + 2, 1) == 2 * num_clusters - 1) {
-      p.tile_counter[0] = 0;
-      p.tile_counter[1] = 0;
-      p.tile_counter[2] = 0;
-      __threadfence();
-    }
-  };
-
-  // ring geometry of a stream
-  auto stage_addr = [&](int cold, int s) {
-    return cold ? base + COLD_RING_OFF + s * COLD_STAGE_BYTES : base + s * STAGE_BYTES;
-  };
 
   // The TMA and MMA roles run WARP-WIDE with one elected lane issuing (elect.sync): inside `if (lane == 0)` ptxas
-  // cannot tell that a single lane is active and wraps every asm statement in an elect / branch loop; the issue
-  // loop of the MMA thread is instruction-bound (measured: ~0.25 us of issue work per 0.30 us k-block), so those
-  // extra instructions cost tensor time.
+  // cannot tell that a single lane is active and wraps every asm statement in an elect / branch loop, and the
+  // MMA issue loop is instruction-bound (ncu: ~0.25 us of issue work per 0.30 us k-block on C2), so those extra
+  // instructions cost tensor time.
   if (warp == 0) {
-    // ===================== TMA producer (one warp per CTA): hot and cold stream, whichever has a free stage =====
-    struct Str { int t, e, n0, brow0, kb, s, n_st; uint32_t ph, tx; const CUtensorMap* tm_b; Feed feed; };
-    Str st[2];
-    auto next_tile = [&](Str& q, int cls) {
-      q.t = feed_next(q.feed, cls, true);
-      if (q.t >= 0) {
-        const TileCoord c = decode(q.t, cls);
-        const int half = c.nt >> 1;                    // this CTA's tokens (multiple of 8, <= 128; 8 in a cold tile)
-        q.e = c.e;
-        q.n0 = c.f_tile * OUT_FEATS + static_cast<int>(rank) * CTA_FEATS;
-        q.brow0 = c.row0 + static_cast<int>(rank) * half;
-        q.tx = 2u * (A_BYTES + static_cast<uint32_t>(half) * (BK * 2));   // the bytes of both CTAs
-        q.tm_b = &tm_act.m[(half >> 3) - 1];
-      }
-    };
-    for (int c = 0; c < 2; ++c) {
-      st[c].feed = {0, 0, -1};
-      st[c].kb = 0; st[c].s = 0; st[c].ph = 0;
-      st[c].n_st = c ? COLD_STAGES : hot_stages;
-      next_tile(st[c], c);
-    }
-    while (st[0].t >= 0 || st[1].t >= 0) {
-      #pragma unroll
-      for (int cls = 0; cls < 2; ++cls) {
-        Str& q = st[cls];
-        if (q.t < 0) continue;
-        // a stream that is alone may block on its barrier; two live streams are polled in turn
-        if (st[cls ^ 1].t >= 0) {
-          if (!__shfl_sync(0xffffffffu, mbar_test(empty_bar(cls, q.s), q.ph ^ 1u) ? 1 : 0, 0)) continue;
-        } else {
-          mbar_wait(empty_bar(cls, q.s), q.ph ^ 1u);   // this CTA's slot is free (multicast commit)
-        }
+    // ===================== TMA producer (one warp per CTA, one elected lane issues) =====================
+    int s = 0;
+    uint32_t ph = 0;
+    Feed feed = {0, 0, -1};
+    for (int t = feed_next(feed, true); t >= 0; t = feed_next(feed, true)) {
+      const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
+      const int n0 = c.f_tile * OUT_FEATS + static_cast<int>(rank) * CTA_FEATS;
+      const int half = c.nt >> 1;                    // this CTA's tokens (multiple of 8, <= 128)
+      const int brow0 = c.row0 + static_cast<int>(rank) * half;
+      const uint32_t tx_pair = 2u * (A_BYTES + static_cast<uint32_t>(half) * (BK * 2));
+      const CUtensorMap* tm_b = &tm_act.m[(half >> 3) - 1];
+      for (int kb = 0; kb < k_blocks; ++kb) {
+        mbar_wait(empty_bar(s), ph ^ 1u);            // this CTA's slot is free (multicast commit)
         if (elect_one()) {
-          const int kb = q.kb;
-          const uint32_t sa = stage_addr(cls, q.s);
+          const uint32_t sa = base + s * STAGE_BYTES;
           const uint32_t sb = sa + A_BYTES;
-          const uint32_t fb = leader_bar(full_bar(cls, q.s));
-          if (rank == 0) mbar_expect_tx(full_bar(cls, q.s), q.tx);
+          const uint32_t fb = leader_bar(full_bar(s));
+          if (rank == 0) mbar_expect_tx(full_bar(s), tx_pair);   // the bytes of both CTAs
           if (p.w4d) {
             // one operation per weight tensor: nblk 64-column blocks in [block][k][64 n] order
-            tma_load_4d_pair(sa, &tm_w0, fb, 0, kb * BK, q.n0 >> 6, q.e);
-            if (GATEUP) tma_load_4d_pair(sa + A_BLK_BYTES, &tm_w1, fb, 0, kb * BK, q.n0 >> 6, q.e);
+            tma_load_4d_pair(sa, &tm_w0, fb, 0, kb * BK, n0 >> 6, c.e);
+            if (GATEUP) tma_load_4d_pair(sa + A_BLK_BYTES, &tm_w1, fb, 0, kb * BK, n0 >> 6, c.e);
           } else if (GATEUP) {
-            tma_load_3d_pair(sa, &tm_w0, fb, q.n0, kb * BK, q.e);
-            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w1, fb, q.n0, kb * BK, q.e);
+            tma_load_3d_pair(sa, &tm_w0, fb, n0, kb * BK, c.e);
+            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w1, fb, n0, kb * BK, c.e);
           } else {
-            tma_load_3d_pair(sa, &tm_w0, fb, q.n0, kb * BK, q.e);
-            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w0, fb, q.n0 + 64, kb * BK, q.e);
+            tma_load_3d_pair(sa, &tm_w0, fb, n0, kb * BK, c.e);
+            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w0, fb, n0 + 64, kb * BK, c.e);
           }
           // this CTA's half of the tokens: one box of exactly `half` rows
-          tma_load_2d_pair(sb, q.tm_b, fb, kb * BK, q.brow0);
+          tma_load_2d_pair(sb, tm_b, fb, kb * BK, brow0);
         }
         __syncwarp();
-        if (++q.s == q.n_st) { q.s = 0; q.ph ^= 1u; }
-        if (++q.kb == k_blocks) {
-          q.kb = 0;
-          next_tile(q, cls);
-        }
+        if (++s == STAGES) { s = 0; ph ^= 1u; }
       }
     }
-  } else if (warp == 2) {
-    // ===================== tile scheduler of the cold list (dynamic feed only; one thread of the leader CTA) ======
-    if (dyn && lane == 0 && rank == 0) run_scheduler(1);
   } else if (warp == 3) {
-    // ===================== tile scheduler of the hot list =====================
-    if (dyn && lane == 0 && rank == 0) run_scheduler(0);
-  } else if (warp == 1) {
-    // ===================== MMA issuer (one warp of the leader CTA, one elected lane issues): both streams =====
-    if (rank == 0) {
-      struct Str { int t, kb, s, it, n_st; uint32_t ph, idesc; bool acc_ok; Feed feed; };
-      Str st[2];
-      auto next_tile = [&](Str& q, int cls) {
-        q.t = feed_next(q.feed, cls, true);
-        if (q.t >= 0) q.idesc = IDESC_BASE | (static_cast<uint32_t>(decode(q.t, cls).nt >> 3) << 17);
-      };
-      for (int c = 0; c < 2; ++c) {
-        st[c].feed = {0, 0, -1};
-        st[c].kb = 0; st[c].s = 0; st[c].ph = 0; st[c].it = 0; st[c].acc_ok = false;
-        st[c].n_st = c ? COLD_STAGES : hot_stages;
-        next_tile(st[c], c);
+    // ===================== tile scheduler (dynamic feed only; one thread of the leader CTA) ==========
+    if (dyn && lane == 0 && rank == 0) {
+      int slot = 0;
+      uint32_t ph = 0;
+      while (true) {
+        mbar_wait(sempty_bar(slot), ph ^ 1u);          // every consumer has read this slot's previous ticket
+        int t = atomicAdd(p.tile_counter, 1);
+        if (t >= total_tiles) t = -1;
+        tile_slot[slot] = t;
+        st_shared_cluster_u32(smem_u32(const_cast<int*>(tile_slot + slot)), 1, static_cast<uint32_t>(t));
+        mbar_arrive(sfull_bar(slot));                  // release.cta: the local store above
+        mbar_arrive_cluster(sfull_bar(slot), 1);       // release.cluster: the remote store above
+        if (t < 0) break;
+        if (++slot == SCHED_SLOTS) { slot = 0; ph ^= 1u; }
       }
-      while (st[0].t >= 0 || st[1].t >= 0) {
-        #pragma unroll
-        for (int cls = 0; cls < 2; ++cls) {
-          Str& q = st[cls];
-          if (q.t < 0) continue;
-          const bool alone = st[cls ^ 1].t < 0;
-          const int as = q.it & 1;
-          if (!q.acc_ok) {                             // both CTAs' epilogues have drained this accumulator
-            const uint32_t aph = (q.it >> 1) & 1u;
-            if (alone) mbar_wait(tempty_bar(cls, as), aph ^ 1u);
-            else if (!__shfl_sync(0xffffffffu, mbar_test(tempty_bar(cls, as), aph ^ 1u) ? 1 : 0, 0)) continue;
-            q.acc_ok = true;
-          }
-          if (alone) mbar_wait(full_bar(cls, q.s), q.ph);
-          else if (!__shfl_sync(0xffffffffu, mbar_test(full_bar(cls, q.s), q.ph) ? 1 : 0, 0)) continue;
+      // the last cluster to run dry re-arms the counters for the next launch
+      if (atomicAdd(p.tile_counter + 1, 1) == num_clusters - 1) {
+        p.tile_counter[0] = 0;
+        p.tile_counter[1] = 0;
+        __threadfence();
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (one warp of the leader CTA, one elected lane issues) =====================
+    if (rank == 0) {
+      int s = 0;
+      uint32_t ph = 0;
+      int it = 0;
+      Feed feed = {0, 0, -1};
+      for (int t = feed_next(feed, true); t >= 0; t = feed_next(feed, true), ++it) {
+        const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
+        const uint32_t idesc = IDESC_BASE | (static_cast<uint32_t>(c.nt >> 3) << 17);
+        const int as = it & 1;
+        const uint32_t aph = (it >> 1) & 1u;
+        mbar_wait(tempty_bar(as), aph ^ 1u);          // both CTAs' epilogues have drained this accumulator
+        const uint32_t d_tmem = tmem_base + as * BN_MAX;
+        for (int kb = 0; kb < k_blocks; ++kb) {
+          mbar_wait(full_bar(s), ph);
           tc_fence_after();
-          const bool last = q.kb + 1 == k_blocks;
           if (elect_one()) {
-            const uint32_t d_tmem = tmem_base + (cls ? cold_tmem_col(as) : as * BN_MAX);
-            const uint32_t a_addr = stage_addr(cls, q.s);
+            const uint32_t a_addr = base + s * STAGE_BYTES;
             const uint32_t b_addr = a_addr + A_BYTES;
             const uint64_t ad = ADESC_HI | ((a_addr >> 4) & 0x3FFFu);
             const uint64_t bd = BDESC_HI | ((b_addr >> 4) & 0x3FFFu);
             #pragma unroll
             for (int kk = 0; kk < BK / UK; ++kk) {
               // A (MN-major): +16 k = two 8-row groups = +2048 bytes; B (K-major): +16 k = +32 bytes in the span
-              umma_f16_pair(d_tmem, ad + ((kk * UK * 128) >> 4), bd + ((kk * UK * 2) >> 4), q.idesc,
-                            (q.kb | kk) != 0 ? 1u : 0u);
+              umma_f16_pair(d_tmem, ad + ((kk * UK * 128) >> 4), bd + ((kk * UK * 2) >> 4), idesc,
+                            (kb | kk) != 0 ? 1u : 0u);
             }
-            umma_commit_pair(empty_bar(cls, q.s));    // both CTAs' slots free once these MMAs retire
-            if (last) umma_commit_pair(tfull_bar(cls, as));   // accumulator complete -> both epilogues
+            umma_commit_pair(empty_bar(s));           // both CTAs' slots free once these MMAs retire
+            if (kb + 1 == k_blocks) umma_commit_pair(tfull_bar(as));   // accumulator complete -> both epilogues
           }
           __syncwarp();
-          if (++q.s == q.n_st) { q.s = 0; q.ph ^= 1u; }
-          if (last) {
-            q.kb = 0;
-            q.it += 1;
-            q.acc_ok = false;
-            next_tile(q, cls);
-          } else {
-            q.kb += 1;
-          }
+          if (++s == STAGES) { s = 0; ph ^= 1u; }
         }
       }
     }
@@ -514,26 +389,39 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     const uint32_t stage_rd = smem_u32(stage) + (lane >> 2) * 64 + (lane & 3) * 16;   // + i * 512
     float* sc_smem = reinterpret_cast<float*>(epi_smem);                        // a8: [2][BN_MAX] gate weights, double-buffered
     const int feat0 = static_cast<int>(rank) * CTA_FEATS + (GATEUP ? (q & 1) : q) * 32;   // in the pair tile
-    const uint32_t lane_base = tmem_base + (static_cast<uint32_t>(q * 32) << 16);
-
-    // One tile: accumulator columns [tcol, tcol + c.nt) -> out rows [c.row0, c.row0 + c.rows_valid).
-    // COLD: one 16-column chunk.  sc (a8): this tile's gate weights by token column (shared memory), or nullptr.
-    auto process_tile = [&](const TileCoord& c, uint32_t tcol, bool cold, const float* sc) {
+    Feed feed = {0, 0, -1};
+    int t = feed_next(feed, true);
+    if (!GATEUP && t >= 0) {                         // gate weights of the first tile -> buffer 0
+      const TileCoord c0 = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
+      float sc = 1.0f;
+      if (p.row_scale != nullptr && ew * 32 + lane < c0.rows_valid) sc = __ldg(p.row_scale + c0.row0 + ew * 32 + lane);
+      sc_smem[ew * 32 + lane] = sc;
+    }
+    int it = 0;
+    for (; t >= 0; ++it) {
+      const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
+      const int tn = feed_next(feed, true);            // this cluster's next tile (-1: none)
+      const int as = it & 1;
+      const uint32_t aph = (it >> 1) & 1u;
       const int n_chunks = (c.nt + 31) >> 5;           // 32-token chunks (the last may be half used)
       const int col = c.f_tile * OUT_FEATS + feat0 + (lane & 3) * 8;            // this lane's 8 output columns
       const bool col_ok = col < p.N;                   // N is a multiple of 8
       __nv_bfloat16* out_tile = p.out + static_cast<int64_t>(c.row0) * p.N + col;
-      const uint32_t taddr = lane_base + tcol;
-      // a 32-column load would run past a cold accumulator (and past the allocation): 16 columns there
-      auto load_chunk = [&](int cc, uint32_t* v) {
-        if (cold) {
-          tmem_ld_32x16(taddr, v);
-          #pragma unroll
-          for (int j = 16; j < 32; ++j) v[j] = 0u;
-        } else {
-          tmem_ld_32x32(taddr + cc * 32, v);
+      float sc_next = 1.0f;
+      if (!GATEUP) {
+        // Gate weights (already in expert order: w_perm[r]) of the NEXT tile: warp ew fetches tokens
+        // ew*32 .. +31 now and parks them in the other buffer after this tile's chunks, so the load
+        // latency never sits on the epilogue's critical path.  The barrier makes this tile's buffer
+        // (written by all eight warps at the end of the previous tile) visible.
+        if (tn >= 0 && p.row_scale != nullptr) {
+          const TileCoord cn = decode_tile(tn, tile_start, t_tiles, p.offsets, E, sg_max);
+          if (ew * 32 + lane < cn.rows_valid) sc_next = __ldg(p.row_scale + cn.row0 + ew * 32 + lane);
         }
-      };
+        named_bar_sync(3, 32 * EPI_WARPS);
+      }
+      mbar_wait(tfull_bar(as), aph);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + as * BN_MAX;
       // token-major write-out of the staged 32 x 32 block of chunk cc
       auto flush_chunk = [&](int cc) {
         __syncwarp();
@@ -560,8 +448,8 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         #pragma unroll 1
         for (int c0 = 0; c0 < n_chunks; c0 += 2) {
           uint32_t v0[32], v1[32];
-          load_chunk(c0, v0);
-          if (c0 + 1 < n_chunks) load_chunk(c0 + 1, v1);
+          tmem_ld_32x32(taddr + c0 * 32, v0);
+          if (c0 + 1 < n_chunks) tmem_ld_32x32(taddr + (c0 + 1) * 32, v1);
           tmem_ld_wait();
           // hand over the chunk the partner finishes: up warp gives chunk c0, gate warp gives chunk c0+1
           #pragma unroll
@@ -591,12 +479,11 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         #pragma unroll 1
         for (int cc = sub; cc < n_chunks; cc += 2) {
           uint32_t v[32];
-          load_chunk(cc, v);
+          tmem_ld_32x32(taddr + cc * 32, v);
           tmem_ld_wait();
           #pragma unroll
           for (int j = 0; j < 32; j += 4) {
-            float4 s4 = make_float4(1.0f, 1.0f, 1.0f, 1.0f);
-            if (sc != nullptr) s4 = *reinterpret_cast<const float4*>(sc + cc * 32 + j);   // broadcast
+            const float4 s4 = *reinterpret_cast<const float4*>(sc_smem + (it & 1) * BN_MAX + cc * 32 + j);   // broadcast
             st_shared_bf16(stage_wr + (j + 0) * 64, __uint_as_float(v[j + 0]) * s4.x);
             st_shared_bf16(stage_wr + (j + 1) * 64, __uint_as_float(v[j + 1]) * s4.y);
             st_shared_bf16(stage_wr + (j + 2) * 64, __uint_as_float(v[j + 2]) * s4.z);
@@ -605,88 +492,12 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
           flush_chunk(cc);
         }
       }
-    };
-    // accumulator drained: one arrival per warp on the LEADER's tmem_empty barrier
-    auto release_acc = [&](int cold, int as) {
+      if (!GATEUP) sc_smem[((it + 1) & 1) * BN_MAX + ew * 32 + lane] = sc_next;
+      // accumulator drained: one arrival per warp on the LEADER's tmem_empty barrier
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive_cluster_relaxed(tempty_bar(cold, as), 0);   // relaxed: must not wait for the stores
-    };
-
-    // ---- cold stream state.  Cold accumulators are drained between two hot tiles, when the first epilogue warp
-    // finds one complete (its verdict goes to the other warps through shared memory: the warps of a CTA must take
-    // the same decision, they exchange data through named barriers), and after the hot stream has ended.
-    Feed cfeed = {0, 0, -1};
-    int tc = feed_next(cfeed, 1, true);
-    int cit = 0;
-    // a8: gate weights of cold accumulator `as` live behind the hot tile's (<= 240 when a cold stream exists) in buffer `as`
-    auto csc = [&](int as) { return sc_smem + as * BN_MAX + BI_HOT_CAP; };
-    auto do_cold_tile = [&]() {
-      const TileCoord c = decode(tc, 1);
-      const int as = cit & 1;
-      if (!GATEUP) {
-        if (p.row_scale != nullptr && ew == 0 && lane < COLD_ROWS)
-          csc(as)[lane] = lane < c.rows_valid ? __ldg(p.row_scale + c.row0 + lane) : 1.0f;
-        named_bar_sync(3, 32 * EPI_WARPS);
-      }
-      tc_fence_after();
-      process_tile(c, cold_tmem_col(as), true, (!GATEUP && p.row_scale != nullptr) ? csc(as) : nullptr);
-      release_acc(1, as);
-      tc = feed_next(cfeed, 1, true);
-      ++cit;
-    };
-    int vote_round = 0;
-    auto drain_ready_cold = [&]() {
-      while (tc >= 0) {
-        if (ew == 0 && lane == 0) epi_vote[vote_round & 1] = mbar_test(tfull_bar(1, cit & 1), (cit >> 1) & 1u) ? 1 : 0;
-        named_bar_sync(4, 32 * EPI_WARPS);
-        const int ready = epi_vote[vote_round & 1];
-        ++vote_round;
-        if (!ready) break;
-        do_cold_tile();
-      }
-    };
-
-    // ---- hot stream
-    Feed feed = {0, 0, -1};
-    int t = feed_next(feed, 0, true);
-    if (!GATEUP && t >= 0) {                         // gate weights of the first tile -> buffer 0
-      const TileCoord c0 = decode(t, 0);
-      float sc = 1.0f;
-      if (p.row_scale != nullptr && ew * 32 + lane < c0.rows_valid) sc = __ldg(p.row_scale + c0.row0 + ew * 32 + lane);
-      sc_smem[ew * 32 + lane] = sc;
-    }
-    int it = 0;
-    for (; t >= 0; ++it) {
-      if (bimodal) drain_ready_cold();
-      const TileCoord c = decode(t, 0);
-      const int tn = feed_next(feed, 0, true);         // this cluster's next tile (-1: none)
-      const int as = it & 1;
-      const uint32_t aph = (it >> 1) & 1u;
-      float sc_next = 1.0f;
-      if (!GATEUP) {
-        // Gate weights (already in expert order: w_perm[r]) of the NEXT tile: warp ew fetches tokens
-        // ew*32 .. +31 now and parks them in the other buffer after this tile's chunks, so the load
-        // latency never sits on the epilogue's critical path.  The barrier makes this tile's buffer
-        // (written by all eight warps at the end of the previous tile) visible.
-        if (tn >= 0 && p.row_scale != nullptr) {
-          const TileCoord cn = decode(tn, 0);
-          if (ew * 32 + lane < cn.rows_valid) sc_next = __ldg(p.row_scale + cn.row0 + ew * 32 + lane);
-        }
-        named_bar_sync(3, 32 * EPI_WARPS);
-      }
-      mbar_wait(tfull_bar(0, as), aph);
-      tc_fence_after();
-      process_tile(c, as * BN_MAX, false, (!GATEUP && p.row_scale != nullptr) ? sc_smem + (it & 1) * BN_MAX : nullptr);
-      // (a hot tile of a bimodal launch has <= 240 rows: ew * 32 + lane >= 240 must not touch the cold tiles' scales)
-      if (!GATEUP && (!bimodal || ew * 32 + lane < BI_HOT_CAP)) sc_smem[((it + 1) & 1) * BN_MAX + ew * 32 + lane] = sc_next;
-      release_acc(0, as);
+      if (lane == 0) mbar_arrive_cluster_relaxed(tempty_bar(as), 0);   // relaxed: must not wait for the stores
       t = tn;
-    }
-    // ---- the hot stream has ended: the remaining cold tiles
-    while (tc >= 0) {
-      mbar_wait(tfull_bar(1, cit & 1), (cit >> 1) & 1u);
-      do_cold_tile();
     }
   }
 
@@ -710,7 +521,6 @@ Params make_params(const GemmLaunch& g) {
   p.w4d = g.w4d;
   p.sg_max = g.sg_max;
   p.tile_counter = g.tile_counter;
-  p.bimodal_mode = g.bimodal_mode;
   return p;
 }
 

@@ -123,9 +123,8 @@ struct GemmLaunch {
   // Valid only when N % 64 == 0 (w4d); otherwise the kernels issue one 3-D box per block.
   CUtensorMap tm_b0_4d, tm_b1_4d;
   bool w4d;
-  int* tile_counter;   // pair kernel, dynamic tile feed: three ints (hot tickets, cold tickets, schedulers finished), zero between launches; nullptr = static
+  int* tile_counter;   // pair kernel, dynamic tile feed: two ints (tickets, clusters finished), zero between launches; nullptr = static
   int sg_max;          // pair kernel: token tiles per super-group (0 = sized from K to ~48 MB of tokens)
-  int bimodal_mode;    // pair kernel: 0 = run a cold stream when the load calls for it, -1 = never, 1 = whenever cold experts exist (tests)
   const int32_t* offsets;  // [E+1]
   int E, K, N;         // N = output columns (f for gate/up, d for down)
   void* out;           // bf16 [rows, N]

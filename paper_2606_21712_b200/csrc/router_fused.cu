@@ -237,12 +237,14 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
   pdl_wait_then_trigger();
   trace(1);
 
-  if (warp == 0) {
-    if (lane == 0) {                              // ---- TMA producer
-      int s = 0;
-      uint32_t ph = 0;
-      for (int it = 0; it < n_iter; ++it) {
-        mbar_wait(empty_bar(s), ph ^ 1u);
+  // TMA and MMA roles run warp-wide with one elected lane issuing (elect.sync): under `if (lane == 0)` ptxas wraps
+  // every asm statement in an elect / branch loop.
+  if (warp == 0) {                                // ---- TMA producer
+    int s = 0;
+    uint32_t ph = 0;
+    for (int it = 0; it < n_iter; ++it) {
+      mbar_wait(empty_bar(s), ph ^ 1u);
+      if (elect_one()) {
         const int kb = kb0 + it / ipk, pc0 = (it % ipk) * pps;
         const uint32_t sa = base + s * stage_bytes, sb = sa + A_BYTES;
         mbar_expect_tx(full_bar(s), ROWS ? stage_bytes - A_BYTES : stage_bytes);
@@ -254,16 +256,17 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
             for (int j = 0; j < n_blk; ++j)
               tma_load_3d(sb + pc * piece_bytes + j * B_BLK_BYTES, &tm_w, full_bar(s), 64 * j, kb * BK, pc0 + pc);
         }
-        if (++s == n_stages) { s = 0; ph ^= 1u; }
       }
+      __syncwarp();
+      if (++s == n_stages) { s = 0; ph ^= 1u; }
     }
-  } else if (warp == 1) {
-    if (lane == 0) {                              // ---- MMA issuer
-      int s = 0;
-      uint32_t ph = 0;
-      for (int it = 0; it < n_iter; ++it) {
-        mbar_wait(full_bar(s), ph);
-        tc_fence_after();
+  } else if (warp == 1) {                         // ---- MMA issuer
+    int s = 0;
+    uint32_t ph = 0;
+    for (int it = 0; it < n_iter; ++it) {
+      mbar_wait(full_bar(s), ph);
+      tc_fence_after();
+      if (elect_one()) {
         const uint32_t sa = base + s * stage_bytes, sb = sa + A_BYTES;
         const uint64_t ad = ADESC_HI | ((sa >> 4) & 0x3FFFu);
         // sequential form: chunk c = kb / kb_per owns its own accumulator, restarted at the chunk's first k-block
@@ -279,10 +282,12 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
                      (first && pc == 0 && kk == 0) ? 0u : 1u);
         }
         umma_commit(empty_bar(s));
-        if (++s == n_stages) { s = 0; ph ^= 1u; }
+        if (it + 1 == n_iter) umma_commit(done_bar);
       }
-      umma_commit(done_bar);
+      __syncwarp();
+      if (++s == n_stages) { s = 0; ph ^= 1u; }
     }
+    if (n_iter == 0 && elect_one()) umma_commit(done_bar);
   } else if (warp >= 4) {
     if (ROWS) {                                   // ---- row loader (thread <-> one row of the 128-token tile)
       const int LAG = min(4, n_stages - 1);       // stages in flight per thread (n_stages >= 3 always)
