@@ -455,6 +455,52 @@ def run_c5_combine(steps: int, device_index: int):
     return res
 
 
+# ----------------------------------------------------------------------------- expert-weight ring buffer
+def run_ring(steps: int, device_index: int):
+    """expert weights in pinned host memory, streamed through a device
+    ring of 16 expert slots while the grouped GEMMs run (bg_moe_set_weights_offloaded).  C3 at T = 32768 (the
+    compute-bound end of the sweep, 1.2 GB of expert weights per step over PCIe).  Reported: the step time with
+    resident weights, the time of the bare host->device copy of the same bytes, the streamed step, and how close
+    the streamed step comes to max(copy, compute) -- 1.0 = the transfer is fully hidden behind the GEMMs or the
+    GEMMs fully behind the transfer."""
+    from paper_2606_21712_b200 import MoELayer
+    cfg = wl.CONFIGS["C3"].with_T(32768)
+    lay = wl.make_layer(cfg, "cuda")
+    layer = MoELayer(cfg.d, cfg.f, cfg.E, cfg.k, cfg.T, device=device_index)
+    layer.set_weights(lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"])
+    hidden, stream = lay["hidden"], torch.cuda.current_stream()
+    out = torch.empty_like(hidden)
+    step = lambda: layer.combined_forward(hidden, out, stream)
+
+    def med(fn):
+        torch.cuda.synchronize()
+        time.sleep(0.5)
+        for _ in range(2):
+            fn()
+        _, per = time_steps(fn, steps, stream)
+        return float(np.median(per))
+
+    ms_res = med(step)
+    ref = out.clone()
+    pinned = [lay[n].cpu().pin_memory() for n in ("W_gate", "W_up", "W_down")]
+    dev_tmp = torch.empty_like(lay["W_gate"])
+
+    def bare_copy():
+        for w in pinned:
+            dev_tmp.copy_(w, non_blocking=True)
+
+    ms_copy = med(bare_copy)
+    layer.set_weights_offloaded(lay["W_r"], lay["b_r"], *pinned, ring_experts=16)
+    ms_ring = med(step)
+    torch.cuda.synchronize()
+    same = bool(torch.equal(out, ref))
+    nbytes = layer.ring_bytes_per_call
+    return {"workload": cfg.name, "ring_experts": 16, "h2d_bytes_per_step": nbytes, "resident_ms": ms_res,
+            "bare_h2d_copy_ms": ms_copy, "bare_h2d_gbs": nbytes / ms_copy / 1e6, "streamed_ms": ms_ring,
+            "streamed_h2d_gbs": nbytes / ms_ring / 1e6, "overlap_efficiency": max(ms_copy, ms_res) / ms_ring,
+            "bit_identical_to_resident": same}
+
+
 # ----------------------------------------------------------------------------- our arm
 def run_ours(args):
     from paper_2606_21712_b200 import MoELayer
@@ -584,6 +630,7 @@ def run_ours(args):
                            "B_moe_tokens": b_moe, "target_reached": reached}
     if rank == 0 and world == 1 and not args.no_sweep:
         line["combine_c5"] = run_c5_combine(args.steps, local)
+        line["ring_c3"] = run_ring(min(args.steps, 10), local)
         # every other BASELINE.json configuration through the same protocol (the north_star claim is "every
         # config"), and the sustained regime for the headline workload
         del layer

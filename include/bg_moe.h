@@ -72,6 +72,27 @@ int bg_moe_destroy(bg_moe_ctx* ctx);
 int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, const void* W_gate,
                        const void* W_up, const void* W_down, void* stream);
 
+/* Expert-weight ring buffer.  The paper keeps model parameters in host memory -- "a single
+ * source of truth ... Parameter movement is unidirectional: host memory serves as the source for GPU
+ * prefetching" -- and streams the experts of a module through a GPU-side "ring parameter buffer" whose slot
+ * ownership "is released after the module completes execution" (§5.2, Fig. 7a), "fully
+ * overlapping parameter transfers with computation" (§6.5).
+ *   W_r, b_r                      DEVICE, as in bg_moe_set_weights (the router stays resident: 4 d E bytes)
+ *   W_gate_host, W_up_host, W_down_host   HOST pointers (pinned memory, or the copies are not asynchronous), the
+ *                                 same layouts as the resident tensors; borrowed, must outlive the calls
+ *   ring_experts                  even, >= 2: the device ring holds this many experts' weights in two halves
+ *                                 (6 d f ring_experts bytes, allocated here, at set-up time)
+ * Afterwards bg_moe_combined_forward (and the _segments / _host forms) runs the expert FFN chunk by chunk:
+ * ring_experts/2 experts are copied into one half on a stream the context owns while the grouped GEMMs of the
+ * previous chunk run out of the other half.  Same kernels, same per-row arithmetic: results are bit-identical to
+ * the resident path.  Every expert is copied (which experts are empty is known only on the device; no host
+ * synchronisation is taken).  The split calls (bg_moe_expert_ffn) need resident weights. */
+int bg_moe_set_weights_offloaded(bg_moe_ctx* ctx, const float* W_r, const float* b_r, const void* W_gate_host,
+                                 const void* W_up_host, const void* W_down_host, int32_t ring_experts,
+                                 void* stream);
+/* Host -> device bytes the ring copied during the last fused call (0 with resident weights). */
+int64_t bg_moe_ring_bytes_per_call(const bg_moe_ctx* ctx);
+
 /* Debug / test switches of the grouped-GEMM tile scheduler; production never calls this.
  *   static_tile_feed != 0     tile t -> cluster (t mod #clusters) instead of the dynamic ticket feed
  *   supergroup_token_tiles    > 0: token tiles per super-group (forces the super-group order on small

@@ -15,7 +15,7 @@ BG_OK, BG_ERR_INVALID_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA, BG_ERR_NOMEM, BG_ERR
 EXPORTS = ["bg_moe_create", "bg_moe_destroy", "bg_moe_set_weights", "bg_moe_route", "bg_moe_permute",
            "bg_moe_expert_ffn", "bg_moe_unpermute", "bg_moe_combined_forward", "bg_moe_combined_forward_host",
            "bg_moe_debug_views", "bg_moe_profile_enable", "bg_moe_profile_read", "bg_moe_launch_count", "bg_moe_workspace_bytes", "bg_moe_strerror",
-           "bg_moe_last_error", "bg_moe_set_debug", "bg_moe_combined_forward_segments", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens"]
+           "bg_moe_last_error", "bg_moe_set_debug", "bg_moe_set_weights_offloaded", "bg_moe_ring_bytes_per_call", "bg_moe_combined_forward_segments", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens"]
 
 
 class BgMoeConfig(ctypes.Structure):
@@ -48,6 +48,9 @@ def load_library() -> ctypes.CDLL:
         lib.bg_moe_destroy.argtypes = [vp]
         lib.bg_moe_set_weights.argtypes = [vp] * 7
         lib.bg_moe_set_debug.argtypes = [vp, i32, i32, i32]
+        lib.bg_moe_set_weights_offloaded.argtypes = [vp, vp, vp, vp, vp, vp, i32, vp]
+        lib.bg_moe_ring_bytes_per_call.argtypes = [vp]
+        lib.bg_moe_ring_bytes_per_call.restype = i64
         lib.bg_moe_route.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
         lib.bg_moe_permute.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp]
         lib.bg_moe_expert_ffn.argtypes = [vp, vp, vp, i32, vp, vp]
@@ -135,6 +138,25 @@ class MoELayer:
         self._weights = (W_r, b_r, W_gate, W_up, W_down)          # keep the borrowed tensors alive
         self._check(self.lib.bg_moe_set_weights(self._ctx, _ptr(W_r), _ptr(b_r), _ptr(W_gate), _ptr(W_up),
                                                 _ptr(W_down), _stream(stream)))
+
+    def set_weights_offloaded(self, W_r, b_r, W_gate_host, W_up_host, W_down_host, ring_experts: int, stream=None):
+        """bg_moe_set_weights_offloaded: expert weights stay in (pinned) host memory and are streamed through a
+        device ring of `ring_experts` expert slots while the grouped GEMMs run."""
+        assert W_r.dtype == torch.float32 and W_r.shape == (self.d, self.E) and W_r.is_contiguous() and W_r.is_cuda
+        assert b_r is None or (b_r.dtype == torch.float32 and b_r.shape == (self.E,) and b_r.is_contiguous()
+                               and b_r.is_cuda)
+        for w, shp in ((W_gate_host, (self.E, self.d, self.f)), (W_up_host, (self.E, self.d, self.f)),
+                       (W_down_host, (self.E, self.f, self.d))):
+            assert w.dtype == torch.bfloat16 and tuple(w.shape) == shp and w.is_contiguous() and not w.is_cuda
+            assert w.is_pinned(), "offloaded expert weights must be in pinned host memory"
+        self._weights = (W_r, b_r, W_gate_host, W_up_host, W_down_host)
+        self._check(self.lib.bg_moe_set_weights_offloaded(self._ctx, _ptr(W_r), _ptr(b_r), _ptr(W_gate_host),
+                                                          _ptr(W_up_host), _ptr(W_down_host), int(ring_experts),
+                                                          _stream(stream)))
+
+    @property
+    def ring_bytes_per_call(self) -> int:
+        return int(self.lib.bg_moe_ring_bytes_per_call(self._ctx))
 
     def route(self, hidden, logits_in=None, want_logits=True, stream=None):
         T = hidden.shape[0] if hidden is not None else logits_in.shape[0]

@@ -56,8 +56,22 @@ struct bg_moe_ctx {
   int host_slot = 0;
   int64_t host_calls = 0;
   // weight tensor maps (encoded in set_weights)
-  CUtensorMap tm_wg, tm_wu, tm_wd, tm_wr, tm_wr1;   // tm_wr1: one-piece box of the 4-D W_r view (E > 128)
-  CUtensorMap tm_wg4, tm_wu4, tm_wd4;   // 4-D block views (kernels.h GemmLaunch), valid when f % 64 == 0 / d % 64 == 0
+  CUtensorMap tm_wr, tm_wr1;    // W_r pieces; tm_wr1: one-piece box of the 4-D view (E > 128)
+  // expert-weight tensor maps: [0] = the resident tensors, [1], [2] = the two halves of the ring (offloaded weights)
+  struct WeightMaps {
+    CUtensorMap wg, wu, wd;      // [E', K, N] boxes {64, 64, 1}
+    CUtensorMap wg4, wu4, wd4;   // 4-D block views (kernels.h GemmLaunch), valid when f % 64 == 0 / d % 64 == 0
+  } wm[3];
+  // expert-weight ring buffer (bg_moe_set_weights_offloaded; "ring parameter buffer")
+  const uint8_t* host_wg = nullptr;   // HOST (pinned) [E,d,f], [E,d,f], [E,f,d] bf16
+  const uint8_t* host_wu = nullptr;
+  const uint8_t* host_wd = nullptr;
+  uint8_t* ring = nullptr;            // device: 2 halves x ring_chunk experts x (W_gate | W_up | W_down)
+  int ring_chunk = 0;                 // experts per half (0 = weights are resident)
+  cudaStream_t st_ring = nullptr;
+  cudaEvent_t ev_ring_ready[2] = {}, ev_ring_free[2] = {};
+  bool ring_used[2] = {false, false};
+  int64_t ring_h2d_bytes = 0;         // bytes copied host -> ring by the last forward
   // activation tensor maps of the workspace x_perm / H (whole capacity: rows past T*k are never stored)
   bg::ActMaps am_x, am_h;
   int sg_max = 0;               // bg_moe_set_debug: overrides the pair kernel's super-group size (tests)
@@ -233,9 +247,13 @@ int do_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits
   return BG_OK;
 }
 
+// offsets: [n_experts + 1] of the experts this launch covers (a slice of the layer's offsets when the weights come
+// through the ring); wm: the tensor maps of those experts' weights.
 int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t T, void* y,
-           const float* row_scale_perm, cudaStream_t st, int mark_between = -1) {
+           const float* row_scale_perm, cudaStream_t st, int mark_between = -1, int which_maps = 0, int n_experts = -1) {
   const bg_moe_config& c = ctx->cfg;
+  const bg_moe_ctx::WeightMaps& wm = ctx->wm[which_maps];
+  if (n_experts < 0) n_experts = c.E;
   const int64_t R = static_cast<int64_t>(T) * c.k;
   bg::GemmLaunch g1;
   if (x_perm == ctx->x_perm) {
@@ -244,15 +262,15 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
     ctx->last_error = "cuTensorMapEncodeTiled(x_perm) failed";
     return BG_ERR_CUDA;
   }
-  g1.tm_b0 = ctx->tm_wg;
-  g1.tm_b1 = ctx->tm_wu;
+  g1.tm_b0 = wm.wg;
+  g1.tm_b1 = wm.wu;
   g1.sg_max = ctx->sg_max;
   g1.tile_counter = ctx->dyn_sched ? ctx->tile_counters : nullptr;
   g1.w4d = c.f % 64 == 0;
-  g1.tm_b0_4d = g1.w4d ? ctx->tm_wg4 : ctx->tm_wg;
-  g1.tm_b1_4d = g1.w4d ? ctx->tm_wu4 : ctx->tm_wu;
+  g1.tm_b0_4d = g1.w4d ? wm.wg4 : wm.wg;
+  g1.tm_b1_4d = g1.w4d ? wm.wu4 : wm.wu;
   g1.offsets = offsets;
-  g1.E = c.E; g1.K = c.d; g1.N = c.f;
+  g1.E = n_experts; g1.K = c.d; g1.N = c.f;
   g1.out = ctx->H;
   g1.row_scale_perm = nullptr;
   g1.num_sms = ctx->num_sms;
@@ -260,19 +278,57 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   if (mark_between >= 0) mark(ctx, mark_between, st);
   bg::GemmLaunch g2;
   g2.tm_act = ctx->am_h;
-  g2.tm_b0 = ctx->tm_wd;
-  g2.tm_b1 = ctx->tm_wd;
+  g2.tm_b0 = wm.wd;
+  g2.tm_b1 = wm.wd;
   g2.sg_max = ctx->sg_max;
   g2.tile_counter = ctx->dyn_sched ? ctx->tile_counters + 4 : nullptr;
   g2.w4d = c.d % 64 == 0;
-  g2.tm_b0_4d = g2.w4d ? ctx->tm_wd4 : ctx->tm_wd;
+  g2.tm_b0_4d = g2.w4d ? wm.wd4 : wm.wd;
   g2.tm_b1_4d = g2.tm_b0_4d;
   g2.offsets = offsets;
-  g2.E = c.E; g2.K = c.f; g2.N = c.d;
+  g2.E = n_experts; g2.K = c.f; g2.N = c.d;
   g2.out = y;
   g2.row_scale_perm = row_scale_perm;
   g2.num_sms = ctx->num_sms;
   BG_LAUNCH(ctx, bg::launch_down_pair(g2, st), "down");
+  return BG_OK;
+}
+
+// Expert-weight ring buffer (§5.2, Fig. 7a "the running and prefetching expert
+// using the ring buffer"; "fully overlapping parameter transfers with computation").  The expert
+// weights live in pinned HOST memory; the device holds two ring halves of `ring_chunk` experts.  Chunk c of the
+// experts is copied into half c & 1 on the context's copy stream while the grouped GEMMs of chunk c-1 run out of
+// the other half on the caller's stream; a half is handed back to the copy engine when its GEMMs have finished
+// ("the buffer slot ownership is released after the module completes execution").  The GEMM kernels are the
+// resident path's: they see `ring_chunk` experts whose offsets are the matching slice of the layer's offsets, so
+// every row runs through exactly the same arithmetic and the result is bit-identical.  Parameter movement is one
+// way, host -> device; every expert is copied (which experts are empty is only known on the device, and this
+// path takes no host synchronisation either).
+int do_ffn_ring(bg_moe_ctx* ctx, int32_t T, cudaStream_t st) {
+  const bg_moe_config& c = ctx->cfg;
+  const int C = ctx->ring_chunk;
+  const size_t gu_bytes = static_cast<size_t>(c.d) * c.f * 2;       // one expert's W_gate (= W_up = W_down) bytes
+  const size_t half_bytes = 3 * gu_bytes * C;
+  ctx->ring_h2d_bytes = 0;
+  for (int e0 = 0, chunk = 0; e0 < c.E; e0 += C, ++chunk) {
+    const int h = chunk & 1;
+    const int n = c.E - e0 < C ? c.E - e0 : C;
+    uint8_t* half = ctx->ring + h * half_bytes;
+    if (ctx->ring_used[h]) BG_CUDA(ctx, cudaStreamWaitEvent(ctx->st_ring, ctx->ev_ring_free[h], 0), "ring half free");
+    BG_CUDA(ctx, cudaMemcpyAsync(half, ctx->host_wg + e0 * gu_bytes, n * gu_bytes, cudaMemcpyHostToDevice, ctx->st_ring),
+            "H2D W_gate chunk");
+    BG_CUDA(ctx, cudaMemcpyAsync(half + C * gu_bytes, ctx->host_wu + e0 * gu_bytes, n * gu_bytes, cudaMemcpyHostToDevice,
+                                 ctx->st_ring), "H2D W_up chunk");
+    BG_CUDA(ctx, cudaMemcpyAsync(half + 2 * C * gu_bytes, ctx->host_wd + e0 * gu_bytes, n * gu_bytes,
+                                 cudaMemcpyHostToDevice, ctx->st_ring), "H2D W_down chunk");
+    ctx->ring_h2d_bytes += 3 * static_cast<int64_t>(n) * gu_bytes;
+    BG_CUDA(ctx, cudaEventRecord(ctx->ev_ring_ready[h], ctx->st_ring), "record ring ready");
+    BG_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_ring_ready[h], 0), "wait ring ready");
+    int rc = do_ffn(ctx, ctx->x_perm, ctx->offsets + e0, T, ctx->Y, ctx->w_perm, st, -1, 1 + h, n);
+    if (rc) return rc;
+    BG_CUDA(ctx, cudaEventRecord(ctx->ev_ring_free[h], st), "record ring free");
+    ctx->ring_used[h] = true;
+  }
   return BG_OK;
 }
 
@@ -287,13 +343,84 @@ int do_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void* out, cudaSt
                        ctx->w_perm};
   BG_LAUNCH(ctx, bg::launch_gather(hidden, pl, T, c.E, c.k, c.d, ctx->x_perm, ctx->num_sms, st, seg), "gather");
   mark(ctx, 2, st);
-  rc = do_ffn(ctx, ctx->x_perm, ctx->offsets, T, ctx->Y, ctx->w_perm, st, /*mark_between=*/3);
-  if (rc) return rc;
+  if (ctx->ring_chunk == 0) {
+    rc = do_ffn(ctx, ctx->x_perm, ctx->offsets, T, ctx->Y, ctx->w_perm, st, /*mark_between=*/3);
+    if (rc) return rc;
+  } else {
+    rc = do_ffn_ring(ctx, T, st);
+    if (rc) return rc;
+    mark(ctx, 3, st);        // per-kernel profile: the whole streamed FFN is reported as "gateup_swiglu", "down" = 0
+  }
   mark(ctx, 4, st);
   BG_LAUNCH(ctx, bg::launch_unpermute(ctx->Y, ctx->inv_perm, nullptr, T, c.k, c.d, out, ctx->num_sms, st, seg),
             "unpermute");
   mark(ctx, 5, st);
   ctx->profile_valid = ctx->profile;
+  return BG_OK;
+}
+
+// The three expert-weight tensors [n_experts, ...] -> the six tensor maps of a WeightMaps set.
+bool encode_weight_maps(bg_moe_ctx* ctx, bg_moe_ctx::WeightMaps* wm, const void* W_gate, const void* W_up,
+                        const void* W_down, int n_experts) {
+  const bg_moe_config& c = ctx->cfg;
+  if (!encode_weight_map(&wm->wg, W_gate, n_experts, c.d, c.f) || !encode_weight_map(&wm->wu, W_up, n_experts, c.d, c.f) ||
+      !encode_weight_map(&wm->wd, W_down, n_experts, c.f, c.d)) {
+    ctx->last_error = "cuTensorMapEncodeTiled(weights) failed";
+    return false;
+  }
+  // block views for the pair kernel: a7 = 1 block of 64 columns per map, a8 = 2
+  if ((c.f % 64 == 0 && (!encode_weight_map_4d(&wm->wg4, W_gate, n_experts, c.d, c.f, 1) ||
+                         !encode_weight_map_4d(&wm->wu4, W_up, n_experts, c.d, c.f, 1))) ||
+      (c.d % 64 == 0 && !encode_weight_map_4d(&wm->wd4, W_down, n_experts, c.f, c.d, 2))) {
+    ctx->last_error = "cuTensorMapEncodeTiled(weight block views) failed";
+    return false;
+  }
+  return true;
+}
+
+// Router weights: the exact bf16 hi/mid/lo split of W_r (router_fused.cu) and its tensor maps.
+int set_router_weights(bg_moe_ctx* ctx, const float* W_r, cudaStream_t st) {
+  const bg_moe_config& c = ctx->cfg;
+  {
+    DeviceGuard guard(c.device);
+    const int64_t E_ld = (c.E + 15) & ~15;
+    EncodeTiledFn fn = get_encode_fn();
+    CUresult res;
+    if (E_ld % 64 == 0) {
+      // [3][d][E_ld] viewed as [3][E_ld/64][d][64]: one box {64 e, 64 k, E_ld/64 blocks, 3 pieces} per
+      // k-block lands every piece and 64-expert block in the [piece][block][k][64 e] order of the MN-major operand
+      cuuint64_t dims[4] = {64, static_cast<cuuint64_t>(c.d), static_cast<cuuint64_t>(E_ld / 64), 3};
+      cuuint64_t strides[3] = {static_cast<cuuint64_t>(E_ld) * 2, 128, static_cast<cuuint64_t>(E_ld) * c.d * 2};
+      cuuint32_t box[4] = {64, 64, static_cast<cuuint32_t>(E_ld / 64), 3};
+      cuuint32_t estr[4] = {1, 1, 1, 1};
+      res = fn(&ctx->tm_wr, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, ctx->wr_pieces, dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      box[3] = 1;
+      if (res == CUDA_SUCCESS)
+        res = fn(&ctx->tm_wr1, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, ctx->wr_pieces, dims, strides, box, estr,
+                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    } else {
+      cuuint64_t dims[3] = {static_cast<cuuint64_t>(E_ld), static_cast<cuuint64_t>(c.d), 3};
+      cuuint64_t strides[2] = {static_cast<cuuint64_t>(E_ld) * 2, static_cast<cuuint64_t>(E_ld) * c.d * 2};
+      cuuint32_t box[3] = {64, 64, 1};
+      cuuint32_t estr[3] = {1, 1, 1};
+      res = fn(&ctx->tm_wr, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, ctx->wr_pieces, dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    }
+    if (E_ld % 64 != 0) ctx->tm_wr1 = ctx->tm_wr;
+    if (res != CUDA_SUCCESS) {
+      ctx->last_error = "cuTensorMapEncodeTiled(W_r pieces) failed";
+      return BG_ERR_CUDA;
+    }
+    int rc = begin_call(ctx, st);      // also orders the split after host-path work that still reads the old pieces
+    if (rc) return rc;
+    BG_LAUNCH(ctx, bg::launch_split_wr(W_r, c.d, c.E, ctx->wr_pieces, st), "split_wr");
+    rc = end_call(ctx, st, false);
+    if (rc) return rc;
+  }
   return BG_OK;
 }
 
@@ -306,6 +433,12 @@ void destroy_ctx(bg_moe_ctx* ctx) {
     if (ctx->ev_d2h[i]) cudaEventDestroy(ctx->ev_d2h[i]);
   }
   if (ctx->ev_device_call) cudaEventDestroy(ctx->ev_device_call);
+  for (int i = 0; i < 2; ++i) {
+    if (ctx->ev_ring_ready[i]) cudaEventDestroy(ctx->ev_ring_ready[i]);
+    if (ctx->ev_ring_free[i]) cudaEventDestroy(ctx->ev_ring_free[i]);
+  }
+  if (ctx->st_ring) cudaStreamDestroy(ctx->st_ring);
+  if (ctx->ring) cudaFree(ctx->ring);
   if (ctx->st_in) cudaStreamDestroy(ctx->st_in);
   if (ctx->st_compute) cudaStreamDestroy(ctx->st_compute);
   if (ctx->st_out) cudaStreamDestroy(ctx->st_out);
@@ -417,6 +550,7 @@ int bg_moe_destroy(bg_moe_ctx* ctx) {
   if (ctx->st_in) cudaStreamSynchronize(ctx->st_in);
   if (ctx->st_compute) cudaStreamSynchronize(ctx->st_compute);
   if (ctx->st_out) cudaStreamSynchronize(ctx->st_out);
+  if (ctx->st_ring) cudaStreamSynchronize(ctx->st_ring);
   destroy_ctx(ctx);
   return BG_OK;
 }
@@ -435,63 +569,59 @@ int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, cons
   if (!ctx || !W_r || !W_gate || !W_up || !W_down) return BG_ERR_INVALID_ARG;
   if (!aligned16(W_r) || !aligned16(W_gate) || !aligned16(W_up) || !aligned16(W_down)) return BG_ERR_INVALID_ARG;
   const bg_moe_config& c = ctx->cfg;
-  if (!encode_weight_map(&ctx->tm_wg, W_gate, c.E, c.d, c.f) || !encode_weight_map(&ctx->tm_wu, W_up, c.E, c.d, c.f) ||
-      !encode_weight_map(&ctx->tm_wd, W_down, c.E, c.f, c.d)) {
-    ctx->last_error = "cuTensorMapEncodeTiled(weights) failed";
-    return BG_ERR_CUDA;
-  }
-  // block views for the pair kernel: a7 = 1 block of 64 columns per map, a8 = 2
-  if ((c.f % 64 == 0 && (!encode_weight_map_4d(&ctx->tm_wg4, W_gate, c.E, c.d, c.f, 1) ||
-                         !encode_weight_map_4d(&ctx->tm_wu4, W_up, c.E, c.d, c.f, 1))) ||
-      (c.d % 64 == 0 && !encode_weight_map_4d(&ctx->tm_wd4, W_down, c.E, c.f, c.d, 2))) {
-    ctx->last_error = "cuTensorMapEncodeTiled(weight block views) failed";
-    return BG_ERR_CUDA;
-  }
-  // exact bf16 hi/mid/lo split of W_r for the tensor-core router (router_fused.cu); [3][d][E_ld]
-  {
-    DeviceGuard guard(c.device);
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const int64_t E_ld = (c.E + 15) & ~15;
-    EncodeTiledFn fn = get_encode_fn();
-    CUresult res;
-    if (E_ld % 64 == 0) {
-      // [3][d][E_ld] viewed as [3][E_ld/64][d][64]: one box {64 e, 64 k, E_ld/64 blocks, 3 pieces} per
-      // k-block lands every piece and 64-expert block in the [piece][block][k][64 e] order of the MN-major operand
-      cuuint64_t dims[4] = {64, static_cast<cuuint64_t>(c.d), static_cast<cuuint64_t>(E_ld / 64), 3};
-      cuuint64_t strides[3] = {static_cast<cuuint64_t>(E_ld) * 2, 128, static_cast<cuuint64_t>(E_ld) * c.d * 2};
-      cuuint32_t box[4] = {64, 64, static_cast<cuuint32_t>(E_ld / 64), 3};
-      cuuint32_t estr[4] = {1, 1, 1, 1};
-      res = fn(&ctx->tm_wr, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, ctx->wr_pieces, dims, strides, box, estr,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-      box[3] = 1;
-      if (res == CUDA_SUCCESS)
-        res = fn(&ctx->tm_wr1, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, ctx->wr_pieces, dims, strides, box, estr,
-                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    } else {
-      cuuint64_t dims[3] = {static_cast<cuuint64_t>(E_ld), static_cast<cuuint64_t>(c.d), 3};
-      cuuint64_t strides[2] = {static_cast<cuuint64_t>(E_ld) * 2, static_cast<cuuint64_t>(E_ld) * c.d * 2};
-      cuuint32_t box[3] = {64, 64, 1};
-      cuuint32_t estr[3] = {1, 1, 1};
-      res = fn(&ctx->tm_wr, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, ctx->wr_pieces, dims, strides, box, estr,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    }
-    if (E_ld % 64 != 0) ctx->tm_wr1 = ctx->tm_wr;
-    if (res != CUDA_SUCCESS) {
-      ctx->last_error = "cuTensorMapEncodeTiled(W_r pieces) failed";
-      return BG_ERR_CUDA;
-    }
-    int rc = begin_call(ctx, st);      // also orders the split after host-path work that still reads the old pieces
-    if (rc) return rc;
-    BG_LAUNCH(ctx, bg::launch_split_wr(W_r, c.d, c.E, ctx->wr_pieces, st), "split_wr");
-    rc = end_call(ctx, st, false);
-    if (rc) return rc;
-  }
+  if (!encode_weight_maps(ctx, &ctx->wm[0], W_gate, W_up, W_down, c.E)) return BG_ERR_CUDA;
+  int rc = set_router_weights(ctx, W_r, static_cast<cudaStream_t>(stream));
+  if (rc) return rc;
   ctx->W_r = W_r; ctx->b_r = b_r; ctx->W_gate = W_gate; ctx->W_up = W_up; ctx->W_down = W_down;
+  ctx->ring_chunk = 0;            // resident weights
   return BG_OK;
 }
+
+int bg_moe_set_weights_offloaded(bg_moe_ctx* ctx, const float* W_r, const float* b_r, const void* W_gate_host,
+                                 const void* W_up_host, const void* W_down_host, int32_t ring_experts, void* stream) {
+  if (!ctx || !W_r || !W_gate_host || !W_up_host || !W_down_host || !aligned16(W_r)) return BG_ERR_INVALID_ARG;
+  const bg_moe_config& c = ctx->cfg;
+  if (ring_experts < 2 || (ring_experts & 1)) return BG_ERR_INVALID_ARG;
+  DeviceGuard guard(c.device);
+  const int chunk = ring_experts / 2 < c.E ? ring_experts / 2 : c.E;
+  const size_t gu_bytes = static_cast<size_t>(c.d) * c.f * 2;
+  const size_t half_bytes = 3 * gu_bytes * chunk;
+  if (ctx->ring == nullptr || ctx->ring_chunk != chunk) {
+    // set-up time allocation (like the caller's own weight tensors); nothing is allocated per call
+    if (ctx->st_ring) BG_CUDA(ctx, cudaStreamSynchronize(ctx->st_ring), "ring stream sync");
+    if (ctx->ring) { cudaFree(ctx->ring); ctx->ring = nullptr; }
+    void* p = nullptr;
+    if (cudaMalloc(&p, 2 * half_bytes) != cudaSuccess) {
+      cudaGetLastError();
+      return BG_ERR_NOMEM;
+    }
+    ctx->ring = static_cast<uint8_t*>(p);
+    if (ctx->st_ring == nullptr) {
+      BG_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->st_ring, cudaStreamNonBlocking), "ring stream");
+      for (int i = 0; i < 2; ++i) {
+        BG_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_ring_ready[i], cudaEventDisableTiming), "ring event");
+        BG_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_ring_free[i], cudaEventDisableTiming), "ring event");
+      }
+    }
+    ctx->ring_used[0] = ctx->ring_used[1] = false;
+  }
+  for (int h = 0; h < 2; ++h) {
+    uint8_t* half = ctx->ring + h * half_bytes;
+    if (!encode_weight_maps(ctx, &ctx->wm[1 + h], half, half + chunk * gu_bytes, half + 2 * chunk * gu_bytes, chunk))
+      return BG_ERR_CUDA;
+  }
+  int rc = set_router_weights(ctx, W_r, static_cast<cudaStream_t>(stream));
+  if (rc) return rc;
+  ctx->W_r = W_r; ctx->b_r = b_r;
+  ctx->host_wg = static_cast<const uint8_t*>(W_gate_host);
+  ctx->host_wu = static_cast<const uint8_t*>(W_up_host);
+  ctx->host_wd = static_cast<const uint8_t*>(W_down_host);
+  ctx->W_gate = W_gate_host; ctx->W_up = W_up_host; ctx->W_down = W_down_host;   // "weights set" for the entry checks
+  ctx->ring_chunk = chunk;
+  return BG_OK;
+}
+
+int64_t bg_moe_ring_bytes_per_call(const bg_moe_ctx* ctx) { return ctx ? ctx->ring_h2d_bytes : 0; }
 
 int bg_moe_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits_in, float* logits_out,
                  int32_t* topk_idx, float* topk_w, int32_t* counts, int32_t* offsets, void* stream) {
@@ -545,7 +675,7 @@ int bg_moe_expert_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offset
   if (rc) return rc;
   if (T == 0) return BG_OK;
   if (!x_perm || !offsets || !y_perm || !aligned16(x_perm) || !aligned16(y_perm)) return BG_ERR_INVALID_ARG;
-  if (ctx->W_gate == nullptr) return BG_ERR_NO_WEIGHTS;
+  if (ctx->W_gate == nullptr || ctx->ring_chunk != 0) return BG_ERR_NO_WEIGHTS;   // needs resident expert weights
   DeviceGuard guard(ctx->cfg.device);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   if ((rc = begin_call(ctx, st))) return rc;

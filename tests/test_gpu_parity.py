@@ -444,6 +444,40 @@ def test_non_finite_logits_are_memory_safe():
     assert np.array_equal(idx[fin], o_idx)
 
 
+@pytest.mark.parametrize("ring_experts", [2, 4, 6, 16], ids=lambda r: f"ring{r}")
+def test_offloaded_weights_ring_buffer_equals_resident(ring_experts):
+    """SURVEY §8(f)-4 / PAPER.md:317-325: expert weights in pinned host memory, streamed through a device ring of
+    `ring_experts` slots (two halves) while the grouped GEMMs run.  The result must be bit-identical to the
+    resident path (same kernels, the experts merely arrive in chunks) and match the oracle; chunk sizes 1, 2, 3
+    (11 experts: a ragged last chunk) and a ring larger than the layer; repeated calls reuse the ring halves."""
+    cfg = wl.small_config(T=600, d=256, E=11, k=3, f=192, index=37)
+    lay, g, layer = make(cfg)
+    ref = layer.combined_forward(g["hidden"]).clone()
+    h2 = g["hidden"].flip(0).contiguous()
+    ref2 = layer.combined_forward(h2).clone()
+    pinned = [lay[n].pin_memory() for n in ("W_gate", "W_up", "W_down")]
+    layer.set_weights_offloaded(g["W_r"], g["b_r"], *pinned, ring_experts=ring_experts)
+    a = layer.combined_forward(g["hidden"]).clone()
+    b = layer.combined_forward(h2).clone()
+    c = layer.combined_forward(g["hidden"]).clone()
+    torch.cuda.synchronize()
+    assert layer.ring_bytes_per_call == 6 * cfg.d * cfg.f * cfg.E * 2 // 2
+    assert torch.equal(a, ref) and torch.equal(b, ref2) and torch.equal(c, ref)
+    L = layer.debug_views(cfg.T)["logits"].cpu().numpy()
+    o = oracle.forward_batched(lay["hidden"], lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"], cfg.k,
+                               logits_in=L)["out"]
+    check_out(c, o, f"ring of {ring_experts}")
+    # host entry point and zero-copy segments ride the same ring
+    host_out = layer.combined_forward_host(lay["hidden"].pin_memory())
+    segs = [g["hidden"][:100].clone(), g["hidden"][100:].clone()]
+    outs = layer.combined_forward_segments(segs)
+    torch.cuda.synchronize()
+    assert torch.equal(host_out, ref.cpu()) and torch.equal(torch.cat(outs), ref)
+    # back to resident weights on the same context
+    layer.set_weights(g["W_r"], g["b_r"], g["W_gate"], g["W_up"], g["W_down"])
+    assert torch.equal(layer.combined_forward(g["hidden"]), ref)
+
+
 def test_planned_workspace_equals_allocated_workspace():
     """bg_moe_workspace_bytes_for (host-only planner) must predict what bg_moe_create allocates."""
     import paper_2606_21712_b200 as pk
