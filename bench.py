@@ -483,11 +483,11 @@ def run_ring(steps: int, device_index: int):
     ms_res = med(step)
     ref = out.clone()
     pinned = [lay[n].cpu().pin_memory() for n in ("W_gate", "W_up", "W_down")]
-    dev_tmp = torch.empty_like(lay["W_gate"])
+    dev_tmp = torch.empty_like(lay["W_gate"]).view(-1)
 
     def bare_copy():
         for w in pinned:
-            dev_tmp.copy_(w, non_blocking=True)
+            dev_tmp.copy_(w.view(-1), non_blocking=True)
 
     ms_copy = med(bare_copy)
     layer.set_weights_offloaded(lay["W_r"], lay["b_r"], *pinned, ring_experts=16)
