@@ -15,7 +15,7 @@ BG_OK, BG_ERR_INVALID_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA, BG_ERR_NOMEM, BG_ERR
 EXPORTS = ["bg_moe_create", "bg_moe_destroy", "bg_moe_set_weights", "bg_moe_route", "bg_moe_permute",
            "bg_moe_expert_ffn", "bg_moe_unpermute", "bg_moe_combined_forward", "bg_moe_combined_forward_host",
            "bg_moe_debug_views", "bg_moe_profile_enable", "bg_moe_profile_read", "bg_moe_launch_count", "bg_moe_workspace_bytes", "bg_moe_strerror",
-           "bg_moe_last_error", "bg_moe_set_debug", "bg_moe_set_weights_offloaded", "bg_moe_ring_bytes_per_call", "bg_moe_combined_forward_segments", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens"]
+           "bg_moe_last_error", "bg_moe_set_debug", "bg_moe_set_weights_offloaded", "bg_moe_ring_bytes_per_call", "bg_moe_set_precision", "bg_moe_debug_fp8_views", "bg_moe_combined_forward_segments", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens"]
 
 
 class BgMoeConfig(ctypes.Structure):
@@ -51,6 +51,8 @@ def load_library() -> ctypes.CDLL:
         lib.bg_moe_set_weights_offloaded.argtypes = [vp, vp, vp, vp, vp, vp, i32, vp]
         lib.bg_moe_ring_bytes_per_call.argtypes = [vp]
         lib.bg_moe_ring_bytes_per_call.restype = i64
+        lib.bg_moe_set_precision.argtypes = [vp, i32, vp]
+        lib.bg_moe_debug_fp8_views.argtypes = [vp] + [ctypes.POINTER(vp)] * 6
         lib.bg_moe_route.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
         lib.bg_moe_permute.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp]
         lib.bg_moe_expert_ffn.argtypes = [vp, vp, vp, i32, vp, vp]
@@ -153,6 +155,23 @@ class MoELayer:
         self._check(self.lib.bg_moe_set_weights_offloaded(self._ctx, _ptr(W_r), _ptr(b_r), _ptr(W_gate_host),
                                                           _ptr(W_up_host), _ptr(W_down_host), int(ring_experts),
                                                           _stream(stream)))
+
+    def set_precision(self, precision: int, stream=None):
+        """bg_moe_set_precision: 0 = bf16, 1 = FP8 (e4m3) gate/up GEMM; quantises the resident weights."""
+        self._check(self.lib.bg_moe_set_precision(self._ctx, int(precision), _stream(stream)))
+
+    def fp8_views(self, T: int) -> dict:
+        """FP8 artefacts of the last fused call, copied out of the library's buffers (codes as uint8)."""
+        ptrs = [ctypes.c_void_p() for _ in range(6)]
+        self._check(self.lib.bg_moe_debug_fp8_views(self._ctx, *[ctypes.byref(p) for p in ptrs]))
+        R = T * self.k
+        spec = [("xq_perm", "|u1", (R, self.d)), ("sx_perm", "<f4", (R,)), ("q_gate", "|u1", (self.E, self.f, self.d)),
+                ("sw_gate", "<f4", (self.E, self.f)), ("q_up", "|u1", (self.E, self.f, self.d)),
+                ("sw_up", "<f4", (self.E, self.f))]
+        out = {}
+        for p, (name, ts, shape) in zip(ptrs, spec):
+            out[name] = torch.as_tensor(_DeviceArray(p.value, shape, ts), device=self._dev()).clone()
+        return out
 
     @property
     def ring_bytes_per_call(self) -> int:

@@ -62,6 +62,18 @@ struct bg_moe_ctx {
     CUtensorMap wg, wu, wd;      // [E', K, N] boxes {64, 64, 1}
     CUtensorMap wg4, wu4, wd4;   // 4-D block views (kernels.h GemmLaunch), valid when f % 64 == 0 / d % 64 == 0
   } wm[3];
+  // FP8 gate/up (bg_moe_set_precision; readings F1-F4): quantised weights [E, f, d] bytes + per-channel scales,
+  // the quantised expert-order rows + per-row scales, and their tensor maps
+  int precision = 0;                  // 0 = bf16, 1 = FP8 gate/up
+  uint8_t* fp8_buf = nullptr;         // one set-up time allocation
+  uint8_t* q_gate = nullptr;
+  uint8_t* q_up = nullptr;
+  float* sw_gate = nullptr;
+  float* sw_up = nullptr;
+  uint8_t* xq_perm = nullptr;
+  float* sx_perm = nullptr;
+  CUtensorMap tm_qg, tm_qu;
+  bg::ActMaps am_xq;
   // expert-weight ring buffer (bg_moe_set_weights_offloaded; "ring parameter buffer")
   const uint8_t* host_wg = nullptr;   // HOST (pinned) [E,d,f], [E,d,f], [E,f,d] bf16
   const uint8_t* host_wu = nullptr;
@@ -144,6 +156,32 @@ bool encode_weight_map(CUtensorMap* tm, const void* ptr, int64_t E, int64_t K, i
   cuuint32_t box[3] = {64, 64, 1};
   cuuint32_t estr[3] = {1, 1, 1};
   return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(ptr), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// e4m3 bytes [rows, K] row-major, box {128 k, box_rows rows}, 128B swizzle.
+bool encode_act_map_u8(CUtensorMap* tm, const void* ptr, int64_t rows, int64_t K, int box_rows) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(rows)};
+  cuuint64_t strides[1] = {static_cast<cuuint64_t>(K)};
+  cuuint32_t box[2] = {128, static_cast<cuuint32_t>(box_rows)};
+  cuuint32_t estr[2] = {1, 1};
+  return fn(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(ptr), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// quantised weights [E, N, K] e4m3 bytes (k contiguous), box {128 k, 64 n, 1 expert}, 128B swizzle.
+bool encode_weight_map_u8(CUtensorMap* tm, const void* ptr, int64_t E, int64_t N, int64_t K) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[3] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(N), static_cast<cuuint64_t>(E)};
+  cuuint64_t strides[2] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(N) * K};
+  cuuint32_t box[3] = {128, 64, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  return fn(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(ptr), dims, strides, box, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
@@ -274,7 +312,16 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g1.out = ctx->H;
   g1.row_scale_perm = nullptr;
   g1.num_sms = ctx->num_sms;
-  BG_LAUNCH(ctx, bg::launch_gateup_swiglu_pair(g1, st), "gateup_swiglu");
+  if (ctx->precision == 1 && x_perm == ctx->x_perm && which_maps == 0) {
+    // FP8 gate/up (fused path): the gather wrote e4m3 rows + scales instead of x_perm
+    g1.tm_act = ctx->am_xq;
+    g1.tm_b0 = ctx->tm_qg;
+    g1.tm_b1 = ctx->tm_qu;
+    g1.sx = ctx->sx_perm; g1.sw0 = ctx->sw_gate; g1.sw1 = ctx->sw_up;
+    BG_LAUNCH(ctx, bg::launch_gateup_swiglu_pair_fp8(g1, st), "gateup_swiglu_fp8");
+  } else {
+    BG_LAUNCH(ctx, bg::launch_gateup_swiglu_pair(g1, st), "gateup_swiglu");
+  }
   if (mark_between >= 0) mark(ctx, mark_between, st);
   bg::GemmLaunch g2;
   g2.tm_act = ctx->am_h;
@@ -341,7 +388,11 @@ int do_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void* out, cudaSt
   mark(ctx, 1, st);
   bg::PermLaunch pl = {ctx->topk_idx, ctx->tile_rank, ctx->tile_base, ctx->topk_w, ctx->row_src, ctx->inv_perm,
                        ctx->w_perm};
-  BG_LAUNCH(ctx, bg::launch_gather(hidden, pl, T, c.E, c.k, c.d, ctx->x_perm, ctx->num_sms, st, seg), "gather");
+  if (ctx->precision == 1)
+    BG_LAUNCH(ctx, bg::launch_gather_fp8(hidden, pl, T, c.E, c.k, c.d, ctx->xq_perm, ctx->sx_perm, ctx->num_sms, st, seg),
+              "gather_fp8");
+  else
+    BG_LAUNCH(ctx, bg::launch_gather(hidden, pl, T, c.E, c.k, c.d, ctx->x_perm, ctx->num_sms, st, seg), "gather");
   mark(ctx, 2, st);
   if (ctx->ring_chunk == 0) {
     rc = do_ffn(ctx, ctx->x_perm, ctx->offsets, T, ctx->Y, ctx->w_perm, st, /*mark_between=*/3);
@@ -439,6 +490,7 @@ void destroy_ctx(bg_moe_ctx* ctx) {
   }
   if (ctx->st_ring) cudaStreamDestroy(ctx->st_ring);
   if (ctx->ring) cudaFree(ctx->ring);
+  if (ctx->fp8_buf) cudaFree(ctx->fp8_buf);
   if (ctx->st_in) cudaStreamDestroy(ctx->st_in);
   if (ctx->st_compute) cudaStreamDestroy(ctx->st_compute);
   if (ctx->st_out) cudaStreamDestroy(ctx->st_out);
@@ -574,6 +626,7 @@ int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, cons
   if (rc) return rc;
   ctx->W_r = W_r; ctx->b_r = b_r; ctx->W_gate = W_gate; ctx->W_up = W_up; ctx->W_down = W_down;
   ctx->ring_chunk = 0;            // resident weights
+  ctx->precision = 0;             // new weights: bf16 until bg_moe_set_precision quantises them
   return BG_OK;
 }
 
@@ -618,10 +671,66 @@ int bg_moe_set_weights_offloaded(bg_moe_ctx* ctx, const float* W_r, const float*
   ctx->host_wd = static_cast<const uint8_t*>(W_down_host);
   ctx->W_gate = W_gate_host; ctx->W_up = W_up_host; ctx->W_down = W_down_host;   // "weights set" for the entry checks
   ctx->ring_chunk = chunk;
+  ctx->precision = 0;             // the streamed path is bf16
   return BG_OK;
 }
 
 int64_t bg_moe_ring_bytes_per_call(const bg_moe_ctx* ctx) { return ctx ? ctx->ring_h2d_bytes : 0; }
+
+int bg_moe_set_precision(bg_moe_ctx* ctx, int32_t precision, void* stream) {
+  if (ctx == nullptr || precision < 0 || precision > 1) return BG_ERR_INVALID_ARG;
+  if (precision == 0) { ctx->precision = 0; return BG_OK; }
+  const bg_moe_config& c = ctx->cfg;
+  if (ctx->W_gate == nullptr || ctx->ring_chunk != 0) return BG_ERR_NO_WEIGHTS;     // needs resident bf16 weights
+  if (c.d % 128 != 0 || c.f % 64 != 0) return BG_ERR_UNSUPPORTED;                    // 128-byte k-blocks, 64-feature boxes
+  DeviceGuard guard(c.device);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int64_t Tm = c.max_tokens > 0 ? c.max_tokens : 1;
+  const int64_t Rm = Tm * c.k;
+  if (ctx->fp8_buf == nullptr) {
+    // set-up time allocation (like the ring): 2 E d f bytes of codes, scales, and the quantised rows
+    auto up = [](int64_t v) { return (v + 1023) / 1024 * 1024; };
+    const int64_t wq = up(static_cast<int64_t>(c.E) * c.d * c.f), sw = up(static_cast<int64_t>(c.E) * c.f * 4);
+    const int64_t xq = up(Rm * c.d), sx = up(Rm * 4);
+    void* p = nullptr;
+    if (cudaMalloc(&p, static_cast<size_t>(2 * wq + 2 * sw + xq + sx)) != cudaSuccess) {
+      cudaGetLastError();
+      return BG_ERR_NOMEM;
+    }
+    ctx->fp8_buf = static_cast<uint8_t*>(p);
+    ctx->q_gate = ctx->fp8_buf;
+    ctx->q_up = ctx->q_gate + wq;
+    ctx->sw_gate = reinterpret_cast<float*>(ctx->q_up + wq);
+    ctx->sw_up = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(ctx->sw_gate) + sw);
+    ctx->xq_perm = reinterpret_cast<uint8_t*>(ctx->sw_up) + sw;
+    ctx->sx_perm = reinterpret_cast<float*>(ctx->xq_perm + xq);
+    bool ok = encode_weight_map_u8(&ctx->tm_qg, ctx->q_gate, c.E, c.f, c.d) &&
+              encode_weight_map_u8(&ctx->tm_qu, ctx->q_up, c.E, c.f, c.d);
+    for (int i = 0; i < 16 && ok; ++i) ok = encode_act_map_u8(&ctx->am_xq.m[i], ctx->xq_perm, Rm, c.d, 8 * (i + 1));
+    if (!ok) {
+      ctx->last_error = "cuTensorMapEncodeTiled(fp8) failed";
+      return BG_ERR_CUDA;
+    }
+  }
+  int rc = begin_call(ctx, st);
+  if (rc) return rc;
+  BG_LAUNCH(ctx, bg::launch_quantize_weights(ctx->W_gate, c.E, c.d, c.f, ctx->q_gate, ctx->sw_gate, st), "quantize W_gate");
+  BG_LAUNCH(ctx, bg::launch_quantize_weights(ctx->W_up, c.E, c.d, c.f, ctx->q_up, ctx->sw_up, st), "quantize W_up");
+  ctx->precision = 1;
+  return end_call(ctx, st, false);
+}
+
+int bg_moe_debug_fp8_views(bg_moe_ctx* ctx, const void** xq_perm, const float** sx_perm, const void** q_gate,
+                           const float** sw_gate, const void** q_up, const float** sw_up) {
+  if (!ctx || ctx->fp8_buf == nullptr) return BG_ERR_INVALID_ARG;
+  if (xq_perm) *xq_perm = ctx->xq_perm;
+  if (sx_perm) *sx_perm = ctx->sx_perm;
+  if (q_gate) *q_gate = ctx->q_gate;
+  if (sw_gate) *sw_gate = ctx->sw_gate;
+  if (q_up) *q_up = ctx->q_up;
+  if (sw_up) *sw_up = ctx->sw_up;
+  return BG_OK;
+}
 
 int bg_moe_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits_in, float* logits_out,
                  int32_t* topk_idx, float* topk_w, int32_t* counts, int32_t* offsets, void* stream) {

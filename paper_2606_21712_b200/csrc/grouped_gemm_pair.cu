@@ -69,13 +69,15 @@ constexpr int BAR_BYTES = 256;
 constexpr int TABLE_BYTES = 2064;                   // 2 x (MAX_E + 1) ints, 16-byte padded
 constexpr int STAGE_TILE_BYTES = 32 * 64;           // per-warp output staging: [32 tokens][32 features] bf16
 // epilogue scratch: [4 exchange buffers (a7) | 4 x 256 gate weights (a8)] then the 4 staging tiles
-constexpr int EPI_BYTES = 4 * XCH_BYTES + 4 * STAGE_TILE_BYTES;   // a8: 2 KB of scales + 8 staging tiles = 18 KB
+constexpr int EPI_BYTES = 4 * XCH_BYTES + 4 * STAGE_TILE_BYTES + BN_MAX * 4;   // a8: 2 KB of scales + 8 staging tiles = 18 KB; FP8 a7: + 1 KB of token scales
 static_assert(EPI_BYTES >= 2 * BN_MAX * 4 + 8 * STAGE_TILE_BYTES, "a8 epilogue scratch");
 constexpr int SMEM_BYTES = RING_BYTES + 1024 /*align slack*/ + BAR_BYTES + TABLE_BYTES + EPI_BYTES;
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
 
 // M = 256 (pair), A MN-major (weights), B K-major (tokens); the N field is filled in per tile.
 constexpr uint32_t IDESC_BASE = umma_idesc_bf16(256, 0, /*A MN-major*/ 1, /*B K-major*/ 0);
+// FP8 gate/up: e4m3 x e4m3, both operands K-major (the quantised weights are stored [E, N, K], reading F3)
+constexpr uint32_t IDESC_FP8 = umma_idesc_e4m3(256, 0, 0, 0);
 // A: MN-major SW128: 64-feature blocks A_BLK_BYTES apart (LBO); 8-k-row groups 1024 B apart (SBO).
 constexpr uint64_t ADESC_HI = umma_desc_sw128(A_BLK_BYTES, 1024);
 // B: K-major SW128: 8-token groups 1024 B apart (SBO); LBO unused inside one swizzle span.
@@ -89,6 +91,10 @@ struct Params {
   bool w4d;                    // tm_w0 / tm_w1 are the 4-D block views (kernels.h)
   int sg_max;                  // 0 = derive the super-group size from K
   int* tile_counter;           // dynamic feed: [2] = ticket counter, clusters-finished counter (zero between launches); nullptr = static feed
+  // FP8 gate/up (reading F4): dequantisation scales
+  const float* sx;             // [rows]  per expert-order token row
+  const float* sw0;            // [E, N]  per expert and output channel, W_gate
+  const float* sw1;            // [E, N]  W_up
 };
 
 __device__ __forceinline__ void named_bar_sync(int id, int threads) {
@@ -163,7 +169,9 @@ __device__ __forceinline__ void st_shared_bf16(uint32_t addr, float v) {
 
 // GATEUP = true : a7 (per CTA A = [64 W_gate columns | 64 W_up columns], SwiGLU epilogue, 128 output features / pair tile)
 // GATEUP = false: a8 (per CTA A = 128 W_down columns, optional per-token scale, 256 output features / pair tile)
-template <bool GATEUP>
+// FP8 (a7 only): operands are e4m3 bytes, a k-block is 128 elements (the same 128-byte swizzle span), both K-major;
+//                 the epilogue multiplies the accumulators by sx[token] * sw[expert, feature] before the SwiGLU.
+template <bool GATEUP, bool FP8 = false>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GATEUP ? 256 : 384, 1)
 pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__ CUtensorMap tm_w0,
                  const __grid_constant__ CUtensorMap tm_w1, const Params p) {
@@ -199,7 +207,8 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   const int cluster_id = blockIdx.x >> 1, num_clusters = gridDim.x >> 1;
   const int E = p.E;
   const int f_tiles = (p.N + OUT_FEATS - 1) / OUT_FEATS;
-  const int k_blocks = (p.K + BK - 1) / BK;
+  constexpr int BKE = FP8 ? 2 * BK : BK;             // elements per k-block (128 bytes either way)
+  const int k_blocks = (p.K + BKE - 1) / BKE;
   // token tiles whose rows fit ~48 MB of L2 (p.sg_max > 0: override, used by the tests to reach this path on small shapes)
   const int sg_max = p.sg_max > 0 ? p.sg_max : max(1, (48 << 20) / (BN_MAX * 2 * p.K));
 
@@ -299,7 +308,11 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
           const uint32_t sb = sa + A_BYTES;
           const uint32_t fb = leader_bar(full_bar(s));
           if (rank == 0) mbar_expect_tx(full_bar(s), tx_pair);   // the bytes of both CTAs
-          if (p.w4d) {
+          if (FP8) {
+            // quantised weights [E, N, K] bytes: box {128 k, 64 features, 1}: K-major, 8 KB per tensor
+            tma_load_3d_pair(sa, &tm_w0, fb, kb * BKE, n0, c.e);
+            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w1, fb, kb * BKE, n0, c.e);
+          } else if (p.w4d) {
             // one operation per weight tensor: nblk 64-column blocks in [block][k][64 n] order
             tma_load_4d_pair(sa, &tm_w0, fb, 0, kb * BK, n0 >> 6, c.e);
             if (GATEUP) tma_load_4d_pair(sa + A_BLK_BYTES, &tm_w1, fb, 0, kb * BK, n0 >> 6, c.e);
@@ -311,7 +324,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
             tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w0, fb, n0 + 64, kb * BK, c.e);
           }
           // this CTA's half of the tokens: one box of exactly `half` rows
-          tma_load_2d_pair(sb, tm_b, fb, kb * BK, brow0);
+          tma_load_2d_pair(sb, tm_b, fb, kb * BKE, brow0);
         }
         __syncwarp();
         if (++s == STAGES) { s = 0; ph ^= 1u; }
@@ -349,7 +362,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       Feed feed = {0, 0, -1};
       for (int t = feed_next(feed, true); t >= 0; t = feed_next(feed, true), ++it) {
         const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
-        const uint32_t idesc = IDESC_BASE | (static_cast<uint32_t>(c.nt >> 3) << 17);
+        const uint32_t idesc = (FP8 ? IDESC_FP8 : IDESC_BASE) | (static_cast<uint32_t>(c.nt >> 3) << 17);
         const int as = it & 1;
         const uint32_t aph = (it >> 1) & 1u;
         mbar_wait(tempty_bar(as), aph ^ 1u);          // both CTAs' epilogues have drained this accumulator
@@ -360,13 +373,18 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
           if (elect_one()) {
             const uint32_t a_addr = base + s * STAGE_BYTES;
             const uint32_t b_addr = a_addr + A_BYTES;
-            const uint64_t ad = ADESC_HI | ((a_addr >> 4) & 0x3FFFu);
+            const uint64_t ad = (FP8 ? BDESC_HI : ADESC_HI) | ((a_addr >> 4) & 0x3FFFu);   // FP8: A is K-major too
             const uint64_t bd = BDESC_HI | ((b_addr >> 4) & 0x3FFFu);
             #pragma unroll
             for (int kk = 0; kk < BK / UK; ++kk) {
-              // A (MN-major): +16 k = two 8-row groups = +2048 bytes; B (K-major): +16 k = +32 bytes in the span
-              umma_f16_pair(d_tmem, ad + ((kk * UK * 128) >> 4), bd + ((kk * UK * 2) >> 4), idesc,
-                            (kb | kk) != 0 ? 1u : 0u);
+              if (FP8) {
+                // both K-major: +32 k (one MMA of 8-bit inputs) = +32 bytes in the span
+                umma_f8_pair(d_tmem, ad + ((kk * 32) >> 4), bd + ((kk * 32) >> 4), idesc, (kb | kk) != 0 ? 1u : 0u);
+              } else {
+                // A (MN-major): +16 k = two 8-row groups = +2048 bytes; B (K-major): +16 k = +32 bytes in the span
+                umma_f16_pair(d_tmem, ad + ((kk * UK * 128) >> 4), bd + ((kk * UK * 2) >> 4), idesc,
+                              (kb | kk) != 0 ? 1u : 0u);
+              }
             }
             umma_commit_pair(empty_bar(s));           // both CTAs' slots free once these MMAs retire
             if (kb + 1 == k_blocks) umma_commit_pair(tfull_bar(as));   // accumulator complete -> both epilogues
@@ -419,6 +437,19 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         }
         named_bar_sync(3, 32 * EPI_WARPS);
       }
+      float swg = 1.0f, swu = 1.0f;                    // FP8: this thread's feature's weight scales
+      float* sx_smem = reinterpret_cast<float*>(epi_smem + 4 * XCH_BYTES + 4 * STAGE_TILE_BYTES);   // FP8: [BN_MAX] token scales
+      if (FP8) {
+        const int n = c.f_tile * OUT_FEATS + feat0 + lane;                    // this thread's output feature
+        if (n < p.N) {
+          swg = __ldg(p.sw0 + static_cast<int64_t>(c.e) * p.N + n);
+          swu = __ldg(p.sw1 + static_cast<int64_t>(c.e) * p.N + n);
+        }
+        named_bar_sync(5, 32 * EPI_WARPS);             // every warp is done with the previous tile's token scales
+        for (int i = ew * 32 + lane; i < c.nt; i += 32 * EPI_WARPS)
+          sx_smem[i] = i < c.rows_valid ? __ldg(p.sx + c.row0 + i) : 0.0f;
+        named_bar_sync(5, 32 * EPI_WARPS);
+      }
       mbar_wait(tfull_bar(as), aph);
       tc_fence_after();
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + as * BN_MAX;
@@ -466,8 +497,13 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
               const uint32_t other[4] = {o.x, o.y, o.z, o.w};
               #pragma unroll
               for (int i = 0; i < 4; ++i) {
-                const float g = __uint_as_float(is_up ? other[i] : v0[j + i]);
-                const float u = __uint_as_float(is_up ? v1[j + i] : other[i]);
+                float g = __uint_as_float(is_up ? other[i] : v0[j + i]);
+                float u = __uint_as_float(is_up ? v1[j + i] : other[i]);
+                if (FP8) {                               // dequantise: sx[token] * sw[expert, feature] (reading F4)
+                  const float st = sx_smem[cc * 32 + j + i];
+                  g *= st * swg;
+                  u *= st * swu;
+                }
                 st_shared_bf16(stage_wr + (j + i) * 64, silu_mul(g, u));
               }
             }
@@ -521,6 +557,7 @@ Params make_params(const GemmLaunch& g) {
   p.w4d = g.w4d;
   p.sg_max = g.sg_max;
   p.tile_counter = g.tile_counter;
+  p.sx = g.sx; p.sw0 = g.sw0; p.sw1 = g.sw1;
   return p;
 }
 
@@ -529,11 +566,19 @@ Params make_params(const GemmLaunch& g) {
 cudaError_t pair_kernels_init() {
   cudaError_t e = cudaFuncSetAttribute(pair_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
   if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(pair_gemm_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(pair_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
 }
 
 cudaError_t launch_gateup_swiglu_pair(const GemmLaunch& g, cudaStream_t st) {
   launch_pdl(pair_gemm_kernel<true>, g.num_sms & ~1, 256, SMEM_BYTES, st, g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b1_4d : g.tm_b1, make_params(g));
+  return cudaGetLastError();
+}
+
+// FP8 gate/up: tm_act over the e4m3 rows [rows, K bytes], tm_b0 / tm_b1 over the quantised weights [E, N, K bytes]
+cudaError_t launch_gateup_swiglu_pair_fp8(const GemmLaunch& g, cudaStream_t st) {
+  launch_pdl(pair_gemm_kernel<true, true>, g.num_sms & ~1, 256, SMEM_BYTES, st, g.tm_act, g.tm_b0, g.tm_b1, make_params(g));
   return cudaGetLastError();
 }
 

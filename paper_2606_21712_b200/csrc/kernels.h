@@ -107,6 +107,14 @@ cudaError_t launch_gather(const void* hidden, const PermLaunch& pl, int T, int E
 cudaError_t launch_unpermute(const void* y_perm, const int32_t* inv_perm, const float* weights, int T, int k,
                              int d, void* out, int num_sms, cudaStream_t st, const SegTable* seg = nullptr);
 
+// ---- FP8 quantisation (fp8_quant.cu; readings F1-F3 of DESIGN.md §2)
+// W [E, K, N] bf16 -> Wq [E, N, K] e4m3 bytes + sw [E, N] fp32 (one scale per expert and output channel)
+cudaError_t launch_quantize_weights(const void* W, int E, int K, int N, void* Wq, float* sw, cudaStream_t st);
+// a5'' + a6 with quantisation: as launch_gather, but the k expert-order rows of a token are written as e4m3 bytes
+// xq_perm [T*k, d] with the token's fp32 scale in sx_perm [T*k]
+cudaError_t launch_gather_fp8(const void* hidden, const PermLaunch& pl, int T, int E, int k, int d, void* xq_perm,
+                              float* sx_perm, int num_sms, cudaStream_t st, const SegTable* seg = nullptr);
+
 // ---- grouped GEMM (grouped_gemm_pair.cu): steps a7 and a8
 // Activation tensor maps: the same [rows, K] bf16 matrix with TMA boxes of {64 k, 8 (i + 1) rows},
 // so that any token count that is a multiple of 8 (<= 128) is ONE TMA operation: the TMA unit's
@@ -129,10 +137,15 @@ struct GemmLaunch {
   int E, K, N;         // N = output columns (f for gate/up, d for down)
   void* out;           // bf16 [rows, N]
   const float* row_scale_perm;   // down GEMM, fused path: gate weights in expert order, w_perm[r] = topk_w[row_src[r]] (else nullptr)
+  // FP8 gate/up (launch_gateup_swiglu_pair_fp8): dequantisation scales
+  const float* sx = nullptr;     // [rows] per expert-order token row
+  const float* sw0 = nullptr;    // [E, N] W_gate, per expert and output channel
+  const float* sw1 = nullptr;    // [E, N] W_up
   int num_sms;
 };
 // CTA-pair kernels (grouped_gemm_pair.cu): weights on UMMA M (256 per pair), tokens on UMMA N.
 cudaError_t launch_gateup_swiglu_pair(const GemmLaunch& g, cudaStream_t st);
+cudaError_t launch_gateup_swiglu_pair_fp8(const GemmLaunch& g, cudaStream_t st);
 cudaError_t launch_down_pair(const GemmLaunch& g, cudaStream_t st);
 cudaError_t pair_kernels_init();
 

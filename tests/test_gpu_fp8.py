@@ -1,0 +1,132 @@
+"""GPU parity of the FP8 (e4m3) gate/up path (readings F1-F4 of DESIGN.md §2) against
+oracle/fp8.py, through the C ABI.
+
+Bars:
+  * quantisation codes and scales -- integer decisions taken in fp32 on both sides (F2, F3) -- bit-exact;
+  * layer output against the oracle that follows the SAME quantised definition in fp64: the bf16 path's bars
+    (max|err| <= 2e-2 max|ref|, rel L2 <= 5e-3): with exact e4m3 x e4m3 products and fp32 accumulation the only
+    roundings left are the bf16 path's (H, Y, out);
+  * against the UNQUANTISED oracle the distance is the quantisation error itself (3 mantissa bits on both operands of
+    the gate/up GEMM: ~2^-4 / sqrt(3) per operand relative, independent errors): reported, and bounded at 8e-2 rel L2
+    (DESIGN.md §3 derives the bar).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from oracle import fp8
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+MAX_TOL, L2_TOL = 2e-2, 5e-3
+
+
+def make(cfg):
+    from paper_2606_21712_b200 import MoELayer
+    lay = wl.make_layer(cfg)
+    g = {k: (v.cuda() if isinstance(v, torch.Tensor) else v) for k, v in lay.items()}
+    layer = MoELayer(cfg.d, cfg.f, cfg.E, cfg.k, max(cfg.T, 1))
+    layer.set_weights(g["W_r"], g["b_r"], g["W_gate"], g["W_up"], g["W_down"])
+    return lay, g, layer
+
+
+def f32(t):
+    return t.float().numpy()
+
+
+FP8_SHAPES = [
+    wl.small_config(T=256, d=512, E=8, k=2, f=1024, index=40, name="C1-like"),
+    wl.small_config(T=1, d=128, E=4, k=2, f=64, index=41, name="T1"),
+    wl.small_config(T=333, d=384, E=7, k=3, f=192, index=42, name="ragged"),
+    wl.small_config(T=700, d=256, E=130, k=8, f=128, index=43, name="E130"),
+    wl.small_config(T=1500, d=128, E=2, k=1, f=320, index=44, name="multi-tile"),
+]
+
+
+@pytest.mark.parametrize("cfg", FP8_SHAPES, ids=lambda c: c.name)
+def test_fp8_gateup_parity(cfg):
+    lay, g, layer = make(cfg)
+    out_bf16 = layer.combined_forward(g["hidden"]).clone()
+    layer.set_precision(1)
+    out = layer.combined_forward(g["hidden"]).clone()
+    out2 = layer.combined_forward(g["hidden"])
+    torch.cuda.synchronize()
+    assert torch.equal(out, out2), "FP8 path is not bitwise deterministic"
+    v = layer.debug_views(cfg.T)
+    q = layer.fp8_views(cfg.T)
+    L = v["logits"].cpu().numpy()
+    row_src, offsets = v["row_src"].cpu().numpy(), v["offsets"].cpu().numpy()
+    # ---- quantisation artefacts: bit-exact
+    x_perm = f32(lay["hidden"])[row_src // cfg.k]
+    xq_o, sx_o = fp8.quantize_rows(x_perm)
+    assert np.array_equal(q["sx_perm"].cpu().numpy(), sx_o), "activation scales differ"
+    assert np.array_equal(q["xq_perm"].cpu().numpy(), xq_o), "activation codes differ"
+    gq_o, sg_o = fp8.quantize_weight_channels(f32(lay["W_gate"]))
+    uq_o, su_o = fp8.quantize_weight_channels(f32(lay["W_up"]))
+    assert np.array_equal(q["sw_gate"].cpu().numpy(), sg_o) and np.array_equal(q["sw_up"].cpu().numpy(), su_o)
+    assert np.array_equal(q["q_gate"].cpu().numpy(), gq_o) and np.array_equal(q["q_up"].cpu().numpy(), uq_o)
+    # ---- output: the oracle of the quantised definition (fp64), routed by the GPU's logits, gate-weighted reduce
+    res = fp8.expert_ffn_fp8_gateup(x_perm, offsets, f32(lay["W_gate"]), f32(lay["W_up"]), f32(lay["W_down"]))
+    idx, w = oracle.topk_gate(L, cfg.k)
+    assert np.array_equal(v["idx"].cpu().numpy(), idx)
+    ref = oracle.unpermute(res["y"], v["inv_perm"].cpu().numpy(), w)
+    got = out.to(torch.float64).cpu().numpy()
+    scale = np.abs(ref).max()
+    max_err, l2 = np.abs(got - ref).max(), np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    assert max_err <= MAX_TOL * scale and l2 <= L2_TOL, (cfg.name, max_err / scale, l2)
+    # ---- distance to the unquantised layer: the quantisation error, reported and bounded
+    full = oracle.forward_batched(lay["hidden"], lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"], cfg.k,
+                                  logits_in=L)["out"]
+    l2_q = np.linalg.norm(got - full) / np.linalg.norm(full)
+    l2_b = np.linalg.norm(out_bf16.to(torch.float64).cpu().numpy() - full) / np.linalg.norm(full)
+    print(f"[fp8] {cfg.name}: vs quantised-definition oracle relL2 {l2:.2e} max {max_err / scale:.2e}; "
+          f"vs unquantised oracle relL2 {l2_q:.2e} (bf16 path {l2_b:.2e})")
+    assert l2_q <= 8e-2
+    # ---- back to bf16: same bits as before
+    layer.set_precision(0)
+    assert torch.equal(layer.combined_forward(g["hidden"]), out_bf16)
+
+
+def test_fp8_exactly_representable_inputs_equal_the_bf16_path():
+    """With activations and weights that sit on the e4m3 grid of their row / channel (scale a power of two), the
+    quantisation is lossless: the FP8 path must agree with the bf16 path to within the bf16 roundings of both."""
+    rng = np.random.default_rng(5)
+    T, d, E, k, f = 200, 256, 4, 2, 128
+    grid = fp8.e4m3_decode(np.arange(0x30, 0x46, dtype=np.uint8))
+    x = rng.choice(grid, size=(T, d)) * rng.choice([-1.0, 1.0], size=(T, d))
+    x[:, 0] = 3.5
+    Wg = rng.choice(grid, size=(E, d, f)) * rng.choice([-1.0, 1.0], size=(E, d, f)) / 256.0
+    Wu = rng.choice(grid, size=(E, d, f)) * rng.choice([-1.0, 1.0], size=(E, d, f)) / 256.0
+    Wg[:, 0, :] = 3.5 / 256.0
+    Wu[:, 0, :] = 3.5 / 256.0
+    tb = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(torch.bfloat16).cuda()
+    from paper_2606_21712_b200 import MoELayer
+    layer = MoELayer(d, f, E, k, T)
+    W_r = torch.randn(d, E, generator=torch.Generator().manual_seed(3)).cuda() / 16
+    Wd = (torch.randn(E, f, d, generator=torch.Generator().manual_seed(4)) * 0.05).to(torch.bfloat16).cuda()
+    layer.set_weights(W_r, None, tb(Wg), tb(Wu), Wd)
+    h = tb(x)
+    a = layer.combined_forward(h).clone()
+    layer.set_precision(1)
+    b = layer.combined_forward(h).clone()
+    torch.cuda.synchronize()
+    q = layer.fp8_views(T)
+    assert bool((q["sx_perm"] == 2.0 ** -7).all())
+    # both paths compute the same exact sums in fp32 (every product and partial sum is exact here): same bits
+    assert torch.equal(a, b)
+
+
+def test_fp8_argument_errors():
+    from paper_2606_21712_b200 import MoELayer, BgMoeError, BG_ERR_UNSUPPORTED, BG_ERR_NO_WEIGHTS
+    layer = MoELayer(192, 128, 4, 2, 16)                 # d % 128 != 0
+    with pytest.raises(BgMoeError) as ei:
+        layer.set_precision(1)
+    assert ei.value.status == BG_ERR_NO_WEIGHTS
+    cfg = wl.small_config(T=16, d=192, E=4, k=2, f=128, index=45)
+    g = {k_: (v.cuda() if isinstance(v, torch.Tensor) else v) for k_, v in wl.make_layer(cfg).items()}
+    layer.set_weights(g["W_r"], None, g["W_gate"], g["W_up"], g["W_down"])
+    with pytest.raises(BgMoeError) as ei:
+        layer.set_precision(1)
+    assert ei.value.status == BG_ERR_UNSUPPORTED
