@@ -18,7 +18,7 @@ import workloads as wl  # noqa: E402
 def declared_symbols():
     hdr = open(os.path.join(ROOT, "include", "bg_moe.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    return sorted(set(re.findall(r"\b(bg_moe_[a-z_]+)\s*\(", hdr)))
+    return sorted(set(re.findall(r"\b(bg_moe_[a-z0-9_]+)\s*\(", hdr)))
 
 
 def test_library_exports_every_declared_symbol():
