@@ -455,6 +455,59 @@ def run_c5_combine(steps: int, device_index: int):
     return res
 
 
+# ----------------------------------------------------------------------------- FP8 gate/up
+def run_fp8(steps: int, peaks: dict, device_index: int):
+    """the gate/up GEMM in FP8 (e4m3, W8A8, per-token x per-channel
+    scales; readings F1-F4), tcgen05 kind::f8f6f4.  Per configuration: step time and gate/up kernel time in bf16
+    and in FP8.  The FP8 gate/up kernel is scored against max(flops / (2 x the measured bf16 peak), bytes / BW): the
+    profiling guide's nominal fp8 : bf16 ratio applied to the measured bf16 number, with its algorithmic bytes
+    (1-byte weights and activations in, bf16 H out)."""
+    from paper_2606_21712_b200 import MoELayer
+    rows = []
+    for name in ("C2", "C3", "C5"):
+        cfg = wl.CONFIGS[name]
+        lay = wl.make_layer(cfg, "cuda")
+        layer = MoELayer(cfg.d, cfg.f, cfg.E, cfg.k, cfg.T, device=device_index)
+        layer.set_weights(lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"])
+        hidden, stream = lay["hidden"], torch.cuda.current_stream()
+        out = torch.empty_like(hidden)
+        step = lambda: layer.combined_forward(hidden, out, stream)
+        res = {}
+        for prec in (0, 1):
+            layer.set_precision(prec)
+            torch.cuda.synchronize()
+            time.sleep(1.0)
+            for _ in range(5):
+                step()
+            total, per = time_steps(step, steps, stream)
+            layer.profile_enable(True)
+            acc = {}
+            for _ in range(5):
+                step()
+                for k_, v in layer.profile_read().items():
+                    acc[k_] = acc.get(k_, 0.0) + v / 5
+            layer.profile_enable(False)
+            res[prec] = (total / steps, float(np.median(per)), acc)
+        counts = layer.debug_views(cfg.T)["counts"].cpu().numpy()
+        E_act = int((counts > 0).sum())
+        R = cfg.T * cfg.k
+        fl = 4.0 * R * cfg.d * cfg.f
+        by = 2.0 * cfg.d * cfg.f * E_act + 1.0 * R * cfg.d + 4.0 * R + 2.0 * R * cfg.f
+        t_bound = max(fl / (2 * peaks["bf16_tflops"] * 1e12), by / (peaks["hbm_gbs"] * 1e9))
+        gu8 = res[1][2]["gateup_swiglu"] * 1e-3
+        rows.append({"workload": cfg.name, "bf16_ms_per_step": res[0][0], "fp8_ms_per_step": res[1][0],
+                     "step_speedup": res[0][0] / res[1][0],
+                     "bf16_gateup_ms": res[0][2]["gateup_swiglu"], "fp8_gateup_ms": res[1][2]["gateup_swiglu"],
+                     "bf16_gather_ms": res[0][2]["gather"], "fp8_gather_ms": res[1][2]["gather"],
+                     "fp8_gateup_tflops": fl / gu8 / 1e12,
+                     "fp8_gateup_roofline": {"bound": "tensor" if fl / (2 * peaks["bf16_tflops"] * 1e12) >= by / (peaks["hbm_gbs"] * 1e9) else "hbm",
+                                             "frac": t_bound / gu8,
+                                             "peak": "2 x measured bf16 burst (guide's nominal fp8 : bf16 ratio)"}})
+        del layer, lay, hidden, out
+        torch.cuda.empty_cache()
+    return rows
+
+
 # ----------------------------------------------------------------------------- expert-weight ring buffer
 def run_ring(steps: int, device_index: int):
     """expert weights in pinned host memory, streamed through a device
@@ -631,6 +684,7 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_sweep:
         line["combine_c5"] = run_c5_combine(args.steps, local)
         line["ring_c3"] = run_ring(min(args.steps, 10), local)
+        line["fp8_gateup"] = run_fp8(args.steps, peaks, local)
         # every other BASELINE.json configuration through the same protocol (the north_star claim is "every
         # config"), and the sustained regime for the headline workload
         del layer
