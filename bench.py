@@ -294,6 +294,28 @@ def sustained_ms(fn, stream, seconds: float = 2.0, chunk: int = 10):
     return float(np.median(tail)), len(chunks) * chunk, float(sum(chunks) * chunk / 1e3)
 
 
+def stage_times(layer, step, rounds: int = 3, burst: int = 8) -> dict:
+    """Per-kernel durations from the library's own CUDA events (bg_moe_profile_enable): `burst` steps back to back
+    with the events recorded in-stream, the LAST call's events read once the burst has drained; median of `rounds`.
+    (The events between the kernels switch off their programmatic overlap, so the sum of the stages is a little
+    above the step time.)"""
+    runs = []
+    for _ in range(rounds):
+        # same starting condition as every timed leg: an idle (cool) GPU, then warm-up -- the part is power-managed,
+        # and kernels timed after seconds of back-to-back work belong to the sustained regime, not to this number
+        torch.cuda.synchronize()
+        time.sleep(1.0)
+        layer.profile_enable(False)
+        for _ in range(3):
+            step()
+        layer.profile_enable(True)
+        for _ in range(burst):
+            step()
+        runs.append(layer.profile_read())
+    layer.profile_enable(False)
+    return {k_: float(np.median([r[k_] for r in runs])) for k_ in runs[0]}
+
+
 def layer_fracs(cfg: wl.MoEConfig, E_act: int, ms: float, peaks: dict) -> dict:
     F, B = cfg.flops(), cfg.min_bytes(E_act)
     t_f, t_b = F / (peaks["bf16_tflops"] * 1e12), B / (peaks["hbm_gbs"] * 1e9)
@@ -329,14 +351,7 @@ def run_config(name: str, steps: int, peaks: dict, device_index: int, sustained:
     ms = total / steps
     row = {"workload": cfg.name, "T": cfg.T, "E_active": E_act, "ms_per_step": ms, "ms_min": float(min(per)),
            "ms_median": float(np.median(per)), **layer_fracs(cfg, E_act, ms, peaks)}
-    layer.profile_enable(True)
-    acc = {}
-    for _ in range(min(steps, 10)):
-        step()
-        for k_, v in layer.profile_read().items():
-            acc[k_] = acc.get(k_, 0.0) + v / min(steps, 10)
-    layer.profile_enable(False)
-    row["stage_ms"] = acc
+    row["stage_ms"] = stage_times(layer, step)
     if sustained:
         sm, n, secs = sustained_ms(step, stream)
         fr = layer_fracs(cfg, E_act, sm, peaks)
@@ -384,10 +399,7 @@ def run_c3_sweep(steps: int, peaks: dict, device_index: int):
         E_act = int((counts > 0).sum())
         row = {"T": T, "ms_per_step": ms, "ms_min": float(min(per)), "ms_median": float(np.median(per)),
                "E_active": E_act, **layer_fracs(cfg, E_act, ms, peaks)}
-        layer.profile_enable(True)
-        step()
-        row["stage_ms"] = layer.profile_read()
-        layer.profile_enable(False)
+        row["stage_ms"] = stage_times(layer, step)
         if T == 16384:
             sm, n, secs = sustained_ms(step, stream)
             fr = layer_fracs(cfg, E_act, sm, peaks)
@@ -480,14 +492,7 @@ def run_fp8(steps: int, peaks: dict, device_index: int):
             for _ in range(5):
                 step()
             total, per = time_steps(step, steps, stream)
-            layer.profile_enable(True)
-            acc = {}
-            for _ in range(5):
-                step()
-                for k_, v in layer.profile_read().items():
-                    acc[k_] = acc.get(k_, 0.0) + v / 5
-            layer.profile_enable(False)
-            res[prec] = (total / steps, float(np.median(per)), acc)
+            res[prec] = (total / steps, float(np.median(per)), stage_times(layer, step))
         counts = layer.debug_views(cfg.T)["counts"].cpu().numpy()
         E_act = int((counts > 0).sum())
         R = cfg.T * cfg.k
@@ -576,6 +581,8 @@ def run_ours(args):
         lay["hidden"] = lay["hidden"].roll(17 * rank, dims=0).contiguous()   # each replica: its own tokens
     layer = MoELayer(cfg.d, cfg.f, cfg.E, cfg.k, cfg.T, device=local)
     layer.set_weights(lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"])
+    if args.fp8:
+        layer.set_precision(1)
     hidden = lay["hidden"]
     out = torch.empty_like(hidden)
     stream = torch.cuda.current_stream()
@@ -607,19 +614,14 @@ def run_ours(args):
     h_host = hidden.cpu().pin_memory()
     o_host = torch.empty_like(h_host).pin_memory()
     e2e_step = lambda: layer.combined_forward_host(h_host, o_host, stream)
+    torch.cuda.synchronize()
+    time.sleep(1.0)
     for _ in range(3):
         e2e_step()
     ms_e2e = timed(e2e_step, args.steps)[0] / args.steps
 
     # ---- per-kernel durations (CUDA events recorded by the library on the launching stream)
-    layer.profile_enable(True)
-    acc = {}
-    for _ in range(args.steps):
-        step()
-        for k_, v in layer.profile_read().items():
-            acc[k_] = acc.get(k_, 0.0) + v
-    layer.profile_enable(False)
-    stage_ms = {k_: v / args.steps for k_, v in acc.items()}
+    stage_ms = stage_times(layer, step, rounds=3, burst=max(4, min(args.steps, 8)))
 
     views = layer.debug_views(cfg.T)
     counts = views["counts"].cpu().numpy()
@@ -653,7 +655,7 @@ def run_ours(args):
     line = {
         "metric": METRIC, "value": tflops, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "vs_baseline": None, "dtype": "fp8-gateup/bf16" if args.fp8 else "bf16", "data": "synthetic",
         "config": config_keys(cfg),
         "load": {"E_active": E_act, "rows_per_expert_min_max": [int(counts.min()), int(counts.max())],
                  "parallelism": "replicas" if world > 1 else "single-gpu"},
@@ -722,6 +724,8 @@ def main():
     ap.add_argument("--T", type=int, default=0, help="override the combined-token count (C3 sweep)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the C3 combine-size sweep (sweep_c3 key)")
+    ap.add_argument("--fp8", action="store_true", help="run the gate/up GEMM in FP8 (bg_moe_set_precision 1); "
+                    "the line is then labelled dtype fp8-gateup/bf16 and is NOT the BASELINE.json bf16 metric")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
