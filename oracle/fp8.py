@@ -17,8 +17,10 @@ the quantisation recipe.  Reading taken (F1-F4):
   F4  scope: the gate/up GEMM (two thirds of the expert FLOPs and weight bytes) runs W8A8:
         g[r,n] = sx[r] * sw_gate[e,n] * sum_k xq[r,k] * Wq_gate[e,n,k]      (products exact, fp32 accumulate on the GPU)
         u[r,n] likewise;  H = silu(g) * u;  Y = H W_down[e] with H and W_down in bf16 as before.
-      H's own per-row scale would need a second pass over H (its row maximum is only known after all feature
-      tiles), or block-scaled MMA; the down GEMM stays bf16.
+      (precision 1: H and the down GEMM stay bf16.)
+  F5  precision 2 adds the down GEMM: H is first rounded to bf16 as in every other path (RNE), then quantised like an
+      activation row (F2: sh[r] = fl32(max_n |Hb[r,n]| / 448), Hq = e4m3(fl32(Hb / sh))), W_down per expert and output
+      channel (F3, stored [E, d, f]), and  Y[r,j] = sh[r] * sw_down[e,j] * sum_n Hq[r,n] * Wq_down[e,j,n].
 
 Every floating-point step of the reference GEMMs is fp64 on exactly decoded values, with no intermediate rounding
 (as in bgo_oracle.cpp); only the quantisation decisions are taken in fp32, as F2 / F3 state.
@@ -108,6 +110,31 @@ def quantize_weight_channels(W: np.ndarray):
 
 def _silu(z: np.ndarray) -> np.ndarray:
     return z / (1.0 + np.exp(-z))
+
+
+def round_bf16(a: np.ndarray) -> np.ndarray:
+    """Round-to-nearest-even of float64 / float32 values to bf16, returned as float32 (exact bit arithmetic on the
+    float32 rounding of the input; the inputs here are far from the float32 rounding boundary cases that would make
+    the double rounding visible -- and the GPU's H is compared through its own bits anyway, reading F5)."""
+    x = np.ascontiguousarray(a, dtype=np.float32)
+    u = x.view(np.uint32).astype(np.uint64)
+    r = ((u + 0x7FFF + ((u >> 16) & 1)) >> 16) << 16
+    return r.astype(np.uint32).view(np.float32).reshape(x.shape)
+
+
+def down_fp8(H_bf16: np.ndarray, offsets: np.ndarray, W_down: np.ndarray) -> dict:
+    """F5.  H_bf16 float32 [R, f] (bf16 values), W_down float32 [E, f, d].  Returns y float64 [R, d] + artefacts."""
+    R, f = H_bf16.shape
+    E, _, d = W_down.shape
+    hq, sh = quantize_rows(H_bf16)
+    dq, sd = quantize_weight_channels(W_down)              # [E, d, f], [E, d]
+    hd = e4m3_decode(hq)
+    y = np.zeros((R, d), np.float64)
+    for e in range(E):
+        r0, r1 = int(offsets[e]), int(offsets[e + 1])
+        if r1 > r0:
+            y[r0:r1] = (hd[r0:r1] @ e4m3_decode(dq[e]).T) * sh[r0:r1, None].astype(np.float64) * sd[e][None, :].astype(np.float64)
+    return dict(y=y, hq=hq, sh=sh, dq=dq, sd=sd)
 
 
 def expert_ffn_fp8_gateup(x_perm: np.ndarray, offsets: np.ndarray, W_gate: np.ndarray, W_up: np.ndarray,

@@ -133,3 +133,36 @@ def test_exactly_representable_data_reduces_to_the_bf16_oracle():
     assert np.all(res["sx"] == np.float32(2.0 ** -7))
     ref = oracle.expert_ffn(xb, off, Wgb, Wub, Wdb)
     assert np.max(np.abs(res["y"] - ref)) <= 1e-12 * np.max(np.abs(ref))
+
+
+def test_round_bf16_matches_torch():
+    rng = np.random.default_rng(6)
+    x = np.concatenate([rng.standard_normal(50000) * s for s in (1e-4, 1.0, 300.0)]).astype(np.float32)
+    x = np.concatenate([x, np.array([1.00390625, 1.01171875, -1.00390625, 0.0, -0.0], np.float32)])   # exact ties
+    ref = torch.from_numpy(x).to(torch.bfloat16).float().numpy()
+    assert np.array_equal(fp8.round_bf16(x).view(np.uint32), ref.view(np.uint32))
+
+
+def test_down_fp8_against_a_pure_python_loop_and_lossless_case():
+    rng = np.random.default_rng(7)
+    R, f, d, E = 6, 12, 8, 2
+    H = fp8.round_bf16(rng.standard_normal((R, f)))
+    Wd = fp8.round_bf16(rng.standard_normal((E, f, d)) * 0.2)
+    off = np.array([0, 2, 6])
+    res = fp8.down_fp8(H, off, Wd)
+    tab = fp8.e4m3_decode_table()
+    for r in range(R):
+        e = 0 if r < 2 else 1
+        for j in range(d):
+            acc = sum(tab[res["hq"][r, n]] * tab[res["dq"][e, j, n]] for n in range(f))
+            want = acc * float(res["sh"][r]) * float(res["sd"][e, j])
+            assert abs(want - res["y"][r, j]) <= 1e-12 * max(1.0, abs(want))
+    # lossless case: values on the e4m3 grid with power-of-two scales -> the plain fp64 product
+    grid = fp8.e4m3_decode(np.arange(0x30, 0x46, dtype=np.uint8))
+    H = rng.choice(grid, size=(R, f)) * rng.choice([-1.0, 1.0], size=(R, f))
+    H[:, 0] = 3.5
+    Wd = rng.choice(grid, size=(E, f, d)) * rng.choice([-1.0, 1.0], size=(E, f, d)) / 32.0
+    Wd[:, 0, :] = 3.5 / 32.0
+    res = fp8.down_fp8(H.astype(np.float32), off, Wd.astype(np.float32))
+    for e, (r0, r1) in enumerate(((0, 2), (2, 6))):
+        assert np.max(np.abs(res["y"][r0:r1] - H[r0:r1] @ Wd[e])) <= 1e-12
