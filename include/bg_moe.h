@@ -98,17 +98,24 @@ int64_t bg_moe_ring_bytes_per_call(const bg_moe_ctx* ctx);
  * of DESIGN.md §2: OCP e4m3, round-to-nearest-even, saturating; activations one fp32 scale per token row
  * (max|x| / 448), weights one fp32 scale per expert and output channel; the gate/up GEMM runs W8A8 on
  * tcgen05 kind::f8f6f4 with fp32 accumulation and the scales applied in its epilogue before the SwiGLU; H and the
- * down GEMM stay bf16.
- *   precision 0: bf16 (default);  1: FP8 gate/up.
- * Switching to 1 quantises the resident bf16 W_gate / W_up on `stream` into library-owned buffers ([E, f, d] e4m3
- * bytes + [E, f] scales; 2 E d f bytes, allocated at the first switch) -- call it again after bg_moe_set_weights.
- * It applies to the fused calls (bg_moe_combined_forward and its _segments / _host forms); the split calls and the
- * offloaded-weights path stay bf16.  BG_ERR_UNSUPPORTED unless d % 128 == 0 and f % 64 == 0. */
+ * down GEMM stay bf16 (precision 1).  Precision 2 (reading F5) runs the down GEMM W8A8 as well: the gate/up epilogue
+ * keeps the row maximum of |H| (integer max on float bits: order-independent), a quantising pass turns the bf16 H
+ * into e4m3 rows with one scale per row, W_down is quantised per expert and output channel.
+ *   precision 0: bf16 (default);  1: FP8 gate/up;  2: FP8 gate/up and down.
+ * Switching to 1 / 2 quantises the resident bf16 weights on `stream` into library-owned buffers ([E, f, d] / [E, d, f]
+ * e4m3 bytes + per-channel scales; 3 E d f bytes, allocated at the first switch) -- call it again after
+ * bg_moe_set_weights.  It applies to the fused calls (bg_moe_combined_forward and its _segments / _host forms); the
+ * split calls and the offloaded-weights path stay bf16.  BG_ERR_UNSUPPORTED unless d % 128 == 0 and f % 64 == 0
+ * (precision 2: f % 128 == 0). */
 int bg_moe_set_precision(bg_moe_ctx* ctx, int32_t precision, void* stream);
 /* Device pointers to the FP8 artefacts of the last fused call / last quantisation (any out-pointer may be NULL):
  * xq_perm e4m3 [T*k, d] and sx_perm fp32 [T*k] in expert order; q_gate / q_up e4m3 [E, f, d]; sw_gate / sw_up fp32 [E, f]. */
 int bg_moe_debug_fp8_views(bg_moe_ctx* ctx, const void** xq_perm, const float** sx_perm, const void** q_gate,
                            const float** sw_gate, const void** q_up, const float** sw_up);
+/* Precision 2: H bf16 [T*k, f] (workspace), its codes hq e4m3 [T*k, f] and scales sh_perm fp32 [T*k] of the last fused
+ * call; q_down e4m3 [E, d, f], sw_down fp32 [E, d]. */
+int bg_moe_debug_fp8_down_views(bg_moe_ctx* ctx, const void** H, const void** hq, const float** sh_perm,
+                                const void** q_down, const float** sw_down);
 
 /* Debug / test switches of the grouped-GEMM tile scheduler; production never calls this.
  *   static_tile_feed != 0     tile t -> cluster (t mod #clusters) instead of the dynamic ticket feed

@@ -15,7 +15,7 @@ BG_OK, BG_ERR_INVALID_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA, BG_ERR_NOMEM, BG_ERR
 EXPORTS = ["bg_moe_create", "bg_moe_destroy", "bg_moe_set_weights", "bg_moe_route", "bg_moe_permute",
            "bg_moe_expert_ffn", "bg_moe_unpermute", "bg_moe_combined_forward", "bg_moe_combined_forward_host",
            "bg_moe_debug_views", "bg_moe_profile_enable", "bg_moe_profile_read", "bg_moe_launch_count", "bg_moe_workspace_bytes", "bg_moe_strerror",
-           "bg_moe_last_error", "bg_moe_set_debug", "bg_moe_set_weights_offloaded", "bg_moe_ring_bytes_per_call", "bg_moe_set_precision", "bg_moe_debug_fp8_views", "bg_moe_combined_forward_segments", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens"]
+           "bg_moe_last_error", "bg_moe_set_debug", "bg_moe_set_weights_offloaded", "bg_moe_ring_bytes_per_call", "bg_moe_set_precision", "bg_moe_debug_fp8_views", "bg_moe_debug_fp8_down_views", "bg_moe_combined_forward_segments", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens"]
 
 
 class BgMoeConfig(ctypes.Structure):
@@ -53,6 +53,7 @@ def load_library() -> ctypes.CDLL:
         lib.bg_moe_ring_bytes_per_call.restype = i64
         lib.bg_moe_set_precision.argtypes = [vp, i32, vp]
         lib.bg_moe_debug_fp8_views.argtypes = [vp] + [ctypes.POINTER(vp)] * 6
+        lib.bg_moe_debug_fp8_down_views.argtypes = [vp] + [ctypes.POINTER(vp)] * 5
         lib.bg_moe_route.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
         lib.bg_moe_permute.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp]
         lib.bg_moe_expert_ffn.argtypes = [vp, vp, vp, i32, vp, vp]
@@ -171,6 +172,19 @@ class MoELayer:
         out = {}
         for p, (name, ts, shape) in zip(ptrs, spec):
             out[name] = torch.as_tensor(_DeviceArray(p.value, shape, ts), device=self._dev()).clone()
+        return out
+
+    def fp8_down_views(self, T: int) -> dict:
+        """Precision-2 artefacts of the last fused call (H as bf16, codes as uint8)."""
+        ptrs = [ctypes.c_void_p() for _ in range(5)]
+        self._check(self.lib.bg_moe_debug_fp8_down_views(self._ctx, *[ctypes.byref(p) for p in ptrs]))
+        R = T * self.k
+        spec = [("H", "<u2", (R, self.f)), ("hq", "|u1", (R, self.f)), ("sh_perm", "<f4", (R,)),
+                ("q_down", "|u1", (self.E, self.d, self.f)), ("sw_down", "<f4", (self.E, self.d))]
+        out = {}
+        for p, (name, ts, shape) in zip(ptrs, spec):
+            t = torch.as_tensor(_DeviceArray(p.value, shape, ts), device=self._dev()).clone()
+            out[name] = t.view(torch.bfloat16) if name == "H" else t
         return out
 
     @property

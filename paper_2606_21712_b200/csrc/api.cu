@@ -64,7 +64,7 @@ struct bg_moe_ctx {
   } wm[3];
   // FP8 gate/up (bg_moe_set_precision; readings F1-F4): quantised weights [E, f, d] bytes + per-channel scales,
   // the quantised expert-order rows + per-row scales, and their tensor maps
-  int precision = 0;                  // 0 = bf16, 1 = FP8 gate/up
+  int precision = 0;                  // 0 = bf16, 1 = FP8 gate/up, 2 = FP8 gate/up + down
   uint8_t* fp8_buf = nullptr;         // one set-up time allocation
   uint8_t* q_gate = nullptr;
   uint8_t* q_up = nullptr;
@@ -74,6 +74,15 @@ struct bg_moe_ctx {
   float* sx_perm = nullptr;
   CUtensorMap tm_qg, tm_qu;
   bg::ActMaps am_xq;
+  // precision 2 (reading F5): quantised W_down [E, d, f] + scales, quantised H rows + row factors
+  uint8_t* q_down = nullptr;
+  float* sw_down = nullptr;
+  uint8_t* hq = nullptr;
+  unsigned* hmax = nullptr;
+  float* sh_perm = nullptr;
+  float* sc_perm = nullptr;
+  CUtensorMap tm_qd;
+  bg::ActMaps am_hq;
   // expert-weight ring buffer (bg_moe_set_weights_offloaded; "ring parameter buffer")
   const uint8_t* host_wg = nullptr;   // HOST (pinned) [E,d,f], [E,d,f], [E,f,d] bf16
   const uint8_t* host_wu = nullptr;
@@ -174,12 +183,12 @@ bool encode_act_map_u8(CUtensorMap* tm, const void* ptr, int64_t rows, int64_t K
 }
 
 // quantised weights [E, N, K] e4m3 bytes (k contiguous), box {128 k, 64 n, 1 expert}, 128B swizzle.
-bool encode_weight_map_u8(CUtensorMap* tm, const void* ptr, int64_t E, int64_t N, int64_t K) {
+bool encode_weight_map_u8(CUtensorMap* tm, const void* ptr, int64_t E, int64_t N, int64_t K, int box_rows = 64) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return false;
   cuuint64_t dims[3] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(N), static_cast<cuuint64_t>(E)};
   cuuint64_t strides[2] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(N) * K};
-  cuuint32_t box[3] = {128, 64, 1};
+  cuuint32_t box[3] = {128, static_cast<cuuint32_t>(box_rows), 1};
   cuuint32_t estr[3] = {1, 1, 1};
   return fn(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(ptr), dims, strides, box, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -312,12 +321,14 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g1.out = ctx->H;
   g1.row_scale_perm = nullptr;
   g1.num_sms = ctx->num_sms;
-  if (ctx->precision == 1 && x_perm == ctx->x_perm && which_maps == 0) {
+  const bool fp8 = ctx->precision >= 1 && x_perm == ctx->x_perm && which_maps == 0;
+  if (fp8) {
     // FP8 gate/up (fused path): the gather wrote e4m3 rows + scales instead of x_perm
     g1.tm_act = ctx->am_xq;
     g1.tm_b0 = ctx->tm_qg;
     g1.tm_b1 = ctx->tm_qu;
     g1.sx = ctx->sx_perm; g1.sw0 = ctx->sw_gate; g1.sw1 = ctx->sw_up;
+    g1.hmax = ctx->precision == 2 ? ctx->hmax : nullptr;
     BG_LAUNCH(ctx, bg::launch_gateup_swiglu_pair_fp8(g1, st), "gateup_swiglu_fp8");
   } else {
     BG_LAUNCH(ctx, bg::launch_gateup_swiglu_pair(g1, st), "gateup_swiglu");
@@ -337,7 +348,18 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
   g2.out = y;
   g2.row_scale_perm = row_scale_perm;
   g2.num_sms = ctx->num_sms;
-  BG_LAUNCH(ctx, bg::launch_down_pair(g2, st), "down");
+  if (fp8 && ctx->precision == 2) {
+    // FP8 down GEMM (reading F5): quantise H with its per-row scale, then W8A8 with the row factor sh * gate weight
+    BG_LAUNCH(ctx, bg::launch_quantize_h(ctx->H, ctx->hmax, row_scale_perm, R, c.f, ctx->hq, ctx->sh_perm, ctx->sc_perm,
+                                         ctx->num_sms, st), "quantize_h");
+    g2.tm_act = ctx->am_hq;
+    g2.tm_b0 = ctx->tm_qd;
+    g2.row_scale_perm = ctx->sc_perm;
+    g2.sw0 = ctx->sw_down;
+    BG_LAUNCH(ctx, bg::launch_down_pair_fp8(g2, st), "down_fp8");
+  } else {
+    BG_LAUNCH(ctx, bg::launch_down_pair(g2, st), "down");
+  }
   return BG_OK;
 }
 
@@ -388,8 +410,9 @@ int do_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void* out, cudaSt
   mark(ctx, 1, st);
   bg::PermLaunch pl = {ctx->topk_idx, ctx->tile_rank, ctx->tile_base, ctx->topk_w, ctx->row_src, ctx->inv_perm,
                        ctx->w_perm};
-  if (ctx->precision == 1)
-    BG_LAUNCH(ctx, bg::launch_gather_fp8(hidden, pl, T, c.E, c.k, c.d, ctx->xq_perm, ctx->sx_perm, ctx->num_sms, st, seg),
+  if (ctx->precision >= 1)
+    BG_LAUNCH(ctx, bg::launch_gather_fp8(hidden, pl, T, c.E, c.k, c.d, ctx->xq_perm, ctx->sx_perm,
+                                         ctx->precision == 2 ? ctx->hmax : nullptr, ctx->num_sms, st, seg),
               "gather_fp8");
   else
     BG_LAUNCH(ctx, bg::launch_gather(hidden, pl, T, c.E, c.k, c.d, ctx->x_perm, ctx->num_sms, st, seg), "gather");
@@ -678,35 +701,46 @@ int bg_moe_set_weights_offloaded(bg_moe_ctx* ctx, const float* W_r, const float*
 int64_t bg_moe_ring_bytes_per_call(const bg_moe_ctx* ctx) { return ctx ? ctx->ring_h2d_bytes : 0; }
 
 int bg_moe_set_precision(bg_moe_ctx* ctx, int32_t precision, void* stream) {
-  if (ctx == nullptr || precision < 0 || precision > 1) return BG_ERR_INVALID_ARG;
+  if (ctx == nullptr || precision < 0 || precision > 2) return BG_ERR_INVALID_ARG;
   if (precision == 0) { ctx->precision = 0; return BG_OK; }
   const bg_moe_config& c = ctx->cfg;
   if (ctx->W_gate == nullptr || ctx->ring_chunk != 0) return BG_ERR_NO_WEIGHTS;     // needs resident bf16 weights
   if (c.d % 128 != 0 || c.f % 64 != 0) return BG_ERR_UNSUPPORTED;                    // 128-byte k-blocks, 64-feature boxes
+  if (precision == 2 && c.f % 128 != 0) return BG_ERR_UNSUPPORTED;                   // the down GEMM's k is f
   DeviceGuard guard(c.device);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const int64_t Tm = c.max_tokens > 0 ? c.max_tokens : 1;
   const int64_t Rm = Tm * c.k;
   if (ctx->fp8_buf == nullptr) {
-    // set-up time allocation (like the ring): 2 E d f bytes of codes, scales, and the quantised rows
+    // set-up time allocation (like the ring): 3 E d f bytes of codes, scales, and the quantised rows
     auto up = [](int64_t v) { return (v + 1023) / 1024 * 1024; };
-    const int64_t wq = up(static_cast<int64_t>(c.E) * c.d * c.f), sw = up(static_cast<int64_t>(c.E) * c.f * 4);
-    const int64_t xq = up(Rm * c.d), sx = up(Rm * 4);
+    const int64_t wq = up(static_cast<int64_t>(c.E) * c.d * c.f);
+    const int64_t swf = up(static_cast<int64_t>(c.E) * c.f * 4), swd = up(static_cast<int64_t>(c.E) * c.d * 4);
+    const int64_t xq = up(Rm * c.d), hq = up(Rm * c.f), rv = up(Rm * 4);
     void* p = nullptr;
-    if (cudaMalloc(&p, static_cast<size_t>(2 * wq + 2 * sw + xq + sx)) != cudaSuccess) {
+    if (cudaMalloc(&p, static_cast<size_t>(3 * wq + 2 * swf + swd + xq + hq + 4 * rv)) != cudaSuccess) {
       cudaGetLastError();
       return BG_ERR_NOMEM;
     }
-    ctx->fp8_buf = static_cast<uint8_t*>(p);
-    ctx->q_gate = ctx->fp8_buf;
-    ctx->q_up = ctx->q_gate + wq;
-    ctx->sw_gate = reinterpret_cast<float*>(ctx->q_up + wq);
-    ctx->sw_up = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(ctx->sw_gate) + sw);
-    ctx->xq_perm = reinterpret_cast<uint8_t*>(ctx->sw_up) + sw;
-    ctx->sx_perm = reinterpret_cast<float*>(ctx->xq_perm + xq);
+    uint8_t* b = static_cast<uint8_t*>(p);
+    ctx->fp8_buf = b;
+    ctx->q_gate = b; b += wq;
+    ctx->q_up = b; b += wq;
+    ctx->q_down = b; b += wq;
+    ctx->sw_gate = reinterpret_cast<float*>(b); b += swf;
+    ctx->sw_up = reinterpret_cast<float*>(b); b += swf;
+    ctx->sw_down = reinterpret_cast<float*>(b); b += swd;
+    ctx->xq_perm = b; b += xq;
+    ctx->hq = b; b += hq;
+    ctx->sx_perm = reinterpret_cast<float*>(b); b += rv;
+    ctx->hmax = reinterpret_cast<unsigned*>(b); b += rv;
+    ctx->sh_perm = reinterpret_cast<float*>(b); b += rv;
+    ctx->sc_perm = reinterpret_cast<float*>(b); b += rv;
     bool ok = encode_weight_map_u8(&ctx->tm_qg, ctx->q_gate, c.E, c.f, c.d) &&
-              encode_weight_map_u8(&ctx->tm_qu, ctx->q_up, c.E, c.f, c.d);
+              encode_weight_map_u8(&ctx->tm_qu, ctx->q_up, c.E, c.f, c.d) &&
+              (c.f % 128 != 0 || encode_weight_map_u8(&ctx->tm_qd, ctx->q_down, c.E, c.d, c.f, 128));
     for (int i = 0; i < 16 && ok; ++i) ok = encode_act_map_u8(&ctx->am_xq.m[i], ctx->xq_perm, Rm, c.d, 8 * (i + 1));
+    for (int i = 0; i < 16 && ok && c.f % 128 == 0; ++i) ok = encode_act_map_u8(&ctx->am_hq.m[i], ctx->hq, Rm, c.f, 8 * (i + 1));
     if (!ok) {
       ctx->last_error = "cuTensorMapEncodeTiled(fp8) failed";
       return BG_ERR_CUDA;
@@ -716,8 +750,21 @@ int bg_moe_set_precision(bg_moe_ctx* ctx, int32_t precision, void* stream) {
   if (rc) return rc;
   BG_LAUNCH(ctx, bg::launch_quantize_weights(ctx->W_gate, c.E, c.d, c.f, ctx->q_gate, ctx->sw_gate, st), "quantize W_gate");
   BG_LAUNCH(ctx, bg::launch_quantize_weights(ctx->W_up, c.E, c.d, c.f, ctx->q_up, ctx->sw_up, st), "quantize W_up");
-  ctx->precision = 1;
+  if (precision == 2)
+    BG_LAUNCH(ctx, bg::launch_quantize_weights(ctx->W_down, c.E, c.f, c.d, ctx->q_down, ctx->sw_down, st), "quantize W_down");
+  ctx->precision = precision;
   return end_call(ctx, st, false);
+}
+
+int bg_moe_debug_fp8_down_views(bg_moe_ctx* ctx, const void** H, const void** hq, const float** sh_perm,
+                                const void** q_down, const float** sw_down) {
+  if (!ctx || ctx->fp8_buf == nullptr) return BG_ERR_INVALID_ARG;
+  if (H) *H = ctx->H;
+  if (hq) *hq = ctx->hq;
+  if (sh_perm) *sh_perm = ctx->sh_perm;
+  if (q_down) *q_down = ctx->q_down;
+  if (sw_down) *sw_down = ctx->sw_down;
+  return BG_OK;
 }
 
 int bg_moe_debug_fp8_views(bg_moe_ctx* ctx, const void** xq_perm, const float** sx_perm, const void** q_gate,

@@ -84,7 +84,8 @@ struct PermArgs {
 template <int KMAX>
 __global__ void __launch_bounds__(256) gather_fp8_kernel(const uint4* __restrict__ hidden, const PermArgs pa, int T, int k,
                                                          int vec_per_row, uint2* __restrict__ xq_perm,
-                                                         float* __restrict__ sx_perm, const SegTable seg) {
+                                                         float* __restrict__ sx_perm, unsigned* __restrict__ hmax,
+                                                         const SegTable seg) {
   pdl_wait_then_trigger();
   const int lane = threadIdx.x & 31;
   const int warps_total = gridDim.x * (blockDim.x >> 5);
@@ -128,7 +129,10 @@ __global__ void __launch_bounds__(256) gather_fp8_kernel(const uint4* __restrict
       const int rs = __shfl_sync(0xffffffffu, r, s);
       ok[s] = s < k && rs >= 0;
       dst[s] = xq_perm + static_cast<int64_t>(ok[s] ? rs : 0) * vec_per_row;
-      if (ok[s] && lane == 0) sx_perm[rs] = sx;
+      if (ok[s] && lane == 0) {
+        sx_perm[rs] = sx;
+        if (hmax != nullptr) hmax[rs] = 0u;
+      }
     }
     // pass 2: quantise 8 values per vector -> 8 bytes
     for (int c = lane; c < vec_per_row; c += 32) {
@@ -148,7 +152,49 @@ __global__ void __launch_bounds__(256) gather_fp8_kernel(const uint4* __restrict
   }
 }
 
+// ---- H rows (reading F5): one warp per expert-order row
+__global__ void __launch_bounds__(256) quantize_h_kernel(const uint4* __restrict__ H, const unsigned* __restrict__ hmax,
+                                                         const float* __restrict__ w_perm, int64_t rows, int vec_per_row,
+                                                         uint2* __restrict__ Hq, float* __restrict__ sh,
+                                                         float* __restrict__ sc) {
+  pdl_wait_then_trigger();
+  const int lane = threadIdx.x & 31;
+  const int64_t warps_total = static_cast<int64_t>(gridDim.x) * (blockDim.x >> 5);
+  for (int64_t r = static_cast<int64_t>(blockIdx.x) * (blockDim.x >> 5) + (threadIdx.x >> 5); r < rows; r += warps_total) {
+    const float amax = __uint_as_float(__ldg(hmax + r));
+    const float s = amax == 0.0f ? 1.0f : __fdiv_rn(amax, 448.0f);
+    if (lane == 0) {
+      sh[r] = s;
+      sc[r] = w_perm != nullptr ? s * __ldg(w_perm + r) : s;
+    }
+    const uint4* src = H + r * vec_per_row;
+    uint2* dst = Hq + r * vec_per_row;
+    for (int c = lane; c < vec_per_row; c += 32) {
+      const uint4 a = __ldg(src + c);
+      const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&a);
+      uint32_t w[2] = {0u, 0u};
+      #pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const float2 f = __bfloat1622float2(h[i]);
+        const uint32_t lo = to_e4m3(__fdiv_rn(f.x, s)), hi = to_e4m3(__fdiv_rn(f.y, s));
+        w[i >> 1] |= (lo | (hi << 8)) << (16 * (i & 1));
+      }
+      dst[c] = make_uint2(w[0], w[1]);
+    }
+  }
+}
+
 }  // namespace
+
+cudaError_t launch_quantize_h(const void* H, const unsigned* hmax, const float* w_perm, int64_t rows, int f, void* Hq,
+                              float* sh, float* sc, int num_sms, cudaStream_t st) {
+  if (rows == 0) return cudaSuccess;
+  const int64_t blocks_needed = (rows + 7) / 8, cap = static_cast<int64_t>(num_sms) * 8;
+  const int grid = static_cast<int>(blocks_needed < cap ? blocks_needed : cap);
+  launch_pdl(quantize_h_kernel, grid, 256, 0, st, static_cast<const uint4*>(H), hmax, w_perm, rows, f / 8,
+             static_cast<uint2*>(Hq), sh, sc);
+  return cudaGetLastError();
+}
 
 cudaError_t launch_quantize_weights(const void* W, int E, int K, int N, void* Wq, float* sw, cudaStream_t st) {
   dim3 grid((N + 31) / 32, E);
@@ -157,7 +203,7 @@ cudaError_t launch_quantize_weights(const void* W, int E, int K, int N, void* Wq
 }
 
 cudaError_t launch_gather_fp8(const void* hidden, const PermLaunch& pl, int T, int E, int k, int d, void* xq_perm,
-                              float* sx_perm, int num_sms, cudaStream_t st, const SegTable* segp) {
+                              float* sx_perm, unsigned* hmax, int num_sms, cudaStream_t st, const SegTable* segp) {
   const SegTable seg = segp ? *segp : SegTable{nullptr, nullptr, nullptr, 0};
   if (T == 0) return cudaSuccess;
   PermArgs pa;
@@ -167,13 +213,13 @@ cudaError_t launch_gather_fp8(const void* hidden, const PermLaunch& pl, int T, i
   const int grid = blocks_needed < cap ? blocks_needed : cap;
   if (k <= 2)
     launch_pdl(gather_fp8_kernel<2>, grid, 256, 0, st, static_cast<const uint4*>(hidden), pa, T, k, d / 8,
-               static_cast<uint2*>(xq_perm), sx_perm, seg);
+               static_cast<uint2*>(xq_perm), sx_perm, hmax, seg);
   else if (k <= 4)
     launch_pdl(gather_fp8_kernel<4>, grid, 256, 0, st, static_cast<const uint4*>(hidden), pa, T, k, d / 8,
-               static_cast<uint2*>(xq_perm), sx_perm, seg);
+               static_cast<uint2*>(xq_perm), sx_perm, hmax, seg);
   else
     launch_pdl(gather_fp8_kernel<8>, grid, 256, 0, st, static_cast<const uint4*>(hidden), pa, T, k, d / 8,
-               static_cast<uint2*>(xq_perm), sx_perm, seg);
+               static_cast<uint2*>(xq_perm), sx_perm, hmax, seg);
   return cudaGetLastError();
 }
 

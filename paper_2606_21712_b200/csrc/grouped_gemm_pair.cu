@@ -95,6 +95,7 @@ struct Params {
   const float* sx;             // [rows]  per expert-order token row
   const float* sw0;            // [E, N]  per expert and output channel, W_gate
   const float* sw1;            // [E, N]  W_up
+  unsigned* hmax;              // a7, FP8 down GEMM downstream (reading F5): [rows] running max |H| (float bits), or nullptr
 };
 
 __device__ __forceinline__ void named_bar_sync(int id, int threads) {
@@ -308,10 +309,12 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
           const uint32_t sb = sa + A_BYTES;
           const uint32_t fb = leader_bar(full_bar(s));
           if (rank == 0) mbar_expect_tx(full_bar(s), tx_pair);   // the bytes of both CTAs
-          if (FP8) {
+          if (FP8 && GATEUP) {
             // quantised weights [E, N, K] bytes: box {128 k, 64 features, 1}: K-major, 8 KB per tensor
             tma_load_3d_pair(sa, &tm_w0, fb, kb * BKE, n0, c.e);
             tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w1, fb, kb * BKE, n0, c.e);
+          } else if (FP8) {
+            tma_load_3d_pair(sa, &tm_w0, fb, kb * BKE, n0, c.e);      // W_down codes: box {128 k, 128 features, 1}
           } else if (p.w4d) {
             // one operation per weight tensor: nblk 64-column blocks in [block][k][64 n] order
             tma_load_4d_pair(sa, &tm_w0, fb, 0, kb * BK, n0 >> 6, c.e);
@@ -465,6 +468,22 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
                        : "=r"(val.x), "=r"(val.y), "=r"(val.z), "=r"(val.w) : "r"(stage_rd + i * 512));
           if (col_ok && r < n_tok)
             *reinterpret_cast<uint4*>(out_tile + static_cast<int64_t>(cc * 32 + r) * p.N) = val;
+          if (GATEUP && p.hmax != nullptr) {
+            // row maximum of |H| for the FP8 down GEMM's per-row scale: integer max on the float bits of
+            // non-negative values (order-independent, hence deterministic); 4 lanes share a token row
+            const __nv_bfloat162* hv = reinterpret_cast<const __nv_bfloat162*>(&val);
+            float m = 0.0f;
+            if (col_ok && r < n_tok) {
+              #pragma unroll
+              for (int x = 0; x < 4; ++x) {
+                const float2 f2 = __bfloat1622float2(hv[x]);
+                m = fmaxf(m, fmaxf(fabsf(f2.x), fabsf(f2.y)));
+              }
+            }
+            m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
+            m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
+            if ((lane & 3) == 0 && r < n_tok) atomicMax(p.hmax + c.row0 + cc * 32 + r, __float_as_uint(m));
+          }
         }
         __syncwarp();
       };
@@ -512,6 +531,11 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
           named_bar_sync(bar_id, 64);                    // exchange buffers free for the next round
         }
       } else {
+        float swf = 1.0f;                              // FP8: this thread's output channel's weight scale (reading F5)
+        if (FP8) {
+          const int n = c.f_tile * OUT_FEATS + feat0 + lane;
+          if (n < p.N) swf = __ldg(p.sw0 + static_cast<int64_t>(c.e) * p.N + n);
+        }
         #pragma unroll 1
         for (int cc = sub; cc < n_chunks; cc += 2) {
           uint32_t v[32];
@@ -519,7 +543,8 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
           tmem_ld_wait();
           #pragma unroll
           for (int j = 0; j < 32; j += 4) {
-            const float4 s4 = *reinterpret_cast<const float4*>(sc_smem + (it & 1) * BN_MAX + cc * 32 + j);   // broadcast
+            float4 s4 = *reinterpret_cast<const float4*>(sc_smem + (it & 1) * BN_MAX + cc * 32 + j);   // broadcast
+            if (FP8) { s4.x *= swf; s4.y *= swf; s4.z *= swf; s4.w *= swf; }
             st_shared_bf16(stage_wr + (j + 0) * 64, __uint_as_float(v[j + 0]) * s4.x);
             st_shared_bf16(stage_wr + (j + 1) * 64, __uint_as_float(v[j + 1]) * s4.y);
             st_shared_bf16(stage_wr + (j + 2) * 64, __uint_as_float(v[j + 2]) * s4.z);
@@ -558,6 +583,7 @@ Params make_params(const GemmLaunch& g) {
   p.sg_max = g.sg_max;
   p.tile_counter = g.tile_counter;
   p.sx = g.sx; p.sw0 = g.sw0; p.sw1 = g.sw1;
+  p.hmax = g.hmax;
   return p;
 }
 
@@ -567,6 +593,8 @@ cudaError_t pair_kernels_init() {
   cudaError_t e = cudaFuncSetAttribute(pair_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(pair_gemm_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(pair_gemm_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
   if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(pair_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
 }
@@ -579,6 +607,12 @@ cudaError_t launch_gateup_swiglu_pair(const GemmLaunch& g, cudaStream_t st) {
 // FP8 gate/up: tm_act over the e4m3 rows [rows, K bytes], tm_b0 / tm_b1 over the quantised weights [E, N, K bytes]
 cudaError_t launch_gateup_swiglu_pair_fp8(const GemmLaunch& g, cudaStream_t st) {
   launch_pdl(pair_gemm_kernel<true, true>, g.num_sms & ~1, 256, SMEM_BYTES, st, g.tm_act, g.tm_b0, g.tm_b1, make_params(g));
+  return cudaGetLastError();
+}
+
+// FP8 down: tm_act over the e4m3 H rows [rows, K bytes], tm_b0 over the quantised W_down [E, N, K bytes] (box of 128 rows)
+cudaError_t launch_down_pair_fp8(const GemmLaunch& g, cudaStream_t st) {
+  launch_pdl(pair_gemm_kernel<false, true>, g.num_sms & ~1, 384, SMEM_BYTES, st, g.tm_act, g.tm_b0, g.tm_b0, make_params(g));
   return cudaGetLastError();
 }
 

@@ -112,8 +112,13 @@ cudaError_t launch_unpermute(const void* y_perm, const int32_t* inv_perm, const 
 cudaError_t launch_quantize_weights(const void* W, int E, int K, int N, void* Wq, float* sw, cudaStream_t st);
 // a5'' + a6 with quantisation: as launch_gather, but the k expert-order rows of a token are written as e4m3 bytes
 // xq_perm [T*k, d] with the token's fp32 scale in sx_perm [T*k]
+// hmax (may be NULL): [T*k] zeroed here for the rows the token owns (the gate/up epilogue accumulates max |H| there)
 cudaError_t launch_gather_fp8(const void* hidden, const PermLaunch& pl, int T, int E, int k, int d, void* xq_perm,
-                              float* sx_perm, int num_sms, cudaStream_t st, const SegTable* seg = nullptr);
+                              float* sx_perm, unsigned* hmax, int num_sms, cudaStream_t st, const SegTable* seg = nullptr);
+// Reading F5: H [rows, f] bf16 + hmax [rows] (float bits of max |H[r,:]|) -> Hq [rows, f] e4m3, sh [rows] = max / 448,
+// sc [rows] = sh * (w_perm ? w_perm[r] : 1): the per-row factor the down GEMM's epilogue applies
+cudaError_t launch_quantize_h(const void* H, const unsigned* hmax, const float* w_perm, int64_t rows, int f, void* Hq,
+                              float* sh, float* sc, int num_sms, cudaStream_t st);
 
 // ---- grouped GEMM (grouped_gemm_pair.cu): steps a7 and a8
 // Activation tensor maps: the same [rows, K] bf16 matrix with TMA boxes of {64 k, 8 (i + 1) rows},
@@ -141,11 +146,13 @@ struct GemmLaunch {
   const float* sx = nullptr;     // [rows] per expert-order token row
   const float* sw0 = nullptr;    // [E, N] W_gate, per expert and output channel
   const float* sw1 = nullptr;    // [E, N] W_up
+  unsigned* hmax = nullptr;      // gate/up GEMM: [rows] running max |H| as float bits (FP8 down GEMM downstream), or nullptr
   int num_sms;
 };
 // CTA-pair kernels (grouped_gemm_pair.cu): weights on UMMA M (256 per pair), tokens on UMMA N.
 cudaError_t launch_gateup_swiglu_pair(const GemmLaunch& g, cudaStream_t st);
 cudaError_t launch_gateup_swiglu_pair_fp8(const GemmLaunch& g, cudaStream_t st);
+cudaError_t launch_down_pair_fp8(const GemmLaunch& g, cudaStream_t st);
 cudaError_t launch_down_pair(const GemmLaunch& g, cudaStream_t st);
 cudaError_t pair_kernels_init();
 

@@ -130,3 +130,58 @@ def test_fp8_argument_errors():
     with pytest.raises(BgMoeError) as ei:
         layer.set_precision(1)
     assert ei.value.status == BG_ERR_UNSUPPORTED
+
+
+FP8_FULL_SHAPES = [
+    wl.small_config(T=256, d=512, E=8, k=2, f=1024, index=46, name="C1-like"),
+    wl.small_config(T=333, d=384, E=7, k=3, f=384, index=47, name="ragged"),
+    wl.small_config(T=1500, d=128, E=2, k=1, f=256, index=48, name="multi-tile"),
+    wl.small_config(T=700, d=256, E=130, k=8, f=128, index=49, name="E130"),
+]
+
+
+@pytest.mark.parametrize("cfg", FP8_FULL_SHAPES, ids=lambda c: c.name)
+def test_fp8_gateup_and_down_parity(cfg):
+    """Precision 2 (reading F5): the down GEMM in FP8 as well.  H is produced by the GPU's gate/up kernel (fp32
+    accumulation, bf16 rounding), so -- as with the router logits (S5) -- the integer decisions that depend on it are
+    checked on the SAME input: the oracle quantises the GPU's H and must find the same codes and scales bit for bit,
+    and the layer output is checked against the oracle's FP8 down GEMM of that H.  The GPU's H itself is checked
+    against the oracle's gate/up (quantised definition) at the bf16 bar."""
+    lay, g, layer = make(cfg)
+    layer.set_precision(2)
+    out = layer.combined_forward(g["hidden"]).clone()
+    out2 = layer.combined_forward(g["hidden"])
+    torch.cuda.synchronize()
+    assert torch.equal(out, out2), "FP8 path is not bitwise deterministic"
+    v = layer.debug_views(cfg.T)
+    dv = layer.fp8_down_views(cfg.T)
+    L = v["logits"].cpu().numpy()
+    row_src, offsets, inv_perm = v["row_src"].cpu().numpy(), v["offsets"].cpu().numpy(), v["inv_perm"].cpu().numpy()
+    x_perm = f32(lay["hidden"])[row_src // cfg.k]
+    # gate/up: GPU H vs the quantised-definition oracle
+    res = fp8.expert_ffn_fp8_gateup(x_perm, offsets, f32(lay["W_gate"]), f32(lay["W_up"]), f32(lay["W_down"]))
+    Hg = dv["H"].float().cpu().numpy()
+    assert np.linalg.norm(Hg - res["H"]) / np.linalg.norm(res["H"]) <= L2_TOL
+    assert np.abs(Hg - res["H"]).max() <= MAX_TOL * np.abs(res["H"]).max()
+    # H quantisation on the GPU's own H: bit-exact
+    d = fp8.down_fp8(Hg, offsets, f32(lay["W_down"]))
+    assert np.array_equal(dv["sh_perm"].cpu().numpy(), d["sh"]), "H row scales differ"
+    assert np.array_equal(dv["hq"].cpu().numpy(), d["hq"]), "H codes differ"
+    assert np.array_equal(dv["sw_down"].cpu().numpy(), d["sd"]) and np.array_equal(dv["q_down"].cpu().numpy(), d["dq"])
+    # output
+    idx, w = oracle.topk_gate(L, cfg.k)
+    ref = oracle.unpermute(d["y"], inv_perm, w)
+    got = out.to(torch.float64).cpu().numpy()
+    scale = np.abs(ref).max()
+    max_err, l2 = np.abs(got - ref).max(), np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    assert max_err <= MAX_TOL * scale and l2 <= L2_TOL, (cfg.name, max_err / scale, l2)
+    full = oracle.forward_batched(lay["hidden"], lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"], cfg.k,
+                                  logits_in=L)["out"]
+    l2_q = np.linalg.norm(got - full) / np.linalg.norm(full)
+    print(f"[fp8 full] {cfg.name}: vs quantised-definition oracle relL2 {l2:.2e} max {max_err / scale:.2e}; "
+          f"vs unquantised oracle relL2 {l2_q:.2e}")
+    assert l2_q <= 1.2e-1
+    layer.set_precision(1)
+    o1 = layer.combined_forward(g["hidden"]).clone()
+    layer.set_precision(2)
+    assert torch.equal(layer.combined_forward(g["hidden"]), out) and not torch.equal(o1, out)
