@@ -582,7 +582,7 @@ def run_ours(args):
     layer = MoELayer(cfg.d, cfg.f, cfg.E, cfg.k, cfg.T, device=local)
     layer.set_weights(lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"])
     if args.fp8:
-        layer.set_precision(1)
+        layer.set_precision(args.fp8)
     hidden = lay["hidden"]
     out = torch.empty_like(hidden)
     stream = torch.cuda.current_stream()
@@ -655,7 +655,7 @@ def run_ours(args):
     line = {
         "metric": METRIC, "value": tflops, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "fp8-gateup/bf16" if args.fp8 else "bf16", "data": "synthetic",
+        "vs_baseline": None, "dtype": {0: "bf16", 1: "fp8-gateup/bf16", 2: "fp8"}[args.fp8], "data": "synthetic",
         "config": config_keys(cfg),
         "load": {"E_active": E_act, "rows_per_expert_min_max": [int(counts.min()), int(counts.max())],
                  "parallelism": "replicas" if world > 1 else "single-gpu"},
@@ -724,8 +724,9 @@ def main():
     ap.add_argument("--T", type=int, default=0, help="override the combined-token count (C3 sweep)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the C3 combine-size sweep (sweep_c3 key)")
-    ap.add_argument("--fp8", action="store_true", help="run the gate/up GEMM in FP8 (bg_moe_set_precision 1); "
-                    "the line is then labelled dtype fp8-gateup/bf16 and is NOT the BASELINE.json bf16 metric")
+    ap.add_argument("--fp8", type=int, default=0, choices=[0, 1, 2],
+                    help="bg_moe_set_precision: 1 = FP8 gate/up GEMM, 2 = FP8 gate/up and down; the line is then labelled "
+                    "with that dtype and is NOT the BASELINE.json bf16 metric")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
