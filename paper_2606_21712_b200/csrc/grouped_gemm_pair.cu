@@ -442,7 +442,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       }
       float swg = 1.0f, swu = 1.0f;                    // FP8: this thread's feature's weight scales
       float* sx_smem = reinterpret_cast<float*>(epi_smem + 4 * XCH_BYTES + 4 * STAGE_TILE_BYTES);   // FP8: [BN_MAX] token scales
-      if (FP8) {
+      if (FP8 && GATEUP) {
         const int n = c.f_tile * OUT_FEATS + feat0 + lane;                    // this thread's output feature
         if (n < p.N) {
           swg = __ldg(p.sw0 + static_cast<int64_t>(c.e) * p.N + n);
