@@ -469,11 +469,11 @@ def run_c5_combine(steps: int, device_index: int):
 
 # ----------------------------------------------------------------------------- FP8 gate/up
 def run_fp8(steps: int, peaks: dict, device_index: int):
-    """the gate/up GEMM in FP8 (e4m3, W8A8, per-token x per-channel
-    scales; readings F1-F4), tcgen05 kind::f8f6f4.  Per configuration: step time and gate/up kernel time in bf16
-    and in FP8.  The FP8 gate/up kernel is scored against max(flops / (2 x the measured bf16 peak), bytes / BW): the
-    profiling guide's nominal fp8 : bf16 ratio applied to the measured bf16 number, with its algorithmic bytes
-    (1-byte weights and activations in, bf16 H out)."""
+    """SURVEY.md §8(f)-2 (PAPER.md:384, 442, 476): the expert GEMMs in FP8 (e4m3, W8A8, per-row x per-channel scales;
+    readings F1-F5), tcgen05 kind::f8f6f4: precision 1 = gate/up, precision 2 = gate/up and down.  Per configuration:
+    step time and GEMM kernel times in bf16 and in FP8.  An FP8 kernel is scored against max(flops / (2 x the measured
+    bf16 peak), bytes / BW): the profiling guide's nominal fp8 : bf16 ratio applied to the measured bf16 number, with
+    that kernel's algorithmic bytes (1-byte weights and activations in, bf16 out)."""
     from paper_2606_21712_b200 import MoELayer
     rows = []
     for name in ("C2", "C3", "C5"):
@@ -485,29 +485,35 @@ def run_fp8(steps: int, peaks: dict, device_index: int):
         out = torch.empty_like(hidden)
         step = lambda: layer.combined_forward(hidden, out, stream)
         res = {}
-        for prec in (0, 1):
+        for prec in (0, 1, 2):
             layer.set_precision(prec)
             torch.cuda.synchronize()
             time.sleep(1.0)
             for _ in range(5):
                 step()
             total, per = time_steps(step, steps, stream)
-            res[prec] = (total / steps, float(np.median(per)), stage_times(layer, step))
+            res[prec] = (total / steps, float(np.median(per)), stage_times(layer, step, rounds=1))
         counts = layer.debug_views(cfg.T)["counts"].cpu().numpy()
         E_act = int((counts > 0).sum())
         R = cfg.T * cfg.k
-        fl = 4.0 * R * cfg.d * cfg.f
-        by = 2.0 * cfg.d * cfg.f * E_act + 1.0 * R * cfg.d + 4.0 * R + 2.0 * R * cfg.f
-        t_bound = max(fl / (2 * peaks["bf16_tflops"] * 1e12), by / (peaks["hbm_gbs"] * 1e9))
-        gu8 = res[1][2]["gateup_swiglu"] * 1e-3
-        rows.append({"workload": cfg.name, "bf16_ms_per_step": res[0][0], "fp8_ms_per_step": res[1][0],
-                     "step_speedup": res[0][0] / res[1][0],
-                     "bf16_gateup_ms": res[0][2]["gateup_swiglu"], "fp8_gateup_ms": res[1][2]["gateup_swiglu"],
-                     "bf16_gather_ms": res[0][2]["gather"], "fp8_gather_ms": res[1][2]["gather"],
-                     "fp8_gateup_tflops": fl / gu8 / 1e12,
-                     "fp8_gateup_roofline": {"bound": "tensor" if fl / (2 * peaks["bf16_tflops"] * 1e12) >= by / (peaks["hbm_gbs"] * 1e9) else "hbm",
-                                             "frac": t_bound / gu8,
-                                             "peak": "2 x measured bf16 burst (guide's nominal fp8 : bf16 ratio)"}})
+        P8, BW = 2 * peaks["bf16_tflops"] * 1e12, peaks["hbm_gbs"] * 1e9
+
+        def score(fl, by, ms):
+            return {"tflops": fl / (ms * 1e-3) / 1e12, "bound": "tensor" if fl / P8 >= by / BW else "hbm",
+                    "frac": max(fl / P8, by / BW) / (ms * 1e-3)}
+
+        gu = score(4.0 * R * cfg.d * cfg.f, 2.0 * cfg.d * cfg.f * E_act + 1.0 * R * cfg.d + 4.0 * R + 2.0 * R * cfg.f,
+                   res[1][2]["gateup_swiglu"])
+        # precision 2's "down" stage holds the H quantising pass + the FP8 down GEMM
+        dn = score(2.0 * R * cfg.d * cfg.f, 1.0 * cfg.d * cfg.f * E_act + 3.0 * R * cfg.f + 1.0 * R * cfg.f + 2.0 * R * cfg.d,
+                   res[2][2]["down"])
+        rows.append({"workload": cfg.name, "bf16_ms_per_step": res[0][0], "fp8_gateup_ms_per_step": res[1][0],
+                     "fp8_full_ms_per_step": res[2][0], "speedup_gateup": res[0][0] / res[1][0],
+                     "speedup_full": res[0][0] / res[2][0],
+                     "stage_ms": {"bf16": res[0][2], "fp8_gateup": res[1][2], "fp8_full": res[2][2]},
+                     "fp8_gateup_kernel": gu, "fp8_down_stage_incl_quantise": dn,
+                     "peak": "2 x measured bf16 burst (guide's nominal fp8 : bf16 ratio)",
+                     "layer_tflops_equiv_fp8_full": cfg.flops() / (res[2][0] * 1e-3) / 1e12})
         del layer, lay, hidden, out
         torch.cuda.empty_cache()
     return rows
@@ -686,7 +692,7 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_sweep:
         line["combine_c5"] = run_c5_combine(args.steps, local)
         line["ring_c3"] = run_ring(min(args.steps, 10), local)
-        line["fp8_gateup"] = run_fp8(args.steps, peaks, local)
+        line["fp8"] = run_fp8(args.steps, peaks, local)
         # every other BASELINE.json configuration through the same protocol (the north_star claim is "every
         # config"), and the sustained regime for the headline workload
         del layer
