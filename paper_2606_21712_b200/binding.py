@@ -79,6 +79,16 @@ def _ptr(t: Optional[torch.Tensor]):
     return None if t is None else ctypes.c_void_p(t.data_ptr())
 
 
+def _chk(t: torch.Tensor, dtype, shape, what: str, cuda: bool = True):
+    """Every tensor that crosses the C ABI as a raw pointer: dtype, device, contiguity and shape are checked here
+    (the library only sees addresses)."""
+    assert isinstance(t, torch.Tensor), f"{what}: tensor expected"
+    assert t.dtype == dtype, f"{what}: dtype {t.dtype}, expected {dtype}"
+    assert t.is_cuda == cuda, f"{what}: must be a {'CUDA' if cuda else 'CPU'} tensor"
+    assert t.is_contiguous(), f"{what}: must be contiguous"
+    assert tuple(t.shape) == tuple(shape), f"{what}: shape {tuple(t.shape)}, expected {tuple(shape)}"
+
+
 def _stream(stream: Optional[torch.cuda.Stream]):
     s = torch.cuda.current_stream() if stream is None else stream
     return ctypes.c_void_p(s.cuda_stream)
@@ -191,8 +201,16 @@ class MoELayer:
     def ring_bytes_per_call(self) -> int:
         return int(self.lib.bg_moe_ring_bytes_per_call(self._ctx))
 
+    def _alloc_stream(self, stream):
+        """Outputs are allocated under the stream the call runs on (caching-allocator reuse is stream-ordered)."""
+        return torch.cuda.stream(stream) if stream is not None else torch.cuda.stream(torch.cuda.current_stream())
+
     def route(self, hidden, logits_in=None, want_logits=True, stream=None):
         T = hidden.shape[0] if hidden is not None else logits_in.shape[0]
+        if hidden is not None:
+            _chk(hidden, torch.bfloat16, (T, self.d), "hidden")
+        if logits_in is not None:
+            _chk(logits_in, torch.float32, (T, self.E), "logits_in")
         dev = self._dev()
         logits = torch.empty(T, self.E, dtype=torch.float32, device=dev) if want_logits else None
         idx = torch.empty(T, self.k, dtype=torch.int32, device=dev)
@@ -205,6 +223,10 @@ class MoELayer:
 
     def permute(self, hidden, topk_idx, offsets, gather=True, stream=None):
         T = topk_idx.shape[0]
+        _chk(topk_idx, torch.int32, (T, self.k), "topk_idx")
+        _chk(offsets, torch.int32, (self.E + 1,), "offsets")
+        if gather:
+            _chk(hidden, torch.bfloat16, (T, self.d), "hidden")
         dev = self._dev()
         row_src = torch.empty(T * self.k, dtype=torch.int32, device=dev)
         inv_perm = torch.empty(T * self.k, dtype=torch.int32, device=dev)
@@ -215,12 +237,17 @@ class MoELayer:
 
     def expert_ffn(self, x_perm, offsets, T=None, stream=None):
         T = x_perm.shape[0] // self.k if T is None else T
+        _chk(x_perm, torch.bfloat16, (T * self.k, self.d), "x_perm")
+        _chk(offsets, torch.int32, (self.E + 1,), "offsets")
         y = torch.empty(T * self.k, self.d, dtype=torch.bfloat16, device=self._dev())
         self._check(self.lib.bg_moe_expert_ffn(self._ctx, _ptr(x_perm), _ptr(offsets), T, _ptr(y), _stream(stream)))
         return y
 
     def unpermute(self, y_perm, inv_perm, topk_w, stream=None):
         T = topk_w.shape[0]
+        _chk(y_perm, torch.bfloat16, (T * self.k, self.d), "y_perm")
+        _chk(inv_perm, torch.int32, (T * self.k,), "inv_perm")
+        _chk(topk_w, torch.float32, (T, self.k), "topk_w")
         out = torch.empty(T, self.d, dtype=torch.bfloat16, device=self._dev())
         self._check(self.lib.bg_moe_unpermute(self._ctx, _ptr(y_perm), _ptr(inv_perm), _ptr(topk_w), T, _ptr(out),
                                               _stream(stream)))
@@ -228,18 +255,23 @@ class MoELayer:
 
     def combined_forward(self, hidden, out=None, stream=None):
         T = hidden.shape[0]
-        assert hidden.dtype == torch.bfloat16 and hidden.is_cuda and hidden.is_contiguous()
+        _chk(hidden, torch.bfloat16, (T, self.d), "hidden")
         if out is None:
-            out = torch.empty(T, self.d, dtype=torch.bfloat16, device=self._dev())
+            with self._alloc_stream(stream):
+                out = torch.empty(T, self.d, dtype=torch.bfloat16, device=self._dev())
+        else:
+            _chk(out, torch.bfloat16, (T, self.d), "out")
         self._check(self.lib.bg_moe_combined_forward(self._ctx, _ptr(hidden), T, _ptr(out), _stream(stream)))
         return out
 
     def combined_forward_host(self, hidden_host, out_host=None, stream=None):
         """hidden_host / out_host: CPU (ideally pinned) bf16 tensors; copies run on `stream`."""
         T = hidden_host.shape[0]
-        assert hidden_host.dtype == torch.bfloat16 and not hidden_host.is_cuda and hidden_host.is_contiguous()
+        _chk(hidden_host, torch.bfloat16, (T, self.d), "hidden_host", cuda=False)
         if out_host is None:
             out_host = torch.empty(T, self.d, dtype=torch.bfloat16).pin_memory()
+        else:
+            _chk(out_host, torch.bfloat16, (T, self.d), "out_host", cuda=False)
         self._check(self.lib.bg_moe_combined_forward_host(self._ctx, _ptr(hidden_host), T, _ptr(out_host),
                                                           _stream(stream)))
         return out_host
