@@ -196,7 +196,8 @@ int bg_moe_debug_views(bg_moe_ctx* ctx, const float** logits, const int32_t** to
 /* Per-kernel timing of the fused chain.  While enabled, bg_moe_combined_forward records a CUDA
  * event on `stream` before and after each of its BG_MOE_NUM_STAGES kernels (in launch order:
  * fused router (logits, top-k, histogram, scan, tile ranks), gather (+ permutation), gate/up
- * GEMM+SwiGLU, down GEMM, un-permute reduce).
+ * GEMM+SwiGLU, down GEMM, un-permute reduce); bg_moe_expert_ffn records its two GEMMs in the same
+ * slots (the other three read 0).
  * bg_moe_profile_read waits for the last recorded call and writes that call's per-kernel
  * durations in milliseconds to ms_out[BG_MOE_NUM_STAGES] (HOST pointer). */
 #define BG_MOE_NUM_STAGES 5

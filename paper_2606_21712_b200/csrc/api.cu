@@ -837,8 +837,12 @@ int bg_moe_expert_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offset
   if ((rc = begin_call(ctx, st))) return rc;
   // no router kernel precedes the GEMMs here: zero their ticket counters on the stream
   BG_CUDA(ctx, cudaMemsetAsync(ctx->tile_counters, 0, 32, st), "memset ticket counters");
-  rc = do_ffn(ctx, x_perm, offsets, T, y_perm, nullptr, st);
+  // per-kernel profile of the split FFN: "gateup_swiglu" and "down" are timed, the other three stages read 0
+  mark(ctx, 0, st); mark(ctx, 1, st); mark(ctx, 2, st);
+  rc = do_ffn(ctx, x_perm, offsets, T, y_perm, nullptr, st, /*mark_between=*/3);
   if (rc) return rc;
+  mark(ctx, 4, st); mark(ctx, 5, st);
+  ctx->profile_valid = ctx->profile;
   return end_call(ctx, st, false);
 }
 
