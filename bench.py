@@ -270,11 +270,29 @@ def time_steps(fn, steps: int, stream):
     return ev[0].elapsed_time(ev[steps]), per
 
 
+def _energy_mj(device_index: int = 0):
+    """The board's cumulative energy counter (NVML, millijoules), or None when NVML is not there."""
+    try:
+        import pynvml
+        pynvml.nvmlInit()
+        try:
+            uuid = torch.cuda.get_device_properties(device_index).uuid
+            h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + str(uuid)).encode())
+        except Exception:
+            h = pynvml.nvmlDeviceGetHandleByIndex(device_index)
+        return int(pynvml.nvmlDeviceGetTotalEnergyConsumption(h))
+    except Exception:
+        return None
+
+
 def sustained_ms(fn, stream, seconds: float = 2.0, chunk: int = 10):
     """>= `seconds` of back-to-back steps with no idle gap; the median per-step time of the
-    chunks in the second half of the run (the part is power-managed: the first few hundred ms are the burst)."""
+    chunks in the second half of the run (the part is power-managed: the first few hundred ms are the burst).
+    Also returns the energy the board drew over the run (NVML counter): joules per step and average watts -- at the
+    1000 W cap the sustained step time IS joules per step / 1000 W."""
     chunks = []
     torch.cuda.synchronize()
+    e_start = _energy_mj(torch.cuda.current_device())
     t0 = time.perf_counter()
     evs = [torch.cuda.Event(enable_timing=True)]
     evs[0].record(stream)
@@ -289,9 +307,15 @@ def sustained_ms(fn, stream, seconds: float = 2.0, chunk: int = 10):
             if time.perf_counter() - t0 >= seconds:
                 break
     torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    e_end = _energy_mj(torch.cuda.current_device())
     chunks = [evs[i].elapsed_time(evs[i + 1]) / chunk for i in range(len(evs) - 1)]
     tail = chunks[len(chunks) // 2:]
-    return float(np.median(tail)), len(chunks) * chunk, float(sum(chunks) * chunk / 1e3)
+    n = len(chunks) * chunk
+    energy = None
+    if e_start is not None and e_end is not None and e_end > e_start:
+        energy = {"joules_per_step": (e_end - e_start) / 1e3 / n, "avg_watts": (e_end - e_start) / 1e3 / wall}
+    return float(np.median(tail)), n, float(sum(chunks) * chunk / 1e3), energy
 
 
 def stage_times(layer, step, rounds: int = 3, burst: int = 8) -> dict:
@@ -353,11 +377,11 @@ def run_config(name: str, steps: int, peaks: dict, device_index: int, sustained:
            "ms_median": float(np.median(per)), **layer_fracs(cfg, E_act, ms, peaks)}
     row["stage_ms"] = stage_times(layer, step)
     if sustained:
-        sm, n, secs = sustained_ms(step, stream)
+        sm, n, secs, energy = sustained_ms(step, stream)
         fr = layer_fracs(cfg, E_act, sm, peaks)
         row["sustained"] = {"ms_per_step_median": sm, "steps": n, "seconds": secs, "tflops": fr["tflops"],
                             "frac_of_measured_sustained": fr["frac_of_measured_sustained"],
-                            "frac_of_measured_burst": fr["frac_of_measured_burst"]}
+                            "frac_of_measured_burst": fr["frac_of_measured_burst"], "energy": energy}
     if note:
         row["note"] = note
     del layer, lay, hidden, out
@@ -401,11 +425,11 @@ def run_c3_sweep(steps: int, peaks: dict, device_index: int):
                "E_active": E_act, **layer_fracs(cfg, E_act, ms, peaks)}
         row["stage_ms"] = stage_times(layer, step)
         if T == 16384:
-            sm, n, secs = sustained_ms(step, stream)
+            sm, n, secs, energy = sustained_ms(step, stream)
             fr = layer_fracs(cfg, E_act, sm, peaks)
             row["sustained"] = {"ms_per_step_median": sm, "steps": n, "seconds": secs, "tflops": fr["tflops"],
                                 "frac_of_measured_sustained": fr["frac_of_measured_sustained"],
-                                "frac_of_measured_burst": fr["frac_of_measured_burst"]}
+                                "frac_of_measured_burst": fr["frac_of_measured_burst"], "energy": energy}
         rows.append(row)
     del layer, lay
     torch.cuda.empty_cache()
@@ -700,8 +724,8 @@ def run_ours(args):
         line["configs"] = [
             run_config("C1", args.steps, peaks, local, note="L2-resident (25 MB of weights): a correctness config, not a roofline point"),
             run_config("C2", args.steps, peaks, local, sustained=True),
-            run_config("C4", args.steps, peaks, local),
-            run_config("C5", args.steps, peaks, local),
+            run_config("C4", args.steps, peaks, local, sustained=True),
+            run_config("C5", args.steps, peaks, local, sustained=True),
         ]
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle

@@ -46,7 +46,6 @@
 // global ticket counter (dynamic feed, see `feed_next`), so the neighbours really run concurrently and a strip
 // is read from HBM once; bg_moe_set_debug(static_tile_feed) keeps the fixed map tile t -> cluster (t mod #clusters).
 // Experts with no rows own no tiles and their weights are never touched.
-#include <cstdlib>
 #include <type_traits>
 
 #include "kernels.h"
@@ -431,9 +430,6 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
             const uint64_t bd = BDESC_HI | ((b_addr >> 4) & 0x3FFFu);
             #pragma unroll
             for (int kk = 0; kk < BK / UK; ++kk) {
-#ifdef BG_PROBE_NOMMA
-              if (c.nt <= 64) continue;   // probe builds only: power of a cold tile without its MMAs
-#endif
               if (FP8) {
                 // both K-major: +32 k (one MMA of 8-bit inputs) = +32 bytes in the span
                 umma_f8_pair(d_tmem, ad + ((kk * 32) >> 4), bd + ((kk * 32) >> 4), idesc, (kb | kk) != 0 ? 1u : 0u);
@@ -653,15 +649,8 @@ cudaError_t pair_kernels_init() {
   return cudaFuncSetAttribute(pair_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
 }
 
-#ifdef BG_PROBE
-// probe builds only (-DBG_PROBE, never the product): BG_PROBE_CTAS caps the grid so that per-CTA stream rates can be measured
-static int probe_ctas(int n) { const char* e = getenv("BG_PROBE_CTAS"); return e ? atoi(e) : n; }
-#else
-static int probe_ctas(int n) { return n; }
-#endif
-
 cudaError_t launch_gateup_swiglu_pair(const GemmLaunch& g, cudaStream_t st) {
-  launch_pdl(pair_gemm_kernel<true>, probe_ctas(g.num_sms) & ~1, GATEUP_THREADS, SMEM_BYTES, st, g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b1_4d : g.tm_b1, make_params(g));
+  launch_pdl(pair_gemm_kernel<true>, g.num_sms & ~1, GATEUP_THREADS, SMEM_BYTES, st, g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b1_4d : g.tm_b1, make_params(g));
   return cudaGetLastError();
 }
 
@@ -678,7 +667,7 @@ cudaError_t launch_down_pair_fp8(const GemmLaunch& g, cudaStream_t st) {
 }
 
 cudaError_t launch_down_pair(const GemmLaunch& g, cudaStream_t st) {
-  launch_pdl(pair_gemm_kernel<false>, probe_ctas(g.num_sms) & ~1, 384, SMEM_BYTES, st, g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b0_4d : g.tm_b0, make_params(g));
+  launch_pdl(pair_gemm_kernel<false>, g.num_sms & ~1, 384, SMEM_BYTES, st, g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b0_4d : g.tm_b0, make_params(g));
   return cudaGetLastError();
 }
 

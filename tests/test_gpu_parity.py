@@ -159,8 +159,9 @@ def test_expert_ffn_parity(rows, d, f):
 def test_expert_ffn_scheduler_variants(env):
     """The same FFN through (i) the pair kernel's super-group tile order, which production shapes only
     reach with experts of several thousand rows (forced here on experts of 3-5 token tiles) and (ii) the
-    static tile feed (the default is the dynamic ticket feed); both selected through bg_moe_set_debug."""
-    rows = [1300, 0, 700, 257, 16, 1]
+    static tile feed (the default is the dynamic ticket feed); both selected through bg_moe_set_debug.  The experts of
+    <= 64 rows are "cold" (their tiles are spread evenly through the ticket order): 64 and 65 rows sit on that boundary."""
+    rows = [1300, 0, 700, 257, 16, 1, 64, 65]
     d, f = 192, 320
     E, R = len(rows), sum(rows)
     cfg = wl.MoEConfig("ffn-sched", 15, T=R, d=d, E=E, k=1, f=f)
