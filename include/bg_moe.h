@@ -121,9 +121,8 @@ int bg_moe_debug_fp8_down_views(bg_moe_ctx* ctx, const void** H, const void** hq
  *   static_tile_feed != 0     tile t -> cluster (t mod #clusters) instead of the dynamic ticket feed
  *   supergroup_token_tiles    > 0: token tiles per super-group (forces the super-group order on small
  *                             shapes); 0: sized from K so that a super-group's tokens fit ~48 MB of L2
- *   router_form               0: the router picks its form from T; 1: plain sequential form (one CTA per 128-token
- *                             tile) wherever it exists; 2: cluster form; 3: streaming form (persistent, pipelined
- *                             sequential form; E <= 128) wherever it exists.  All forms give the same bits. */
+ *   router_form               0: the router picks its form from T; 1: sequential form (one CTA per 128-token
+ *                             tile) wherever it exists; 2: cluster form.  Both forms give the same bits. */
 int bg_moe_set_debug(bg_moe_ctx* ctx, int32_t static_tile_feed, int32_t supergroup_token_tiles,
                      int32_t router_form);
 

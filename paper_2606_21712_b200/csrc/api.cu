@@ -96,7 +96,7 @@ struct bg_moe_ctx {
   // activation tensor maps of the workspace x_perm / H (whole capacity: rows past T*k are never stored)
   bg::ActMaps am_x, am_h;
   int sg_max = 0;               // bg_moe_set_debug: overrides the pair kernel's super-group size (tests)
-  int router_form = 0;          // bg_moe_set_debug: 0 = by T, 1 = sequential, 2 = cluster, 3 = streaming
+  int router_form = 0;          // bg_moe_set_debug: 0 = by T, 1 = sequential, 2 = cluster
   int64_t launches = 0;
   std::string last_error;
   // optional per-kernel timing of the fused chain
@@ -270,7 +270,6 @@ int do_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* logits
   if (logits_in == nullptr) {
     bg::RouterLaunch r;
     r.T = T; r.d = c.d; r.E = c.E; r.k = c.k;
-    r.hidden = seg ? nullptr : hidden;
     r.b_r = ctx->b_r;
     r.logits_out = logits_buf;
     r.topk_idx = topk_idx; r.topk_w = topk_w;
@@ -632,7 +631,7 @@ int bg_moe_destroy(bg_moe_ctx* ctx) {
 }
 
 int bg_moe_set_debug(bg_moe_ctx* ctx, int32_t static_tile_feed, int32_t supergroup_token_tiles, int32_t router_form) {
-  if (ctx == nullptr || supergroup_token_tiles < 0 || router_form < 0 || router_form > 3)
+  if (ctx == nullptr || supergroup_token_tiles < 0 || router_form < 0 || router_form > 2)
     return BG_ERR_INVALID_ARG;
   ctx->dyn_sched = static_tile_feed == 0;
   ctx->sg_max = supergroup_token_tiles;

@@ -26,10 +26,9 @@
 // The weights are consumed in the layout the layer is given (reading S14): no transpose/prepack.
 //
 // Warp roles (persistent, one CTA per SM, 74 clusters; every launch uses programmatic dependent launch):
-//   warp 0       : TMA producer of the first weight tensor, one elected lane issues (both CTAs; transaction bytes of both land on the leader's barrier)
+//   warp 0       : TMA producer, one elected lane issues (both CTAs; transaction bytes of both land on the leader's barrier)
 //   warp 1       : tcgen05.mma issuer, one elected lane issues (leader CTA only); commits are multicast to both CTAs
-//   warp 2       : TMEM allocator, then TMA producer of the token boxes
-//   warp 8 (a7)  : TMA producer of the W_up boxes (a TMA instruction holds its thread ~95 ns: one operand stream per warp)
+//   warp 2       : TMEM allocator
 //   warp 3 lane 0: tile scheduler (leader only): ticket counter -> 4-slot ring in both CTAs' shared memory
 //   warps 4-7    : epilogue (TMEM -> registers -> SwiGLU | gate weight -> bf16 -> smem transpose -> global);
 //                  a8 adds warps 8-11 (384 threads): its k loops are short, two warps serve each TMEM lane quarter
@@ -46,8 +45,6 @@
 // global ticket counter (dynamic feed, see `feed_next`), so the neighbours really run concurrently and a strip
 // is read from HBM once; bg_moe_set_debug(static_tile_feed) keeps the fixed map tile t -> cluster (t mod #clusters).
 // Experts with no rows own no tiles and their weights are never touched.
-#include <type_traits>
-
 #include "kernels.h"
 #include "ptx_sm100.cuh"
 
@@ -64,9 +61,7 @@ constexpr int A_BYTES = 2 * A_BLK_BYTES;            // 16 KB: this CTA's 128 M r
 constexpr int B_BYTES = (BN_MAX / 2) * BK * 2;      // 16 KB: this CTA's half of the tokens
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;      // 32 KB
 constexpr int RING_BYTES = STAGES * STAGE_BYTES;    // 192 KB
-constexpr int COLD_ROWS = 64;                       // an expert with <= COLD_ROWS rows is cold (tile order)
-constexpr int MAX_THREADS = 384;             // 4 role warps + 4 (a7) or 8 (a8) epilogue warps (+ a7's second weight producer)
-constexpr int GATEUP_THREADS = 288;          // a7: warps 0-3 roles, 4-7 epilogue, 8 = W_up producer
+constexpr int MAX_THREADS = 384;             // 4 role warps + 4 (a7) or 8 (a8) epilogue warps
 constexpr int MAX_E = 256;
 constexpr int XCH_PITCH = 36;                       // words per lane row of an exchange buffer (conflict-free v4)
 constexpr int XCH_BYTES = 32 * XCH_PITCH * 4;       // 4608 B
@@ -108,31 +103,19 @@ __device__ __forceinline__ void named_bar_sync(int id, int threads) {
 }
 
 struct TileCoord {
-  int e, row0, rows_valid, nt, f_tile, t_tile, tt;
+  int e, row0, rows_valid, nt, f_tile, t_tile;
 };
 
-// Two prefix tables in shared memory: hot_start[e] = tiles of the HOT experts before e, cold_start[e] = tiles of the
-// COLD experts before e (an expert is cold when all its rows fit one tile of <= COLD_ROWS tokens: its tiles stream
-// their weight strip once and do next to no tensor work); [E] = the totals H and C.
-// Ticket order: the cold tiles are spread evenly through the hot ones (ticket t is cold iff floor((t+1) C / (H+C)) >
-// floor(t C / (H+C))), so that at any moment a constant share of the clusters streams cold weights from HBM while the
-// rest run tensor-bound hot tiles out of L2 -- in plain expert order every cluster reaches a run of cold experts at the
-// same time, the tensor cores idle while HBM saturates, and then HBM idles while the next hot expert computes.
-// Inside a hot expert the order is feature-tile-major / token-tile-minor, so the token tiles that share a
+// tile_start[e] = first linear tile index of expert e (tile_start[E] = total);
+// t_tiles[e] = token tiles of expert e.  Both live in shared memory.
+// Inside an expert the order is feature-tile-major / token-tile-minor, so the token tiles that share a
 // weight strip run at the same time.  When an expert's token matrix is too large to stay in L2 between
 // two feature tiles (DeepSeek-shaped hot experts: thousands of rows x 14 KB), that order re-streams the
 // tokens from HBM once per feature tile; such experts are cut into super-groups of `sg_max` token tiles
 // (sized to ~48 MB of tokens) and each super-group runs through all feature tiles before the next starts:
 // the tokens stay in L2 and the expert's weights are streamed once per super-group instead.
-__device__ __forceinline__ TileCoord decode_tile(int t, const int* hot_start, const int* cold_start,
+__device__ __forceinline__ TileCoord decode_tile(int t, const int* tile_start, const int* t_tiles,
                                                  const int32_t* offsets, int E, int sg_max) {
-  const int H = hot_start[E], C = cold_start[E];
-  const int* tile_start = hot_start;
-  if (C != 0) {
-    const int c_before = static_cast<int>((static_cast<int64_t>(t) * C) / (H + C));
-    const int c_after = static_cast<int>((static_cast<int64_t>(t + 1) * C) / (H + C));
-    if (c_after > c_before) { tile_start = cold_start; t = c_before; } else { t -= c_before; }
-  }
   int lo = 0, hi = E;              // largest e with tile_start[e] <= t
   while (hi - lo > 1) {
     const int mid = (lo + hi) >> 1;
@@ -141,10 +124,8 @@ __device__ __forceinline__ TileCoord decode_tile(int t, const int* hot_start, co
   // experts with zero tiles share tile_start with their successor: the search above lands on the
   // last expert whose start <= t, which is the one that owns t (its successors start later).
   const int e = lo;
-  const int beg = __ldg(offsets + e), end = __ldg(offsets + e + 1);
-  const int n_e = end - beg;
   const int local = t - tile_start[e];
-  const int tt = (n_e + BN_MAX - 1) / BN_MAX;
+  const int tt = t_tiles[e];
   int f_tile, t_tile;
   if (tt <= sg_max) {
     f_tile = local / tt;
@@ -160,6 +141,8 @@ __device__ __forceinline__ TileCoord decode_tile(int t, const int* hot_start, co
     f_tile = r / g_here;
     t_tile = sg * g + (r - f_tile * g_here);
   }
+  const int beg = __ldg(offsets + e), end = __ldg(offsets + e + 1);
+  const int n_e = end - beg;
   const int base = (((n_e + tt - 1) / tt) + 15) & ~15;      // rows per token tile, multiple of 16, <= 256
   TileCoord c;
   c.e = e;
@@ -168,7 +151,6 @@ __device__ __forceinline__ TileCoord decode_tile(int t, const int* hot_start, co
   c.nt = (c.rows_valid + 15) & ~15;
   c.f_tile = f_tile;
   c.t_tile = t_tile;
-  c.tt = tt;
   return c;
 }
 
@@ -191,7 +173,7 @@ __device__ __forceinline__ void st_shared_bf16(uint32_t addr, float v) {
 // FP8 (a7 only): operands are e4m3 bytes, a k-block is 128 elements (the same 128-byte swizzle span), both K-major;
 //                 the epilogue multiplies the accumulators by sx[token] * sw[expert, feature] before the SwiGLU.
 template <bool GATEUP, bool FP8 = false>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GATEUP ? GATEUP_THREADS : 384, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GATEUP ? 256 : 384, 1)
 pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__ CUtensorMap tm_w0,
                  const __grid_constant__ CUtensorMap tm_w1, const Params p) {
   constexpr int CTA_FEATS = GATEUP ? 64 : 128;       // output features per CTA and tile
@@ -216,15 +198,9 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   static_assert(8 * NBAR + 16 + 4 * SCHED_SLOTS <= BAR_BYTES, "barrier area");
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + RING_BYTES + 8 * NBAR);
   volatile int* tile_slot = reinterpret_cast<volatile int*>(smem + RING_BYTES + 8 * NBAR + 16);
-  // TMA issue is spread over warps: one TMA instruction occupies its issuing thread for ~95 ns whatever the box size
-  // (measured: a thread sustains 9.7 bulk operations/us, three warps 28/us), so with one producer thread the three
-  // operations of an a7 k-block cost 0.29 us -- the whole MMA time of a 256-token k-block, and a 55 GB/s ceiling on a
-  // CTA that streams the weights of a cold expert.  a7: warp 0 = W_gate boxes, warp 8 = W_up boxes, warp 2 = tokens;
-  // a8: warp 0 = W_down boxes, warp 2 = tokens.
-  constexpr int PROD_WARPS = GATEUP ? 3 : 2;
-  constexpr int N_CONSUMERS = 2 * PROD_WARPS + 1 + 2 * EPI_WARPS;   // every producer warp, the MMA thread, every epilogue warp of the pair
+  constexpr int N_CONSUMERS = 3 + 2 * EPI_WARPS;      // two producers, the MMA thread, every epilogue warp of the pair
   int* tile_start = reinterpret_cast<int*>(smem + RING_BYTES + BAR_BYTES);
-  int* cold_start = tile_start + (MAX_E + 1);
+  int* t_tiles = tile_start + (MAX_E + 1);
   uint8_t* epi_smem = smem + RING_BYTES + BAR_BYTES + TABLE_BYTES;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -253,31 +229,28 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   }
   // ---- everything below reads what the previous kernels wrote (offsets, activations)
   pdl_wait_then_trigger();
-  // ---- per-CTA tile tables: inclusive scans of the hot and of the cold experts' tile counts (E <= 256 <= blockDim)
+  // ---- per-CTA tile table: inclusive scan of per-expert tile counts (E <= 256 = blockDim)
   {
-    unsigned long long v = 0;                     // low word: hot tiles, high word: cold tiles
+    int tt = 0;
     if (threadIdx.x < E) {
       const int cnt = __ldg(p.offsets + threadIdx.x + 1) - __ldg(p.offsets + threadIdx.x);
-      const int tt = (cnt + BN_MAX - 1) / BN_MAX;
-      const bool cold = cnt <= COLD_ROWS;
-      v = cold ? (static_cast<unsigned long long>(tt * f_tiles) << 32) : static_cast<unsigned long long>(tt * f_tiles);
+      tt = (cnt + BN_MAX - 1) / BN_MAX;
+      t_tiles[threadIdx.x] = tt;
     }
+    int v = tt * f_tiles;
     #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const unsigned long long u = __shfl_up_sync(0xffffffffu, v, o);
+      const int u = __shfl_up_sync(0xffffffffu, v, o);
       if (lane >= o) v += u;
     }
-    __shared__ unsigned long long warp_tot[MAX_THREADS / 32];
+    __shared__ int warp_tot[MAX_THREADS / 32];
     if (lane == 31) warp_tot[warp] = v;
     __syncthreads();
-    unsigned long long add = 0;
+    int add = 0;
     for (int w = 0; w < warp; ++w) add += warp_tot[w];
     v += add;                                   // inclusive prefix for thread's expert
-    if (threadIdx.x < E) {
-      tile_start[threadIdx.x + 1] = static_cast<int>(v & 0xffffffffu);
-      cold_start[threadIdx.x + 1] = static_cast<int>(v >> 32);
-    }
-    if (threadIdx.x == 0) { tile_start[0] = 0; cold_start[0] = 0; }
+    if (threadIdx.x < E) tile_start[threadIdx.x + 1] = v;
+    if (threadIdx.x == 0) tile_start[0] = 0;
   }
 
   tc_fence_before();
@@ -285,7 +258,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   cluster_sync_all();                                 // the peer's barriers are initialised, its TMEM allocated
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
-  const int total_tiles = tile_start[E] + cold_start[E];
+  const int total_tiles = tile_start[E];
 
   // ---- tile feed.  Static (tile_counter == nullptr): cluster c takes tiles c, c + 74, ...  Dynamic: tiles
   // are handed out in linear order from a global ticket counter by one thread of the leader CTA (warp 3),
@@ -317,15 +290,13 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   // cannot tell that a single lane is active and wraps every asm statement in an elect / branch loop, and the
   // MMA issue loop is instruction-bound (ncu: ~0.25 us of issue work per 0.30 us k-block on C2), so those extra
   // instructions cost tensor time.
-  // ===================== TMA producers (one warp per operand stream and CTA, one elected lane issues) =====================
-  // ROLE bits: 1 = first weight tensor (W_gate | W_down) + the transaction count, 2 = second weight tensor (W_up), 4 = tokens
-  auto producer = [&](auto role_tag) {
-    constexpr int ROLE = decltype(role_tag)::value;
+  if (warp == 0) {
+    // ===================== TMA producer (one warp per CTA, one elected lane issues) =====================
     int s = 0;
     uint32_t ph = 0;
     Feed feed = {0, 0, -1};
     for (int t = feed_next(feed, true); t >= 0; t = feed_next(feed, true)) {
-      const TileCoord c = decode_tile(t, tile_start, cold_start, p.offsets, E, sg_max);
+      const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
       const int n0 = c.f_tile * OUT_FEATS + static_cast<int>(rank) * CTA_FEATS;
       const int half = c.nt >> 1;                    // this CTA's tokens (multiple of 8, <= 128)
       const int brow0 = c.row0 + static_cast<int>(rank) * half;
@@ -335,7 +306,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       // evict-first policy so that they do not displace what is reused (token tiles, routing tables, W_r pieces).
       // Measured: C3 at T = 64 / 1024 0.220 -> 0.213 / 0.254 -> 0.247 ms, T = 4096 and C2 unchanged; the same hint on
       // experts with two token tiles, or evict-last on the x_perm / H / Y stores, was slower.
-      const bool once = c.tt == 1;
+      const bool once = t_tiles[c.e] == 1;
       const uint64_t pol = l2_policy_evict_first();
       for (int kb = 0; kb < k_blocks; ++kb) {
         mbar_wait(empty_bar(s), ph ^ 1u);            // this CTA's slot is free (multicast commit)
@@ -343,46 +314,34 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
           const uint32_t sa = base + s * STAGE_BYTES;
           const uint32_t sb = sa + A_BYTES;
           const uint32_t fb = leader_bar(full_bar(s));
-          if ((ROLE & 1) && rank == 0) mbar_expect_tx(full_bar(s), tx_pair);   // the bytes of both CTAs, all streams
-          if (ROLE & 1) {
-            if (FP8) {
-              // quantised weights [E, N, K] bytes: box {128 k, 64 (a7) | 128 (a8) features, 1}: K-major
-              tma_load_3d_pair(sa, &tm_w0, fb, kb * BKE, n0, c.e);
-            } else if (p.w4d && once) {
-              tma_load_4d_pair_hint(sa, &tm_w0, fb, 0, kb * BK, n0 >> 6, c.e, pol);
-            } else if (p.w4d) {
-              // one operation per weight tensor: nblk 64-column blocks in [block][k][64 n] order
-              tma_load_4d_pair(sa, &tm_w0, fb, 0, kb * BK, n0 >> 6, c.e);
-            } else {
-              tma_load_3d_pair(sa, &tm_w0, fb, n0, kb * BK, c.e);
-              if (!GATEUP) tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w0, fb, n0 + 64, kb * BK, c.e);
-            }
-          }
-          if (GATEUP && (ROLE & 2)) {
-            if (FP8) {
-              tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w1, fb, kb * BKE, n0, c.e);
-            } else if (p.w4d && once) {
-              tma_load_4d_pair_hint(sa + A_BLK_BYTES, &tm_w1, fb, 0, kb * BK, n0 >> 6, c.e, pol);
-            } else if (p.w4d) {
-              tma_load_4d_pair(sa + A_BLK_BYTES, &tm_w1, fb, 0, kb * BK, n0 >> 6, c.e);
-            } else {
-              tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w1, fb, n0, kb * BK, c.e);
-            }
+          if (rank == 0) mbar_expect_tx(full_bar(s), tx_pair);   // the bytes of both CTAs
+          if (FP8 && GATEUP) {
+            // quantised weights [E, N, K] bytes: box {128 k, 64 features, 1}: K-major, 8 KB per tensor
+            tma_load_3d_pair(sa, &tm_w0, fb, kb * BKE, n0, c.e);
+            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w1, fb, kb * BKE, n0, c.e);
+          } else if (FP8) {
+            tma_load_3d_pair(sa, &tm_w0, fb, kb * BKE, n0, c.e);      // W_down codes: box {128 k, 128 features, 1}
+          } else if (p.w4d && once) {
+            tma_load_4d_pair_hint(sa, &tm_w0, fb, 0, kb * BK, n0 >> 6, c.e, pol);
+            if (GATEUP) tma_load_4d_pair_hint(sa + A_BLK_BYTES, &tm_w1, fb, 0, kb * BK, n0 >> 6, c.e, pol);
+          } else if (p.w4d) {
+            // one operation per weight tensor: nblk 64-column blocks in [block][k][64 n] order
+            tma_load_4d_pair(sa, &tm_w0, fb, 0, kb * BK, n0 >> 6, c.e);
+            if (GATEUP) tma_load_4d_pair(sa + A_BLK_BYTES, &tm_w1, fb, 0, kb * BK, n0 >> 6, c.e);
+          } else if (GATEUP) {
+            tma_load_3d_pair(sa, &tm_w0, fb, n0, kb * BK, c.e);
+            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w1, fb, n0, kb * BK, c.e);
+          } else {
+            tma_load_3d_pair(sa, &tm_w0, fb, n0, kb * BK, c.e);
+            tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w0, fb, n0 + 64, kb * BK, c.e);
           }
           // this CTA's half of the tokens: one box of exactly `half` rows
-          if (ROLE & 4) tma_load_2d_pair(sb, tm_b, fb, kb * BKE, brow0);
+          tma_load_2d_pair(sb, tm_b, fb, kb * BKE, brow0);
         }
         __syncwarp();
         if (++s == STAGES) { s = 0; ph ^= 1u; }
       }
     }
-  };
-  if (warp == 0) {
-    producer(std::integral_constant<int, 1>{});
-  } else if (warp == 2) {
-    producer(std::integral_constant<int, 4>{});
-  } else if (GATEUP && warp == 4 + EPI_WARPS) {
-    producer(std::integral_constant<int, 2>{});
   } else if (warp == 3) {
     // ===================== tile scheduler (dynamic feed only; one thread of the leader CTA) ==========
     if (dyn && lane == 0 && rank == 0) {
@@ -414,7 +373,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       int it = 0;
       Feed feed = {0, 0, -1};
       for (int t = feed_next(feed, true); t >= 0; t = feed_next(feed, true), ++it) {
-        const TileCoord c = decode_tile(t, tile_start, cold_start, p.offsets, E, sg_max);
+        const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
         const uint32_t idesc = (FP8 ? IDESC_FP8 : IDESC_BASE) | (static_cast<uint32_t>(c.nt >> 3) << 17);
         const int as = it & 1;
         const uint32_t aph = (it >> 1) & 1u;
@@ -447,7 +406,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         }
       }
     }
-  } else if (warp >= 4 && warp < 4 + EPI_WARPS) {
+  } else if (warp >= 4) {
     // ===================== epilogue: TMEM -> registers -> shared (transpose) -> global ==========
     // A thread owns one feature (TMEM lane) and reads 32 tokens (columns) at a time; the output is
     // token-major, so each warp turns its 32 feature x 32 token block around in a private 2 KB
@@ -463,14 +422,14 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     Feed feed = {0, 0, -1};
     int t = feed_next(feed, true);
     if (!GATEUP && t >= 0) {                         // gate weights of the first tile -> buffer 0
-      const TileCoord c0 = decode_tile(t, tile_start, cold_start, p.offsets, E, sg_max);
+      const TileCoord c0 = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
       float sc = 1.0f;
       if (p.row_scale != nullptr && ew * 32 + lane < c0.rows_valid) sc = __ldg(p.row_scale + c0.row0 + ew * 32 + lane);
       sc_smem[ew * 32 + lane] = sc;
     }
     int it = 0;
     for (; t >= 0; ++it) {
-      const TileCoord c = decode_tile(t, tile_start, cold_start, p.offsets, E, sg_max);
+      const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
       const int tn = feed_next(feed, true);            // this cluster's next tile (-1: none)
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1u;
@@ -485,7 +444,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         // latency never sits on the epilogue's critical path.  The barrier makes this tile's buffer
         // (written by all eight warps at the end of the previous tile) visible.
         if (tn >= 0 && p.row_scale != nullptr) {
-          const TileCoord cn = decode_tile(tn, tile_start, cold_start, p.offsets, E, sg_max);
+          const TileCoord cn = decode_tile(tn, tile_start, t_tiles, p.offsets, E, sg_max);
           if (ew * 32 + lane < cn.rows_valid) sc_next = __ldg(p.row_scale + cn.row0 + ew * 32 + lane);
         }
         named_bar_sync(3, 32 * EPI_WARPS);
@@ -650,13 +609,13 @@ cudaError_t pair_kernels_init() {
 }
 
 cudaError_t launch_gateup_swiglu_pair(const GemmLaunch& g, cudaStream_t st) {
-  launch_pdl(pair_gemm_kernel<true>, g.num_sms & ~1, GATEUP_THREADS, SMEM_BYTES, st, g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b1_4d : g.tm_b1, make_params(g));
+  launch_pdl(pair_gemm_kernel<true>, g.num_sms & ~1, 256, SMEM_BYTES, st, g.tm_act, g.w4d ? g.tm_b0_4d : g.tm_b0, g.w4d ? g.tm_b1_4d : g.tm_b1, make_params(g));
   return cudaGetLastError();
 }
 
 // FP8 gate/up: tm_act over the e4m3 rows [rows, K bytes], tm_b0 / tm_b1 over the quantised weights [E, N, K bytes]
 cudaError_t launch_gateup_swiglu_pair_fp8(const GemmLaunch& g, cudaStream_t st) {
-  launch_pdl(pair_gemm_kernel<true, true>, g.num_sms & ~1, GATEUP_THREADS, SMEM_BYTES, st, g.tm_act, g.tm_b0, g.tm_b1, make_params(g));
+  launch_pdl(pair_gemm_kernel<true, true>, g.num_sms & ~1, 256, SMEM_BYTES, st, g.tm_act, g.tm_b0, g.tm_b1, make_params(g));
   return cudaGetLastError();
 }
 

@@ -39,7 +39,6 @@ inline int route_num_tiles(int T) { return (T + 127) / 128; }
 
 struct RouterLaunch {
   int T, d, E, k;
-  const void* hidden = nullptr;   // the contiguous [T,d] bf16 matrix (nullptr when the rows come through a segment table)
   const float* b_r;         // [E] or nullptr
   float* logits_out;        // [T,E]
   int32_t* topk_idx;        // [T,k]
@@ -52,7 +51,7 @@ struct RouterLaunch {
   int32_t* done_counter;    // one int, zero between launches (re-armed by the kernel)
   int32_t* gemm_counters;   // eight ints zeroed by the kernel's last tile (or nullptr)
   int num_sms;
-  int force_form;           // 0 = choose from T (router_sequential); tests: 1 = plain sequential form, 2 = cluster form, 3 = streaming form
+  int force_form;           // 0 = choose from T (router_sequential); 1 = sequential form; 2 = cluster form (tests)
 };
 
 // ---- segments (zero-copy COMBINE): the combined tokens given as a list

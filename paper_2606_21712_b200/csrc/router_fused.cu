@@ -107,7 +107,6 @@ struct RouterParams {
   const void* const* seg_hidden;
   const int32_t* seg_start;
   int n_segs;
-  const void* hidden;       // the contiguous [T, d] matrix (streaming form), or nullptr
 };
 
 #ifdef BG_ROUTER_TRACE
@@ -523,7 +522,7 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
     if (*last_flag) {
       // ---- 4. the last tile: scan over tiles and experts; re-arm the counters
       __threadfence();
-      scan_tiles_block256(p.tile_counts, n_tiles, E, p.tile_base, p.counts, p.offsets, scan_scratch, [] { __syncthreads(); });
+      scan_tiles_block256(p.tile_counts, n_tiles, E, p.tile_base, p.counts, p.offsets, scan_scratch);
       if (threadIdx.x == 0) {
         *p.done_counter = 0;
         if (p.gemm_counters != nullptr)
@@ -535,352 +534,6 @@ router_fused_kernel(const __grid_constant__ CUtensorMap tm_h, const __grid_const
   tc_fence_before();
   __syncthreads();
   if (warp == 2) { tc_fence_after(); tmem_dealloc(tmem_base, tmem_cols); }
-}
-
-// ===================== streaming form (large T, E <= 128, one contiguous hidden matrix) =====================
-// The same arithmetic as the sequential form -- chunk c of K accumulates in its own TMEM accumulator, the chunk sums are
-// added in ascending order, then the bias -- hence the same bits, organised for throughput instead of latency:
-//   * persistent: min(#tiles, #SMs) CTAs, CTA b runs tiles b, b + grid, ...; the loaders and the MMA warp work on tile
-//     i+1 while the epilogue warps finish tile i (the sequential form spends a third of a tile's time in an epilogue
-//     during which nothing is in flight);
-//   * two rings with their own barriers: the hidden tile (16 KB per k-block, from HBM) is copied by two warps with
-//     16-byte cp.async into the 128B-swizzled layout (as the segment path does), 3-4 k-blocks in flight per thread, and TMA
-//     carries only the three W_r pieces (one 4-D box per k-block, from L2).  The main loop itself stays bound by the
-//     MMA issue path: a k-block is 12 tcgen05.mma of M = 128, N <= 128 plus its commits, and one thread gets those out at
-//     ~85 clocks each (measured with a stand-alone issue loop: 76 clk per MMA at N = 128 with no commit, 87 with
-//     three), i.e. ~0.55 us per k-block whatever the loaders do -- the price of the exact three-piece product;
-//   * the epilogue is two threads per token row (eight warps; the MMA warp's TMEM accumulators are handed back as soon
-//     as the row's partial sums are in registers): each adds the nch partial rows of its 32-expert chunks in ascending
-//     chunk order (+ bias), writes those logits, and keeps a sorted k-list in registers; the two lists are merged
-//     through shared memory under the order of reading S3; then gates, the tile's stable ranks and histogram.
-// NC = 32-column chunks of a logit row (n_mma <= 32 NC).
-constexpr int ST_THREADS = 384;     // warps 0, 3: hidden loaders; 1: MMA; 2: TMEM + TMA (W_r pieces); 4-11: epilogue
-constexpr int ST_LOADERS = 64;
-constexpr int ST_MERGE_BYTES = BM * 16 * 4;           // the second thread's k-list of every row: [128][8 keys | 8 experts]
-constexpr int ST_BAR_BYTES = 512;
-constexpr int ST_SMEM_BYTES = RING_BYTES + 1024 + ST_BAR_BYTES + ST_MERGE_BYTES + MASK_BYTES;
-static_assert(ST_SMEM_BYTES <= 227 * 1024, "shared memory budget");
-
-template <int NC, int KMAX>
-__global__ void __launch_bounds__(ST_THREADS, 1)
-router_stream_kernel(const __grid_constant__ CUtensorMap tm_w, const RouterParams p, const int nA, const int nB) {
-  constexpr int NH = (NC + 1) / 2;                // chunks per epilogue thread
-  extern __shared__ uint8_t smem_raw[];
-  const uint32_t raw = smem_u32(smem_raw);
-  const uint32_t base = (raw + 1023u) & ~1023u;
-  uint8_t* smem = smem_raw + (base - raw);
-  const uint32_t bar_base = base + RING_BYTES;
-  constexpr int MAX_A = 8, MAX_B = 8;
-  auto fullA = [&](int s) { return bar_base + 8u * s; };
-  auto emptyA = [&](int s) { return bar_base + 8u * (MAX_A + s); };
-  auto fullB = [&](int s) { return bar_base + 8u * (2 * MAX_A + s); };
-  auto emptyB = [&](int s) { return bar_base + 8u * (2 * MAX_A + MAX_B + s); };
-  auto tfull = [&](int b) { return bar_base + 8u * (2 * MAX_A + 2 * MAX_B + b); };
-  auto tempty = [&](int b) { return bar_base + 8u * (2 * MAX_A + 2 * MAX_B + 2 + b); };
-  constexpr int NBAR = 2 * MAX_A + 2 * MAX_B + 4;
-  static_assert(8 * NBAR + 16 <= ST_BAR_BYTES, "barrier area");
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + RING_BYTES + 8 * NBAR);
-  int* last_flag = reinterpret_cast<int*>(smem + RING_BYTES + 8 * NBAR + 8);
-  uint32_t* merge = reinterpret_cast<uint32_t*>(smem + RING_BYTES + ST_BAR_BYTES);                  // [128][16]
-  uint32_t* mask = reinterpret_cast<uint32_t*>(smem + RING_BYTES + ST_BAR_BYTES + ST_MERGE_BYTES);  // [E][4]
-  int* scan_scratch = reinterpret_cast<int*>(smem);          // the ring, once every tile of this CTA is done
-
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-#ifdef BG_ROUTER_TRACE
-  auto trace = [&](int slot) {
-    if (threadIdx.x == 128 && blockIdx.x < 8 && slot < 16) {
-      unsigned long long t;
-      asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-      g_router_trace[blockIdx.x * 16 + slot] = t;
-    }
-  };
-#else
-  auto trace = [](int) {};
-#endif
-  trace(0);
-  const int T = p.T, d = p.d, E = p.E, k = p.k, nch = p.nch;
-  const int n_tiles = (T + BM - 1) / BM;
-  const int k_blocks = (d + BK - 1) / BK;
-  const int kb_per = (k_blocks + nch - 1) / nch;
-  const int n_mma = (E + 15) & ~15;
-  const int n_blk = (E + 63) / 64;
-  const uint32_t piece_bytes = n_blk * B_BLK_BYTES;
-  const uint32_t b_bytes = 3 * piece_bytes;
-  const uint32_t baseB = base + static_cast<uint32_t>(nA) * A_BYTES;
-  const bool w4d = (n_mma & 63) == 0;
-  const uint32_t idesc = umma_idesc_bf16(BM, n_mma, 0, 1);
-  const int acc_cols = nch * n_mma;                          // one tile's accumulators
-  const int n_buf = 2 * acc_cols <= 512 ? 2 : 1;             // accumulator sets (tile i+1 accumulates while tile i drains)
-  uint32_t tmem_cols = 32;
-  while (static_cast<int>(tmem_cols) < n_buf * acc_cols) tmem_cols <<= 1;
-
-  if (warp == 0 && lane == 0) {
-    tma_prefetch_desc(&tm_w);
-    for (int s = 0; s < MAX_A; ++s) { mbar_init(fullA(s), ST_LOADERS); mbar_init(emptyA(s), 1); }
-    for (int s = 0; s < MAX_B; ++s) { mbar_init(fullB(s), 1); mbar_init(emptyB(s), 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(tfull(b), 1); mbar_init(tempty(b), 8); }
-    fence_barrier_init();
-  }
-  if (warp == 2) { tmem_alloc(smem_u32(tmem_slot), tmem_cols); tmem_relinquish(); }
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot;
-  pdl_wait_then_trigger();
-  trace(1);
-
-  int my_tiles = 0;
-  if (warp == 0 || warp == 3) {                   // ---- hidden loaders: 64 threads, 16 x 16 bytes each per k-block
-    // Eight consecutive lanes copy the eight 16-byte chunks of one row's 128-byte k-span into the position the
-    // 128B swizzle gives them (row * 128 + ((chunk ^ (row & 7)) << 4)); thread li owns rows (li >> 3) + 8 j.
-    const int li = (warp == 0 ? 0 : 32) + lane, chunk = li & 7, r0 = li >> 3;
-    const int LAG = nA - 1 < 4 ? nA - 1 : 4;      // k-blocks in flight per thread (nA >= 3)
-    const uint8_t* hidden = static_cast<const uint8_t*>(p.hidden);
-    const int64_t row_bytes = static_cast<int64_t>(d) * 2;
-    int s = 0, pub_s = 0, issued = 0;
-    uint32_t ph = 0;
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-      const int t0 = tile * BM + r0;
-      const uint8_t* src0 = hidden + static_cast<int64_t>(t0) * row_bytes + chunk * 16;
-      for (int kb = 0; kb < k_blocks; ++kb) {
-        if (issued >= LAG) {                      // publish the k-block issued LAG iterations ago
-          if (LAG == 4) asm volatile("cp.async.wait_group 3;" ::: "memory");
-          else if (LAG == 3) asm volatile("cp.async.wait_group 2;" ::: "memory");
-          else asm volatile("cp.async.wait_group 1;" ::: "memory");
-          fence_proxy_async();
-          mbar_arrive_relaxed(fullA(pub_s));
-          if (++pub_s == nA) pub_s = 0;
-        }
-        mbar_wait(emptyA(s), ph ^ 1u);
-        const uint32_t sa = base + s * A_BYTES + r0 * 128 + ((chunk ^ r0) << 4);
-        const bool k_ok = kb * BK + chunk * 8 < d;            // k past d must read as zero
-        #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          const bool ok = k_ok && t0 + 8 * j < T;
-          cp_async_16(sa + j * 1024, ok ? src0 + static_cast<int64_t>(8 * j) * row_bytes + kb * (BK * 2) : hidden,
-                      ok ? 16u : 0u);
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-        ++issued;
-        if (++s == nA) { s = 0; ph ^= 1u; }
-      }
-    }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-    fence_proxy_async();
-    for (int i = issued > LAG ? LAG : issued; i > 0; --i) {
-      mbar_arrive_relaxed(fullA(pub_s));
-      if (++pub_s == nA) pub_s = 0;
-    }
-  } else if (warp == 2) {                         // ---- TMA producer: the three W_r pieces of a k-block
-    int s = 0;
-    uint32_t ph = 0;
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x)
-      for (int kb = 0; kb < k_blocks; ++kb) {
-        mbar_wait(emptyB(s), ph ^ 1u);
-        if (elect_one()) {
-          const uint32_t sb = baseB + s * b_bytes;
-          mbar_expect_tx(fullB(s), b_bytes);
-          if (w4d) {                                // one operation: [piece][block][k][64 e]
-            tma_load_4d(sb, &tm_w, fullB(s), 0, kb * BK, 0, 0);
-          } else {
-            for (int pc = 0; pc < 3; ++pc)
-              for (int j = 0; j < n_blk; ++j)
-                tma_load_3d(sb + pc * piece_bytes + j * B_BLK_BYTES, &tm_w, fullB(s), 64 * j, kb * BK, pc);
-          }
-        }
-        __syncwarp();
-        if (++s == nB) { s = 0; ph ^= 1u; }
-      }
-  } else if (warp == 1) {                         // ---- MMA issuer
-    int sa = 0, sb = 0, it = 0;
-    uint32_t pha = 0, phb = 0;
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
-      const int buf = n_buf == 2 ? (it & 1) : 0;
-      const uint32_t use = static_cast<uint32_t>(n_buf == 2 ? (it >> 1) : it);
-      mbar_wait(tempty(buf), (use & 1u) ^ 1u);     // the epilogue has pulled this accumulator set's previous tile
-      tc_fence_after();
-      for (int kb = 0; kb < k_blocks; ++kb) {
-        mbar_wait(fullA(sa), pha);
-        mbar_wait(fullB(sb), phb);
-        tc_fence_after();
-        if (elect_one()) {
-          const uint32_t a_addr = base + sa * A_BYTES, b_addr = baseB + sb * b_bytes;
-          const uint64_t ad = ADESC_HI | ((a_addr >> 4) & 0x3FFFu);
-          const int chunk = kb / kb_per;
-          const bool first = kb - chunk * kb_per == 0;
-          const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(buf * acc_cols + chunk * n_mma);
-          for (int pc = 0; pc < 3; ++pc) {          // hidden * hi + hidden * mid + hidden * lo, one accumulator
-            const uint64_t bd = BDESC_HI | (((b_addr + pc * piece_bytes) >> 4) & 0x3FFFu);
-            #pragma unroll
-            for (int kk = 0; kk < BK / UK; ++kk)
-              umma_f16(d_tmem, ad + ((kk * UK * 2) >> 4), bd + ((kk * UK * 128) >> 4), idesc,
-                       (first && pc == 0 && kk == 0) ? 0u : 1u);
-          }
-          umma_commit(emptyA(sa));
-          umma_commit(emptyB(sb));
-          if (kb + 1 == k_blocks) umma_commit(tfull(buf));
-        }
-        __syncwarp();
-        if (++sa == nA) { sa = 0; pha ^= 1u; }
-        if (++sb == nB) { sb = 0; phb ^= 1u; }
-      }
-    }
-  } else if (warp >= 4) {                         // ---- epilogue: two threads per token row of the tile
-    const int q = warp & 3, half = (warp - 4) >> 2, row = q * 32 + lane;
-    int it = 0;
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it, ++my_tiles) {
-      const int buf = n_buf == 2 ? (it & 1) : 0;
-      const uint32_t use = static_cast<uint32_t>(n_buf == 2 ? (it >> 1) : it);
-      const int t = tile * BM + row;
-      if (half == 0) {
-        named_bar_sync(1, 128);                   // the previous tile's histogram has been read
-        for (int i = row; i < ROUTE_MAX_E * 4; i += BM) mask[i] = 0u;
-      }
-      mbar_wait(tfull(buf), use & 1u);
-      tc_fence_after();
-      trace(2 + it * 5);
-      const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + static_cast<uint32_t>(buf * acc_cols);
-      float x[32 * NH];                           // this thread's chunks: half, half + 2
-      #pragma unroll
-      for (int ii = 0; ii < NH; ++ii) {
-        const int c0 = (2 * ii + half) * 32;
-        const int cols = n_mma - c0;              // columns of this chunk that exist (multiple of 16)
-        uint32_t v[32];
-        #pragma unroll
-        for (int j = 0; j < 32; ++j) v[j] = 0u;
-        if (cols >= 32) tmem_ld_32x32(taddr + c0, v);
-        else if (cols > 0) tmem_ld_32x16(taddr + c0, v);
-        tmem_ld_wait();
-        for (int c = 1; c < nch; ++c) {           // + chunk c, ascending: the cluster form's summation order
-          uint32_t u[32];
-          #pragma unroll
-          for (int j = 0; j < 32; ++j) u[j] = 0u;
-          if (cols >= 32) tmem_ld_32x32(taddr + c * n_mma + c0, u);
-          else if (cols > 0) tmem_ld_32x16(taddr + c * n_mma + c0, u);
-          tmem_ld_wait();
-          #pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(u[j]));
-        }
-        #pragma unroll
-        for (int j = 0; j < 32; ++j) x[ii * 32 + j] = __uint_as_float(v[j]);
-      }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(tempty(buf));    // accumulator set handed back
-      trace(3 + it * 5);
-      // ---- logits (+ bias), k-list over this thread's experts in ascending order
-      uint32_t bk[KMAX];
-      int be[KMAX];
-      #pragma unroll
-      for (int s = 0; s < KMAX; ++s) { bk[s] = 0u; be[s] = 0x7fffffff; }
-      const bool vec_ok = (E & 3) == 0;
-      float* lrow = p.logits_out + static_cast<int64_t>(t) * E;
-      #pragma unroll
-      for (int ii = 0; ii < NH; ++ii) {
-        const int c0 = (2 * ii + half) * 32;
-        if (p.b_r != nullptr) {
-          #pragma unroll
-          for (int j = 0; j < 32; ++j)
-            if (c0 + j < E) x[ii * 32 + j] += __ldg(p.b_r + c0 + j);
-        }
-        if (t < T) {
-          #pragma unroll
-          for (int j = 0; j < 32; j += 4)
-            if (c0 + j < E) {
-              if (vec_ok) {
-                *reinterpret_cast<float4*>(lrow + c0 + j) =
-                    make_float4(x[ii * 32 + j], x[ii * 32 + j + 1], x[ii * 32 + j + 2], x[ii * 32 + j + 3]);
-              } else {
-                #pragma unroll
-                for (int jj = 0; jj < 4; ++jj)
-                  if (c0 + j + jj < E) lrow[c0 + j + jj] = x[ii * 32 + j + jj];
-              }
-            }
-        }
-        #pragma unroll
-        for (int j = 0; j < 32; ++j)
-          if (c0 + j < E) klist_insert<KMAX, false>(bk, be, float_to_ordered(x[ii * 32 + j]), c0 + j);
-      }
-      trace(4 + it * 5);
-      // ---- merge the row's two lists (reading S3: key descending, expert index ascending)
-      if (half == 1) {
-        #pragma unroll
-        for (int s = 0; s < KMAX; ++s) {
-          merge[row * 16 + s] = bk[s];
-          merge[row * 16 + 8 + s] = static_cast<uint32_t>(be[s]);
-        }
-      }
-      named_bar_sync(2, 256);
-      if (half == 0) {
-        #pragma unroll
-        for (int s = 0; s < KMAX; ++s)
-          klist_insert<KMAX, true>(bk, be, merge[row * 16 + s], static_cast<int>(merge[row * 16 + 8 + s]));
-      }
-      named_bar_sync(2, 256);                     // the lists have been read: the next tile may overwrite them
-      if (half == 0) {
-        int e[ROUTE_MAX_K], rk[ROUTE_MAX_K];
-        #pragma unroll
-        for (int s = 0; s < ROUTE_MAX_K; ++s) e[s] = -1;
-        finish_token<KMAX>(bk, be, k, t, T, p, [&](int s, int ee) { e[s] = ee; });
-        trace(5 + it * 5);
-        tile_rank_and_counts(mask, row, e, k, E, rk, p.tile_counts + static_cast<int64_t>(tile) * E, row,
-                             [] { named_bar_sync(1, 128); });
-        #pragma unroll
-        for (int s = 0; s < ROUTE_MAX_K; ++s)
-          if (s < k && e[s] >= 0) p.tile_rank[static_cast<int64_t>(t) * k + s] = rk[s];
-        __threadfence();
-        trace(6 + it * 5);
-      }
-    }
-  }
-  tc_fence_before();
-  __syncthreads();
-  trace(14);
-  // ---- the CTA that completes the count of finished tiles scans the tile histograms; re-arms the counters
-  if (threadIdx.x == 128) *last_flag = (atomicAdd(p.done_counter, my_tiles) + my_tiles == n_tiles) ? 1 : 0;
-  __syncthreads();
-  if (*last_flag && threadIdx.x < 256) {
-    __threadfence();
-    scan_tiles_block256(p.tile_counts, n_tiles, E, p.tile_base, p.counts, p.offsets, scan_scratch,
-                        [] { named_bar_sync(3, 256); });
-    if (threadIdx.x == 0) {
-      *p.done_counter = 0;
-      if (p.gemm_counters != nullptr)
-        for (int i = 0; i < 8; ++i) p.gemm_counters[i] = 0;
-    }
-  }
-  __syncthreads();
-  trace(15);
-  if (warp == 2) { tc_fence_after(); tmem_dealloc(tmem_base, tmem_cols); }
-}
-
-// Ring split of the streaming form: nB slots of the three-piece box, the rest of the ring in 16 KB hidden tiles.
-inline bool stream_ring(int E, int* nA, int* nB) {
-  const int n_blk = (E + 63) / 64;
-  const int b_bytes = 3 * n_blk * B_BLK_BYTES;
-  *nB = 3;
-  *nA = (RING_BYTES - *nB * b_bytes) / A_BYTES;
-  if (*nA > 8) *nA = 8;
-  return E <= 128 && *nA >= 3;
-}
-
-template <int NC>
-cudaError_t launch_stream(const CUtensorMap& tm_w, const RouterParams& p, int num_sms, cudaStream_t st) {
-  int nA, nB;
-  stream_ring(p.E, &nA, &nB);
-  const int n_tiles = (p.T + BM - 1) / BM;
-  const int grid = n_tiles < num_sms ? n_tiles : num_sms;
-  if (p.k <= 2) return launch_pdl(router_stream_kernel<NC, 2>, grid, ST_THREADS, ST_SMEM_BYTES, st, tm_w, p, nA, nB);
-  if (p.k <= 4) return launch_pdl(router_stream_kernel<NC, 4>, grid, ST_THREADS, ST_SMEM_BYTES, st, tm_w, p, nA, nB);
-  return launch_pdl(router_stream_kernel<NC, 8>, grid, ST_THREADS, ST_SMEM_BYTES, st, tm_w, p, nA, nB);
-}
-
-template <int NC>
-cudaError_t init_stream() {
-  cudaError_t e;
-  if ((e = cudaFuncSetAttribute(router_stream_kernel<NC, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, ST_SMEM_BYTES)) != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute(router_stream_kernel<NC, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, ST_SMEM_BYTES)) != cudaSuccess) return e;
-  return cudaFuncSetAttribute(router_stream_kernel<NC, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, ST_SMEM_BYTES);
 }
 
 template <bool ROWS, bool SEQ, int KMAX>
@@ -934,10 +587,7 @@ cudaError_t router_kernels_init() {
   if ((e = init_k<false, false>()) != cudaSuccess) return e;
   if ((e = init_k<false, true>()) != cudaSuccess) return e;
   if ((e = init_k<true, false>()) != cudaSuccess) return e;
-  if ((e = init_k<true, true>()) != cudaSuccess) return e;
-  if ((e = init_stream<1>()) != cudaSuccess) return e;
-  if ((e = init_stream<2>()) != cudaSuccess) return e;
-  return init_stream<4>();
+  return init_k<true, true>();
 }
 
 #ifdef BG_ROUTER_TRACE
@@ -987,24 +637,11 @@ cudaError_t launch_router_fused(const CUtensorMap* tm_h, const CUtensorMap& tm_w
   p.tile_rank = r.tile_rank; p.tile_counts = r.tile_counts; p.tile_base = r.tile_base;
   p.counts = r.counts; p.offsets = r.offsets;
   p.done_counter = r.done_counter; p.gemm_counters = r.gemm_counters;
-  p.hidden = r.hidden;
   p.seg_hidden = seg ? seg->hidden : nullptr;
   p.seg_start = seg ? seg->start : nullptr;
   p.n_segs = seg ? seg->n : 0;
-  const int n_mma = (r.E + 15) & ~15;
-  const bool fits = p.nch == 1 || p.nch * n_mma <= 512;             // nch accumulators in TMEM
-  const bool seq = r.force_form == 0 ? router_sequential(r.T, r.d, r.E, r.num_sms) : (r.force_form != 2 && fits);
-  int nA, nB;
-  // The streaming form (persistent CTAs, the epilogue of a tile overlapped with the next tile's main loop) pays once
-  // most CTAs run two or more tiles (measured, C3: T = 32768 113 -> 97 us; at T = 16384, one tile per CTA, 64 -> 70 us);
-  // force_form 3 selects it wherever it exists, force_form 1 keeps the plain sequential form reachable (tests).
-  const int n_tiles = (r.T + BM - 1) / BM;
-  const bool want_stream = r.force_form == 3 || (r.force_form == 0 && 2 * n_tiles >= 3 * r.num_sms);
-  if (seq && want_stream && seg == nullptr && r.hidden != nullptr && stream_ring(r.E, &nA, &nB)) {
-    if (n_mma <= 32) return launch_stream<1>(tm_w, p, r.num_sms, st);
-    if (n_mma <= 64) return launch_stream<2>(tm_w, p, r.num_sms, st);
-    return launch_stream<4>(tm_w, p, r.num_sms, st);
-  }
+  const bool seq = r.force_form == 0 ? router_sequential(r.T, r.d, r.E, r.num_sms)
+                                     : (r.force_form == 1 && (p.nch * ((r.E + 15) & ~15) <= 512 || p.nch == 1));
   if (seg != nullptr) return seq ? launch_k<true, true>(tm_w, tm_w, tm_w1, p, st) : launch_k<true, false>(tm_w, tm_w, tm_w1, p, st);
   return seq ? launch_k<false, true>(*tm_h, tm_w, tm_w1, p, st) : launch_k<false, false>(*tm_h, tm_w, tm_w1, p, st);
 }

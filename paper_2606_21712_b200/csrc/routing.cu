@@ -112,7 +112,7 @@ __global__ void __launch_bounds__(256) scan_kernel(const int32_t* __restrict__ t
                                                    int32_t* __restrict__ offsets) {
   pdl_wait_then_trigger();
   __shared__ int scratch[2 * 256 + 8];
-  scan_tiles_block256(tile_counts, n_tiles, E, tile_base, counts, offsets, scratch, [] { __syncthreads(); });
+  scan_tiles_block256(tile_counts, n_tiles, E, tile_base, counts, offsets, scratch);
 }
 
 }  // namespace

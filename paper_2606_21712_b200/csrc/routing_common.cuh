@@ -65,12 +65,10 @@ __device__ __forceinline__ void tile_rank_and_counts(uint32_t* mask, int row, co
 // Step a4 for all tiles, by ONE block of 256 threads:
 //   counts[e] = sum_tiles tile_counts[tile][e];  offsets = exclusive scan over e, offsets[E] = total;
 //   tile_base[tile][e] = offsets[e] + sum_{tile' < tile} tile_counts[tile'][e].
-// scratch: shared, >= 2 * 256 + 8 ints.  counts / offsets may be nullptr.  Called by threads 0..255 of the block;
-// `sync256` is a barrier over exactly those threads (__syncthreads in a 256-thread block).
-template <typename Sync>
+// scratch: shared, >= 2 * 256 + 8 ints.  counts / offsets may be nullptr.
 __device__ __forceinline__ void scan_tiles_block256(const int32_t* tile_counts, int n_tiles, int E,
                                                     int32_t* tile_base, int32_t* counts, int32_t* offsets,
-                                                    int* scratch, Sync sync256) {
+                                                    int* scratch) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   int EW = 32;
   while (EW < E) EW <<= 1;                       // lanes per tile row (power of two, <= 256)
@@ -87,7 +85,7 @@ __device__ __forceinline__ void scan_tiles_block256(const int32_t* tile_counts, 
     for (int b = b0; b < b1; ++b) part += __ldcg(tile_counts + static_cast<int64_t>(b) * E + e);
   }
   gsum[tid] = part;
-  sync256();
+  __syncthreads();
   int total = 0;
   if (tid < EW)
     for (int gg = 0; gg < G; ++gg) total += gsum[gg * EW + tid];
@@ -98,7 +96,7 @@ __device__ __forceinline__ void scan_tiles_block256(const int32_t* tile_counts, 
     if (lane >= o) v += u;
   }
   if (lane == 31) wtot[warp] = v;
-  sync256();
+  __syncthreads();
   int add = 0;
   for (int w = 0; w < warp; ++w) add += wtot[w];
   const int incl = v + add;
@@ -110,7 +108,7 @@ __device__ __forceinline__ void scan_tiles_block256(const int32_t* tile_counts, 
       if (tid == E - 1) offsets[E] = incl;
     }
   }
-  sync256();
+  __syncthreads();
   if (e < E) {
     int run = excl[e];
     for (int gg = 0; gg < g; ++gg) run += gsum[gg * EW + e];

@@ -159,8 +159,7 @@ def test_expert_ffn_parity(rows, d, f):
 def test_expert_ffn_scheduler_variants(env):
     """The same FFN through (i) the pair kernel's super-group tile order, which production shapes only
     reach with experts of several thousand rows (forced here on experts of 3-5 token tiles) and (ii) the
-    static tile feed (the default is the dynamic ticket feed); both selected through bg_moe_set_debug.  The experts of
-    <= 64 rows are "cold" (their tiles are spread evenly through the ticket order): 64 and 65 rows sit on that boundary."""
+    static tile feed (the default is the dynamic ticket feed); both selected through bg_moe_set_debug."""
     rows = [1300, 0, 700, 257, 16, 1, 64, 65]
     d, f = 192, 320
     E, R = len(rows), sum(rows)
@@ -314,23 +313,21 @@ def test_combine_invariance_large_d(d, E, k):
 
 
 @pytest.mark.parametrize("T,d,E,k", [(1000, 2048, 128, 8), (333, 4096, 8, 2), (700, 1024, 64, 6), (130, 2048, 33, 3),
-                                     (40000, 512, 100, 4), (19000, 2048, 128, 8)])
+                                     (19000, 2048, 128, 8)])
 def test_router_forms_are_bit_identical(T, d, E, k):
-    """The router's cluster form (K chunks on the CTAs of a cluster, partials reduced through DSMEM), its
-    sequential form (one CTA per tile, one TMEM accumulator per chunk) and its streaming form (persistent CTAs,
-    several tiles each, one thread per token row in the epilogue) add the same partial sums in the same order:
+    """The router's cluster form (K chunks on the CTAs of a cluster, partials reduced through DSMEM) and its
+    sequential form (one CTA, one TMEM accumulator per chunk) add the same partial sums in the same order:
     logits, indices, gates and every routing table must agree bit for bit, and match the oracle."""
     cfg = wl.small_config(T=T, d=d, E=E, k=k, f=64, index=36)
     lay, g, layer = make(cfg)
     res = {}
-    for form in (1, 2, 3):
+    for form in (1, 2):
         layer.set_debug(router_form=form)
         r = layer.route(g["hidden"])
         p = layer.permute(g["hidden"], r["idx"], r["offsets"], gather=False)
         res[form] = {**r, **{kk: p[kk] for kk in ("row_src", "inv_perm")}}
     for key in ("logits", "idx", "w", "counts", "offsets", "row_src", "inv_perm"):
-        assert torch.equal(res[1][key], res[2][key]), f"{key} differs between the sequential and the cluster form"
-        assert torch.equal(res[1][key], res[3][key]), f"{key} differs between the sequential and the streaming form"
+        assert torch.equal(res[1][key], res[2][key]), f"{key} differs between the router forms"
     r = res[1]
     check_routing_against_oracle(r["logits"], r["idx"], r["w"], r["counts"], r["offsets"], r["row_src"],
                                  r["inv_perm"], E, k)
