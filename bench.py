@@ -377,11 +377,13 @@ def run_config(name: str, steps: int, peaks: dict, device_index: int, sustained:
            "ms_median": float(np.median(per)), **layer_fracs(cfg, E_act, ms, peaks)}
     row["stage_ms"] = stage_times(layer, step)
     if sustained:
+        sampler = ClockSampler(device_index)     # >= 2 s: long enough for NVML's clock / power readings to follow
         sm, n, secs, energy = sustained_ms(step, stream)
         fr = layer_fracs(cfg, E_act, sm, peaks)
         row["sustained"] = {"ms_per_step_median": sm, "steps": n, "seconds": secs, "tflops": fr["tflops"],
                             "frac_of_measured_sustained": fr["frac_of_measured_sustained"],
-                            "frac_of_measured_burst": fr["frac_of_measured_burst"], "energy": energy}
+                            "frac_of_measured_burst": fr["frac_of_measured_burst"], "energy": energy,
+                            "clocks": sampler.stop()}
     if note:
         row["note"] = note
     del layer, lay, hidden, out
@@ -425,11 +427,13 @@ def run_c3_sweep(steps: int, peaks: dict, device_index: int):
                "E_active": E_act, **layer_fracs(cfg, E_act, ms, peaks)}
         row["stage_ms"] = stage_times(layer, step)
         if T == 16384:
+            sampler = ClockSampler(device_index)
             sm, n, secs, energy = sustained_ms(step, stream)
             fr = layer_fracs(cfg, E_act, sm, peaks)
             row["sustained"] = {"ms_per_step_median": sm, "steps": n, "seconds": secs, "tflops": fr["tflops"],
                                 "frac_of_measured_sustained": fr["frac_of_measured_sustained"],
-                                "frac_of_measured_burst": fr["frac_of_measured_burst"], "energy": energy}
+                                "frac_of_measured_burst": fr["frac_of_measured_burst"], "energy": energy,
+                                "clocks": sampler.stop()}
         rows.append(row)
     del layer, lay
     torch.cuda.empty_cache()
