@@ -608,7 +608,10 @@ cudaError_t launch_split_wr(const float* W_r, int d, int E, void* pieces, cudaSt
 // depends on the combined-batch size.  Every chunk holds at least one k-block.
 int router_nch(int d) {
   const int k_blocks = (d + BK - 1) / BK;
-  if (k_blocks >= 96) return 8;
+  // At most 4 chunks: with 8 (tried for d >= 6144) a tile's cluster is 8 CTAs and T = 8192 runs 3.5 waves of them, each
+  // paying the cluster's two DSMEM barriers and the reduce-scatter for 14 k-blocks of work.  Measured at d = 7168, E = 256
+  // (one call, alternating builds): route() 160 -> 112 us at T = 8192, 90 -> 55 us at T = 4096, 59 -> 48 us at T = 2048, and
+  // 30 -> 42 us at T <= 1024, where a layer of that width spends milliseconds streaming its expert weights.
   if (k_blocks >= 32) return 4;
   if (k_blocks >= 16) return 2;
   return 1;
