@@ -42,20 +42,30 @@ struct PermArgs {
 
 template <int KMAX>
 __global__ void __launch_bounds__(256) gather_kernel(const uint4* __restrict__ hidden, const PermArgs pa, int T, int k,
-                                                     int vec_per_row, uint4* __restrict__ x_perm, const SegTable seg) {
+                                                     int vec_per_row, uint4* __restrict__ x_perm, const SegTable seg,
+                                                     int parts) {
   pdl_wait_then_trigger();
   const int lane = threadIdx.x & 31;
   const int warps_total = gridDim.x * (blockDim.x >> 5);
-  for (int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); t < T; t += warps_total) {
+  // `parts` warps share a token (a power of two; > 1 at small T, where one warp per token leaves the SMs a few dozen
+  // warps each and the kernel latency-bound): warp unit u moves columns [part, part + 1) * vec_per_row / parts of token
+  // u / parts; part 0 also records the permutation.
+  const int units = T * parts;
+  const int span = (vec_per_row + parts - 1) / parts;
+  for (int u = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); u < units; u += warps_total) {
+    const int t = u / parts, part = u - t * parts;
+    const int c_begin = part * span, c_end = min(vec_per_row, c_begin + span);
     int r = -1;
     if (lane < k) {
       const int64_t i = static_cast<int64_t>(t) * k + lane;
       const int e = __ldg(pa.topk_idx + i);
       if (e >= 0 && e < pa.E) {
         r = __ldg(pa.tile_base + static_cast<int64_t>(t >> 7) * pa.E + e) + __ldg(pa.tile_rank + i);
-        pa.inv_perm[i] = r;
-        pa.row_src[r] = static_cast<int32_t>(i);
-        if (pa.w_perm != nullptr) pa.w_perm[r] = __ldg(pa.topk_w + i);
+        if (part == 0) {
+          pa.inv_perm[i] = r;
+          pa.row_src[r] = static_cast<int32_t>(i);
+          if (pa.w_perm != nullptr) pa.w_perm[r] = __ldg(pa.topk_w + i);
+        }
       }
     }
     if (x_perm == nullptr) continue;
@@ -74,8 +84,8 @@ __global__ void __launch_bounds__(256) gather_kernel(const uint4* __restrict__ h
       ok[s] = s < k && rs >= 0;
       dst[s] = x_perm + static_cast<int64_t>(ok[s] ? rs : 0) * vec_per_row;
     }
-    int c = lane;
-    for (; c + 96 < vec_per_row; c += 128) {
+    int c = c_begin + lane;
+    for (; c + 96 < c_end; c += 128) {
       const uint4 a0 = ld_stream(src + c), a1 = ld_stream(src + c + 32), a2 = ld_stream(src + c + 64),
                   a3 = ld_stream(src + c + 96);
       #pragma unroll
@@ -87,7 +97,7 @@ __global__ void __launch_bounds__(256) gather_kernel(const uint4* __restrict__ h
           st_stream(dst[s] + c + 96, a3);
         }
     }
-    for (; c < vec_per_row; c += 32) {
+    for (; c < c_end; c += 32) {
       const uint4 a = ld_stream(src + c);
       #pragma unroll
       for (int s = 0; s < KMAX; ++s)
@@ -110,11 +120,16 @@ template <int KMAX>
 __global__ void __launch_bounds__(256) unpermute_kernel(const uint4* __restrict__ y_perm,
                                                         const int32_t* __restrict__ inv_perm,
                                                         const float* __restrict__ weights, int T, int k,
-                                                        int vec_per_row, uint4* __restrict__ out, const SegTable seg) {
+                                                        int vec_per_row, uint4* __restrict__ out, const SegTable seg,
+                                                        int parts) {
   pdl_wait_then_trigger();
   const int lane = threadIdx.x & 31;
   const int warps_total = gridDim.x * (blockDim.x >> 5);
-  for (int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); t < T; t += warps_total) {
+  const int units = T * parts;                 // `parts` warps share a token, each a column range (see gather_kernel)
+  const int span = (vec_per_row + parts - 1) / parts;
+  for (int u = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); u < units; u += warps_total) {
+    const int t = u / parts, part = u - t * parts;
+    const int c_begin = part * span, c_end = min(vec_per_row, c_begin + span);
     const uint4* rows[KMAX];
     float w[KMAX];
     #pragma unroll
@@ -133,7 +148,7 @@ __global__ void __launch_bounds__(256) unpermute_kernel(const uint4* __restrict_
     } else {
       dst = out + static_cast<int64_t>(t) * vec_per_row;
     }
-    for (int c = lane; c < vec_per_row; c += 32) {
+    for (int c = c_begin + lane; c < c_end; c += 32) {
       uint4 v[KMAX];
       #pragma unroll
       for (int s = 0; s < KMAX; ++s)
@@ -155,6 +170,13 @@ __global__ void __launch_bounds__(256) unpermute_kernel(const uint4* __restrict_
   }
 }
 
+// Warps per token: enough warps for ~48 per SM, each keeping at least one warp-wide pass of 16-byte vectors.
+inline int row_mover_parts(int T, int vec_per_row, int num_sms) {
+  int parts = 1;
+  while (parts < 8 && static_cast<int64_t>(T) * parts < 48ll * num_sms && vec_per_row / (2 * parts) >= 32) parts *= 2;
+  return parts;
+}
+
 inline int row_mover_grid(int rows, int num_sms) {
   const int blocks_needed = (rows + 7) / 8;
   const int cap = num_sms * 8;     // 8 resident blocks of 256 threads per SM
@@ -170,16 +192,17 @@ cudaError_t launch_gather(const void* hidden, const PermLaunch& pl, int T, int E
   PermArgs pa;
   pa.topk_idx = pl.topk_idx; pa.tile_rank = pl.tile_rank; pa.tile_base = pl.tile_base; pa.topk_w = pl.topk_w;
   pa.row_src = pl.row_src; pa.inv_perm = pl.inv_perm; pa.w_perm = pl.w_perm; pa.E = E;
-  const int grid = row_mover_grid(T, num_sms);
+  const int parts = row_mover_parts(T, d / 8, num_sms);
+  const int grid = row_mover_grid(T * parts, num_sms);
   if (k <= 2)
     launch_pdl(gather_kernel<2>, grid, 256, 0, st, static_cast<const uint4*>(hidden), pa, T, k, d / 8,
-                                           static_cast<uint4*>(x_perm), seg);
+                                           static_cast<uint4*>(x_perm), seg, parts);
   else if (k <= 4)
     launch_pdl(gather_kernel<4>, grid, 256, 0, st, static_cast<const uint4*>(hidden), pa, T, k, d / 8,
-                                           static_cast<uint4*>(x_perm), seg);
+                                           static_cast<uint4*>(x_perm), seg, parts);
   else
     launch_pdl(gather_kernel<8>, grid, 256, 0, st, static_cast<const uint4*>(hidden), pa, T, k, d / 8,
-                                           static_cast<uint4*>(x_perm), seg);
+                                           static_cast<uint4*>(x_perm), seg, parts);
   return cudaGetLastError();
 }
 
@@ -187,16 +210,17 @@ cudaError_t launch_unpermute(const void* y_perm, const int32_t* inv_perm, const 
                              int d, void* out, int num_sms, cudaStream_t st, const SegTable* segp) {
   const SegTable seg = segp ? *segp : SegTable{nullptr, nullptr, nullptr, 0};
   if (T == 0) return cudaSuccess;
-  const int grid = row_mover_grid(T, num_sms);
+  const int parts = row_mover_parts(T, d / 8, num_sms);
+  const int grid = row_mover_grid(T * parts, num_sms);
   if (k <= 2)
     launch_pdl(unpermute_kernel<2>, grid, 256, 0, st, static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
-                                              static_cast<uint4*>(out), seg);
+                                              static_cast<uint4*>(out), seg, parts);
   else if (k <= 4)
     launch_pdl(unpermute_kernel<4>, grid, 256, 0, st, static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
-                                              static_cast<uint4*>(out), seg);
+                                              static_cast<uint4*>(out), seg, parts);
   else
     launch_pdl(unpermute_kernel<8>, grid, 256, 0, st, static_cast<const uint4*>(y_perm), inv_perm, weights, T, k, d / 8,
-                                              static_cast<uint4*>(out), seg);
+                                              static_cast<uint4*>(out), seg, parts);
   return cudaGetLastError();
 }
 
