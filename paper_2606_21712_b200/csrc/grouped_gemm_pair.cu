@@ -66,7 +66,7 @@ constexpr int MAX_E = 256;
 constexpr int XCH_PITCH = 36;                       // words per lane row of an exchange buffer (conflict-free v4)
 constexpr int XCH_BYTES = 32 * XCH_PITCH * 4;       // 4608 B
 constexpr int BAR_BYTES = 256;
-constexpr int TABLE_BYTES = 2064;                   // 2 x (MAX_E + 1) ints, 16-byte padded
+constexpr int TABLE_BYTES = 3104;                   // 3 x (MAX_E + 1) ints (tile_start, t_tiles, offsets), 16-byte padded
 constexpr int STAGE_TILE_BYTES = 32 * 64;           // per-warp output staging: [32 tokens][32 features] bf16
 // epilogue scratch: [4 exchange buffers (a7) | 4 x 256 gate weights (a8)] then the 4 staging tiles
 constexpr int EPI_BYTES = 4 * XCH_BYTES + 4 * STAGE_TILE_BYTES + BN_MAX * 4;   // a8: 2 KB of scales + 8 staging tiles = 18 KB; FP8 a7: + 1 KB of token scales
@@ -141,7 +141,7 @@ __device__ __forceinline__ TileCoord decode_tile(int t, const int* tile_start, c
     f_tile = r / g_here;
     t_tile = sg * g + (r - f_tile * g_here);
   }
-  const int beg = __ldg(offsets + e), end = __ldg(offsets + e + 1);
+  const int beg = offsets[e], end = offsets[e + 1];    // the CTA's shared-memory copy (a global load here sits on every role's path at every tile)
   const int n_e = end - beg;
   const int base = (((n_e + tt - 1) / tt) + 15) & ~15;      // rows per token tile, multiple of 16, <= 256
   TileCoord c;
@@ -201,6 +201,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   constexpr int N_CONSUMERS = 3 + 2 * EPI_WARPS;      // two producers, the MMA thread, every epilogue warp of the pair
   int* tile_start = reinterpret_cast<int*>(smem + RING_BYTES + BAR_BYTES);
   int* t_tiles = tile_start + (MAX_E + 1);
+  int* offs = t_tiles + (MAX_E + 1);                  // offsets[0..E], copied once
   uint8_t* epi_smem = smem + RING_BYTES + BAR_BYTES + TABLE_BYTES;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -233,9 +234,12 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   {
     int tt = 0;
     if (threadIdx.x < E) {
-      const int cnt = __ldg(p.offsets + threadIdx.x + 1) - __ldg(p.offsets + threadIdx.x);
+      const int o0 = __ldg(p.offsets + threadIdx.x), o1 = __ldg(p.offsets + threadIdx.x + 1);
+      const int cnt = o1 - o0;
       tt = (cnt + BN_MAX - 1) / BN_MAX;
       t_tiles[threadIdx.x] = tt;
+      offs[threadIdx.x] = o0;
+      if (threadIdx.x == E - 1) offs[E] = o1;
     }
     int v = tt * f_tiles;
     #pragma unroll
@@ -296,7 +300,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     uint32_t ph = 0;
     Feed feed = {0, 0, -1};
     for (int t = feed_next(feed, true); t >= 0; t = feed_next(feed, true)) {
-      const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
+      const TileCoord c = decode_tile(t, tile_start, t_tiles, offs, E, sg_max);
       const int n0 = c.f_tile * OUT_FEATS + static_cast<int>(rank) * CTA_FEATS;
       const int half = c.nt >> 1;                    // this CTA's tokens (multiple of 8, <= 128)
       const int brow0 = c.row0 + static_cast<int>(rank) * half;
@@ -373,7 +377,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       int it = 0;
       Feed feed = {0, 0, -1};
       for (int t = feed_next(feed, true); t >= 0; t = feed_next(feed, true), ++it) {
-        const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
+        const TileCoord c = decode_tile(t, tile_start, t_tiles, offs, E, sg_max);
         const uint32_t idesc = (FP8 ? IDESC_FP8 : IDESC_BASE) | (static_cast<uint32_t>(c.nt >> 3) << 17);
         const int as = it & 1;
         const uint32_t aph = (it >> 1) & 1u;
@@ -422,14 +426,14 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     Feed feed = {0, 0, -1};
     int t = feed_next(feed, true);
     if (!GATEUP && t >= 0) {                         // gate weights of the first tile -> buffer 0
-      const TileCoord c0 = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
+      const TileCoord c0 = decode_tile(t, tile_start, t_tiles, offs, E, sg_max);
       float sc = 1.0f;
       if (p.row_scale != nullptr && ew * 32 + lane < c0.rows_valid) sc = __ldg(p.row_scale + c0.row0 + ew * 32 + lane);
       sc_smem[ew * 32 + lane] = sc;
     }
     int it = 0;
     for (; t >= 0; ++it) {
-      const TileCoord c = decode_tile(t, tile_start, t_tiles, p.offsets, E, sg_max);
+      const TileCoord c = decode_tile(t, tile_start, t_tiles, offs, E, sg_max);
       const int tn = feed_next(feed, true);            // this cluster's next tile (-1: none)
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1u;
@@ -444,7 +448,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         // latency never sits on the epilogue's critical path.  The barrier makes this tile's buffer
         // (written by all eight warps at the end of the previous tile) visible.
         if (tn >= 0 && p.row_scale != nullptr) {
-          const TileCoord cn = decode_tile(tn, tile_start, t_tiles, p.offsets, E, sg_max);
+          const TileCoord cn = decode_tile(tn, tile_start, t_tiles, offs, E, sg_max);
           if (ew * 32 + lane < cn.rows_valid) sc_next = __ldg(p.row_scale + cn.row0 + ew * 32 + lane);
         }
         named_bar_sync(3, 32 * EPI_WARPS);
