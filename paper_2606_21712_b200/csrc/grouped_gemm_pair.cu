@@ -42,7 +42,7 @@
 // tt_e = ceil(n_e/256) token tiles of ceil16(ceil(n_e/tt_e)) rows (the last one shorter) times
 // ceil(N_out/OUT_FEATS) feature tiles, ordered feature-tile-major / token-tile-minor so that the
 // clusters running at the same time share weight strips through L2.  Tiles are drawn in that order from a
-// global ticket counter (dynamic feed, see `feed_next`), so the neighbours really run concurrently and a strip
+// global ticket counter (dynamic feed, see `feed_tile`), so the neighbours really run concurrently and a strip
 // is read from HBM once; bg_moe_set_debug(static_tile_feed) keeps the fixed map tile t -> cluster (t mod #clusters).
 // Experts with no rows own no tiles and their weights are never touched.
 #include "kernels.h"
@@ -55,7 +55,8 @@ constexpr int BN_MAX = 256;        // UMMA N max: tokens per tile
 constexpr int BK = 64;             // k per pipeline stage = one 128-byte swizzle span of bf16
 constexpr int UK = 16;             // UMMA K for 16-bit inputs
 constexpr int STAGES = 6;
-constexpr int SCHED_SLOTS = 4;     // tile indices published ahead by the dynamic scheduler
+constexpr int SCHED_SLOTS = 4;     // tiles published ahead by the dynamic scheduler
+constexpr int SLOT_WORDS = 8;      // a published tile: ticket, expert, row0, rows_valid, f_tile, t_tile, token tiles of the expert
 constexpr int A_BLK_BYTES = 64 * BK * 2;            // 8 KB: one 64-feature block of weights
 constexpr int A_BYTES = 2 * A_BLK_BYTES;            // 16 KB: this CTA's 128 M rows
 constexpr int B_BYTES = (BN_MAX / 2) * BK * 2;      // 16 KB: this CTA's half of the tokens
@@ -65,7 +66,7 @@ constexpr int MAX_THREADS = 384;             // 4 role warps + 4 (a7) or 8 (a8) 
 constexpr int MAX_E = 256;
 constexpr int XCH_PITCH = 36;                       // words per lane row of an exchange buffer (conflict-free v4)
 constexpr int XCH_BYTES = 32 * XCH_PITCH * 4;       // 4608 B
-constexpr int BAR_BYTES = 256;
+constexpr int BAR_BYTES = 512;
 constexpr int TABLE_BYTES = 3104;                   // 3 x (MAX_E + 1) ints (tile_start, t_tiles, offsets), 16-byte padded
 constexpr int STAGE_TILE_BYTES = 32 * 64;           // per-warp output staging: [32 tokens][32 features] bf16
 // epilogue scratch: [4 exchange buffers (a7) | 4 x 256 gate weights (a8)] then the 4 staging tiles
@@ -103,7 +104,7 @@ __device__ __forceinline__ void named_bar_sync(int id, int threads) {
 }
 
 struct TileCoord {
-  int e, row0, rows_valid, nt, f_tile, t_tile;
+  int e, row0, rows_valid, nt, f_tile, t_tile, tt;
 };
 
 // tile_start[e] = first linear tile index of expert e (tile_start[E] = total);
@@ -151,6 +152,7 @@ __device__ __forceinline__ TileCoord decode_tile(int t, const int* tile_start, c
   c.nt = (c.rows_valid + 15) & ~15;
   c.f_tile = f_tile;
   c.t_tile = t_tile;
+  c.tt = tt;
   return c;
 }
 
@@ -195,7 +197,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   auto sfull_bar = [&](int i) { return bar_base + 8u * (2 * STAGES + 4 + i); };
   auto sempty_bar = [&](int i) { return bar_base + 8u * (2 * STAGES + 4 + SCHED_SLOTS + i); };
   constexpr int NBAR = 2 * STAGES + 4 + 2 * SCHED_SLOTS;
-  static_assert(8 * NBAR + 16 + 4 * SCHED_SLOTS <= BAR_BYTES, "barrier area");
+  static_assert(8 * NBAR + 16 + 4 * SLOT_WORDS * SCHED_SLOTS <= BAR_BYTES, "barrier area");
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + RING_BYTES + 8 * NBAR);
   volatile int* tile_slot = reinterpret_cast<volatile int*>(smem + RING_BYTES + 8 * NBAR + 16);
   constexpr int N_CONSUMERS = 3 + 2 * EPI_WARPS;      // two producers, the MMA thread, every epilogue warp of the pair
@@ -272,22 +274,31 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
   // share a weight strip stay concurrent however unequal the tiles of a launch are.
   const bool dyn = p.tile_counter != nullptr;
   struct Feed { int slot; uint32_t ph; int t; };
-  auto feed_next = [&](Feed& f, bool warp_collective) -> int {
+  // Next tile of this cluster into `c`; false = the stream has ended.  Dynamic feed: the scheduler thread has already
+  // DECODED the ticket (binary search over the experts, the divisions of the tile order): a consumer reads seven words
+  // instead of repeating ~0.3 us of dependent integer work at the head of every tile -- the k loops of the down GEMM are
+  // 12 k-blocks (3-5 us) long.
+  auto feed_tile = [&](Feed& f, TileCoord& c) -> bool {
     if (!dyn) {
       f.t = (f.t < 0) ? cluster_id : f.t + num_clusters;
-      return f.t < total_tiles ? f.t : -1;
+      if (f.t >= total_tiles) return false;
+      c = decode_tile(f.t, tile_start, t_tiles, offs, E, sg_max);
+      return true;
     }
     mbar_wait_cluster(sfull_bar(f.slot), f.ph);
-    const int t = tile_slot[f.slot];
-    // Hand the slot back with a RELAXED arrive whose address depends on the ticket just read (so it cannot
-    // pass the read): a releasing arrive is a fence that waits for the thread's outstanding work -- the
+    const volatile int* w = tile_slot + f.slot * SLOT_WORDS;
+    const int t = w[0];
+    c.e = w[1]; c.row0 = w[2]; c.rows_valid = w[3]; c.f_tile = w[4]; c.t_tile = w[5]; c.tt = w[6];
+    c.nt = (c.rows_valid + 15) & ~15;
+    // Hand the slot back with a RELAXED arrive whose address depends on the words just read (so it cannot
+    // pass the reads): a releasing arrive is a fence that waits for the thread's outstanding work -- the
     // epilogue's global stores, the MMA thread's in-flight tcgen05 operations -- once per tile.
     uint32_t zero;
-    asm volatile("and.b32 %0, %1, 0;" : "=r"(zero) : "r"(t));
-    if (warp_collective) __syncwarp();                 // all 32 lanes have read; one lane arrives
-    if (!warp_collective || lane == 0) mbar_arrive_cluster_relaxed(sempty_bar(f.slot) + zero, 0);
+    asm volatile("and.b32 %0, %1, 0;" : "=r"(zero) : "r"(t | c.e | c.row0 | c.rows_valid | c.f_tile | c.t_tile | c.tt));
+    __syncwarp();                                      // all 32 lanes have read; one lane arrives
+    if (lane == 0) mbar_arrive_cluster_relaxed(sempty_bar(f.slot) + zero, 0);
     if (++f.slot == SCHED_SLOTS) { f.slot = 0; f.ph ^= 1u; }
-    return t;
+    return t >= 0;
   };
 
   // The TMA and MMA roles run WARP-WIDE with one elected lane issuing (elect.sync): inside `if (lane == 0)` ptxas
@@ -299,8 +310,8 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     int s = 0;
     uint32_t ph = 0;
     Feed feed = {0, 0, -1};
-    for (int t = feed_next(feed, true); t >= 0; t = feed_next(feed, true)) {
-      const TileCoord c = decode_tile(t, tile_start, t_tiles, offs, E, sg_max);
+    TileCoord c;
+    while (feed_tile(feed, c)) {
       const int n0 = c.f_tile * OUT_FEATS + static_cast<int>(rank) * CTA_FEATS;
       const int half = c.nt >> 1;                    // this CTA's tokens (multiple of 8, <= 128)
       const int brow0 = c.row0 + static_cast<int>(rank) * half;
@@ -310,7 +321,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       // evict-first policy so that they do not displace what is reused (token tiles, routing tables, W_r pieces).
       // Measured: C3 at T = 64 / 1024 0.220 -> 0.213 / 0.254 -> 0.247 ms, T = 4096 and C2 unchanged; the same hint on
       // experts with two token tiles, or evict-last on the x_perm / H / Y stores, was slower.
-      const bool once = t_tiles[c.e] == 1;
+      const bool once = c.tt == 1;
       const uint64_t pol = l2_policy_evict_first();
       for (int kb = 0; kb < k_blocks; ++kb) {
         mbar_wait(empty_bar(s), ph ^ 1u);            // this CTA's slot is free (multicast commit)
@@ -355,8 +366,16 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         mbar_wait(sempty_bar(slot), ph ^ 1u);          // every consumer has read this slot's previous ticket
         int t = atomicAdd(p.tile_counter, 1);
         if (t >= total_tiles) t = -1;
-        tile_slot[slot] = t;
-        st_shared_cluster_u32(smem_u32(const_cast<int*>(tile_slot + slot)), 1, static_cast<uint32_t>(t));
+        int w[7] = {t, 0, 0, 0, 0, 0, 0};
+        if (t >= 0) {
+          const TileCoord c = decode_tile(t, tile_start, t_tiles, offs, E, sg_max);
+          w[1] = c.e; w[2] = c.row0; w[3] = c.rows_valid; w[4] = c.f_tile; w[5] = c.t_tile; w[6] = c.tt;
+        }
+        #pragma unroll
+        for (int i = 0; i < 7; ++i) {
+          tile_slot[slot * SLOT_WORDS + i] = w[i];
+          st_shared_cluster_u32(smem_u32(const_cast<int*>(tile_slot + slot * SLOT_WORDS + i)), 1, static_cast<uint32_t>(w[i]));
+        }
         mbar_arrive(sfull_bar(slot));                  // release.cta: the local store above
         mbar_arrive_cluster(sfull_bar(slot), 1);       // release.cluster: the remote store above
         if (t < 0) break;
@@ -376,8 +395,8 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       uint32_t ph = 0;
       int it = 0;
       Feed feed = {0, 0, -1};
-      for (int t = feed_next(feed, true); t >= 0; t = feed_next(feed, true), ++it) {
-        const TileCoord c = decode_tile(t, tile_start, t_tiles, offs, E, sg_max);
+      TileCoord c;
+      for (; feed_tile(feed, c); ++it) {
         const uint32_t idesc = (FP8 ? IDESC_FP8 : IDESC_BASE) | (static_cast<uint32_t>(c.nt >> 3) << 17);
         const int as = it & 1;
         const uint32_t aph = (it >> 1) & 1u;
@@ -424,17 +443,16 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
     float* sc_smem = reinterpret_cast<float*>(epi_smem);                        // a8: [2][BN_MAX] gate weights, double-buffered
     const int feat0 = static_cast<int>(rank) * CTA_FEATS + (GATEUP ? (q & 1) : q) * 32;   // in the pair tile
     Feed feed = {0, 0, -1};
-    int t = feed_next(feed, true);
-    if (!GATEUP && t >= 0) {                         // gate weights of the first tile -> buffer 0
-      const TileCoord c0 = decode_tile(t, tile_start, t_tiles, offs, E, sg_max);
+    TileCoord c, cn;
+    bool have = feed_tile(feed, c);
+    if (!GATEUP && have) {                           // gate weights of the first tile -> buffer 0
       float sc = 1.0f;
-      if (p.row_scale != nullptr && ew * 32 + lane < c0.rows_valid) sc = __ldg(p.row_scale + c0.row0 + ew * 32 + lane);
+      if (p.row_scale != nullptr && ew * 32 + lane < c.rows_valid) sc = __ldg(p.row_scale + c.row0 + ew * 32 + lane);
       sc_smem[ew * 32 + lane] = sc;
     }
     int it = 0;
-    for (; t >= 0; ++it) {
-      const TileCoord c = decode_tile(t, tile_start, t_tiles, offs, E, sg_max);
-      const int tn = feed_next(feed, true);            // this cluster's next tile (-1: none)
+    for (; have; ++it) {
+      const bool have_next = feed_tile(feed, cn);      // this cluster's next tile (false: none)
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1u;
       const int n_chunks = (c.nt + 31) >> 5;           // 32-token chunks (the last may be half used)
@@ -447,8 +465,7 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
         // ew*32 .. +31 now and parks them in the other buffer after this tile's chunks, so the load
         // latency never sits on the epilogue's critical path.  The barrier makes this tile's buffer
         // (written by all eight warps at the end of the previous tile) visible.
-        if (tn >= 0 && p.row_scale != nullptr) {
-          const TileCoord cn = decode_tile(tn, tile_start, t_tiles, offs, E, sg_max);
+        if (have_next && p.row_scale != nullptr) {
           if (ew * 32 + lane < cn.rows_valid) sc_next = __ldg(p.row_scale + cn.row0 + ew * 32 + lane);
         }
         named_bar_sync(3, 32 * EPI_WARPS);
@@ -571,7 +588,8 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive_cluster_relaxed(tempty_bar(as), 0);   // relaxed: must not wait for the stores
-      t = tn;
+      c = cn;
+      have = have_next;
     }
   }
 
