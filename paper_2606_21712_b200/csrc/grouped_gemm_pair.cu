@@ -323,6 +323,12 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       // experts with two token tiles, or evict-last on the x_perm / H / Y stores, was slower.
       const bool once = c.tt == 1;
       const uint64_t pol = l2_policy_evict_first();
+      // a8 with an expert's weight matrix larger than ~half of L2 (Mixtral: 117 MB): every feature tile streams 7 MB of
+      // weights past the expert's H tiles, which all later feature tiles need again -- the H tiles are loaded evict-last.
+      // Measured on C2 (ncu, same call): down reads 2.02 -> 1.66 GB (algorithmic 1.17), 686 -> 665 us; step 2.11 -> 2.09 ms.
+      // With small experts (C3: 3 MB) the sticky lines only crowd the next kernels' data (C3 T=16384 1.181 -> 1.186 ms).
+      const uint64_t pol_last = l2_policy_evict_last();
+      const bool keep_tokens = !GATEUP && static_cast<int64_t>(p.K) * p.N * 2 > (48ll << 20);
       for (int kb = 0; kb < k_blocks; ++kb) {
         mbar_wait(empty_bar(s), ph ^ 1u);            // this CTA's slot is free (multicast commit)
         if (elect_one()) {
@@ -351,7 +357,8 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
             tma_load_3d_pair(sa + A_BLK_BYTES, &tm_w0, fb, n0 + 64, kb * BK, c.e);
           }
           // this CTA's half of the tokens: one box of exactly `half` rows
-          tma_load_2d_pair(sb, tm_b, fb, kb * BKE, brow0);
+          if (keep_tokens && c.tt > 1) tma_load_2d_pair_hint(sb, tm_b, fb, kb * BKE, brow0, pol_last);
+          else tma_load_2d_pair(sb, tm_b, fb, kb * BKE, brow0);
         }
         __syncwarp();
         if (++s == STAGES) { s = 0; ph ^= 1u; }
