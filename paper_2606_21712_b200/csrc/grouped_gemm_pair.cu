@@ -325,7 +325,8 @@ pair_gemm_kernel(const __grid_constant__ ActMaps tm_act, const __grid_constant__
       const uint64_t pol = l2_policy_evict_first();
       // a8 with an expert's weight matrix larger than ~half of L2 (Mixtral: 117 MB): every feature tile streams 7 MB of
       // weights past the expert's H tiles, which all later feature tiles need again -- the H tiles are loaded evict-last.
-      // Measured on C2 (ncu, same call): down reads 2.02 -> 1.66 GB (algorithmic 1.17), 686 -> 665 us; step 2.11 -> 2.09 ms.
+      // Measured on C2: down reads 1.66-1.80 GB per launch instead of 1.73-2.02 GB (ncu, four captures; algorithmic 1.17 GB),
+      // step 2.103 / 2.102 -> 2.095 / 2.086 ms (same call, alternating builds).
       // With small experts (C3: 3 MB) the sticky lines only crowd the next kernels' data (C3 T=16384 1.181 -> 1.186 ms).
       const uint64_t pol_last = l2_policy_evict_last();
       const bool keep_tokens = !GATEUP && static_cast<int64_t>(p.K) * p.N * 2 > (48ll << 20);
