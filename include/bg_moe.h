@@ -137,6 +137,48 @@ int bg_moe_route(bg_moe_ctx* ctx, const void* hidden, int32_t T, const float* lo
                  float* logits_out, int32_t* topk_idx, float* topk_w, int32_t* counts,
                  int32_t* offsets, void* stream);
 
+/* Steps a2-a4 from given logits WITHOUT any allocation and without a context: the same results as
+ * bg_moe_route(ctx, NULL, T, logits, NULL, ...) -- same selection order, same gate arithmetic, same
+ * counts / offsets.
+ *
+ * Why it exists.  bg_moe_create cudaMallocs a workspace, and some users of this library cannot do
+ * that: a serving runtime that has already given all of HBM to pools it manages itself (the paper's
+ * runtime fills the device with KV cache and its ring parameter buffer, so a
+ * library-side cudaMalloc fails or eats memory its planner counted on), and code on a
+ * latency-critical path where cudaMalloc / cudaFree are banned because they serialise with all work
+ * in flight on the device.  This call allocates nothing -- no cudaMalloc, no cudaFree, no
+ * allocating library routine, on any call -- because the only global memory it needs beyond its
+ * arguments (per-tile expert histograms and a tile ticket) is a fixed array inside the library image.
+ *
+ * The price, all of it a consequence of that array:
+ *  - Limit: T <= BG_MOE_NOALLOC_MAX_TOKENS and E <= 256 (k <= 8).  A larger T is refused with
+ *    BG_ERR_INVALID_ARG and a message saying so in bg_moe_noalloc_last_error(); nothing is launched.
+ *  - Footprint: 131,328 bytes of device memory on EVERY GPU that loads the library, held until the
+ *    process exits whether or not this call is ever made.
+ *  - One array per GPU, shared by all calls, threads and streams.  Two calls whose kernels can be on
+ *    the same GPU at the same time (different streams without an event between them) RACE on it and
+ *    produce garbage counts; calls on one stream, or ordered by events, are fine.  The array keeps
+ *    the previous call's contents; the call clears the one word that has to start at zero itself.
+ *  - The call works on the CURRENT device: `stream` and every pointer must belong to it.  The first
+ *    call on each device looks up that device's copy of the array (cudaGetSymbolAddress, which may
+ *    make the runtime load the library's kernels onto the device); make that first call during
+ *    set-up, before any stream capture is begun.  Later calls only enqueue a 256-byte memset and
+ *    one kernel on `stream`.
+ *
+ *   logits    DEVICE fp32 [T,E] (row-major), read only
+ *   topk_idx  DEVICE int32 [T,k]; topk_w DEVICE fp32 [T,k]   (may be NULL only when T == 0)
+ *   counts    DEVICE int32 [E];   offsets DEVICE int32 [E+1], offsets[E] = T*k
+ * T == 0 writes zero counts / offsets.  All buffers are the caller's; the call is asynchronous on
+ * `stream` and never synchronises.  Returns BG_OK, BG_ERR_INVALID_ARG, BG_ERR_UNSUPPORTED (E > 256,
+ * k > 8, device not sm_100) or BG_ERR_CUDA. */
+#define BG_MOE_NOALLOC_MAX_TOKENS 16384
+int bg_moe_route_logits_noalloc(const float* logits, int32_t T, int32_t E, int32_t k,
+                                int32_t* topk_idx, float* topk_w, int32_t* counts, int32_t* offsets,
+                                void* stream);
+/* Why the calling thread's last bg_moe_route_logits_noalloc failed ("" after a success).  The
+ * string is thread-local and owned by the library. */
+const char* bg_moe_noalloc_last_error(void);
+
 /* Steps a5-a6: stable counting sort of flat index i = t*k+s by expert, and the row gather.
  *   row_src  int32 [T*k]: row_src[r] = i;   inv_perm int32 [T*k]: inv_perm[i] = r
  *   x_perm   bf16 [T*k,d]: x_perm[r,:] = hidden[row_src[r]/k,:]   (may be NULL: skip the gather) */

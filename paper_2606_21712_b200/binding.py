@@ -15,7 +15,8 @@ BG_OK, BG_ERR_INVALID_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA, BG_ERR_NOMEM, BG_ERR
 EXPORTS = ["bg_moe_create", "bg_moe_destroy", "bg_moe_set_weights", "bg_moe_route", "bg_moe_permute",
            "bg_moe_expert_ffn", "bg_moe_unpermute", "bg_moe_combined_forward", "bg_moe_combined_forward_host",
            "bg_moe_debug_views", "bg_moe_profile_enable", "bg_moe_profile_read", "bg_moe_launch_count", "bg_moe_workspace_bytes", "bg_moe_strerror",
-           "bg_moe_last_error", "bg_moe_set_debug", "bg_moe_set_weights_offloaded", "bg_moe_ring_bytes_per_call", "bg_moe_set_precision", "bg_moe_debug_fp8_views", "bg_moe_debug_fp8_down_views", "bg_moe_combined_forward_segments", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens"]
+           "bg_moe_last_error", "bg_moe_set_debug", "bg_moe_set_weights_offloaded", "bg_moe_ring_bytes_per_call", "bg_moe_set_precision", "bg_moe_debug_fp8_views", "bg_moe_debug_fp8_down_views", "bg_moe_combined_forward_segments", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens",
+           "bg_moe_route_logits_noalloc", "bg_moe_noalloc_last_error"]
 
 
 class BgMoeConfig(ctypes.Structure):
@@ -71,6 +72,9 @@ def load_library() -> ctypes.CDLL:
         lib.bg_moe_strerror.restype = ctypes.c_char_p
         lib.bg_moe_last_error.argtypes = [vp]
         lib.bg_moe_last_error.restype = ctypes.c_char_p
+        lib.bg_moe_route_logits_noalloc.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp]
+        lib.bg_moe_noalloc_last_error.argtypes = []
+        lib.bg_moe_noalloc_last_error.restype = ctypes.c_char_p
         _lib = lib
     return _lib
 
@@ -387,3 +391,34 @@ def choose_tokens(d: int, f: int, E: int, k: int, fit: BgMoeFit, target_util: fl
                                               ctypes.c_int64(memory_budget_bytes), ctypes.c_int32(granularity),
                                               ctypes.byref(tok), ctypes.byref(reached)))
     return int(tok.value), bool(reached.value)
+
+
+# ---------------------------------------------------------------------- routing without allocation
+NOALLOC_MAX_TOKENS = 16384   # BG_MOE_NOALLOC_MAX_TOKENS of include/bg_moe.h
+
+
+def route_logits_noalloc(logits, k: int, topk_idx, topk_w, counts, offsets, stream=None) -> None:
+    """bg_moe_route_logits_noalloc: top-k + gates + histogram + exclusive scan from fp32 logits [T,E], for callers
+    that may not allocate device memory (a runtime that owns all of HBM through its own pools, or a latency-critical
+    section where cudaMalloc's device-wide serialisation is banned).  No context and no workspace: the library's
+    scratch is a fixed array in its own image, which is why T <= NOALLOC_MAX_TOKENS, and why calls that may run
+    concurrently on one GPU must be ordered by the caller (they share that array).  In keeping with that, this
+    wrapper allocates nothing either: ALL four outputs are passed in (topk_idx int32 [T,k], topk_w fp32 [T,k],
+    counts int32 [E], offsets int32 [E+1]) and are overwritten.  Runs on the device of `logits`, asynchronously on
+    `stream` (default: torch's current stream).  Make the first call on a device during set-up, outside any
+    stream capture."""
+    lib = load_library()
+    assert isinstance(logits, torch.Tensor) and logits.dim() == 2, "logits: [T,E] tensor expected"
+    T, E = logits.shape
+    _chk(logits, torch.float32, (T, E), "logits")
+    _chk(topk_idx, torch.int32, (T, k), "topk_idx")
+    _chk(topk_w, torch.float32, (T, k), "topk_w")
+    _chk(counts, torch.int32, (E,), "counts")
+    _chk(offsets, torch.int32, (E + 1,), "offsets")
+    for t in (topk_idx, topk_w, counts, offsets):
+        assert t.device == logits.device, "all tensors must live on the device of `logits`"
+    with torch.cuda.device(logits.device):
+        rc = lib.bg_moe_route_logits_noalloc(_ptr(logits), T, E, k, _ptr(topk_idx), _ptr(topk_w), _ptr(counts),
+                                             _ptr(offsets), _stream(stream))
+        if rc != BG_OK:
+            raise BgMoeError(rc, lib.bg_moe_strerror(rc).decode() + " -- " + lib.bg_moe_noalloc_last_error().decode())

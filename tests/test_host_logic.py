@@ -43,6 +43,29 @@ def test_strerror_and_null_handling_without_gpu():
     assert lib.bg_moe_launch_count(None) == 0
 
 
+def test_noalloc_route_checks_its_limits_before_touching_the_gpu():
+    """bg_moe_route_logits_noalloc refuses what its fixed scratch array cannot hold, with a message, before any CUDA
+    call (so this runs without a GPU)."""
+    from paper_2606_21712_b200 import load_library, NOALLOC_MAX_TOKENS
+    lib = load_library()
+    hdr = open(os.path.join(ROOT, "include", "bg_moe.h")).read()
+    assert int(re.search(r"#define\s+BG_MOE_NOALLOC_MAX_TOKENS\s+(\d+)", hdr).group(1)) == NOALLOC_MAX_TOKENS
+    one = ctypes.c_void_p(256)            # never dereferenced: the size check comes first
+    assert lib.bg_moe_route_logits_noalloc(one, NOALLOC_MAX_TOKENS + 1, 8, 2, one, one, one, one, None) == -1
+    msg = lib.bg_moe_noalloc_last_error().decode()
+    assert "BG_MOE_NOALLOC_MAX_TOKENS" in msg and str(NOALLOC_MAX_TOKENS + 1) in msg
+    assert lib.bg_moe_route_logits_noalloc(one, 16, 257, 2, one, one, one, one, None) == -2      # E > 256
+    assert lib.bg_moe_route_logits_noalloc(one, 16, 8, 9, one, one, one, one, None) == -1        # k > E
+    assert lib.bg_moe_route_logits_noalloc(one, 16, 16, 9, one, one, one, one, None) == -2       # k > 8
+    assert lib.bg_moe_route_logits_noalloc(one, -1, 8, 2, one, one, one, one, None) == -1
+    assert lib.bg_moe_route_logits_noalloc(one, 16, 8, 2, one, one, None, one, None) == -1       # counts NULL
+    assert lib.bg_moe_route_logits_noalloc(None, 16, 8, 2, one, one, one, one, None) == -1       # logits NULL
+    # and its translation unit calls no allocating routine at all
+    src = open(os.path.join(ROOT, "paper_2606_21712_b200", "csrc", "route_noalloc.cu")).read()
+    assert not re.search(r"\b(cudaMalloc\w*|cudaFree\w*|cudaHostAlloc|cuMemAlloc\w*|malloc|new)\s*[\(\[]", src)
+    assert "cudaGetSymbolAddress" in src and "static __device__ __align__(256)" in src
+
+
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
 def test_no_cpu_fallback_create_fails_loudly():
     from paper_2606_21712_b200 import MoELayer, BgMoeError
