@@ -180,6 +180,11 @@ int bg_moe_route_logits_noalloc(const float* logits, int32_t T, int32_t E, int32
 const char* bg_moe_noalloc_last_error(void);
 
 /* Steps a5-a6: stable counting sort of flat index i = t*k+s by expert, and the row gather.
+ *   topk_idx int32 [T,k], every entry in [0,E).  Any list is sorted correctly: a token may name the
+ *            same expert in several slots (each entry gets its own row, lower slot first).
+ *   offsets  int32 [E+1]: must be the exclusive scan of topk_idx's histogram (what bg_moe_route
+ *            returned for these indices).  The permutation is rebuilt from topk_idx alone; offsets is
+ *            not read, and a table that disagrees with topk_idx does not change the result.
  *   row_src  int32 [T*k]: row_src[r] = i;   inv_perm int32 [T*k]: inv_perm[i] = r
  *   x_perm   bf16 [T*k,d]: x_perm[r,:] = hidden[row_src[r]/k,:]   (may be NULL: skip the gather) */
 int bg_moe_permute(bg_moe_ctx* ctx, const void* hidden, int32_t T, const int32_t* topk_idx,
@@ -222,18 +227,37 @@ int bg_moe_combined_forward_segments(bg_moe_ctx* ctx, const bg_moe_segment* segm
 /* Same, but `hidden_host` and `out_host` are HOST pointers (pinned memory, or the copies are not
  * asynchronous): hidden host->device, the fused chain, out device->host.  The three run on streams the
  * context owns, over two staging slots, so that consecutive calls overlap the upload of call i+1 and the
- * download of call i-1 with the GEMMs of call i.  Ordering: hidden_host must hold its data when the call is
- * made (host memory is not stream-ordered); the call is ordered after every earlier call on the context;
- * `stream` is made to wait for the download, so work enqueued on `stream` afterwards -- or a synchronize
- * on it -- sees out_host complete. */
+ * download of call i-1 with the GEMMs of call i.
+ * Ordering and lifetime of the two host buffers:
+ *  - The upload does NOT run on `stream` and does not wait for it (if it did, call i+1's upload would
+ *    queue behind call i's download and nothing would overlap).  hidden_host must therefore hold its
+ *    data when the call is made -- work still pending on `stream` that fills it (a D2H copy, a host
+ *    function) is NOT ordered before the upload; finish it first.
+ *  - hidden_host is read asynchronously after the call returns: keep it alive and unmodified until the
+ *    upload has finished.  bg_moe_host_input_sync(ctx) blocks the calling thread until the upload of the
+ *    most recent host call is done (it does not wait for the GEMMs); a synchronize on `stream` after the
+ *    call implies it too.  A caller cycling through >= 2 input buffers needs neither.
+ *  - The call is ordered after every earlier call on the context; `stream` is made to wait for the
+ *    download, so work enqueued on `stream` afterwards -- or a synchronize on it -- sees out_host
+ *    complete.  out_host must stay alive until then. */
 int bg_moe_combined_forward_host(bg_moe_ctx* ctx, const void* hidden_host, int32_t T,
                                  void* out_host, void* stream);
+/* Blocks until the host->device upload of the most recent bg_moe_combined_forward_host call has
+ * finished, i.e. until that call's hidden_host may be overwritten or freed.  BG_OK at once if no
+ * host call has been made. */
+int bg_moe_host_input_sync(bg_moe_ctx* ctx);
 
 /* Device pointers into the workspace holding the routing artefacts of the LAST fused call
  * (valid until the next call on this context).  Any out-pointer may be NULL. */
 int bg_moe_debug_views(bg_moe_ctx* ctx, const float** logits, const int32_t** topk_idx,
                        const float** topk_w, const int32_t** counts, const int32_t** offsets,
                        const int32_t** row_src, const int32_t** inv_perm);
+
+/* The two intermediates of the expert FFN of the LAST fused call, in expert order (row r = the r-th row of
+ * row_src): H bf16 [T*k, f] = silu(x W_gate) . (x W_up), and Y bf16 [T*k, d] = the down GEMM's output,
+ * already multiplied by the row's gate weight in the fused chain.  Workspace pointers, valid until the next
+ * call on this context; either out-pointer may be NULL.  For tests that check one expert's rows. */
+int bg_moe_debug_ffn_views(bg_moe_ctx* ctx, const void** H, const void** Y);
 
 /* Per-kernel timing of the fused chain.  While enabled, bg_moe_combined_forward records a CUDA
  * event on `stream` before and after each of its BG_MOE_NUM_STAGES kernels (in launch order:

@@ -16,7 +16,7 @@ EXPORTS = ["bg_moe_create", "bg_moe_destroy", "bg_moe_set_weights", "bg_moe_rout
            "bg_moe_expert_ffn", "bg_moe_unpermute", "bg_moe_combined_forward", "bg_moe_combined_forward_host",
            "bg_moe_debug_views", "bg_moe_profile_enable", "bg_moe_profile_read", "bg_moe_launch_count", "bg_moe_workspace_bytes", "bg_moe_strerror",
            "bg_moe_last_error", "bg_moe_set_debug", "bg_moe_set_weights_offloaded", "bg_moe_ring_bytes_per_call", "bg_moe_set_precision", "bg_moe_debug_fp8_views", "bg_moe_debug_fp8_down_views", "bg_moe_combined_forward_segments", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens",
-           "bg_moe_route_logits_noalloc", "bg_moe_noalloc_last_error"]
+           "bg_moe_route_logits_noalloc", "bg_moe_noalloc_last_error", "bg_moe_host_input_sync", "bg_moe_debug_ffn_views"]
 
 
 class BgMoeConfig(ctypes.Structure):
@@ -61,6 +61,8 @@ def load_library() -> ctypes.CDLL:
         lib.bg_moe_unpermute.argtypes = [vp, vp, vp, vp, i32, vp, vp]
         lib.bg_moe_combined_forward.argtypes = [vp, vp, i32, vp, vp]
         lib.bg_moe_combined_forward_host.argtypes = [vp, vp, i32, vp, vp]
+        lib.bg_moe_host_input_sync.argtypes = [vp]
+        lib.bg_moe_debug_ffn_views.argtypes = [vp] + [ctypes.POINTER(vp)] * 2
         lib.bg_moe_debug_views.argtypes = [vp] + [ctypes.POINTER(vp)] * 7
         lib.bg_moe_profile_enable.argtypes = [vp, ctypes.c_int]
         lib.bg_moe_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
@@ -201,6 +203,19 @@ class MoELayer:
             out[name] = t.view(torch.bfloat16) if name == "H" else t
         return out
 
+    def ffn_views(self, T: int, rows=None) -> dict:
+        """bg_moe_debug_ffn_views: H bf16 [T*k, f] and Y bf16 [T*k, d] of the last fused call (expert order), copied out
+        of the workspace; rows = (r0, r1) copies only that row range."""
+        ptrs = [ctypes.c_void_p() for _ in range(2)]
+        self._check(self.lib.bg_moe_debug_ffn_views(self._ctx, *[ctypes.byref(p) for p in ptrs]))
+        R = T * self.k
+        r0, r1 = (0, R) if rows is None else rows
+        out = {}
+        for p, (name, width) in zip(ptrs, (("H", self.f), ("Y", self.d))):
+            t = torch.as_tensor(_DeviceArray(p.value, (R, width), "<u2"), device=self._dev())
+            out[name] = t[r0:r1].clone().view(torch.bfloat16)
+        return out
+
     @property
     def ring_bytes_per_call(self) -> int:
         return int(self.lib.bg_moe_ring_bytes_per_call(self._ctx))
@@ -269,7 +284,9 @@ class MoELayer:
         return out
 
     def combined_forward_host(self, hidden_host, out_host=None, stream=None):
-        """hidden_host / out_host: CPU (ideally pinned) bf16 tensors; copies run on `stream`."""
+        """hidden_host / out_host: CPU (ideally pinned) bf16 tensors.  The copies run on streams the context owns;
+        `stream` waits for the download.  Keep hidden_host alive and unmodified until host_input_sync() (or a
+        synchronize on `stream`) -- the upload is asynchronous and torch's host allocator does not know of it."""
         T = hidden_host.shape[0]
         _chk(hidden_host, torch.bfloat16, (T, self.d), "hidden_host", cuda=False)
         if out_host is None:
@@ -279,6 +296,10 @@ class MoELayer:
         self._check(self.lib.bg_moe_combined_forward_host(self._ctx, _ptr(hidden_host), T, _ptr(out_host),
                                                           _stream(stream)))
         return out_host
+
+    def host_input_sync(self):
+        """bg_moe_host_input_sync: blocks until the last combined_forward_host's upload has finished."""
+        self._check(self.lib.bg_moe_host_input_sync(self._ctx))
 
     def build_segments(self, hidden_segments, out_segments):
         """The bg_moe_segment array for a list of per-coroutine tensors (marshalling only; reusable)."""

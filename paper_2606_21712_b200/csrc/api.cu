@@ -89,6 +89,7 @@ struct bg_moe_ctx {
   const uint8_t* host_wd = nullptr;
   uint8_t* ring = nullptr;            // device: 2 halves x ring_chunk experts x (W_gate | W_up | W_down)
   int ring_chunk = 0;                 // experts per half (0 = weights are resident)
+  size_t ring_bytes = 0;              // size of the `ring` allocation
   cudaStream_t st_ring = nullptr;
   cudaEvent_t ev_ring_ready[2] = {}, ev_ring_free[2] = {};
   bool ring_used[2] = {false, false};
@@ -639,15 +640,29 @@ int bg_moe_set_debug(bg_moe_ctx* ctx, int32_t static_tile_feed, int32_t supergro
   return BG_OK;
 }
 
+// A failed parameter update must not leave a half-new layer behind (new expert tensor maps with the old router
+// pieces, or a freed ring with the old chunk size): after any failure past the argument checks the context holds
+// NO weights, and every forward call answers BG_ERR_NO_WEIGHTS until a set_weights call succeeds.
+static void drop_weights(bg_moe_ctx* ctx) {
+  ctx->W_r = nullptr; ctx->b_r = nullptr;
+  ctx->W_gate = ctx->W_up = ctx->W_down = nullptr;
+  ctx->host_wg = ctx->host_wu = ctx->host_wd = nullptr;
+  ctx->ring_chunk = 0;
+  ctx->precision = 0;
+}
+
 int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, const void* W_gate, const void* W_up,
                        const void* W_down, void* stream) {
   if (!ctx || !W_r || !W_gate || !W_up || !W_down) return BG_ERR_INVALID_ARG;
   if (!aligned16(W_r) || !aligned16(W_gate) || !aligned16(W_up) || !aligned16(W_down)) return BG_ERR_INVALID_ARG;
   const bg_moe_config& c = ctx->cfg;
-  if (!encode_weight_maps(ctx, &ctx->wm[0], W_gate, W_up, W_down, c.E)) return BG_ERR_CUDA;
+  bg_moe_ctx::WeightMaps maps;                     // encoded aside, committed once nothing can fail any more
+  if (!encode_weight_maps(ctx, &maps, W_gate, W_up, W_down, c.E)) return BG_ERR_CUDA;   // context untouched
   int rc = set_router_weights(ctx, W_r, static_cast<cudaStream_t>(stream));
-  if (rc) return rc;
+  if (rc) { drop_weights(ctx); return rc; }        // the router pieces may be half written
+  ctx->wm[0] = maps;
   ctx->W_r = W_r; ctx->b_r = b_r; ctx->W_gate = W_gate; ctx->W_up = W_up; ctx->W_down = W_down;
+  ctx->host_wg = ctx->host_wu = ctx->host_wd = nullptr;
   ctx->ring_chunk = 0;            // resident weights
   ctx->precision = 0;             // new weights: bf16 until bg_moe_set_precision quantises them
   return BG_OK;
@@ -662,16 +677,24 @@ int bg_moe_set_weights_offloaded(bg_moe_ctx* ctx, const float* W_r, const float*
   const int chunk = ring_experts / 2 < c.E ? ring_experts / 2 : c.E;
   const size_t gu_bytes = static_cast<size_t>(c.d) * c.f * 2;
   const size_t half_bytes = 3 * gu_bytes * chunk;
-  if (ctx->ring == nullptr || ctx->ring_chunk != chunk) {
-    // set-up time allocation (like the caller's own weight tensors); nothing is allocated per call
-    if (ctx->st_ring) BG_CUDA(ctx, cudaStreamSynchronize(ctx->st_ring), "ring stream sync");
-    if (ctx->ring) { cudaFree(ctx->ring); ctx->ring = nullptr; }
+  if (ctx->ring == nullptr || ctx->ring_bytes != 2 * half_bytes) {
+    // set-up time allocation (like the caller's own weight tensors); nothing is allocated per call.  The old ring
+    // goes first (both need not fit at once), so a context that was streaming its weights has none from here on
+    // until this call succeeds.
+    if (ctx->st_ring && cudaStreamSynchronize(ctx->st_ring) != cudaSuccess) {
+      ctx->last_error = std::string("ring stream sync: ") + cudaGetErrorString(cudaGetLastError());
+      drop_weights(ctx);
+      return BG_ERR_CUDA;
+    }
+    if (ctx->ring) { cudaFree(ctx->ring); ctx->ring = nullptr; ctx->ring_bytes = 0; }
+    if (ctx->ring_chunk != 0) drop_weights(ctx);   // streamed weights lose their ring; resident ones are unaffected
     void* p = nullptr;
     if (cudaMalloc(&p, 2 * half_bytes) != cudaSuccess) {
       cudaGetLastError();
       return BG_ERR_NOMEM;
     }
     ctx->ring = static_cast<uint8_t*>(p);
+    ctx->ring_bytes = 2 * half_bytes;
     if (ctx->st_ring == nullptr) {
       BG_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->st_ring, cudaStreamNonBlocking), "ring stream");
       for (int i = 0; i < 2; ++i) {
@@ -681,13 +704,15 @@ int bg_moe_set_weights_offloaded(bg_moe_ctx* ctx, const float* W_r, const float*
     }
     ctx->ring_used[0] = ctx->ring_used[1] = false;
   }
+  bg_moe_ctx::WeightMaps maps[2];
   for (int h = 0; h < 2; ++h) {
     uint8_t* half = ctx->ring + h * half_bytes;
-    if (!encode_weight_maps(ctx, &ctx->wm[1 + h], half, half + chunk * gu_bytes, half + 2 * chunk * gu_bytes, chunk))
-      return BG_ERR_CUDA;
+    if (!encode_weight_maps(ctx, &maps[h], half, half + chunk * gu_bytes, half + 2 * chunk * gu_bytes, chunk))
+      return BG_ERR_CUDA;                          // nothing committed yet
   }
   int rc = set_router_weights(ctx, W_r, static_cast<cudaStream_t>(stream));
-  if (rc) return rc;
+  if (rc) { drop_weights(ctx); return rc; }
+  ctx->wm[1] = maps[0]; ctx->wm[2] = maps[1];
   ctx->W_r = W_r; ctx->b_r = b_r;
   ctx->host_wg = static_cast<const uint8_t*>(W_gate_host);
   ctx->host_wu = static_cast<const uint8_t*>(W_up_host);
@@ -764,6 +789,13 @@ int bg_moe_debug_fp8_down_views(bg_moe_ctx* ctx, const void** H, const void** hq
   if (sh_perm) *sh_perm = ctx->sh_perm;
   if (q_down) *q_down = ctx->q_down;
   if (sw_down) *sw_down = ctx->sw_down;
+  return BG_OK;
+}
+
+int bg_moe_debug_ffn_views(bg_moe_ctx* ctx, const void** H, const void** Y) {
+  if (!ctx) return BG_ERR_INVALID_ARG;
+  if (H) *H = ctx->H;
+  if (Y) *Y = ctx->Y;
   return BG_OK;
 }
 
@@ -982,6 +1014,14 @@ int bg_moe_combined_forward_host(bg_moe_ctx* ctx, const void* hidden_host, int32
   ctx->host_slot ^= 1;
   ctx->host_calls += 1;
   ctx->host_call_pending = true;
+  return BG_OK;
+}
+
+int bg_moe_host_input_sync(bg_moe_ctx* ctx) {
+  if (!ctx) return BG_ERR_INVALID_ARG;
+  if (ctx->host_calls == 0) return BG_OK;
+  DeviceGuard guard(ctx->cfg.device);
+  BG_CUDA(ctx, cudaEventSynchronize(ctx->ev_h2d[ctx->host_slot ^ 1]), "wait for the last upload");
   return BG_OK;
 }
 

@@ -24,7 +24,7 @@ __global__ void __launch_bounds__(256) quantize_weights_kernel(const __nv_bfloat
                                                                uint8_t* __restrict__ Wq, float* __restrict__ sw) {
   __shared__ float red[8][33];
   __shared__ float scale[32];
-  __shared__ uint8_t tile[32][36];                        // [channel][k within a 32-row slab] (+4: bank spread)
+  __shared__ __align__(16) uint8_t tile[32][36];                        // [channel][k within a 32-row slab] (+4: bank spread)
   const int e = blockIdx.y, n0 = blockIdx.x * 32;
   const int cn = threadIdx.x & 31, kl = threadIdx.x >> 5; // channel within the block, k lane 0..7
   const int n = n0 + cn;

@@ -83,14 +83,20 @@ __global__ void __launch_bounds__(ROUTE_TILE) topk_tile_kernel(const float* __re
 }
 
 // Per-tile histogram and tile-local rank from caller-supplied indices (entries outside [0,E) are skipped).
+// Unlike the router's own top-k, a caller's list may name the same expert in several slots of one token, so the
+// single bit per (expert, token) of tile_rank_and_counts is not enough here: one bit plane per SLOT.  Bit `row` of
+// plane[s][e] is set iff entry (row, s) goes to expert e; the stable rank of entry (row, s) -- entries ordered by
+// flat index t*k+s -- is the number of entries of e in lower rows (any slot) plus the number of lower slots of the
+// same row that name e, and counts[e] is the number of ENTRIES, not of tokens.
 __global__ void __launch_bounds__(ROUTE_TILE) tile_rank_kernel(const int32_t* __restrict__ topk_idx, int T, int E, int k,
                                                                int32_t* __restrict__ tile_rank,
                                                                int32_t* __restrict__ tile_counts) {
   pdl_wait_then_trigger();
-  __shared__ uint32_t mask[ROUTE_MAX_E * 4];
-  for (int i = threadIdx.x; i < ROUTE_MAX_E * 4; i += ROUTE_TILE) mask[i] = 0u;
+  __shared__ uint32_t plane[ROUTE_MAX_K][ROUTE_MAX_E * 4];     // 32 KB
+  for (int s = 0; s < k; ++s)
+    for (int i = threadIdx.x; i < E * 4; i += ROUTE_TILE) plane[s][i] = 0u;
   const int row = threadIdx.x, t = blockIdx.x * ROUTE_TILE + row;
-  int e[ROUTE_MAX_K], rk[ROUTE_MAX_K];
+  int e[ROUTE_MAX_K];
   #pragma unroll
   for (int s = 0; s < ROUTE_MAX_K; ++s) {
     e[s] = -1;
@@ -100,11 +106,36 @@ __global__ void __launch_bounds__(ROUTE_TILE) tile_rank_kernel(const int32_t* __
     }
   }
   __syncthreads();
-  tile_rank_and_counts(mask, row, e, k, E, rk, tile_counts + static_cast<int64_t>(blockIdx.x) * E, threadIdx.x,
-                       [] { bar128(); });
   #pragma unroll
   for (int s = 0; s < ROUTE_MAX_K; ++s)
-    if (s < k && e[s] >= 0) tile_rank[static_cast<int64_t>(t) * k + s] = rk[s];
+    if (s < k && e[s] >= 0) atomicOr(&plane[s][e[s] * 4 + (row >> 5)], 1u << (row & 31));
+  __syncthreads();
+  const int w = row >> 5;
+  const uint32_t below = (1u << (row & 31)) - 1u;
+  #pragma unroll
+  for (int s = 0; s < ROUTE_MAX_K; ++s)
+    if (s < k && e[s] >= 0) {
+      int r = 0;
+      for (int s2 = 0; s2 < k; ++s2) {
+        const uint32_t* m = plane[s2] + e[s] * 4;
+        r += __popc(m[w] & below);
+        #pragma unroll
+        for (int j = 0; j < 3; ++j)
+          if (j < w) r += __popc(m[j]);
+      }
+      #pragma unroll
+      for (int s2 = 0; s2 < ROUTE_MAX_K; ++s2)
+        if (s2 < s && e[s2] == e[s]) ++r;
+      tile_rank[static_cast<int64_t>(t) * k + s] = r;
+    }
+  for (int x = threadIdx.x; x < E; x += ROUTE_TILE) {
+    int c = 0;
+    for (int s2 = 0; s2 < k; ++s2) {
+      const uint32_t* m = plane[s2] + x * 4;
+      c += __popc(m[0]) + __popc(m[1]) + __popc(m[2]) + __popc(m[3]);
+    }
+    tile_counts[static_cast<int64_t>(blockIdx.x) * E + x] = c;
+  }
 }
 
 __global__ void __launch_bounds__(256) scan_kernel(const int32_t* __restrict__ tile_counts, int n_tiles, int E,

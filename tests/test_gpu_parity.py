@@ -109,6 +109,33 @@ def test_route_logits_in_ties_and_bias():
     check_routing_against_oracle(r["logits"], r["idx"], r["w"], r["counts"], r["offsets"], None, None, E, k)
 
 
+@pytest.mark.parametrize("T,E,k", [(300, 5, 4), (129, 8, 8), (1000, 200, 8), (77, 3, 3), (513, 256, 2), (64, 1, 1)])
+def test_permute_accepts_duplicate_experts_in_a_token(T, E, k):
+    """bg_moe_permute sorts ANY caller-supplied index list (include/bg_moe.h): a token may name one expert in
+    several slots.  Each entry must get its own row, lower slot first -- the plain stable counting sort of the
+    oracle -- and the gathered rows must follow."""
+    rng = np.random.default_rng(100 + T)
+    idx = rng.integers(0, E, size=(T, k)).astype(np.int32)
+    idx[0, :] = idx[0, 0]                        # one token, the same expert in every slot
+    if T > 130:
+        idx[127, :2] = idx[128, :2] = 0          # duplicates on both sides of a tile boundary
+    assert k == 1 or any(len(set(r)) < k for r in idx.tolist())
+    o_counts, o_offsets, o_rs, o_ip = oracle.hist_scan_perm(idx, E)
+    cfg = wl.small_config(T=T, d=64, E=E, k=k, f=64, index=14)
+    lay = wl.make_layer(cfg)
+    from paper_2606_21712_b200 import MoELayer
+    layer = MoELayer(64, 64, E, k, T)
+    hidden = lay["hidden"].cuda()
+    p = layer.permute(hidden, torch.from_numpy(idx).cuda(), torch.from_numpy(o_offsets).cuda())
+    torch.cuda.synchronize()
+    rs, ip = p["row_src"].cpu().numpy(), p["inv_perm"].cpu().numpy()
+    assert np.array_equal(np.sort(ip), np.arange(T * k)), "inv_perm is not a bijection"
+    assert np.array_equal(rs, o_rs) and np.array_equal(ip, o_ip)
+    xo = oracle.gather(lay["hidden"], o_rs, k)
+    xg = p["x_perm"].view(torch.int16).cpu().numpy().view(np.uint16)
+    assert np.array_equal(xg, xo), "gathered rows differ"
+
+
 def test_one_expert_gets_everything_and_empty_experts():
     T, E, k = 500, 16, 2
     L = np.full((T, E), -5.0, np.float32)
@@ -292,7 +319,7 @@ def test_combine_invariance_large_d(d, E, k):
     """the router's K partition (cluster of router_nch(d) CTAs, partials added in chunk order) is a
     function of d only, so the fp32 logits of a row -- and everything downstream -- cannot depend on how many
     tokens it was combined with.  T=4096 against its two halves and against single 128-token tiles, at the d of
-    C3 / C2,C5 / C4 (4 / 4 / 8 K chunks)."""
+    C3 / C2,C5 / C4 (2 / 4 / 4 K chunks: router_nch caps at 4)."""
     cfg = wl.small_config(T=4096, d=d, E=E, k=k, f=128, index=33)
     lay, g, layer = make(cfg)
     h = g["hidden"]
@@ -339,9 +366,12 @@ def test_host_entry_point_and_zero_tokens():
     cfg = wl.small_config(T=200, d=128, E=8, k=2, f=128, index=29)
     lay, g, layer = make(cfg)
     dev_out = layer.combined_forward(g["hidden"])
-    host_out = layer.combined_forward_host(lay["hidden"].pin_memory())
+    h_pinned = lay["hidden"].pin_memory()     # referenced until the upload is done (include/bg_moe.h: lifetime rule)
+    host_out = layer.combined_forward_host(h_pinned)
+    layer.host_input_sync()                   # the upload is finished: the input may be overwritten ...
+    h_pinned.zero_()
     torch.cuda.synchronize()
-    assert torch.equal(host_out, dev_out.cpu())
+    assert torch.equal(host_out, dev_out.cpu())   # ... without touching the result
     # pipelined back-to-back host calls with different inputs and sizes (two staging slots, the context's own
     # copy / compute streams): every result must equal the device-pointer path on the same rows
     gen = torch.Generator().manual_seed(5)
@@ -469,7 +499,8 @@ def test_offloaded_weights_ring_buffer_equals_resident(ring_experts):
                                logits_in=L)["out"]
     check_out(c, o, f"ring of {ring_experts}")
     # host entry point and zero-copy segments ride the same ring
-    host_out = layer.combined_forward_host(lay["hidden"].pin_memory())
+    h_pinned = lay["hidden"].pin_memory()     # kept referenced until the synchronize below
+    host_out = layer.combined_forward_host(h_pinned)
     segs = [g["hidden"][:100].clone(), g["hidden"][100:].clone()]
     outs = layer.combined_forward_segments(segs)
     torch.cuda.synchronize()
@@ -477,6 +508,39 @@ def test_offloaded_weights_ring_buffer_equals_resident(ring_experts):
     # back to resident weights on the same context
     layer.set_weights(g["W_r"], g["b_r"], g["W_gate"], g["W_up"], g["W_down"])
     assert torch.equal(layer.combined_forward(g["hidden"]), ref)
+
+
+def test_failed_ring_allocation_leaves_no_half_state():
+    """A bg_moe_set_weights_offloaded call that cannot get its ring must leave the context either as it was
+    (resident weights) or without weights (BG_ERR_NO_WEIGHTS from the next forward) -- never with a freed ring and
+    the old chunk size.  The impossible request is a ring of 2 x 256 Mixtral-sized experts (~180 GB); the host
+    pointers are never read because no forward succeeds while they are installed... except the small first ring,
+    which is only installed, not run."""
+    import ctypes
+    from paper_2606_21712_b200 import MoELayer, BgMoeError, BG_ERR_NO_WEIGHTS, BG_ERR_NOMEM
+    d, f, E, k = 4096, 14336, 256, 2
+    layer = MoELayer(d, f, E, k, 8)
+    W_r = torch.zeros(d, E, device="cuda")
+    fake = torch.zeros(64, dtype=torch.uint8).pin_memory()          # stands for three 30 GB host tensors: never read
+    hp = ctypes.c_void_p(fake.data_ptr())
+    st = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    call = lambda ring: layer.lib.bg_moe_set_weights_offloaded(layer._ctx, ctypes.c_void_p(W_r.data_ptr()), None, hp, hp,
+                                                               hp, ring, st)
+    assert call(2) == 0                                             # 0.7 GB ring: fits
+    assert call(512) == BG_ERR_NOMEM                                # 2 x 256 experts: cannot fit
+    x = torch.zeros(8, d, dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(BgMoeError) as ei:
+        layer.combined_forward(x)
+    assert ei.value.status == BG_ERR_NO_WEIGHTS
+    torch.cuda.synchronize()
+    layer.close()
+    # resident weights survive a failed switch to a ring
+    cfg = wl.small_config(T=100, d=128, E=8, k=2, f=128, index=41)
+    lay, g, small = make(cfg)
+    ref = small.combined_forward(g["hidden"]).clone()
+    rc = small.lib.bg_moe_set_weights_offloaded(small._ctx, ctypes.c_void_p(g["W_r"].data_ptr()), None, hp, hp, hp, 1, st)
+    assert rc == -1                                                 # odd ring: refused, nothing touched
+    assert torch.equal(small.combined_forward(g["hidden"]), ref)
 
 
 def test_planned_workspace_equals_allocated_workspace():
@@ -523,6 +587,70 @@ def test_zero_copy_segments_equal_the_concatenation(lengths):
     ref = oracle.forward_batched(lay["hidden"], lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"],
                                  cfg.k, logits_in=L)["out"]
     check_out(got, ref, f"segments {lengths[:4]}...")
+
+
+@pytest.mark.parametrize("router_form", [1, 2], ids=["sequential", "cluster"])
+@pytest.mark.parametrize("T,d,E,k", [(700, 2048, 128, 8), (333, 4096, 8, 2), (600, 7168, 256, 8), (1500, 1024, 40, 4)])
+def test_zero_copy_segments_large_d_both_router_forms(T, d, E, k, router_form):
+    """The segment path where the router splits K over several chunks (d >= 1024: router_nch(d) = 2 or 4), in BOTH
+    router forms -- the cluster form with its DSMEM reduce-scatter and the sequential form with one TMEM accumulator
+    per chunk read their token rows through the segment table here (C1's d = 512 has one chunk).
+    Segments: a boundary inside a 128-token router tile and off the 8-row grid, empty segments, single-token
+    (decode) segments, ragged tails.  Bit-identical to the concatenated call on every routing artefact and on the
+    output, and that output against the oracle."""
+    lengths = [130, 0, 1, 1, 57, 0]
+    rest = T - sum(lengths)
+    lengths += [rest // 2 + 3, 0, rest - rest // 2 - 3]
+    assert sum(lengths) == T and min(lengths) == 0
+    cfg = wl.small_config(T=T, d=d, E=E, k=k, f=128, index=60 + E % 7)
+    lay, g, layer = make(cfg)
+    layer.set_debug(router_form=router_form)
+    ref_out = layer.combined_forward(g["hidden"]).clone()
+    v0 = {kk: x.clone() for kk, x in layer.debug_views(T).items()}
+    torch.cuda.synchronize()
+    segs, pos = [], 0
+    for n in lengths:
+        segs.append(g["hidden"][pos:pos + n].clone())      # every segment in its own allocation
+        pos += n
+    outs = layer.combined_forward_segments(segs)
+    torch.cuda.synchronize()
+    v1 = layer.debug_views(T)
+    for key in ("logits", "idx", "w", "counts", "offsets", "row_src", "inv_perm"):
+        assert torch.equal(v0[key], v1[key]), key
+    got = torch.cat(outs, dim=0)
+    assert torch.equal(got, ref_out), "segment path differs from the concatenated path"
+    L = v1["logits"].cpu().numpy()
+    own = oracle.router_logits(lay["hidden"], lay["W_r"], lay["b_r"])
+    assert np.all(np.abs(L - own) <= 1e-4 * np.maximum(1.0, np.abs(own)))
+    check_routing_against_oracle(v1["logits"], v1["idx"], v1["w"], v1["counts"], v1["offsets"], v1["row_src"],
+                                 v1["inv_perm"], E, k)
+    ref = oracle.forward_batched(lay["hidden"], lay["W_r"], lay["b_r"], lay["W_gate"], lay["W_up"], lay["W_down"],
+                                 k, logits_in=L)["out"]
+    check_out(got, ref, f"segments d={d} form={router_form}")
+
+
+@pytest.mark.parametrize("precision", [1, 2])
+def test_fp8_through_segments_and_host_entry_points(precision):
+    """The FP8 path through the other two fused entry points: the quantising gather has its own
+    segment-table branch and the host pipeline runs the same chain on its own streams -- both must give the bits of
+    the device-pointer FP8 call."""
+    cfg = wl.small_config(T=700, d=256, E=12, k=3, f=256, index=66)
+    lay, g, layer = make(cfg)
+    bf16_out = layer.combined_forward(g["hidden"]).clone()
+    layer.set_precision(precision)
+    ref = layer.combined_forward(g["hidden"]).clone()
+    assert not torch.equal(ref, bf16_out)
+    lengths = [130, 0, 1, 1, 57, 0, 300, 211]
+    segs, pos = [], 0
+    for n in lengths:
+        segs.append(g["hidden"][pos:pos + n].clone())
+        pos += n
+    outs = layer.combined_forward_segments(segs)
+    h_pinned = lay["hidden"].pin_memory()
+    host_out = layer.combined_forward_host(h_pinned)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.cat(outs), ref), "FP8 segments differ from the FP8 device-pointer call"
+    assert torch.equal(host_out, ref.cpu()), "FP8 host entry point differs from the FP8 device-pointer call"
 
 
 def test_zero_copy_segments_argument_errors_and_empty_batch():
