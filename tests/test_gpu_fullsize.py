@@ -25,7 +25,7 @@ pytestmark = pytest.mark.gpu
 MAX_TOL, L2_TOL = 2e-2, 5e-3
 
 
-def run_fullsize(cfg: wl.MoEConfig, shuffle_segments: bool = False):
+def run_fullsize(cfg: wl.MoEConfig, shuffle_segments: bool = False, via_segments: bool = False):
     from paper_2606_21712_b200 import MoELayer
     lay = wl.make_layer(cfg, "cuda")
     hidden = lay["hidden"]
@@ -42,6 +42,28 @@ def run_fullsize(cfg: wl.MoEConfig, shuffle_segments: bool = False):
     torch.cuda.synchronize()
     assert torch.equal(out, out2), "fused path is not bitwise deterministic"
     v = layer.debug_views(cfg.T)
+    if via_segments:
+        # zero-copy COMBINE at full size: the config's own coroutine list -- C5: 30 prefill segments
+        # of 512 rows + 1024 single-token decode segments = 1054 -- each in its own allocation, in both router forms.
+        # Every routing artefact and the output must carry the bits of the concatenated call; what is then checked
+        # against the oracle below is the SEGMENT path's result.
+        lengths = wl.segment_lengths(cfg)
+        assert sum(lengths) == cfg.T
+        segs, pos = [], 0
+        for n in lengths:
+            segs.append(hidden[pos:pos + n].clone())
+            pos += n
+        for form in (1, 2, 0):
+            layer.set_debug(router_form=form)
+            outs = layer.combined_forward_segments(segs)
+            torch.cuda.synchronize()
+            vs = layer.debug_views(cfg.T)
+            for key in ("logits", "idx", "w", "counts", "offsets", "row_src", "inv_perm"):
+                assert torch.equal(v[key], vs[key]), f"segments, router form {form}: {key} differs"
+            seg_out = torch.cat(outs, dim=0)
+            assert torch.equal(seg_out, out), f"segments, router form {form}: output differs from the concatenated call"
+        print(f"[fullsize] {cfg.name}: {len(lengths)} segments, bit-identical to the concatenated call in all router forms")
+        out, v = seg_out, vs
     T, k, E, R = cfg.T, cfg.k, cfg.E, cfg.T * cfg.k
 
     # ---- routing: whole tensors, bit-exact given the GPU's logits
@@ -112,6 +134,10 @@ def test_c4_zipf_skewed_full():
 
 def test_c5_mixed_prefill_decode_full():
     run_fullsize(wl.C5)
+
+
+def test_c5_zero_copy_segments_full():
+    run_fullsize(wl.C5, via_segments=True)
 
 
 def test_c5_segment_order_shuffled():
