@@ -10,6 +10,11 @@ gives no formula; the reading taken (R6) is the two-segment roofl
 Pinned in tests/test_plan.py by exact synthetic data (parameters recovered), by the closed forms
 T_flat = ceil(u*t_floor/s), T_line = ceil(u*t0/((1-u)*s)), and by monotonicity.  Shares no code with the
 library; only tests import it.
+
+workspace_bytes() is the memory side: the sum of the slabs DESIGN.md §4 lists for the context's workspace, each
+rounded up to 1 KB, written out from that list (it is the oracle's own arithmetic, not a call into the library).
+Pinned in tests/test_plan.py by a hand-computed small case, by its exact linear growth per 128 tokens and by what
+the slabs must at least hold.
 """
 from __future__ import annotations
 
@@ -67,3 +72,35 @@ def choose_tokens(fit: dict, target_util: float, memory_budget_bytes: int, granu
             return T, True
         T += granularity
     return t_mem, False
+
+
+def _kb(n: int) -> int:
+    return -(-n // 1024) * 1024
+
+
+def workspace_bytes(d: int, f: int, E: int, k: int, tokens: int) -> int:
+    """Device workspace of a context with max_tokens = tokens ("Library workspace"): every slab is
+    rounded up to a multiple of 1 KB.  T = max(tokens, 1), R = T k, tiles = ceil(T / 128)."""
+    T = max(int(tokens), 1)
+    R = T * k
+    tiles = -(-T // 128)
+    E16 = -(-E // 16) * 16
+    slabs = [
+        4 * T * E,                   # logits [T,E] f32
+        4 * R, 4 * R,                # topk_idx, topk_w [T,k]
+        2 * 3 * d * E16,             # W_r pieces [3][d][ceil16(E)] bf16
+        4 * E, 4 * (E + 1),          # counts [E], offsets [E+1]
+        4 * tiles * E,               # per-tile histograms
+        4 * tiles * E,               # per-tile bases
+        4 * R,                       # tile-local ranks
+        4 * R, 4 * R,                # row_src, inv_perm
+        4 * R,                       # w_perm f32
+        2 * R * d,                   # x_perm bf16
+        2 * R * f,                   # H bf16
+        2 * R * d,                   # Y bf16
+        2 * 2 * T * d,               # host entry point: two [T,d] bf16 staging slots in ...
+        2 * 2 * T * d,               # ... and two out
+        8 * T + 8 * T + 4 * (T + 1), # segment table: hidden pointers, out pointers, start offsets
+        64,                          # counters
+    ]
+    return sum(_kb(b) for b in slabs)
