@@ -50,7 +50,7 @@ def load_traffic(cfg_key: str, kernel: str):
     """DRAM bytes per launch of `kernel` from the committed `ncu --set full` capture of this configuration
     (profiles/r0N_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum; newest round first), and the file
     it came from; (None, None) if there is no capture."""
-    for name in ("r02_traffic.csv", "r01_traffic.csv"):
+    for name in ("r03_traffic.csv", "r02_traffic.csv"):
         p = os.path.join(ROOT, "profiles", name)
         try:
             for ln in open(p).read().splitlines()[1:]:
@@ -351,6 +351,13 @@ def layer_fracs(cfg: wl.MoEConfig, E_act: int, ms: float, peaks: dict) -> dict:
             "frac_of_nominal": max(F / (NOMINAL["bf16_tflops"] * 1e12), B / (NOMINAL["hbm_gbs"] * 1e9)) / (ms * 1e-3)}
 
 
+def burst_fracs(cfg: wl.MoEConfig, E_act: int, ms: float, peaks: dict) -> dict:
+    """layer_fracs for a leg timed in a short burst: a burst time is never divided by the sustained peak."""
+    fr = layer_fracs(cfg, E_act, ms, peaks)
+    fr.pop("frac_of_measured_sustained")
+    return fr
+
+
 def run_config(name: str, steps: int, peaks: dict, device_index: int, sustained: bool = False, note: str = None):
     """One BASELINE.json configuration through the same fused chain and timing protocol as the headline line
     (CUDA events on the launching stream, warm-up, min / median over the timed steps, each point from an idle
@@ -374,7 +381,7 @@ def run_config(name: str, steps: int, peaks: dict, device_index: int, sustained:
     E_act = int((counts > 0).sum())
     ms = total / steps
     row = {"workload": cfg.name, "T": cfg.T, "E_active": E_act, "ms_per_step": ms, "ms_min": float(min(per)),
-           "ms_median": float(np.median(per)), **layer_fracs(cfg, E_act, ms, peaks)}
+           "ms_median": float(np.median(per)), **burst_fracs(cfg, E_act, ms, peaks)}
     row["stage_ms"] = stage_times(layer, step)
     if sustained:
         sampler = ClockSampler(device_index)     # >= 2 s: long enough for NVML's clock / power readings to follow
@@ -424,7 +431,7 @@ def run_c3_sweep(steps: int, peaks: dict, device_index: int):
         counts = layer.debug_views(T)["counts"].cpu().numpy()
         E_act = int((counts > 0).sum())
         row = {"T": T, "ms_per_step": ms, "ms_min": float(min(per)), "ms_median": float(np.median(per)),
-               "E_active": E_act, **layer_fracs(cfg, E_act, ms, peaks)}
+               "E_active": E_act, **burst_fracs(cfg, E_act, ms, peaks)}
         row["stage_ms"] = stage_times(layer, step)
         if T == 16384:
             sampler = ClockSampler(device_index)
@@ -593,7 +600,28 @@ def run_ring(steps: int, device_index: int):
     torch.cuda.synchronize()
     same = bool(torch.equal(out, ref))
     nbytes = layer.ring_bytes_per_call
-    return {"workload": cfg.name, "ring_experts": 16, "h2d_bytes_per_step": nbytes, "resident_ms": ms_res,
+    # skewed routing (a Zipf bias as in BASELINE config C4) at T = 4096, where the step is bound by the PCIe copy:
+    # bg_moe_set_ring_skip_empty copies only the experts that received rows
+    import dataclasses
+    zcfg = dataclasses.replace(cfg.with_T(4096), zipf_s=2.0)
+    _, zb = wl.make_router(zcfg, "cuda")
+    zh, zo = hidden[:4096].contiguous(), torch.empty_like(hidden[:4096])
+    zstep = lambda: layer.combined_forward(zh, zo, stream)
+    layer.set_weights(lay["W_r"], zb, lay["W_gate"], lay["W_up"], lay["W_down"])
+    zstep()
+    zref = zo.clone()
+    n_live = int((layer.debug_views(4096)["counts"] > 0).sum())
+    layer.set_weights_offloaded(lay["W_r"], zb, *pinned, ring_experts=16)
+    ms_all = med(zstep)
+    bytes_all = layer.ring_bytes_per_call
+    layer.set_ring_skip_empty(True)
+    ms_skip = med(zstep)
+    torch.cuda.synchronize()
+    skip = {"workload": "C3 weights, T=4096, Zipf(2.0) router bias", "experts_with_rows": n_live, "experts": cfg.E,
+            "copy_all_ms": ms_all, "copy_all_bytes": bytes_all, "skip_empty_ms": ms_skip,
+            "skip_empty_bytes": layer.ring_bytes_per_call, "bit_identical_to_resident": bool(torch.equal(zo, zref)),
+            "note": "one host synchronisation per call (this call's counts are read back before the copies are issued)"}
+    return {"skip_empty": skip, "workload": cfg.name, "ring_experts": 16, "h2d_bytes_per_step": nbytes, "resident_ms": ms_res,
             "bare_h2d_copy_ms": ms_copy, "bare_h2d_gbs": nbytes / ms_copy / 1e6, "streamed_ms": ms_ring,
             "streamed_h2d_gbs": nbytes / ms_ring / 1e6, "overlap_efficiency": max(ms_copy, ms_res) / ms_ring,
             "bit_identical_to_resident": same}
@@ -659,6 +687,16 @@ def run_ours(args):
     for _ in range(3):
         e2e_step()
     ms_e2e = timed(e2e_step, args.steps)[0] / args.steps
+    # the same call one at a time: host buffers -> result back on the host, nothing else in flight (latency of ONE
+    # call; the number above is the throughput of back-to-back calls pipelined over the two staging slots)
+    lat = []
+    for _ in range(5):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        e2e_step()
+        torch.cuda.synchronize()
+        lat.append((time.perf_counter() - t0) * 1e3)
+    ms_e2e_single = float(np.median(lat))
 
     # ---- per-kernel durations (CUDA events recorded by the library on the launching stream)
     stage_ms = stage_times(layer, step, rounds=3, burst=max(4, min(args.steps, 8)))
@@ -671,7 +709,6 @@ def run_ours(args):
     B_min = cfg.min_bytes(E_act)
     tflops = whole_job_rate(F, world, ms_step) / 1e12
     t_roof_burst = max(F / (peaks["bf16_tflops"] * 1e12), B_min / (peaks["hbm_gbs"] * 1e9))
-    t_roof_sust = max(F / (peaks["bf16_tflops_sustained"] * 1e12), B_min / (peaks["hbm_gbs"] * 1e9))
     t_roof_nom = max(F / (NOMINAL["bf16_tflops"] * 1e12), B_min / (NOMINAL["hbm_gbs"] * 1e9))
 
     # dominant kernel and its roofline: algorithmic work of THAT launch against max(flops / P, bytes / BW)
@@ -703,13 +740,16 @@ def run_ours(args):
         "tokens_per_s": whole_job_rate(cfg.T, world, ms_step),
         "layer_roofline": {"F_gflop": F / 1e9, "B_min_mb": B_min / 1e6,
                            "frac_of_measured_burst": t_roof_burst / (ms_step * 1e-3),
-                           "frac_of_measured_sustained": t_roof_sust / (ms_step * 1e-3),
                            "frac_of_nominal": t_roof_nom / (ms_step * 1e-3), "peaks": peaks,
                            "peak_source": peak_src},
         "stage_ms": stage_ms,
         "roofline": roofline,
         "e2e": {"value": whole_job_rate(F, world, ms_e2e) / 1e12, "unit": "TFLOP/s", "ms_per_step": ms_e2e,
-                "h2d_bytes_per_step": int(cfg.T * cfg.d * 2), "d2h_bytes_per_step": int(cfg.T * cfg.d * 2)},
+                "h2d_bytes_per_step": int(cfg.T * cfg.d * 2), "d2h_bytes_per_step": int(cfg.T * cfg.d * 2),
+                "mode": "pipelined: back-to-back bg_moe_combined_forward_host calls over 2 staging slots (throughput)",
+                "single_call_latency_ms": ms_e2e_single,
+                "single_call_note": "one host call alone, host wall clock from the call to the result on the host "
+                                    "(upload, chain and download in series)"},
         "gpu_launches": int(launches),
         "clocks": clocks,
     }

@@ -85,11 +85,22 @@ int bg_moe_set_weights(bg_moe_ctx* ctx, const float* W_r, const float* b_r, cons
  * Afterwards bg_moe_combined_forward (and the _segments / _host forms) runs the expert FFN chunk by chunk:
  * ring_experts/2 experts are copied into one half on a stream the context owns while the grouped GEMMs of the
  * previous chunk run out of the other half.  Same kernels, same per-row arithmetic: results are bit-identical to
- * the resident path.  Every expert is copied (which experts are empty is known only on the device; no host
- * synchronisation is taken).  The split calls (bg_moe_expert_ffn) need resident weights. */
+ * the resident path.  By default every expert is copied (which experts are empty is known only on the device; no
+ * host synchronisation is taken) -- see bg_moe_set_ring_skip_empty.  The split calls (bg_moe_expert_ffn) need
+ * resident weights. */
 int bg_moe_set_weights_offloaded(bg_moe_ctx* ctx, const float* W_r, const float* b_r, const void* W_gate_host,
                                  const void* W_up_host, const void* W_down_host, int32_t ring_experts,
                                  void* stream);
+/* Skip the experts nobody was routed to (the ring holds "the running and prefetching expert";
+ * offloaded experts are streamed only when they run).  With enable != 0 a fused call on offloaded
+ * weights reads its own per-expert counts back into pinned memory (copied on the ring's stream as soon as the
+ * router kernel has finished, while the gather runs) and copies into the ring only the experts that received at
+ * least one row; chunks with no such expert are skipped altogether.  Same kernels, same rows: the result stays
+ * bit-identical to the resident path.  Cost: ONE host synchronisation per call -- the calling thread blocks until
+ * this call's router has finished (and so until everything queued before it on `stream` has) -- which is why it is
+ * opt-in; it pays when routing is skewed (BASELINE config C4: ~60 of 256 experts are empty at T = 8192) and the
+ * step is bound by the PCIe copy anyway.  Set-up time allocation: E pinned ints.  No effect on resident weights. */
+int bg_moe_set_ring_skip_empty(bg_moe_ctx* ctx, int32_t enable);
 /* Host -> device bytes the ring copied during the last fused call (0 with resident weights). */
 int64_t bg_moe_ring_bytes_per_call(const bg_moe_ctx* ctx);
 

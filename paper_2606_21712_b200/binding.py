@@ -16,7 +16,7 @@ EXPORTS = ["bg_moe_create", "bg_moe_destroy", "bg_moe_set_weights", "bg_moe_rout
            "bg_moe_expert_ffn", "bg_moe_unpermute", "bg_moe_combined_forward", "bg_moe_combined_forward_host",
            "bg_moe_debug_views", "bg_moe_profile_enable", "bg_moe_profile_read", "bg_moe_launch_count", "bg_moe_workspace_bytes", "bg_moe_strerror",
            "bg_moe_last_error", "bg_moe_set_debug", "bg_moe_set_weights_offloaded", "bg_moe_ring_bytes_per_call", "bg_moe_set_precision", "bg_moe_debug_fp8_views", "bg_moe_debug_fp8_down_views", "bg_moe_combined_forward_segments", "bg_moe_fit_roofline", "bg_moe_workspace_bytes_for", "bg_moe_choose_tokens",
-           "bg_moe_route_logits_noalloc", "bg_moe_noalloc_last_error", "bg_moe_host_input_sync", "bg_moe_debug_ffn_views"]
+           "bg_moe_route_logits_noalloc", "bg_moe_noalloc_last_error", "bg_moe_host_input_sync", "bg_moe_debug_ffn_views", "bg_moe_set_ring_skip_empty"]
 
 
 class BgMoeConfig(ctypes.Structure):
@@ -51,6 +51,7 @@ def load_library() -> ctypes.CDLL:
         lib.bg_moe_set_debug.argtypes = [vp, i32, i32, i32]
         lib.bg_moe_set_weights_offloaded.argtypes = [vp, vp, vp, vp, vp, vp, i32, vp]
         lib.bg_moe_ring_bytes_per_call.argtypes = [vp]
+        lib.bg_moe_set_ring_skip_empty.argtypes = [vp, i32]
         lib.bg_moe_ring_bytes_per_call.restype = i64
         lib.bg_moe_set_precision.argtypes = [vp, i32, vp]
         lib.bg_moe_debug_fp8_views.argtypes = [vp] + [ctypes.POINTER(vp)] * 6
@@ -215,6 +216,11 @@ class MoELayer:
             t = torch.as_tensor(_DeviceArray(p.value, (R, width), "<u2"), device=self._dev())
             out[name] = t[r0:r1].clone().view(torch.bfloat16)
         return out
+
+    def set_ring_skip_empty(self, enable: bool = True):
+        """bg_moe_set_ring_skip_empty: offloaded weights only -- copy just the experts that received rows (one host
+        synchronisation per call)."""
+        self._check(self.lib.bg_moe_set_ring_skip_empty(self._ctx, int(bool(enable))))
 
     @property
     def ring_bytes_per_call(self) -> int:

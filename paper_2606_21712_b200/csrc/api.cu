@@ -94,6 +94,11 @@ struct bg_moe_ctx {
   cudaEvent_t ev_ring_ready[2] = {}, ev_ring_free[2] = {};
   bool ring_used[2] = {false, false};
   int64_t ring_h2d_bytes = 0;         // bytes copied host -> ring by the last forward
+  // bg_moe_set_ring_skip_empty: this call's expert counts are read back (pinned, event-ordered on st_ring) and only
+  // experts that received rows are copied into the ring
+  bool ring_skip_empty = false;
+  int32_t* counts_host = nullptr;     // pinned [E]
+  cudaEvent_t ev_router_done = nullptr, ev_counts = nullptr;
   // activation tensor maps of the workspace x_perm / H (whole capacity: rows past T*k are never stored)
   bg::ActMaps am_x, am_h;
   int sg_max = 0;               // bg_moe_set_debug: overrides the pair kernel's super-group size (tests)
@@ -372,26 +377,45 @@ int do_ffn(bg_moe_ctx* ctx, const void* x_perm, const int32_t* offsets, int32_t 
 // ("the buffer slot ownership is released after the module completes execution").  The GEMM kernels are the
 // resident path's: they see `ring_chunk` experts whose offsets are the matching slice of the layer's offsets, so
 // every row runs through exactly the same arithmetic and the result is bit-identical.  Parameter movement is one
-// way, host -> device; every expert is copied (which experts are empty is only known on the device, and this
-// path takes no host synchronisation either).
+// way, host -> device.  By default every expert is copied (which experts are empty is only known on the device, and
+// this path takes no host synchronisation either); with bg_moe_set_ring_skip_empty the call reads its own counts
+// back first and copies only the experts that received rows.
 int do_ffn_ring(bg_moe_ctx* ctx, int32_t T, cudaStream_t st) {
   const bg_moe_config& c = ctx->cfg;
   const int C = ctx->ring_chunk;
   const size_t gu_bytes = static_cast<size_t>(c.d) * c.f * 2;       // one expert's W_gate (= W_up = W_down) bytes
   const size_t half_bytes = 3 * gu_bytes * C;
   ctx->ring_h2d_bytes = 0;
-  for (int e0 = 0, chunk = 0; e0 < c.E; e0 += C, ++chunk) {
-    const int h = chunk & 1;
+  const bool skip = ctx->ring_skip_empty;
+  if (skip)   // the ONE host synchronisation of this mode: this call's counts have landed in pinned memory
+    BG_CUDA(ctx, cudaEventSynchronize(ctx->ev_counts), "wait for this call's expert counts");
+  for (int e0 = 0, used = 0; e0 < c.E; e0 += C) {
     const int n = c.E - e0 < C ? c.E - e0 : C;
+    if (skip) {                          // a chunk none of whose experts received a row: no copy, no GEMM launch
+      bool any = false;
+      for (int e = e0; e < e0 + n; ++e) any = any || ctx->counts_host[e] > 0;
+      if (!any) continue;
+    }
+    const int h = used & 1;
+    ++used;
     uint8_t* half = ctx->ring + h * half_bytes;
     if (ctx->ring_used[h]) BG_CUDA(ctx, cudaStreamWaitEvent(ctx->st_ring, ctx->ev_ring_free[h], 0), "ring half free");
-    BG_CUDA(ctx, cudaMemcpyAsync(half, ctx->host_wg + e0 * gu_bytes, n * gu_bytes, cudaMemcpyHostToDevice, ctx->st_ring),
-            "H2D W_gate chunk");
-    BG_CUDA(ctx, cudaMemcpyAsync(half + C * gu_bytes, ctx->host_wu + e0 * gu_bytes, n * gu_bytes, cudaMemcpyHostToDevice,
-                                 ctx->st_ring), "H2D W_up chunk");
-    BG_CUDA(ctx, cudaMemcpyAsync(half + 2 * C * gu_bytes, ctx->host_wd + e0 * gu_bytes, n * gu_bytes,
-                                 cudaMemcpyHostToDevice, ctx->st_ring), "H2D W_down chunk");
-    ctx->ring_h2d_bytes += 3 * static_cast<int64_t>(n) * gu_bytes;
+    // runs of consecutive experts to copy: the whole chunk, or (skip mode) the maximal runs of non-empty experts;
+    // an expert keeps its slot (e - e0) in the half either way, so the tensor maps and offsets do not change
+    for (int a = 0; a < n;) {
+      if (skip && ctx->counts_host[e0 + a] == 0) { ++a; continue; }
+      int b = a + 1;
+      while (b < n && (!skip || ctx->counts_host[e0 + b] > 0)) ++b;
+      const size_t src = (e0 + a) * gu_bytes, dst = a * gu_bytes, len = (b - a) * gu_bytes;
+      BG_CUDA(ctx, cudaMemcpyAsync(half + dst, ctx->host_wg + src, len, cudaMemcpyHostToDevice, ctx->st_ring),
+              "H2D W_gate chunk");
+      BG_CUDA(ctx, cudaMemcpyAsync(half + C * gu_bytes + dst, ctx->host_wu + src, len, cudaMemcpyHostToDevice,
+                                   ctx->st_ring), "H2D W_up chunk");
+      BG_CUDA(ctx, cudaMemcpyAsync(half + 2 * C * gu_bytes + dst, ctx->host_wd + src, len, cudaMemcpyHostToDevice,
+                                   ctx->st_ring), "H2D W_down chunk");
+      ctx->ring_h2d_bytes += 3 * static_cast<int64_t>(len);
+      a = b;
+    }
     BG_CUDA(ctx, cudaEventRecord(ctx->ev_ring_ready[h], ctx->st_ring), "record ring ready");
     BG_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_ring_ready[h], 0), "wait ring ready");
     int rc = do_ffn(ctx, ctx->x_perm, ctx->offsets + e0, T, ctx->Y, ctx->w_perm, st, -1, 1 + h, n);
@@ -408,6 +432,15 @@ int do_forward(bg_moe_ctx* ctx, const void* hidden, int32_t T, void* out, cudaSt
   mark(ctx, 0, st);
   int rc = do_route(ctx, hidden, T, nullptr, ctx->logits, ctx->topk_idx, ctx->topk_w, ctx->counts, ctx->offsets, st, seg);
   if (rc) return rc;
+  if (ctx->ring_chunk != 0 && ctx->ring_skip_empty) {
+    // counts are final once the router kernel has finished: bring them to the host on the ring's copy stream while
+    // the gather runs on `st`
+    BG_CUDA(ctx, cudaEventRecord(ctx->ev_router_done, st), "record router done");
+    BG_CUDA(ctx, cudaStreamWaitEvent(ctx->st_ring, ctx->ev_router_done, 0), "ring stream waits for the router");
+    BG_CUDA(ctx, cudaMemcpyAsync(ctx->counts_host, ctx->counts, sizeof(int32_t) * c.E, cudaMemcpyDeviceToHost,
+                                 ctx->st_ring), "D2H counts");
+    BG_CUDA(ctx, cudaEventRecord(ctx->ev_counts, ctx->st_ring), "record counts on host");
+  }
   mark(ctx, 1, st);
   bg::PermLaunch pl = {ctx->topk_idx, ctx->tile_rank, ctx->tile_base, ctx->topk_w, ctx->row_src, ctx->inv_perm,
                        ctx->w_perm};
@@ -512,6 +545,9 @@ void destroy_ctx(bg_moe_ctx* ctx) {
     if (ctx->ev_ring_ready[i]) cudaEventDestroy(ctx->ev_ring_ready[i]);
     if (ctx->ev_ring_free[i]) cudaEventDestroy(ctx->ev_ring_free[i]);
   }
+  if (ctx->ev_router_done) cudaEventDestroy(ctx->ev_router_done);
+  if (ctx->ev_counts) cudaEventDestroy(ctx->ev_counts);
+  if (ctx->counts_host) cudaFreeHost(ctx->counts_host);
   if (ctx->st_ring) cudaStreamDestroy(ctx->st_ring);
   if (ctx->ring) cudaFree(ctx->ring);
   if (ctx->fp8_buf) cudaFree(ctx->fp8_buf);
@@ -720,6 +756,23 @@ int bg_moe_set_weights_offloaded(bg_moe_ctx* ctx, const float* W_r, const float*
   ctx->W_gate = W_gate_host; ctx->W_up = W_up_host; ctx->W_down = W_down_host;   // "weights set" for the entry checks
   ctx->ring_chunk = chunk;
   ctx->precision = 0;             // the streamed path is bf16
+  return BG_OK;
+}
+
+int bg_moe_set_ring_skip_empty(bg_moe_ctx* ctx, int32_t enable) {
+  if (!ctx) return BG_ERR_INVALID_ARG;
+  if (enable && ctx->counts_host == nullptr) {      // set-up time: E pinned ints and two events
+    DeviceGuard guard(ctx->cfg.device);
+    void* p = nullptr;
+    if (cudaHostAlloc(&p, sizeof(int32_t) * ctx->cfg.E, cudaHostAllocDefault) != cudaSuccess) {
+      cudaGetLastError();
+      return BG_ERR_NOMEM;
+    }
+    ctx->counts_host = static_cast<int32_t*>(p);
+    BG_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_router_done, cudaEventDisableTiming), "router-done event");
+    BG_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_counts, cudaEventDisableTiming), "counts event");
+  }
+  ctx->ring_skip_empty = enable != 0;
   return BG_OK;
 }
 

@@ -510,23 +510,72 @@ def test_offloaded_weights_ring_buffer_equals_resident(ring_experts):
     assert torch.equal(layer.combined_forward(g["hidden"]), ref)
 
 
+@pytest.mark.parametrize("ring_experts", [2, 6, 32])
+def test_ring_buffer_skips_experts_without_rows(ring_experts):
+    """bg_moe_set_ring_skip_empty: on a skewed layer -- a router bias that starves most
+    experts, as BASELINE config C4's Zipf bias does -- only the experts that received rows are copied into the ring
+    (the byte counter says exactly which), whole chunks of empty experts are skipped, and the result keeps the bits
+    of the resident path; switching the option off copies everything again."""
+    cfg = wl.small_config(T=500, d=256, E=19, k=2, f=192, index=38)
+    lay, g, layer = make(cfg)
+    b = torch.full((cfg.E,), -40.0)
+    live = [0, 1, 5, 6, 7, 13, 18]                       # runs of 2, 3, 1, 1 experts; chunks of 3 / 16 with none at all
+    b[live] = 0.0
+    layer.set_weights(g["W_r"], b.cuda(), g["W_gate"], g["W_up"], g["W_down"])
+    ref = layer.combined_forward(g["hidden"]).clone()
+    counts = layer.debug_views(cfg.T)["counts"].cpu().numpy()
+    assert set(np.nonzero(counts)[0].tolist()) <= set(live) and (counts == 0).sum() >= cfg.E - len(live)
+    n_live = int((counts > 0).sum())
+    pinned = [lay[n].pin_memory() for n in ("W_gate", "W_up", "W_down")]
+    layer.set_weights_offloaded(g["W_r"], b.cuda(), *pinned, ring_experts=ring_experts)
+    per_expert = 6 * cfg.d * cfg.f
+    a = layer.combined_forward(g["hidden"]).clone()
+    torch.cuda.synchronize()
+    assert layer.ring_bytes_per_call == per_expert * cfg.E and torch.equal(a, ref)      # default: every expert
+    layer.set_ring_skip_empty(True)
+    h2 = g["hidden"].flip(0).contiguous()
+    for x in (g["hidden"], h2, g["hidden"]):
+        got = layer.combined_forward(x).clone()
+        torch.cuda.synchronize()
+        c = layer.debug_views(cfg.T)["counts"].cpu().numpy()
+        assert layer.ring_bytes_per_call == per_expert * int((c > 0).sum()), "copied bytes != non-empty experts"
+        if x is g["hidden"]:
+            assert torch.equal(got, ref), "skip-empty ring differs from the resident path"
+    assert layer.ring_bytes_per_call == per_expert * n_live
+    # segments and the host entry point ride the same path
+    segs = [g["hidden"][:77].clone(), g["hidden"][77:].clone()]
+    outs = layer.combined_forward_segments(segs)
+    h_pinned = lay["hidden"].pin_memory()
+    host_out = layer.combined_forward_host(h_pinned)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.cat(outs), ref) and torch.equal(host_out, ref.cpu())
+    layer.set_ring_skip_empty(False)
+    assert torch.equal(layer.combined_forward(g["hidden"]), ref)
+    torch.cuda.synchronize()
+    assert layer.ring_bytes_per_call == per_expert * cfg.E
+    L = layer.debug_views(cfg.T)["logits"].cpu().numpy()
+    o = oracle.forward_batched(lay["hidden"], lay["W_r"], b, lay["W_gate"], lay["W_up"], lay["W_down"], cfg.k,
+                               logits_in=L)["out"]
+    check_out(ref, o, "skewed layer")
+
+
 def test_failed_ring_allocation_leaves_no_half_state():
     """A bg_moe_set_weights_offloaded call that cannot get its ring must leave the context either as it was
     (resident weights) or without weights (BG_ERR_NO_WEIGHTS from the next forward) -- never with a freed ring and
-    the old chunk size.  The impossible request is a ring of 2 x 256 Mixtral-sized experts (~180 GB); the host
+    the old chunk size.  The impossible request is a ring of 2 x 256 experts of 3 x 268 MB (~412 GB); the host
     pointers are never read because no forward succeeds while they are installed... except the small first ring,
     which is only installed, not run."""
     import ctypes
     from paper_2606_21712_b200 import MoELayer, BgMoeError, BG_ERR_NO_WEIGHTS, BG_ERR_NOMEM
-    d, f, E, k = 4096, 14336, 256, 2
+    d, f, E, k = 8192, 16384, 256, 2
     layer = MoELayer(d, f, E, k, 8)
     W_r = torch.zeros(d, E, device="cuda")
-    fake = torch.zeros(64, dtype=torch.uint8).pin_memory()          # stands for three 30 GB host tensors: never read
+    fake = torch.zeros(64, dtype=torch.uint8).pin_memory()          # stands for three 69 GB host tensors: never read
     hp = ctypes.c_void_p(fake.data_ptr())
     st = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
     call = lambda ring: layer.lib.bg_moe_set_weights_offloaded(layer._ctx, ctypes.c_void_p(W_r.data_ptr()), None, hp, hp,
                                                                hp, ring, st)
-    assert call(2) == 0                                             # 0.7 GB ring: fits
+    assert call(2) == 0                                             # 1.6 GB ring: fits
     assert call(512) == BG_ERR_NOMEM                                # 2 x 256 experts: cannot fit
     x = torch.zeros(8, d, dtype=torch.bfloat16, device="cuda")
     with pytest.raises(BgMoeError) as ei:
