@@ -11,7 +11,7 @@
 // For them the per-tile histograms and the tile ticket -- the only global memory this kernel needs beyond its
 // inputs and outputs -- live in a fixed array that is part of the library image (g_scratch below).  Its size fixes
 // the largest call: BG_MOE_NOALLOC_MAX_TOKENS tokens, E <= 256.  Every GPU on which the library's module is loaded
-// holds its own copy of the array (129 KB + 256 B) until the process exits.
+// holds its own copy of the array (128 KiB + 256 B = 131,328 bytes) until the process exits.
 //
 // This file is self-contained on purpose: the array, the one place that asks the runtime for its device address and
 // the kernel that uses it must be in ONE translation unit (the array has internal linkage), and nothing here touches
